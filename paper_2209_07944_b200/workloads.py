@@ -1,0 +1,187 @@
+"""Seeded synthetic workloads (BASELINE.json `configs`; recipe in DESIGN.md §5).
+
+This module holds NONE of the method's arithmetic: it only draws initial particle states and source
+histories with ``numpy.random.default_rng`` and converts them to the units of the C-ABI (positions in grid
+units, momenta u = gamma v / c).  It is the one module shared by the CUDA path's harness and the tests'
+oracle harness; it imports neither.  The inputs stand in for the paper's own set-ups (§3), which
+are self-defined simulations, not a public dataset.
+"""
+from __future__ import annotations
+
+import math
+from dataclasses import dataclass
+from typing import Dict, Iterator, Optional
+
+import numpy as np
+
+# Physical constants (DESIGN.md §3 reading A18)
+C_SI = 299792458.0
+EPS0_SI = 8.8541878128e-12
+E_CHARGE = 1.602176634e-19
+M_E = 9.1093837015e-31
+M_P = 1.67262192369e-27
+SEED0 = 20220907
+
+
+@dataclass(frozen=True)
+class Workload:
+    """Grid + run description of one BASELINE.json config."""
+
+    name: str
+    config: int
+    n: int  # cubic grid n^3
+    dx: float
+    steps: int
+    field_only: bool = False
+
+    @property
+    def dt(self) -> float:
+        return self.dx / (2.0 * C_SI)  # dt = dx/(2c) in every config
+
+    @property
+    def N(self) -> int:
+        return self.n ** 3
+
+    @property
+    def H(self) -> int:
+        # BASELINE.json: H = ceil(sqrt(3) * n * dx / (c dt)) + 2
+        return int(math.ceil(math.sqrt(3.0 * (self.n * self.dx) ** 2) / (C_SI * self.dt))) + 2
+
+    @property
+    def seed(self) -> int:
+        return SEED0 + self.config
+
+
+WORKLOADS: Dict[int, Workload] = {
+    1: Workload("cfg1_16c_electron_cloud", 1, 16, 1e-4, 64),
+    2: Workload("cfg2_32c_neutral_plasma", 2, 32, 1e-4, 100),
+    3: Workload("cfg3_64c_electron_beam", 3, 64, 5e-5, 200),
+    4: Workload("cfg4_96c_field_only", 4, 96, 1e-4, 1, field_only=True),
+    5: Workload("cfg5_128c_two_stream", 5, 128, 5e-5, 50),
+}
+
+
+def _sigma_u(kT_eV: float, mass: float) -> float:
+    """Maxwellian: each momentum component u = gamma v/c is Gaussian with sigma = sqrt(kT/(m c^2))."""
+    return math.sqrt(kT_eV * E_CHARGE / (mass * C_SI * C_SI))
+
+
+def _gauss_inside(rng, mean, sigma, n, lo, hi):
+    """Gaussian draws, rejecting and redrawing values outside [lo, hi)."""
+    out = rng.normal(mean, sigma, n)
+    bad = (out < lo) | (out >= hi)
+    while bad.any():
+        out[bad] = rng.normal(mean, sigma, int(bad.sum()))
+        bad = (out < lo) | (out >= hi)
+    return out
+
+
+def _species(x, y, z, ux, uy, uz, charge, mass, weight):
+    n = x.shape[0]
+    return dict(x=x, y=y, z=z, ux=ux, uy=uy, uz=uz,
+                qw=np.full(n, charge * weight), qm=np.full(n, charge / mass))
+
+
+def _concat(parts):
+    keys = ("x", "y", "z", "ux", "uy", "uz", "qw", "qm")
+    out = {k: np.concatenate([p[k] for p in parts]).astype(np.float32) for k in keys}
+    out["alive"] = np.ones(out["x"].shape[0], dtype=np.uint8)
+    return out
+
+
+def particles(config: int, scale: float = 1.0) -> Dict[str, np.ndarray]:
+    """Initial macro-particles of a PIC config as fp32 arrays (positions in grid units, u = gamma v/c).
+
+    ``scale`` < 1 draws proportionally fewer macro-particles with proportionally larger weight (same total
+    charge); used only by CPU-sized tests.  Keys: x y z ux uy uz qw (C per macro-particle) qm (q/m) alive.
+    """
+    w = WORKLOADS[config]
+    rng = np.random.default_rng(w.seed)
+    n = float(w.n)
+    if config == 1:
+        P = max(1, int(round(4096 * scale)))
+        wt = 1e6 / scale
+        su = _sigma_u(1000.0, M_E)
+        pos = [_gauss_inside(rng, n / 2, 3.0, P, 0.0, n) for _ in range(3)]
+        mom = [rng.normal(0.0, su, P) for _ in range(3)]
+        return _concat([_species(*pos, *mom, -E_CHARGE, M_E, wt)])
+    if config == 2:
+        P = max(1, int(round(100000 * scale)))
+        wt = 1e6 / scale
+        parts = []
+        for charge, mass, kT in ((-E_CHARGE, M_E, 1000.0), (E_CHARGE, M_P, 10.0)):
+            su = _sigma_u(kT, mass)
+            pos = [rng.uniform(n / 2 - 8.0, n / 2 + 8.0, P) for _ in range(3)]
+            mom = [rng.normal(0.0, su, P) for _ in range(3)]
+            parts.append(_species(*pos, *mom, charge, mass, wt))
+        return _concat(parts)
+    if config == 3:
+        P = max(1, int(round(1000000 * scale)))
+        wt = 5e4 / scale
+        su = _sigma_u(10.0, M_E)
+        x = _gauss_inside(rng, n / 2, 4.0, P, 0.0, n)
+        y = _gauss_inside(rng, n / 2, 4.0, P, 0.0, n)
+        z = rng.uniform(16.0, 48.0, P)
+        beta = 0.5
+        drift = beta / math.sqrt(1.0 - beta * beta)  # gamma_d * beta_d, added in u-space
+        mom = [rng.normal(0.0, su, P), rng.normal(0.0, su, P), rng.normal(0.0, su, P) + drift]
+        return _concat([_species(x, y, z, *mom, -E_CHARGE, M_E, wt)])
+    if config == 5:
+        Pb = max(1, int(round(2000000 * scale)))
+        Pp = max(1, int(round(4000000 * scale)))
+        wt = 2e5 / scale
+        su = _sigma_u(100.0, M_E)
+        parts = []
+        for sign in (+1.0, -1.0):
+            beta = 0.3
+            drift = sign * beta / math.sqrt(1.0 - beta * beta)
+            x = rng.uniform(0.0, n, Pb)
+            y = _gauss_inside(rng, n / 2, 8.0, Pb, 0.0, n)
+            z = _gauss_inside(rng, n / 2, 8.0, Pb, 0.0, n)
+            mom = [rng.normal(0.0, su, Pb) + drift, rng.normal(0.0, su, Pb), rng.normal(0.0, su, Pb)]
+            parts.append(_species(x, y, z, *mom, -E_CHARGE, M_E, wt))
+        pos = [rng.uniform(0.0, n, Pp) for _ in range(3)]
+        zero = [np.zeros(Pp) for _ in range(3)]
+        parts.append(_species(*pos, *zero, E_CHARGE, M_P, wt))
+        out = _concat(parts)
+        # fp32 rounding of a draw just below n can land on n exactly; keep every start position inside [0, n)
+        for k in ("x", "y", "z"):
+            np.minimum(out[k], np.nextafter(np.float32(n), np.float32(0)), out=out[k])
+        return out
+    raise ValueError(f"config {config} has no particles")
+
+
+def history_slices(n_cells: int, H: int, seed: int, j_scale: float = 1.0) -> Iterator[np.ndarray]:
+    """Config-4 style source history: H slices of [4][N] fp32, i.i.d. uniform in [-1, 1].
+
+    Slot t uses its own generator ``default_rng([seed, t])`` so any slice can be regenerated alone.
+    ``j_scale`` multiplies Jx,Jy,Jz (the parity-only variant uses j_scale = c so that the J-dot term of
+    Eq. (2.4) is visible next to the rho terms; SURVEY.md §8(d) config 4 caveat).
+    """
+    for t in range(H):
+        yield history_slice(n_cells, t, seed, j_scale)
+
+
+def history_slice(n_cells: int, t: int, seed: int, j_scale: float = 1.0) -> np.ndarray:
+    rng = np.random.default_rng([seed, t])
+    s = rng.uniform(-1.0, 1.0, (4, n_cells))
+    if j_scale != 1.0:
+        s[1:] *= j_scale
+    return s.astype(np.float32)
+
+
+def sample_obs(n_cells_axis: int, count: int, seed: int) -> np.ndarray:
+    """Seeded observation-cell sample for sampled parity: `count` random cells + 8 corners, 6 face centres
+    and the centre cell."""
+    n = n_cells_axis
+    rng = np.random.default_rng([seed, 777])
+    idx = rng.integers(0, n ** 3, size=count, dtype=np.int64)
+    m, c = n - 1, n // 2
+    special = []
+    for k in (0, m):
+        for j in (0, m):
+            for i in (0, m):
+                special.append((i, j, k))
+    special += [(0, c, c), (m, c, c), (c, 0, c), (c, m, c), (c, c, 0), (c, c, m), (c, c, c)]
+    sp = np.array([i + n * (j + n * k) for i, j, k in special], dtype=np.int64)
+    return np.concatenate([idx, sp])
