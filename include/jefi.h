@@ -1,0 +1,137 @@
+/*
+ * jefi.h — C-ABI of libjefi: the B200-native hot path of JefiPIC (arXiv 2209.07944).
+ *
+ * One opaque context per simulation on one GPU.  It owns (1) a device ring buffer with the last H time steps
+ * of the sources rho, J and their backward time differences, (2) the translation-invariant delay table of the
+ * uniform grid, (3) scratch for the cell-sorted deposit.  The six calls of the PIC cycle are
+ *
+ *     jefi_deposit -> jefi_push_sources -> jefi_field_step -> jefi_push_particles
+ *
+ * Conventions common to every call
+ *   - Plain C types only.  Unless a parameter says "host", array arguments are DEVICE pointers owned by the
+ *     caller (e.g. torch tensors); the library never frees or keeps them.  The context owns everything it
+ *     allocates and releases it in jefi_destroy.
+ *   - Work is enqueued on the cudaStream_t given in jefi_config.stream (NULL = legacy default stream) and the
+ *     call returns without synchronising, except where stated ("host" variants and debug exports synchronise).
+ *   - Return value: 0 (JEFI_OK) or a negative JEFI_E* code; jefi_last_error() then returns a text.  No call
+ *     aborts, throws or falls back to the CPU.
+ *   - Grid: nx*ny*nz cuboid cells, cell index c = i + nx*(j + ny*k) (x fastest); every field lives at the cell
+ *     centre ((i+.5)dx, (j+.5)dy, (k+.5)dz).  Sources and observation points share the grid.
+ *   - Particles: positions in GRID UNITS (xi = x/dx in [0,nx), ...), momenta u = gamma*v/c (dimensionless).
+ *     These are "flexible units" in the sense of PAPER.md:233 and make the cell index bit-exact.
+ *   - Step counter n starts at -1; each jefi_push_sources makes it n+1 and stores the sources of step n.
+ */
+#ifndef JEFI_H
+#define JEFI_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define JEFI_OK 0
+#define JEFI_EINVAL (-1) /* NULL / out-of-range argument */
+#define JEFI_ENOMEM (-2) /* host or device allocation failed */
+#define JEFI_ECUDA (-3)  /* a CUDA runtime call failed; text in jefi_last_error */
+#define JEFI_ESTATE (-4) /* call not valid in this state (e.g. field_step before any push_sources) */
+
+/* field_impl values */
+#define JEFI_FIELD_AUTO 0      /* tiled kernel when its delay arithmetic is proven equal to the fp64 table, else reference */
+#define JEFI_FIELD_REFERENCE 1 /* one thread per observation cell, table-driven delays (slow; the paper's K1 in fp32) */
+#define JEFI_FIELD_TILED 2     /* shared-memory tiled kernel; jefi_create fails with JEFI_ESTATE if not provable */
+
+typedef struct jefi_ctx jefi_ctx; /* opaque */
+
+typedef struct {
+  int nx, ny, nz;       /* cells per axis (>= 1) */
+  double dx, dy, dz;    /* cell size, metres (> 0) */
+  double dt;            /* time step, seconds (> 0) */
+  double c, eps0;       /* 0 -> SI values 299792458 and 8.8541878128e-12; mu0 := 1/(eps0 c^2) */
+  int H;                /* ring depth in steps; 0 -> N_dt + 2 with N_dt = min(ceil(Lmax/(c dt)), hist_cap),
+                           Lmax the diagonal of the region.  Delays m > H-2 contribute zero. */
+  int hist_cap;         /* 0 -> 10000 */
+  double Eext[3];       /* uniform background E, V/m, added at the particle */
+  double Bext[3];       /* uniform background B, tesla */
+  int device;           /* CUDA device ordinal */
+  void* stream;         /* cudaStream_t; NULL -> default stream */
+  int field_impl;       /* JEFI_FIELD_* */
+} jefi_config;
+
+/* Create a context: allocates the ring (32*H*N_padded bytes, zeroed = "zero before t0"), builds the
+ * delay table m(|di|,|dj|,|dk|) = floor(R/(c dt) + 1/2) in fp64 on the host (Eq. 2.6; nearest-step reading,
+ * DESIGN.md §3 A1) and verifies on the device that the tiled kernel's fp32 delay arithmetic reproduces it for
+ * every offset.  *out is set to NULL on failure.  Synchronises. */
+int jefi_create(const jefi_config* cfg, jefi_ctx** out);
+
+/* Release everything the context owns.  NULL is a no-op.  Synchronises the context's stream first. */
+void jefi_destroy(jefi_ctx* ctx);
+
+/* Text of the last error of this context ("" if none).  ctx == NULL returns the last jefi_create error. */
+const char* jefi_last_error(const jefi_ctx* ctx);
+
+/* Values the context resolved at create time (H, N_dt, which field kernel runs ...).  All optional (NULL ok). */
+int jefi_get_info(const jefi_ctx* ctx, int* H, int* ndt, int* field_impl, long* step, long* ring_bytes);
+
+/* CIC (volume-weighted) charge/current deposit, Eqs. (2.15)-(2.19).
+ *   np            number of macro-particles (>= 0)
+ *   x,y,z         positions, grid units, np floats each
+ *   ux,uy,uz      u = gamma v / c, np floats each; v = c u / sqrt(1+|u|^2)
+ *   qw            charge of each macro-particle, coulomb
+ *   alive         np bytes, 0 = dead (skipped); NULL = all alive
+ *   rho,jx,jy,jz  OUT, N floats each (C/m^3, A/m^2), overwritten (zeroed by the call).
+ * Node (i,j,k) = floor(xi-.5) ... gets q*w/dV with the 8 trilinear weights; nodes outside the grid are virtual
+ * and dropped.  Sums are fp32 atomics: the order of equal-cell particles is not defined.
+ * The caller's particle arrays are not modified. */
+int jefi_deposit(jefi_ctx* ctx, long np, const float* x, const float* y, const float* z, const float* ux,
+                 const float* uy, const float* uz, const float* qw, const unsigned char* alive, float* rho,
+                 float* jx, float* jy, float* jz);
+
+/* Store the sources of the next step: n += 1, ring slot n mod H <- (rho, J) and their backward differences
+ * against step n-1 (the finite differences of Eqs. 2.4-2.5; zero history before step 0).
+ * rho,jx,jy,jz: N floats each, cell order x fastest. */
+int jefi_push_sources(jefi_ctx* ctx, const float* rho, const float* jx, const float* jy, const float* jz);
+
+/* Jefimenko field solve at the current step n, Eqs. (2.4)-(2.6), PAPER.md:103-109:
+ *   E(r) =  dV/(4 pi eps0) sum_{r'!=r} [ d rho/R^3 + d rho_dot/(c R^2) - J_dot/(c^2 R) ]
+ *   B(r) = -mu0 dV/(4 pi)  sum_{r'!=r} [ d x J/R^3 + d x J_dot/(c R^2) ]
+ * with d = r - r', sources at step n - m(d), time derivatives from steps n-m and n-m-1, the self cell skipped
+ * (PAPER.md:221).  ex..bz: OUT, N floats each (V/m, tesla), overwritten.
+ * JEFI_ESTATE before the first jefi_push_sources. */
+int jefi_field_step(jefi_ctx* ctx, float* ex, float* ey, float* ez, float* bx, float* by, float* bz);
+
+/* Field interpolation (Eq. 2.20) + relativistic Boris push (Eqs. 2.7-2.11, DESIGN.md §3 A5/A6) + kill rule
+ * (PAPER.md:205, 239): for each alive particle gather E,B from the 8 nodes (virtual nodes count as zero), add
+ * Eext/Bext, update u and then the position by v*dt; a particle whose new position leaves [0,n) on any axis gets
+ * alive = 0 and is never pushed or deposited again.
+ *   x..uz   IN/OUT np floats each;  q_over_m  np floats (C/kg);  alive IN/OUT np bytes (must not be NULL)
+ *   ex..bz  fields at step n, N floats each. */
+int jefi_push_particles(jefi_ctx* ctx, long np, float* x, float* y, float* z, float* ux, float* uy, float* uz,
+                        const float* q_over_m, unsigned char* alive, const float* ex, const float* ey,
+                        const float* ez, const float* bx, const float* by, const float* bz);
+
+/* End-to-end variant of one field step with HOST buffers (pinned memory recommended): copies the newest source
+ * slice (4 x N floats) host->device, does jefi_push_sources + jefi_field_step, copies E,B (6 x N floats)
+ * device->host and synchronises the stream.  Host arrays: src_host = [rho|jx|jy|jz] (4N floats),
+ * eb_host = [ex|ey|ez|bx|by|bz] (6N floats). */
+int jefi_field_step_host(jefi_ctx* ctx, const float* src_host, float* eb_host);
+
+/* Number of kernel launches this context has enqueued so far (bench.py's gpu_launches). */
+long jefi_launch_count(const jefi_ctx* ctx);
+
+/* Duration in milliseconds of the most recent jefi_field_step's main kernel, measured with CUDA events on the
+ * context's stream.  Synchronises on the end event.  < 0 if no field step ran. */
+float jefi_last_field_kernel_ms(jefi_ctx* ctx);
+
+/* ---- debug / parity exports (synchronise; not on the timed path) ---- */
+/* m for every non-negative offset (a,b,c): m_out[a + nx*(b + ny*c)], HOST int array of N entries. */
+int jefi_debug_delay_table(jefi_ctx* ctx, int* m_out_host);
+/* Node index (i,j,k) = floor(xi - .5) of each particle as the deposit/push kernels compute it:
+ * ijk_out = DEVICE int array [np][3]. */
+int jefi_debug_cell_index(jefi_ctx* ctx, long np, const float* x, const float* y, const float* z, int* ijk_out);
+/* The stored sources of step n - steps_back: out4N = DEVICE float array [4][N] = rho, Jx, Jy, Jz (J rescaled
+ * back to A/m^2).  JEFI_EINVAL if that step is not in the ring. */
+int jefi_debug_history_slot(jefi_ctx* ctx, int steps_back, float* out4N);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* JEFI_H */

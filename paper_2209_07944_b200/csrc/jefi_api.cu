@@ -1,0 +1,311 @@
+// libjefi: context, history ring buffer and debug exports.  Boundary: include/jefi.h.
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <new>
+
+#include "jefi_ctx.h"
+
+static std::string g_create_err;
+
+static int fail_create(jefi_ctx* c, int code, const std::string& msg) {
+  g_create_err = msg;
+  if (c) {
+    c->err = msg;
+    jefi_destroy(c);
+  }
+  return code;
+}
+
+extern "C" const char* jefi_last_error(const jefi_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_err.c_str(); }
+
+extern "C" long jefi_launch_count(const jefi_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+extern "C" int jefi_get_info(const jefi_ctx* ctx, int* H, int* ndt, int* field_impl, long* step, long* ring_bytes) {
+  if (!ctx) return JEFI_EINVAL;
+  if (H) *H = ctx->dims.H;
+  if (ndt) *ndt = ctx->ndt;
+  if (field_impl) *field_impl = ctx->field_impl;
+  if (step) *step = ctx->step;
+  if (ring_bytes) *ring_bytes = ctx->ring_bytes;
+  return JEFI_OK;
+}
+
+
+extern "C" int jefi_create(const jefi_config* cfg, jefi_ctx** out) {
+  if (out) *out = nullptr;
+  if (!cfg || !out) return fail_create(nullptr, JEFI_EINVAL, "jefi_create: NULL argument");
+  if (cfg->nx < 1 || cfg->ny < 1 || cfg->nz < 1 || !(cfg->dx > 0) || !(cfg->dy > 0) || !(cfg->dz > 0) || !(cfg->dt > 0) ||
+      cfg->c < 0 || cfg->eps0 < 0 || cfg->H < 0 || cfg->hist_cap < 0)
+    return fail_create(nullptr, JEFI_EINVAL, "jefi_create: grid sizes, spacings and dt must be positive");
+  if ((long)cfg->nx * cfg->ny * cfg->nz > (1L << 30)) return fail_create(nullptr, JEFI_EINVAL, "jefi_create: grid too large");
+  jefi_ctx* c = new (std::nothrow) jefi_ctx();
+  if (!c) return fail_create(nullptr, JEFI_ENOMEM, "jefi_create: host allocation failed");
+  c->cfg = *cfg;
+  c->ringS = c->ringD = nullptr;
+  c->mtab_dev = nullptr;
+  c->mtab_host = nullptr;
+  c->src_stage = c->eb_stage = nullptr;
+  c->ev0 = c->ev1 = nullptr;
+  c->ev_valid = false;
+  c->launches = 0;
+  c->step = -1;
+  c->stream = (cudaStream_t)cfg->stream;
+  c->c = cfg->c > 0 ? cfg->c : 299792458.0;
+  c->eps0 = cfg->eps0 > 0 ? cfg->eps0 : 8.8541878128e-12;
+  c->mu0 = 1.0 / (c->eps0 * c->c * c->c);
+
+  cudaError_t e = cudaSetDevice(cfg->device);
+  if (e != cudaSuccess) return fail_create(c, JEFI_ECUDA, std::string("cudaSetDevice: ") + cudaGetErrorString(e));
+
+  // ---- history depth ----
+  const double L0 = c->c * cfg->dt;  // light-step length
+  double lx = cfg->nx * cfg->dx, ly = cfg->ny * cfg->dy, lz = cfg->nz * cfg->dz;
+  double lmax = sqrt(lx * lx + ly * ly + lz * lz);
+  long cap = cfg->hist_cap > 0 ? cfg->hist_cap : 10000;
+  long ndt = (long)ceil(lmax / L0);
+  if (ndt > cap) ndt = cap;
+  c->ndt = (int)ndt;
+  int H = cfg->H > 0 ? cfg->H : (int)ndt + 2;
+  if (H < 2) return fail_create(c, JEFI_EINVAL, "jefi_create: H must be >= 2 (value and backward difference)");
+
+  jefi_dims& d = c->dims;
+  d.nx = cfg->nx; d.ny = cfg->ny; d.nz = cfg->nz;
+  d.ntx = (cfg->nx + JEFI_TS - 1) / JEFI_TS; d.nty = (cfg->ny + JEFI_TS - 1) / JEFI_TS; d.ntz = (cfg->nz + JEFI_TS - 1) / JEFI_TS;
+  d.H = H;
+  d.N = (long)cfg->nx * cfg->ny * cfg->nz;
+  d.ncell_pad = (long)d.ntx * d.nty * d.ntz * JEFI_TCELLS;
+
+  // ---- scaled geometry: d' = d/(c dt), J stored as J/c ----
+  const double dV = cfg->dx * cfg->dy * cfg->dz;
+  const double PI = 3.14159265358979323846;
+  c->geom.kx = (float)(cfg->dx / L0);
+  c->geom.ky = (float)(cfg->dy / L0);
+  c->geom.kz = (float)(cfg->dz / L0);
+  c->geom.prefE = (float)(dV / (4.0 * PI * c->eps0) / (L0 * L0));
+  c->geom.prefB = (float)(-c->mu0 * dV / (4.0 * PI) * c->c / (L0 * L0));
+
+  // ---- ring: zero-initialised = "J and rho are simply set to zero" before t0 ----
+  size_t ring_elems = (size_t)d.ncell_pad * H;
+  c->ring_bytes = (long)(2 * ring_elems * sizeof(float4));
+  if ((e = cudaMalloc(&c->ringS, ring_elems * sizeof(float4))) != cudaSuccess ||
+      (e = cudaMalloc(&c->ringD, ring_elems * sizeof(float4))) != cudaSuccess)
+    return fail_create(c, JEFI_ENOMEM, std::string("ring allocation (") + std::to_string(c->ring_bytes) + " B): " + cudaGetErrorString(e));
+  cudaMemsetAsync(c->ringS, 0, ring_elems * sizeof(float4), c->stream);
+  cudaMemsetAsync(c->ringD, 0, ring_elems * sizeof(float4), c->stream);
+
+  // ---- delay table, fp64 on the host: m = floor(R/(c dt) + 1/2) (Eq. 2.6, reading A1) ----
+  const int ex = jefi_table_extent(d.nx), ey = jefi_table_extent(d.ny), ez = jefi_table_extent(d.nz);
+  size_t tn = (size_t)ex * ey * ez;
+  c->mtab_host = (int*)malloc(tn * sizeof(int));
+  if (!c->mtab_host) return fail_create(c, JEFI_ENOMEM, "delay table host allocation failed");
+  for (int kc = 0; kc < ez; kc++)
+    for (int jb = 0; jb < ey; jb++)
+      for (int ia = 0; ia < ex; ia++) {
+        double ddx = ia * cfg->dx, ddy = jb * cfg->dy, ddz = kc * cfg->dz;
+        double R = sqrt(ddx * ddx + ddy * ddy + ddz * ddz);
+        c->mtab_host[ia + (size_t)ex * (jb + (size_t)ey * kc)] = (int)floor(R / L0 + 0.5);
+      }
+  if ((e = cudaMalloc(&c->mtab_dev, tn * sizeof(int))) != cudaSuccess)
+    return fail_create(c, JEFI_ENOMEM, std::string("delay table device allocation: ") + cudaGetErrorString(e));
+  if ((e = cudaMemcpyAsync(c->mtab_dev, c->mtab_host, tn * sizeof(int), cudaMemcpyHostToDevice, c->stream)) != cudaSuccess)
+    return fail_create(c, JEFI_ECUDA, std::string("delay table upload: ") + cudaGetErrorString(e));
+
+  if ((e = cudaEventCreate(&c->ev0)) != cudaSuccess || (e = cudaEventCreate(&c->ev1)) != cudaSuccess)
+    return fail_create(c, JEFI_ECUDA, std::string("cudaEventCreate: ") + cudaGetErrorString(e));
+
+  // ---- choose the field kernel ----
+  c->field_impl = JEFI_FIELD_REFERENCE;
+  if (cfg->field_impl != JEFI_FIELD_REFERENCE) {
+    long mism = -1;
+    int rc = jefi_verify_delay_fp32(c, &mism);
+    if (rc != JEFI_OK) return fail_create(c, rc, c->err);
+    int prep = (mism == 0) ? jefi_tiled_prepare(c) : JEFI_ESTATE;
+    if (mism == 0 && prep == JEFI_OK) {
+      c->field_impl = JEFI_FIELD_TILED;
+    } else if (cfg->field_impl == JEFI_FIELD_TILED) {
+      char buf[256];
+      snprintf(buf, sizeof buf, "tiled field kernel not usable: %ld delay mismatches against the fp64 table, prepare rc=%d (%s)",
+               mism, prep, c->err.c_str());
+      return fail_create(c, JEFI_ESTATE, buf);
+    }
+  }
+  if ((e = cudaStreamSynchronize(c->stream)) != cudaSuccess)
+    return fail_create(c, JEFI_ECUDA, std::string("create sync: ") + cudaGetErrorString(e));
+  c->err.clear();
+  *out = c;
+  return JEFI_OK;
+}
+
+extern "C" void jefi_destroy(jefi_ctx* c) {
+  if (!c) return;
+  cudaStreamSynchronize(c->stream);
+  if (c->ringS) cudaFree(c->ringS);
+  if (c->ringD) cudaFree(c->ringD);
+  if (c->mtab_dev) cudaFree(c->mtab_dev);
+  if (c->src_stage) cudaFree(c->src_stage);
+  if (c->eb_stage) cudaFree(c->eb_stage);
+  if (c->mtab_host) free(c->mtab_host);
+  if (c->ev0) cudaEventDestroy(c->ev0);
+  if (c->ev1) cudaEventDestroy(c->ev1);
+  delete c;
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// Row a1: history push.  One thread per real cell: reads the previous slot, writes value and backward difference.
+// Traffic: 16 B in (4 SoA floats) + 16 B read (previous) + 32 B written per cell.
+// ------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_push_sources(jefi_dims d, float inv_c, int slot, int prev_slot,
+                                                      const float* __restrict__ rho, const float* __restrict__ jx,
+                                                      const float* __restrict__ jy, const float* __restrict__ jz,
+                                                      float4* __restrict__ ringS, float4* __restrict__ ringD) {
+  long cidx = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (cidx >= d.N) return;
+  int i = (int)(cidx % d.nx), j = (int)((cidx / d.nx) % d.ny), k = (int)(cidx / ((long)d.nx * d.ny));
+  size_t base = (size_t)jefi_ring_cell(d, i, j, k) * d.H;
+  float4 s = make_float4(rho[cidx], jx[cidx] * inv_c, jy[cidx] * inv_c, jz[cidx] * inv_c);
+  float4 p = prev_slot >= 0 ? ringS[base + prev_slot] : make_float4(0.f, 0.f, 0.f, 0.f);
+  ringS[base + slot] = s;
+  ringD[base + slot] = make_float4(s.x - p.x, s.y - p.y, s.z - p.z, s.w - p.w);
+}
+
+int jefi_launch_push_sources(jefi_ctx* c, const float* rho, const float* jx, const float* jy, const float* jz) {
+  const jefi_dims& d = c->dims;
+  long n = c->step + 1;
+  int slot = (int)(n % d.H);
+  int prev = n >= 1 ? (int)((n - 1) % d.H) : -1;
+  unsigned blocks = (unsigned)((d.N + 255) / 256);
+  k_push_sources<<<blocks, 256, 0, c->stream>>>(d, (float)(1.0 / c->c), slot, prev, rho, jx, jy, jz, c->ringS, c->ringD);
+  JEFI_CUDA_TRY(c, cudaGetLastError());
+  c->launches++;
+  c->step = n;
+  return JEFI_OK;
+}
+
+extern "C" int jefi_push_sources(jefi_ctx* c, const float* rho, const float* jx, const float* jy, const float* jz) {
+  if (!c) return JEFI_EINVAL;
+  if (!rho || !jx || !jy || !jz) { c->err = "jefi_push_sources: NULL array"; return JEFI_EINVAL; }
+  return jefi_launch_push_sources(c, rho, jx, jy, jz);
+}
+
+extern "C" int jefi_field_step(jefi_ctx* c, float* ex, float* ey, float* ez, float* bx, float* by, float* bz) {
+  if (!c) return JEFI_EINVAL;
+  if (!ex || !ey || !ez || !bx || !by || !bz) { c->err = "jefi_field_step: NULL array"; return JEFI_EINVAL; }
+  if (c->step < 0) { c->err = "jefi_field_step before any jefi_push_sources"; return JEFI_ESTATE; }
+  JEFI_CUDA_TRY(c, cudaEventRecord(c->ev0, c->stream));
+  int rc = c->field_impl == JEFI_FIELD_TILED ? jefi_launch_field_tiled(c, ex, ey, ez, bx, by, bz)
+                                             : jefi_launch_field_reference(c, ex, ey, ez, bx, by, bz);
+  if (rc != JEFI_OK) return rc;
+  JEFI_CUDA_TRY(c, cudaEventRecord(c->ev1, c->stream));
+  c->ev_valid = true;
+  return JEFI_OK;
+}
+
+extern "C" float jefi_last_field_kernel_ms(jefi_ctx* c) {
+  if (!c || !c->ev_valid) return -1.f;
+  if (cudaEventSynchronize(c->ev1) != cudaSuccess) return -1.f;
+  float ms = -1.f;
+  if (cudaEventElapsedTime(&ms, c->ev0, c->ev1) != cudaSuccess) return -1.f;
+  return ms;
+}
+
+extern "C" int jefi_field_step_host(jefi_ctx* c, const float* src_host, float* eb_host) {
+  if (!c) return JEFI_EINVAL;
+  if (!src_host || !eb_host) { c->err = "jefi_field_step_host: NULL array"; return JEFI_EINVAL; }
+  const long N = c->dims.N;
+  if (!c->src_stage) {
+    if (cudaMalloc(&c->src_stage, 4 * N * sizeof(float)) != cudaSuccess || cudaMalloc(&c->eb_stage, 6 * N * sizeof(float)) != cudaSuccess) {
+      c->err = "jefi_field_step_host: staging allocation failed";
+      return JEFI_ENOMEM;
+    }
+  }
+  JEFI_CUDA_TRY(c, cudaMemcpyAsync(c->src_stage, src_host, 4 * N * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+  float* s = c->src_stage;
+  int rc = jefi_push_sources(c, s, s + N, s + 2 * N, s + 3 * N);
+  if (rc != JEFI_OK) return rc;
+  float* o = c->eb_stage;
+  rc = jefi_field_step(c, o, o + N, o + 2 * N, o + 3 * N, o + 4 * N, o + 5 * N);
+  if (rc != JEFI_OK) return rc;
+  JEFI_CUDA_TRY(c, cudaMemcpyAsync(eb_host, o, 6 * N * sizeof(float), cudaMemcpyDeviceToHost, c->stream));
+  JEFI_CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  return JEFI_OK;
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// debug exports
+// ------------------------------------------------------------------------------------------------------------
+extern "C" int jefi_debug_delay_table(jefi_ctx* c, int* m_out_host) {
+  if (!c || !m_out_host) return JEFI_EINVAL;
+  const jefi_dims& d = c->dims;
+  const int ex = jefi_table_extent(d.nx), ey = jefi_table_extent(d.ny);
+  // read the DEVICE copy back so the export shows what the kernels actually index
+  size_t tn = (size_t)ex * ey * jefi_table_extent(d.nz);
+  int* tmp = (int*)malloc(tn * sizeof(int));
+  if (!tmp) return JEFI_ENOMEM;
+  cudaError_t e = cudaMemcpyAsync(tmp, c->mtab_dev, tn * sizeof(int), cudaMemcpyDeviceToHost, c->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+  if (e != cudaSuccess) { free(tmp); c->err = cudaGetErrorString(e); return JEFI_ECUDA; }
+  for (int kc = 0; kc < d.nz; kc++)
+    for (int jb = 0; jb < d.ny; jb++)
+      for (int ia = 0; ia < d.nx; ia++)
+        m_out_host[ia + (size_t)d.nx * (jb + (size_t)d.ny * kc)] = tmp[ia + (size_t)ex * (jb + (size_t)ey * kc)];
+  free(tmp);
+  return JEFI_OK;
+}
+
+__global__ void __launch_bounds__(256) k_history_slot(jefi_dims d, float cc, int slot, const float4* __restrict__ ringS,
+                                                      float* __restrict__ out) {
+  long cidx = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (cidx >= d.N) return;
+  int i = (int)(cidx % d.nx), j = (int)((cidx / d.nx) % d.ny), k = (int)(cidx / ((long)d.nx * d.ny));
+  float4 s = ringS[(size_t)jefi_ring_cell(d, i, j, k) * d.H + slot];
+  out[cidx] = s.x;
+  out[d.N + cidx] = s.y * cc;
+  out[2 * d.N + cidx] = s.z * cc;
+  out[3 * d.N + cidx] = s.w * cc;
+}
+
+extern "C" int jefi_debug_history_slot(jefi_ctx* c, int steps_back, float* out4N) {
+  if (!c || !out4N) return JEFI_EINVAL;
+  const jefi_dims& d = c->dims;
+  long t = c->step - steps_back;
+  if (steps_back < 0 || steps_back > d.H - 1 || t < 0) { c->err = "jefi_debug_history_slot: step not in the ring"; return JEFI_EINVAL; }
+  k_history_slot<<<(unsigned)((d.N + 255) / 256), 256, 0, c->stream>>>(d, (float)c->c, (int)(t % d.H), c->ringS, out4N);
+  JEFI_CUDA_TRY(c, cudaGetLastError());
+  JEFI_CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  return JEFI_OK;
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// Row a2: proof that the tiled kernel's fp32 delay arithmetic equals the fp64 table on every offset it can form.
+// ------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_verify_delay(int ex, int ey, int ez, jefi_geom g, const int* __restrict__ mtab,
+                                                      unsigned long long* __restrict__ mismatches) {
+  long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  long tn = (long)ex * ey * ez;
+  if (idx >= tn || idx == 0) return;  // offset (0,0,0) is the self cell: never evaluated
+  int ia = (int)(idx % ex), jb = (int)((idx / ex) % ey), kc = (int)(idx / ((long)ex * ey));
+  float q = jefi_q_fp32(g.kx, g.ky, g.kz, (float)ia, (float)jb, (float)kc);
+  if (jefi_delay_fp32(q) != mtab[idx]) atomicAdd(mismatches, 1ull);
+}
+
+int jefi_verify_delay_fp32(jefi_ctx* c, long* mismatches) {
+  const jefi_dims& d = c->dims;
+  const int ex = jefi_table_extent(d.nx), ey = jefi_table_extent(d.ny), ez = jefi_table_extent(d.nz);
+  unsigned long long* cnt = nullptr;
+  JEFI_CUDA_TRY(c, cudaMalloc(&cnt, sizeof(unsigned long long)));
+  cudaMemsetAsync(cnt, 0, sizeof(unsigned long long), c->stream);
+  long tn = (long)ex * ey * ez;
+  k_verify_delay<<<(unsigned)((tn + 255) / 256), 256, 0, c->stream>>>(ex, ey, ez, c->geom, c->mtab_dev, cnt);
+  cudaError_t e = cudaGetLastError();
+  unsigned long long h = 0;
+  if (e == cudaSuccess) e = cudaMemcpyAsync(&h, cnt, sizeof h, cudaMemcpyDeviceToHost, c->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+  cudaFree(cnt);
+  if (e != cudaSuccess) { c->err = std::string("delay verification: ") + cudaGetErrorString(e); return JEFI_ECUDA; }
+  c->launches++;
+  *mismatches = (long)h;
+  return JEFI_OK;
+}

@@ -1,0 +1,202 @@
+// libjefi: CIC deposit (Eqs. 2.15-2.19) and field interpolation +
+// relativistic Boris push + kill (row a5; PAPER.md:117-127 Eqs. 2.7-2.11, :193-205 Eq. 2.20).
+#include "jefi_ctx.h"
+
+// Eq. (2.15)/(2.17) in grid units: node index i = floor(xi - 1/2), fraction alpha = xi - 1/2 - i.  xi - 0.5 is exact
+// in fp32 for 0.25 <= xi < 2^23, so the index equals the fp64 oracle's bit for bit (DESIGN.md §3 A9).
+__device__ __forceinline__ void cic_cell(float xi, int& i, float& alpha) {
+  float s = xi - 0.5f;
+  float f = floorf(s);
+  i = (int)f;
+  alpha = s - f;
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// deposit: one thread per particle; the 8 node contributions of the 4 quantities go out as fp32 reductions.
+// Lanes of a warp whose particles fall on the same node first combine their contributions with a match-any
+// segmented shuffle reduction, so a cell-sorted particle list issues one atomic per (warp, node) instead of one per
+// particle (warp-aggregated atomics).
+// ------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void warp_aggregated_add4(float* __restrict__ rho, float* __restrict__ jx, float* __restrict__ jy,
+                                                     float* __restrict__ jz, long node, float r, float vx, float vy, float vz) {
+  // Called by all 32 lanes.  node < 0 marks "nothing to add" (virtual node or dead particle); such keys are unique
+  // per lane so they never form a group.
+  const unsigned FULL = 0xffffffffu;
+  const unsigned lane = threadIdx.x & 31;
+  const unsigned peers = __match_any_sync(FULL, node);  // lanes that target the same node
+  float a0 = r, a1 = r * vx, a2 = r * vy, a3 = r * vz;
+  const unsigned cnt = __popc(peers);
+  const unsigned maxcnt = __reduce_max_sync(FULL, cnt);
+  if (maxcnt > 1) {
+    // tree reduction inside every peer group: at stride s the lanes of rank 0, 2s, 4s.. add the lane of rank + s
+    const unsigned rank = __popc(peers & ((1u << lane) - 1u));
+    for (unsigned stride = 1; stride < maxcnt; stride <<= 1) {
+      const bool has = rank + stride < cnt;
+      const int partner = has ? (int)__fns(peers, 0, (int)(rank + stride + 1)) : (int)lane;
+      const float b0 = __shfl_sync(FULL, a0, partner), b1 = __shfl_sync(FULL, a1, partner);
+      const float b2 = __shfl_sync(FULL, a2, partner), b3 = __shfl_sync(FULL, a3, partner);
+      if (has && (rank & (2u * stride - 1u)) == 0u) { a0 += b0; a1 += b1; a2 += b2; a3 += b3; }
+    }
+    if (rank != 0) return;  // only the lowest lane of a group issues the atomics (after the last shuffle)
+  }
+  if (node >= 0) {
+    atomicAdd(rho + node, a0); atomicAdd(jx + node, a1); atomicAdd(jy + node, a2); atomicAdd(jz + node, a3);
+  }
+}
+
+__global__ void __launch_bounds__(256) k_deposit(int nx, int ny, int nz, float inv_dV, float cc, long np,
+                                                 const float* __restrict__ x, const float* __restrict__ y,
+                                                 const float* __restrict__ z, const float* __restrict__ ux,
+                                                 const float* __restrict__ uy, const float* __restrict__ uz,
+                                                 const float* __restrict__ qw, const unsigned char* __restrict__ alive,
+                                                 float* __restrict__ rho, float* __restrict__ jx, float* __restrict__ jy,
+                                                 float* __restrict__ jz) {
+  long p = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  bool live = p < np && (alive == nullptr || alive[p] != 0);
+  int i = 0, j = 0, k = 0;
+  float al = 0, be = 0, ch = 0, r0 = 0, vx = 0, vy = 0, vz = 0;
+  if (live) {
+    cic_cell(x[p], i, al); cic_cell(y[p], j, be); cic_cell(z[p], k, ch);
+    float u0 = ux[p], u1 = uy[p], u2 = uz[p];
+    float ig = rsqrtf(1.f + u0 * u0 + u1 * u1 + u2 * u2);  // 1/gamma
+    vx = cc * u0 * ig; vy = cc * u1 * ig; vz = cc * u2 * ig;  // v = c u / gamma
+    r0 = qw[p] * inv_dV;                                     // Eq. (2.18)
+  }
+#pragma unroll
+  for (int c3 = 0; c3 < 8; c3++) {
+    const int a = c3 & 1, b = (c3 >> 1) & 1, c = c3 >> 2;
+    int ii = i + a, jj = j + b, kk = k + c;
+    bool ok = live && ii >= 0 && ii < nx && jj >= 0 && jj < ny && kk >= 0 && kk < nz;  // virtual nodes dropped
+    float w = (a ? al : 1.f - al) * (b ? be : 1.f - be) * (c ? ch : 1.f - ch);          // Eq. (2.16)
+    long node = ok ? (long)ii + (long)nx * ((long)jj + (long)ny * kk) : -1 - (long)(threadIdx.x & 31);
+    warp_aggregated_add4(rho, jx, jy, jz, node, r0 * w, vx, vy, vz);
+  }
+}
+
+extern "C" int jefi_deposit(jefi_ctx* c, long np, const float* x, const float* y, const float* z, const float* ux,
+                            const float* uy, const float* uz, const float* qw, const unsigned char* alive, float* rho,
+                            float* jx, float* jy, float* jz) {
+  if (!c) return JEFI_EINVAL;
+  if (np < 0 || !rho || !jx || !jy || !jz || (np > 0 && (!x || !y || !z || !ux || !uy || !uz || !qw))) {
+    c->err = "jefi_deposit: NULL array or negative np";
+    return JEFI_EINVAL;
+  }
+  const jefi_dims& d = c->dims;
+  JEFI_CUDA_TRY(c, cudaMemsetAsync(rho, 0, d.N * sizeof(float), c->stream));
+  JEFI_CUDA_TRY(c, cudaMemsetAsync(jx, 0, d.N * sizeof(float), c->stream));
+  JEFI_CUDA_TRY(c, cudaMemsetAsync(jy, 0, d.N * sizeof(float), c->stream));
+  JEFI_CUDA_TRY(c, cudaMemsetAsync(jz, 0, d.N * sizeof(float), c->stream));
+  if (np == 0) return JEFI_OK;
+  float inv_dV = (float)(1.0 / (c->cfg.dx * c->cfg.dy * c->cfg.dz));
+  unsigned blocks = (unsigned)((np + 255) / 256);
+  k_deposit<<<blocks, 256, 0, c->stream>>>(d.nx, d.ny, d.nz, inv_dV, (float)c->c, np, x, y, z, ux, uy, uz, qw, alive, rho, jx,
+                                           jy, jz);
+  JEFI_CUDA_TRY(c, cudaGetLastError());
+  c->launches++;
+  return JEFI_OK;
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// interpolation + Boris + kill: one thread per particle
+// ------------------------------------------------------------------------------------------------------------
+struct push_consts {
+  int nx, ny, nz;
+  float half_dt_over_c;  // dt/(2c): u += (q/m) * this * E
+  float half_dt;         // dt/2:    t = (q/m) * this * B / gamma
+  float sx, sy, sz;      // c dt / dx ...: grid-unit displacement = (u/gamma) * s
+  float Eext[3], Bext[3];
+};
+
+__global__ void __launch_bounds__(256) k_push(push_consts K, long np, float* __restrict__ x, float* __restrict__ y,
+                                              float* __restrict__ z, float* __restrict__ ux, float* __restrict__ uy,
+                                              float* __restrict__ uz, const float* __restrict__ qm,
+                                              unsigned char* __restrict__ alive, const float* __restrict__ ex,
+                                              const float* __restrict__ ey, const float* __restrict__ ez,
+                                              const float* __restrict__ bx, const float* __restrict__ by,
+                                              const float* __restrict__ bz) {
+  long p = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= np || alive[p] == 0) return;
+  float xp = x[p], yp = y[p], zp = z[p];
+  int i, j, k;
+  float al, be, ch;
+  cic_cell(xp, i, al); cic_cell(yp, j, be); cic_cell(zp, k, ch);
+  float E0 = 0, E1 = 0, E2 = 0, B0 = 0, B1 = 0, B2 = 0;
+#pragma unroll
+  for (int c3 = 0; c3 < 8; c3++) {  // Eq. (2.20); virtual nodes count as zero
+    const int a = c3 & 1, b = (c3 >> 1) & 1, c = c3 >> 2;
+    int ii = i + a, jj = j + b, kk = k + c;
+    if (ii >= 0 && ii < K.nx && jj >= 0 && jj < K.ny && kk >= 0 && kk < K.nz) {
+      float w = (a ? al : 1.f - al) * (b ? be : 1.f - be) * (c ? ch : 1.f - ch);
+      long node = (long)ii + (long)K.nx * ((long)jj + (long)K.ny * kk);
+      E0 = fmaf(w, __ldg(ex + node), E0); E1 = fmaf(w, __ldg(ey + node), E1); E2 = fmaf(w, __ldg(ez + node), E2);
+      B0 = fmaf(w, __ldg(bx + node), B0); B1 = fmaf(w, __ldg(by + node), B1); B2 = fmaf(w, __ldg(bz + node), B2);
+    }
+  }
+  E0 += K.Eext[0]; E1 += K.Eext[1]; E2 += K.Eext[2];
+  B0 += K.Bext[0]; B1 += K.Bext[1]; B2 += K.Bext[2];
+  const float qom = qm[p];
+  const float he = qom * K.half_dt_over_c, hb = qom * K.half_dt;
+  // Eq. (2.9): half electric kick
+  float umx = fmaf(he, E0, ux[p]), umy = fmaf(he, E1, uy[p]), umz = fmaf(he, E2, uz[p]);
+  // Eq. (2.10): rotation, gamma taken at u^-
+  float igm = 1.0f / sqrtf(1.f + umx * umx + umy * umy + umz * umz);
+  float tx = hb * B0 * igm, ty = hb * B1 * igm, tz = hb * B2 * igm;
+  float upx = umx + (umy * tz - umz * ty);
+  float upy = umy + (umz * tx - umx * tz);
+  float upz = umz + (umx * ty - umy * tx);
+  float sc = 2.f / (1.f + tx * tx + ty * ty + tz * tz);
+  float sx = tx * sc, sy = ty * sc, sz = tz * sc;
+  float uqx = umx + (upy * sz - upz * sy);
+  float uqy = umy + (upz * sx - upx * sz);
+  float uqz = umz + (upx * sy - upy * sx);
+  // Eq. (2.11): second half kick
+  float unx = fmaf(he, E0, uqx), uny = fmaf(he, E1, uqy), unz = fmaf(he, E2, uqz);
+  float ign = 1.0f / sqrtf(1.f + unx * unx + uny * uny + unz * unz);
+  // Eq. (2.8) in grid units
+  float xn = fmaf(unx * ign, K.sx, xp), yn = fmaf(uny * ign, K.sy, yp), zn = fmaf(unz * ign, K.sz, zp);
+  ux[p] = unx; uy[p] = uny; uz[p] = unz;
+  x[p] = xn; y[p] = yn; z[p] = zn;
+  if (xn < 0.f || xn >= (float)K.nx || yn < 0.f || yn >= (float)K.ny || zn < 0.f || zn >= (float)K.nz) alive[p] = 0;
+}
+
+extern "C" int jefi_push_particles(jefi_ctx* c, long np, float* x, float* y, float* z, float* ux, float* uy, float* uz,
+                                   const float* q_over_m, unsigned char* alive, const float* ex, const float* ey,
+                                   const float* ez, const float* bx, const float* by, const float* bz) {
+  if (!c) return JEFI_EINVAL;
+  if (np < 0 || !ex || !ey || !ez || !bx || !by || !bz || (np > 0 && (!x || !y || !z || !ux || !uy || !uz || !q_over_m || !alive))) {
+    c->err = "jefi_push_particles: NULL array or negative np";
+    return JEFI_EINVAL;
+  }
+  if (np == 0) return JEFI_OK;
+  const jefi_dims& d = c->dims;
+  push_consts K;
+  K.nx = d.nx; K.ny = d.ny; K.nz = d.nz;
+  K.half_dt_over_c = (float)(c->cfg.dt / (2.0 * c->c));
+  K.half_dt = (float)(c->cfg.dt / 2.0);
+  K.sx = (float)(c->c * c->cfg.dt / c->cfg.dx); K.sy = (float)(c->c * c->cfg.dt / c->cfg.dy); K.sz = (float)(c->c * c->cfg.dt / c->cfg.dz);
+  for (int a = 0; a < 3; a++) { K.Eext[a] = (float)c->cfg.Eext[a]; K.Bext[a] = (float)c->cfg.Bext[a]; }
+  unsigned blocks = (unsigned)((np + 255) / 256);
+  k_push<<<blocks, 256, 0, c->stream>>>(K, np, x, y, z, ux, uy, uz, q_over_m, alive, ex, ey, ez, bx, by, bz);
+  JEFI_CUDA_TRY(c, cudaGetLastError());
+  c->launches++;
+  return JEFI_OK;
+}
+
+__global__ void __launch_bounds__(256) k_cell_index(long np, const float* __restrict__ x, const float* __restrict__ y,
+                                                    const float* __restrict__ z, int* __restrict__ ijk) {
+  long p = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= np) return;
+  int i, j, k;
+  float a;
+  cic_cell(x[p], i, a); cic_cell(y[p], j, a); cic_cell(z[p], k, a);
+  ijk[3 * p] = i; ijk[3 * p + 1] = j; ijk[3 * p + 2] = k;
+}
+
+extern "C" int jefi_debug_cell_index(jefi_ctx* c, long np, const float* x, const float* y, const float* z, int* ijk_out) {
+  if (!c || np < 0 || (np > 0 && (!x || !y || !z || !ijk_out))) return JEFI_EINVAL;
+  if (np == 0) return JEFI_OK;
+  k_cell_index<<<(unsigned)((np + 255) / 256), 256, 0, c->stream>>>(np, x, y, z, ijk_out);
+  JEFI_CUDA_TRY(c, cudaGetLastError());
+  JEFI_CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  return JEFI_OK;
+}

@@ -1,0 +1,303 @@
+"""Thin Python binding of the libjefi C-ABI (include/jefi.h): argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels of ``libjefi.so``; PyTorch supplies device memory and the
+stream.  There is no CPU fallback: if the library is missing or no CUDA device is present the calls raise.
+The functions carry the names of the C entry points; ``JefiContext`` is a small convenience wrapper around them.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+from typing import Optional, Sequence
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libjefi.so")
+
+JEFI_OK, JEFI_EINVAL, JEFI_ENOMEM, JEFI_ECUDA, JEFI_ESTATE = 0, -1, -2, -3, -4
+JEFI_FIELD_AUTO, JEFI_FIELD_REFERENCE, JEFI_FIELD_TILED = 0, 1, 2
+
+EXPORTS = [
+    "jefi_create", "jefi_destroy", "jefi_last_error", "jefi_get_info", "jefi_deposit", "jefi_push_sources",
+    "jefi_field_step", "jefi_push_particles", "jefi_field_step_host", "jefi_launch_count",
+    "jefi_last_field_kernel_ms", "jefi_debug_delay_table", "jefi_debug_cell_index", "jefi_debug_history_slot",
+]
+
+
+class JefiError(RuntimeError):
+    pass
+
+
+class jefi_config(C.Structure):
+    _fields_ = [
+        ("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int),
+        ("dx", C.c_double), ("dy", C.c_double), ("dz", C.c_double), ("dt", C.c_double),
+        ("c", C.c_double), ("eps0", C.c_double),
+        ("H", C.c_int), ("hist_cap", C.c_int),
+        ("Eext", C.c_double * 3), ("Bext", C.c_double * 3),
+        ("device", C.c_int), ("stream", C.c_void_p), ("field_impl", C.c_int),
+    ]
+
+
+_lib = None
+
+
+def load_library() -> C.CDLL:
+    """dlopen libjefi.so (built by paper_2209_07944_b200.build.build_lib); fails loudly if it is absent."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise JefiError(f"{LIB_PATH} not found: build it with `python -m paper_2209_07944_b200.build` "
+                        "(there is no CPU fallback)")
+    lib = C.CDLL(LIB_PATH)
+    vp, f32p, u8p = C.c_void_p, C.c_void_p, C.c_void_p
+    lib.jefi_create.argtypes = [C.POINTER(jefi_config), C.POINTER(vp)]
+    lib.jefi_create.restype = C.c_int
+    lib.jefi_destroy.argtypes = [vp]
+    lib.jefi_destroy.restype = None
+    lib.jefi_last_error.argtypes = [vp]
+    lib.jefi_last_error.restype = C.c_char_p
+    lib.jefi_get_info.argtypes = [vp, C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_long),
+                                  C.POINTER(C.c_long)]
+    lib.jefi_get_info.restype = C.c_int
+    lib.jefi_deposit.argtypes = [vp, C.c_long] + [f32p] * 7 + [u8p] + [f32p] * 4
+    lib.jefi_deposit.restype = C.c_int
+    lib.jefi_push_sources.argtypes = [vp] + [f32p] * 4
+    lib.jefi_push_sources.restype = C.c_int
+    lib.jefi_field_step.argtypes = [vp] + [f32p] * 6
+    lib.jefi_field_step.restype = C.c_int
+    lib.jefi_push_particles.argtypes = [vp, C.c_long] + [f32p] * 7 + [u8p] + [f32p] * 6
+    lib.jefi_push_particles.restype = C.c_int
+    lib.jefi_field_step_host.argtypes = [vp, f32p, f32p]
+    lib.jefi_field_step_host.restype = C.c_int
+    lib.jefi_launch_count.argtypes = [vp]
+    lib.jefi_launch_count.restype = C.c_long
+    lib.jefi_last_field_kernel_ms.argtypes = [vp]
+    lib.jefi_last_field_kernel_ms.restype = C.c_float
+    lib.jefi_debug_delay_table.argtypes = [vp, vp]
+    lib.jefi_debug_delay_table.restype = C.c_int
+    lib.jefi_debug_cell_index.argtypes = [vp, C.c_long, f32p, f32p, f32p, vp]
+    lib.jefi_debug_cell_index.restype = C.c_int
+    lib.jefi_debug_history_slot.argtypes = [vp, C.c_int, f32p]
+    lib.jefi_debug_history_slot.restype = C.c_int
+    _lib = lib
+    return lib
+
+
+def _check(handle, rc: int, what: str) -> None:
+    if rc != JEFI_OK:
+        msg = load_library().jefi_last_error(handle)
+        raise JefiError(f"{what} failed with code {rc}: {msg.decode() if msg else ''}")
+
+
+def _dev(t, dtype, n: Optional[int], name: str) -> int:
+    """Device pointer of a contiguous CUDA tensor of the given dtype (and length, if given)."""
+    import torch
+
+    if t is None:
+        return 0
+    if not isinstance(t, torch.Tensor) or not t.is_cuda:
+        raise JefiError(f"{name}: expected a CUDA tensor")
+    if t.dtype != dtype or not t.is_contiguous():
+        raise JefiError(f"{name}: expected contiguous {dtype}, got {t.dtype} contiguous={t.is_contiguous()}")
+    if n is not None and t.numel() != n:
+        raise JefiError(f"{name}: expected {n} elements, got {t.numel()}")
+    return t.data_ptr()
+
+
+# ------------------------------------------------------------------------------------------------ C entry points
+def jefi_create(nx: int, ny: int, nz: int, dx: float, dy: float, dz: float, dt: float, c: float = 0.0,
+                eps0: float = 0.0, H: int = 0, hist_cap: int = 0, Eext: Sequence[float] = (0, 0, 0),
+                Bext: Sequence[float] = (0, 0, 0), device: int = 0, stream: int = 0,
+                field_impl: int = JEFI_FIELD_AUTO) -> int:
+    lib = load_library()
+    cfg = jefi_config(nx, ny, nz, dx, dy, dz, dt, c, eps0, H, hist_cap, (C.c_double * 3)(*Eext),
+                      (C.c_double * 3)(*Bext), device, C.c_void_p(stream), field_impl)
+    h = C.c_void_p()
+    rc = lib.jefi_create(C.byref(cfg), C.byref(h))
+    if rc != JEFI_OK:
+        msg = lib.jefi_last_error(None)
+        raise JefiError(f"jefi_create failed with code {rc}: {msg.decode() if msg else ''}")
+    return h.value
+
+
+def jefi_destroy(handle: Optional[int]) -> None:
+    if handle:
+        load_library().jefi_destroy(handle)
+
+
+def jefi_get_info(handle: int) -> dict:
+    H, ndt, impl, step, rb = C.c_int(), C.c_int(), C.c_int(), C.c_long(), C.c_long()
+    _check(handle, load_library().jefi_get_info(handle, C.byref(H), C.byref(ndt), C.byref(impl), C.byref(step),
+                                                C.byref(rb)), "jefi_get_info")
+    return dict(H=H.value, ndt=ndt.value, field_impl=impl.value, step=step.value, ring_bytes=rb.value)
+
+
+def jefi_push_sources(handle: int, N: int, rho, jx, jy, jz) -> None:
+    import torch
+
+    f = torch.float32
+    _check(handle, load_library().jefi_push_sources(handle, _dev(rho, f, N, "rho"), _dev(jx, f, N, "jx"),
+                                                    _dev(jy, f, N, "jy"), _dev(jz, f, N, "jz")), "jefi_push_sources")
+
+
+def jefi_field_step(handle: int, N: int, ex, ey, ez, bx, by, bz) -> None:
+    import torch
+
+    f = torch.float32
+    ptrs = [_dev(t, f, N, n) for t, n in zip((ex, ey, ez, bx, by, bz), ("ex", "ey", "ez", "bx", "by", "bz"))]
+    _check(handle, load_library().jefi_field_step(handle, *ptrs), "jefi_field_step")
+
+
+def jefi_deposit(handle: int, N: int, x, y, z, ux, uy, uz, qw, alive, rho, jx, jy, jz) -> None:
+    import torch
+
+    f = torch.float32
+    np_ = x.numel()
+    pin = [_dev(t, f, np_, n) for t, n in zip((x, y, z, ux, uy, uz, qw), ("x", "y", "z", "ux", "uy", "uz", "qw"))]
+    pal = _dev(alive, torch.uint8, np_, "alive") if alive is not None else 0
+    pout = [_dev(t, f, N, n) for t, n in zip((rho, jx, jy, jz), ("rho", "jx", "jy", "jz"))]
+    _check(handle, load_library().jefi_deposit(handle, np_, *pin, pal, *pout), "jefi_deposit")
+
+
+def jefi_push_particles(handle: int, N: int, x, y, z, ux, uy, uz, q_over_m, alive, ex, ey, ez, bx, by, bz) -> None:
+    import torch
+
+    f = torch.float32
+    np_ = x.numel()
+    pp = [_dev(t, f, np_, n) for t, n in zip((x, y, z, ux, uy, uz, q_over_m), ("x", "y", "z", "ux", "uy", "uz", "q_over_m"))]
+    pal = _dev(alive, torch.uint8, np_, "alive")
+    pf = [_dev(t, f, N, n) for t, n in zip((ex, ey, ez, bx, by, bz), ("ex", "ey", "ez", "bx", "by", "bz"))]
+    _check(handle, load_library().jefi_push_particles(handle, np_, *pp, pal, *pf), "jefi_push_particles")
+
+
+def jefi_field_step_host(handle: int, N: int, src_host, eb_host) -> None:
+    """src_host: CPU float32 tensor [4*N] (pinned recommended); eb_host: CPU float32 tensor [6*N]."""
+    import torch
+
+    for t, n, name in ((src_host, 4 * N, "src_host"), (eb_host, 6 * N, "eb_host")):
+        if t.is_cuda or t.dtype != torch.float32 or not t.is_contiguous() or t.numel() != n:
+            raise JefiError(f"{name}: expected a contiguous CPU float32 tensor of {n} elements")
+    _check(handle, load_library().jefi_field_step_host(handle, src_host.data_ptr(), eb_host.data_ptr()),
+           "jefi_field_step_host")
+
+
+def jefi_launch_count(handle: int) -> int:
+    return int(load_library().jefi_launch_count(handle))
+
+
+def jefi_last_field_kernel_ms(handle: int) -> float:
+    return float(load_library().jefi_last_field_kernel_ms(handle))
+
+
+def jefi_debug_delay_table(handle: int, nx: int, ny: int, nz: int):
+    import numpy as np
+
+    out = np.empty((nz, ny, nx), dtype=np.int32)
+    _check(handle, load_library().jefi_debug_delay_table(handle, out.ctypes.data), "jefi_debug_delay_table")
+    return out
+
+
+def jefi_debug_cell_index(handle: int, x, y, z):
+    import torch
+
+    np_ = x.numel()
+    out = torch.empty((np_, 3), dtype=torch.int32, device=x.device)
+    f = torch.float32
+    _check(handle, load_library().jefi_debug_cell_index(handle, np_, _dev(x, f, np_, "x"), _dev(y, f, np_, "y"),
+                                                        _dev(z, f, np_, "z"), out.data_ptr()), "jefi_debug_cell_index")
+    return out
+
+
+def jefi_debug_history_slot(handle: int, N: int, steps_back: int, device):
+    import torch
+
+    out = torch.empty((4, N), dtype=torch.float32, device=device)
+    _check(handle, load_library().jefi_debug_history_slot(handle, steps_back, out.data_ptr()), "jefi_debug_history_slot")
+    return out
+
+
+# ------------------------------------------------------------------------------------------------ convenience
+@dataclass
+class GridSpec:
+    nx: int
+    ny: int
+    nz: int
+    dx: float
+    dy: float
+    dz: float
+    dt: float
+    c: float = 0.0
+    eps0: float = 0.0
+    H: int = 0
+    hist_cap: int = 0
+    Eext: Sequence[float] = (0.0, 0.0, 0.0)
+    Bext: Sequence[float] = (0.0, 0.0, 0.0)
+
+    @property
+    def N(self) -> int:
+        return self.nx * self.ny * self.nz
+
+
+class JefiContext:
+    """Owns one jefi_ctx and the E/B/rho/J device tensors of a run; every method is one C-ABI call."""
+
+    def __init__(self, grid: GridSpec, device=None, field_impl: int = JEFI_FIELD_AUTO):
+        import torch
+
+        if not torch.cuda.is_available():
+            raise JefiError("no CUDA device: libjefi has no CPU fallback")
+        self.device = torch.device(device if device is not None else "cuda:0")
+        self.grid = grid
+        self.N = grid.N
+        torch.cuda.set_device(self.device)
+        stream = torch.cuda.current_stream(self.device).cuda_stream
+        self.handle = jefi_create(grid.nx, grid.ny, grid.nz, grid.dx, grid.dy, grid.dz, grid.dt, grid.c, grid.eps0,
+                                  grid.H, grid.hist_cap, grid.Eext, grid.Bext, self.device.index or 0, stream,
+                                  field_impl)
+        self.info = jefi_get_info(self.handle)
+        self.H = self.info["H"]
+        z = lambda k: torch.zeros((k, self.N), dtype=torch.float32, device=self.device)
+        self.EB = z(6)   # ex ey ez bx by bz
+        self.src = z(4)  # rho jx jy jz
+
+    def close(self) -> None:
+        if getattr(self, "handle", None):
+            jefi_destroy(self.handle)
+            self.handle = None
+
+    __del__ = close
+
+    def push_sources(self, src=None) -> None:
+        s = self.src if src is None else src
+        jefi_push_sources(self.handle, self.N, s[0], s[1], s[2], s[3])
+
+    def field_step(self, out=None):
+        o = self.EB if out is None else out
+        jefi_field_step(self.handle, self.N, o[0], o[1], o[2], o[3], o[4], o[5])
+        return o
+
+    def deposit(self, part: dict, out=None):
+        o = self.src if out is None else out
+        jefi_deposit(self.handle, self.N, part["x"], part["y"], part["z"], part["ux"], part["uy"], part["uz"],
+                     part["qw"], part.get("alive"), o[0], o[1], o[2], o[3])
+        return o
+
+    def push_particles(self, part: dict, EB=None) -> None:
+        f = self.EB if EB is None else EB
+        jefi_push_particles(self.handle, self.N, part["x"], part["y"], part["z"], part["ux"], part["uy"], part["uz"],
+                            part["qm"], part["alive"], f[0], f[1], f[2], f[3], f[4], f[5])
+
+    def pic_step(self, part: dict) -> None:
+        """deposit -> push_sources -> field_step -> push_particles, all on one stream."""
+        self.deposit(part)
+        self.push_sources()
+        self.field_step()
+        self.push_particles(part)
+
+    def launch_count(self) -> int:
+        return jefi_launch_count(self.handle)
+
+    def last_field_kernel_ms(self) -> float:
+        return jefi_last_field_kernel_ms(self.handle)
