@@ -1,0 +1,332 @@
+#!/usr/bin/env python
+"""bench.py — Jefimenko field-solve throughput on B200 (BASELINE.json metric), one JSON line on stdout.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload 4] [--no-pic] [--impl reference]
+
+Product arm: the timed "step" is one pass of the field path over the 96^3 field-only workload (BASELINE.json
+configs[3], the one the metric "G source-obs pairs/s and % FP32 peak" is quoted on): jefi_push_sources of a fresh
+seeded source slice already resident in HBM + jefi_field_step.  The ring (9.5 GB) is far larger than L2, so no
+L2 flush is needed between iterations.  `e2e` repeats it through jefi_field_step_host with pinned HOST buffers.
+`pic` adds PIC steps/s (deposit -> push_sources -> field_step -> push_particles) on configs 1-3.
+Reference arm (--impl reference): the fp64 CPU oracle, as it stands, on a bounded sample of the same workload.
+N > 1: replicas only: every rank runs the same workload on its own GPU, no data-path collective.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2209_07944_b200 import workloads as wl  # noqa: E402
+
+# FP32 roofline of the field kernel ("bound": "alu"): 148 SMs x 128 FP32 lanes x 2 FLOP x max SM clock.
+N_SM, LANES = 148, 128
+FLOP_PER_PAIR = 48.0  # 24 FMA per source-observation pair
+
+
+def log(*a):
+    print(*a, file=sys.stderr, flush=True)
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons during the timed region (NVML, every 100 ms)."""
+
+    REASONS = {0x2: "applications_clocks_setting", 0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x10: "sync_boost",
+               0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown", 0x80: "hw_power_brake_slowdown",
+               0x100: "display_clock_setting"}
+
+    def __init__(self, index: int):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thr = None
+        try:
+            import pynvml
+
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception as e:  # noqa: BLE001
+            log("clock sampler unavailable:", e)
+            self.nv = None
+
+    def _run(self):
+        nv = self.nv
+        while not self._stop.is_set():
+            try:
+                self.samples.append(float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                mask = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                for bit, name in self.REASONS.items():
+                    if mask & bit:
+                        self.reasons.add(name)
+            except Exception:  # noqa: BLE001
+                pass
+            self._stop.wait(0.1)
+
+    def start(self):
+        if self.nv is not None:
+            self._thr = threading.Thread(target=self._run, daemon=True)
+            self._thr.start()
+
+    def stop(self) -> dict:
+        self._stop.set()
+        if self._thr is not None:
+            self._thr.join()
+        med = float(np.median(self.samples)) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+def visible_gpu_index(local_rank: int) -> int:
+    vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+    if vis:
+        try:
+            return int(vis.split(",")[local_rank])
+        except Exception:  # noqa: BLE001
+            return local_rank
+    return local_rank
+
+
+# --------------------------------------------------------------------------------------------------- reference arm
+def oracle_sample_rate(w: wl.Workload, ring_host: np.ndarray, n_obs: int, seed_tag: int):
+    """Oracle pairs/s on n_obs seeded observation cells against all sources (fp64, all host cores)."""
+    import oracle
+
+    cfg = oracle.OracleConfig(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt)
+    obs = np.random.default_rng([w.seed, seed_tag]).integers(0, w.N, size=n_obs, dtype=np.int64)
+    t0 = time.perf_counter()
+    oracle.field(cfg, w.H - 1, ring_host, obs)
+    dt = time.perf_counter() - t0
+    return n_obs * (w.N - 1) / dt, dt
+
+
+def host_ring(w: wl.Workload) -> np.ndarray:
+    ring = np.empty((w.H, 4, w.N), dtype=np.float32)
+    for t in range(w.H):
+        ring[t] = wl.history_slice(w.N, t, w.seed)
+    return ring
+
+
+def run_reference(args, w: wl.Workload) -> dict:
+    import oracle
+
+    cores = oracle.num_threads()
+    log(f"[reference] building the {w.H}-slot host history of {w.name} ...")
+    ring = host_ring(w)
+    n_obs = args.ref_obs
+    rates = []
+    for i in range(args.warmup + args.steps):
+        r, dt = oracle_sample_rate(w, ring, n_obs, i)
+        log(f"[reference] step {i}: {n_obs} obs cells x {w.N - 1} sources in {dt:.2f} s -> {r / 1e9:.4f} Gpairs/s")
+        if i >= args.warmup:
+            rates.append((r, dt))
+    tot_pairs = sum(r * dt for r, dt in rates)
+    tot_t = sum(dt for _, dt in rates)
+    val = tot_pairs / tot_t / 1e9
+    sample = f"{n_obs} seeded observation cells x all {w.N - 1} source cells per step (of {w.N} cells)"
+    return {"impl": "reference", "metric": "jefimenko_source_obs_pairs_per_s", "value": val, "unit": "Gpairs/s",
+            "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / len(rates),
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": w.name, "grid": [w.n] * 3, "H": w.H, "dx": w.dx, "dt": w.dt},
+            "cpu_baseline": {"value": val, "unit": "Gpairs/s", "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": "Gpairs/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+
+
+# --------------------------------------------------------------------------------------------------- product arm
+def time_pic(J, torch, device, config: int, steps: int, warmup: int) -> dict:
+    w = wl.WORKLOADS[config]
+    ctx = J.JefiContext(J.GridSpec(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt), device=device)
+    part = {k: torch.from_numpy(v).to(device) for k, v in wl.particles(config).items()}
+    for _ in range(warmup):
+        ctx.pic_step(part)
+    torch.cuda.synchronize(device)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l0 = ctx.launch_count()
+    e0.record()
+    for _ in range(steps):
+        ctx.pic_step(part)
+    e1.record()
+    torch.cuda.synchronize(device)
+    ms = e0.elapsed_time(e1) / steps
+    fk = ctx.last_field_kernel_ms()
+    out = {"workload": w.name, "steps": steps, "warmup": warmup, "ms_per_step": ms, "steps_per_s": 1e3 / ms,
+           "particles": int(part["x"].numel()), "field_kernel_ms": fk, "launches": ctx.launch_count() - l0,
+           "field_impl": ctx.info["field_impl"]}
+    ctx.close()
+    return out
+
+
+def run_product(args, w: wl.Workload) -> dict:
+    import torch
+
+    from paper_2209_07944_b200 import jefi as J
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    device = torch.device(f"cuda:{local}")
+    torch.cuda.set_device(device)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=device)
+    J.load_library()
+
+    ctx = J.JefiContext(J.GridSpec(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt), device=device)
+    N, H = w.N, ctx.H
+    assert H == w.H
+    keep_host = (rank == 0 and world == 1 and not args.no_cpu_baseline)
+    ring_host = np.empty((H, 4, N), dtype=np.float32) if keep_host else None
+    log(f"[rank {rank}] {w.name}: N={N} H={H} ring={ctx.info['ring_bytes'] / 1e9:.2f} GB field_impl={ctx.info['field_impl']}")
+    t0 = time.perf_counter()
+    for t in range(H):  # fill the history so that every delay is valid at the timed steps
+        s = wl.history_slice(N, t, w.seed)
+        if keep_host:
+            ring_host[t] = s
+        ctx.push_sources(torch.from_numpy(s).to(device, non_blocking=False))
+    torch.cuda.synchronize(device)
+    log(f"[rank {rank}] history filled in {time.perf_counter() - t0:.1f} s")
+
+    nfresh = args.warmup + args.steps
+    fresh = [torch.from_numpy(wl.history_slice(N, H + i, w.seed)).to(device) for i in range(min(nfresh, 8))]
+    pairs = float(N) * float(N - 1)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize(device)
+
+    # ---- device-resident timing ----
+    for i in range(args.warmup):
+        ctx.push_sources(fresh[i % len(fresh)])
+        ctx.field_step()
+    barrier()
+    sampler = ClockSampler(visible_gpu_index(local))
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l0 = ctx.launch_count()
+    barrier()
+    e0.record()
+    for i in range(args.steps):
+        ctx.push_sources(fresh[(args.warmup + i) % len(fresh)])
+        ctx.field_step()
+    e1.record()
+    barrier()
+    clocks = sampler.stop()
+    launches = ctx.launch_count() - l0
+    step_ms = e0.elapsed_time(e1) / args.steps
+    # per-launch duration of the dominant kernel: CUDA events recorded by the library on the launching stream
+    # around the kernel alone, over a second pass of the same launches (keeps the timed region free of syncs)
+    kms = []
+    for i in range(max(3, min(args.steps, 8))):
+        ctx.push_sources(fresh[i % len(fresh)])
+        ctx.field_step()
+        kms.append(ctx.last_field_kernel_ms())
+    kernel_ms = float(np.mean(kms))
+    t_ms = torch.tensor([step_ms], dtype=torch.float64, device=device)
+    if dist is not None:
+        dist.all_reduce(t_ms, op=dist.ReduceOp.MAX)
+    step_ms_max = float(t_ms.item())
+    value = world * pairs / (step_ms_max * 1e-3) / 1e9
+
+    # ---- end to end through the C-ABI with host buffers ----
+    src_pin = torch.empty(4 * N, dtype=torch.float32).pin_memory()
+    eb_pin = torch.empty(6 * N, dtype=torch.float32).pin_memory()
+    src_pin.copy_(torch.from_numpy(wl.history_slice(N, H + 100, w.seed).reshape(-1)))
+    J.jefi_field_step_host(ctx.handle, N, src_pin, eb_pin)  # warm-up (allocates the staging buffers)
+    barrier()
+    e2e_steps = max(1, min(args.steps, 3))
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        J.jefi_field_step_host(ctx.handle, N, src_pin, eb_pin)
+    torch.cuda.synchronize(device)
+    e2e_ms = (time.perf_counter() - t0) * 1e3 / e2e_steps
+    t_e = torch.tensor([e2e_ms], dtype=torch.float64, device=device)
+    if dist is not None:
+        dist.all_reduce(t_e, op=dist.ReduceOp.MAX)
+    e2e_val = world * pairs / (float(t_e.item()) * 1e-3) / 1e9
+    checksum = float(eb_pin[:N].double().abs().sum())
+
+    impl = ctx.info["field_impl"]
+    ctx.close()
+    torch.cuda.empty_cache()
+
+    out = None
+    if rank == 0:
+        sm_max = clocks.get("sm_max_mhz") or 1965.0
+        peak = N_SM * LANES * 2 * sm_max * 1e6 / 1e12
+        achieved = FLOP_PER_PAIR * pairs / (kernel_ms * 1e-3) / 1e12
+        out = {"metric": "jefimenko_source_obs_pairs_per_s", "value": value, "unit": "Gpairs/s", "n_gpus": world,
+               "steps": args.steps, "warmup": args.warmup, "ms_per_step": step_ms_max, "higher_is_better": True,
+               "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+               "config": {"workload": w.name, "grid": [w.n] * 3, "H": H, "dx": w.dx, "dt": w.dt,
+                          "pairs_per_step": pairs, "l2": "inputs (9.5 GB ring) larger than L2, no flush",
+                          "parallelism": "replicas" if world > 1 else "single", "field_impl": impl},
+               "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+                            "traffic": None, "kernel": "k_field_tiled" if impl == 2 else "k_field_reference",
+                            "kernel_ms": kernel_ms, "flop_per_pair": FLOP_PER_PAIR,
+                            "peak_source": "148 SM x 128 FP32 lanes x 2 FLOP x clocks.max.sm (derived, DESIGN.md §7)"},
+               "e2e": {"value": e2e_val, "unit": "Gpairs/s", "h2d_bytes_per_step": 16 * N, "d2h_bytes_per_step": 24 * N,
+                       "ms_per_step": float(t_e.item()), "checksum_abs_ex": checksum},
+               "gpu_launches": int(launches), "clocks": clocks}
+        if not args.no_pic and world == 1:
+            out["pic"] = []
+            for cfgno, st, wu in ((1, 64, 5), (2, 20, 3), (3, 10, 3)):
+                try:
+                    out["pic"].append(time_pic(J, torch, device, cfgno, st, wu))
+                except Exception as e:  # noqa: BLE001
+                    out["pic"].append({"workload": wl.WORKLOADS[cfgno].name, "error": str(e)})
+        if keep_host:
+            import oracle
+
+            r, dt = oracle_sample_rate(w, ring_host, args.cpu_obs, 0)
+            out["cpu_baseline"] = {"value": r / 1e9, "unit": "Gpairs/s", "cores": oracle.num_threads(), "kind": "oracle",
+                                   "sample": f"{args.cpu_obs} seeded observation cells x all {N - 1} source cells "
+                                             f"({dt:.1f} s of fp64 CPU work)"}
+        else:
+            out["cpu_baseline"] = None
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+    return out
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="jefi", choices=["jefi", "reference"])
+    ap.add_argument("--workload", type=int, default=4, help="BASELINE.json config number of the field workload (4 = 96^3)")
+    ap.add_argument("--no-pic", action="store_true", help="skip the PIC steps/s legs on configs 1-3")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-obs", type=int, default=4096, help="observation cells of the cpu_baseline sample")
+    ap.add_argument("--ref-obs", type=int, default=1024, help="observation cells per step of --impl reference")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "jefi" else max(args.warmup, 0)
+    w = wl.WORKLOADS[args.workload]
+    rank = int(os.environ.get("RANK", "0"))
+    if args.impl == "reference":
+        if rank != 0:
+            return  # rank 0 alone runs the CPU oracle
+        res = run_reference(args, w)
+    else:
+        res = run_product(args, w)
+    if res is not None:
+        print(json.dumps(res), flush=True)
+
+
+if __name__ == "__main__":
+    main()
