@@ -57,6 +57,7 @@ struct jefi_ctx {
   int* mtab_host;
   // tiled-kernel launch parameters
   int wmax;             // largest slot window over all (obs tile, source tile) pairs
+  int wpitch;           // compiled shared-memory pitch chosen for it
   size_t tiled_smem;
   // particles scratch
   float* src_stage;     // 4N floats, device staging of jefi_field_step_host

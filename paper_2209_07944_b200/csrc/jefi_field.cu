@@ -67,6 +67,18 @@ int jefi_launch_field_reference(jefi_ctx* c, float* ex, float* ey, float* ez, fl
 
 // ------------------------------------------------------------------------------------------------------------
 // tiled kernel
+//
+// CTA = 256 threads = one 8x8x8 observation tile, two cells per thread (z and z+4); 2 CTAs per SM.
+// For every 4x4x4 source tile the CTA stages, per source cell, the window of ring slots [m_lo, m_hi] that the tile
+// pair can address (m from the extreme offsets), S window and D window, with one TMA bulk copy per (cell, array)
+// (cp.async.bulk + mbarrier; the ring layout [tile][cell][slot] makes each window one contiguous run, two when the
+// ring wraps).  Shared-memory index j = m_hi - m, so that memory order equals slot order.
+// Pair evaluation: the source cell is warp-uniform, the delay per lane:
+//   q = |d'|^2 (1 FFMA), rs = rsqrt(q) (MUFU), t = q*rs + 1.5*2^23 (1 FFMA, integer m in the mantissa),
+//   address = K - 16*bits(t) (1 IMAD), 2 x LDS.128, then 20 FP32 ops:
+//   u = rs*S + D (4), r2 = rs^2 (1), a' = r2*d' (3), E += a'*u.x - rs*D.yzw (6), B += a' x u.yzw (6).
+// The lanes of a quarter-warp form a compact 2x2x2 box, so one LDS.128 phase touches few distinct slots of the same
+// cell row (16 B apart: conflict-free).
 // ------------------------------------------------------------------------------------------------------------
 constexpr int OB = 8;            // observation tile edge
 constexpr int TILED_THREADS = 256;
@@ -77,18 +89,36 @@ struct tiled_params {
   jefi_geom g;
   long n;          // current step
   int nslot;       // n mod H
-  int wpitch;      // float4 entries per cell row in shared memory (>= largest window)
   int nobx, noby, nobz;
   const float4* ringS;
   const float4* ringD;
   float *ex, *ey, *ez, *bx, *by, *bz;
 };
 
-__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src, bool valid) {
-  int sz = valid ? 16 : 0;  // src-size 0 -> the 16 destination bytes are zero-filled
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(sz) : "memory");
+// ---- mbarrier / TMA bulk-copy primitives (PTX ISA: mbarrier, cp.async.bulk) ----
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
 }
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra DONE_%=;\n"
+      "bra WAIT_%=;\n"
+      "DONE_%=:\n"
+      "}\n" ::"r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst), "l"(src),
+               "r"(bytes), "r"(bar)
+               : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
 // min / max of |a| over the integer interval [lo, hi]
 __device__ __forceinline__ void abs_range(int lo, int hi, int& mn, int& mx) {
@@ -97,62 +127,71 @@ __device__ __forceinline__ void abs_range(int lo, int hi, int& mn, int& mx) {
   mn = (lo <= 0 && hi >= 0) ? 0 : min(alo, ahi);
 }
 
-template <bool SELF>
-__device__ __forceinline__ void tile_pairs(const unsigned char* __restrict__ smS, uint32_t dOff, uint32_t pitchB, float kx,
-                                           float ky, float kz, const float (&fx0)[P_OBS], const float (&fy0)[P_OBS],
-                                           const float (&fz0)[P_OBS], uint32_t cconst, float (&acc)[P_OBS][6]) {
+template <int IMM>
+__device__ __forceinline__ float4 lds128_imm(uint32_t addr) {
+  float4 v;
+  asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4+%5];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr), "n"(IMM));
+  return v;
+}
+
+// One observation cell against one source cell.  K = shared address of the cell's S window + 16*(m_hi + MAGICBITS).
+template <int WP, bool SELF, int CELL>
+__device__ __forceinline__ void one_pair(uint32_t K, float ax, float ay, float az, float qyz, float (&loc)[6]) {
+  constexpr int SOFF = CELL * WP * 16;
+  constexpr int DOFF = SOFF + JEFI_TCELLS * WP * 16;
+  float q = fmaf(ax, ax, qyz);
+  float rs = jefi_rsqrt(q);
+  if (SELF) rs = q > 0.f ? rs : 0.f;        // the self cell contributes exactly zero
+  float t = fmaf(q, rs, JEFI_MAGIC);        // MAGIC + round(s): m sits in the mantissa
+  uint32_t addr = K - (uint32_t)__float_as_int(t) * 16u;   // window entry j = m_hi - m
+  const float4 S = lds128_imm<SOFF>(addr);
+  const float4 D = lds128_imm<DOFF>(addr);
+  float r2 = rs * rs;
+  float u0 = fmaf(rs, S.x, D.x), u1 = fmaf(rs, S.y, D.y), u2 = fmaf(rs, S.z, D.z), u3 = fmaf(rs, S.w, D.w);
+  float bxr = ax * r2, byr = ay * r2, bzr = az * r2;      // d' rs^2
+  loc[0] = fmaf(bxr, u0, loc[0]); loc[1] = fmaf(byr, u0, loc[1]); loc[2] = fmaf(bzr, u0, loc[2]);
+  loc[0] = fmaf(-rs, D.y, loc[0]); loc[1] = fmaf(-rs, D.z, loc[1]); loc[2] = fmaf(-rs, D.w, loc[2]);
+  loc[3] = fmaf(byr, u3, loc[3]); loc[3] = fmaf(-bzr, u2, loc[3]);
+  loc[4] = fmaf(bzr, u1, loc[4]); loc[4] = fmaf(-bxr, u3, loc[4]);
+  loc[5] = fmaf(bxr, u2, loc[5]); loc[5] = fmaf(-byr, u1, loc[5]);
+}
+
+template <int WP, bool SELF, int LY>
+__device__ __forceinline__ void one_row(uint32_t Kz, const float (&ax)[JEFI_TS], float ay, const float (&az)[P_OBS],
+                                        const float (&az2)[P_OBS], float (&loc)[P_OBS][6]) {
+  float qyz[P_OBS];
+#pragma unroll
+  for (int p = 0; p < P_OBS; p++) qyz[p] = fmaf(ay, ay, az2[p]);
+#pragma unroll
+  for (int p = 0; p < P_OBS; p++) {
+    one_pair<WP, SELF, JEFI_TS * LY + 0>(Kz, ax[0], ay, az[p], qyz[p], loc[p]);
+    one_pair<WP, SELF, JEFI_TS * LY + 1>(Kz, ax[1], ay, az[p], qyz[p], loc[p]);
+    one_pair<WP, SELF, JEFI_TS * LY + 2>(Kz, ax[2], ay, az[p], qyz[p], loc[p]);
+    one_pair<WP, SELF, JEFI_TS * LY + 3>(Kz, ax[3], ay, az[p], qyz[p], loc[p]);
+  }
+}
+
+template <int WP, bool SELF>
+__device__ __forceinline__ void tile_pairs(uint32_t K, float kz, const float (&ax)[JEFI_TS], const float (&ay)[JEFI_TS],
+                                           const float (&fz0)[P_OBS], float (&acc)[P_OBS][6]) {
   float loc[P_OBS][6];
 #pragma unroll
   for (int p = 0; p < P_OBS; p++)
 #pragma unroll
     for (int a = 0; a < 6; a++) loc[p][a] = 0.f;
-
 #pragma unroll 1
   for (int lz = 0; lz < JEFI_TS; lz++) {
-#pragma unroll 2
-    for (int ly = 0; ly < JEFI_TS; ly++) {
-      float ay[P_OBS], az[P_OBS], qyz[P_OBS];
+    float az[P_OBS], az2[P_OBS];
 #pragma unroll
-      for (int p = 0; p < P_OBS; p++) {
-        ay[p] = ky * (fy0[p] - (float)ly);
-        az[p] = kz * (fz0[p] - (float)lz);
-        qyz[p] = fmaf(ay[p], ay[p], az[p] * az[p]);
-      }
-      const unsigned char* row = smS + (uint32_t)(JEFI_TS * (ly + JEFI_TS * lz)) * pitchB;
-#pragma unroll
-      for (int lx = 0; lx < JEFI_TS; lx++) {
-        const unsigned char* cellp = row + (uint32_t)lx * pitchB;
-#pragma unroll
-        for (int p = 0; p < P_OBS; p++) {
-          float ax = kx * (fx0[p] - (float)lx);
-          float q = fmaf(ax, ax, qyz[p]);
-          float rs = jefi_rsqrt(q);
-          if (SELF) rs = q > 0.f ? rs : 0.f;  // the self cell contributes exactly zero
-          float t = fmaf(q, rs, JEFI_MAGIC);   // MAGIC + round(s)
-          uint32_t off = (uint32_t)__float_as_int(t) * 16u + cconst;  // byte offset of slot m - m_lo in the cell's window
-          if (SELF) off = q > 0.f ? off : 0u;
-          const float4 S = *reinterpret_cast<const float4*>(cellp + off);
-          const float4 D = *reinterpret_cast<const float4*>(cellp + off + dOff);
-          float rs2 = rs * rs, rs3 = rs2 * rs;
-          float qq = fmaf(rs2, D.x, rs3 * S.x);
-          loc[p][0] = fmaf(ax, qq, loc[p][0]);
-          loc[p][1] = fmaf(ay[p], qq, loc[p][1]);
-          loc[p][2] = fmaf(az[p], qq, loc[p][2]);
-          loc[p][0] = fmaf(-rs, D.y, loc[p][0]);
-          loc[p][1] = fmaf(-rs, D.z, loc[p][1]);
-          loc[p][2] = fmaf(-rs, D.w, loc[p][2]);
-          float wx = fmaf(rs2, D.y, rs3 * S.y);
-          float wy = fmaf(rs2, D.z, rs3 * S.z);
-          float wz = fmaf(rs2, D.w, rs3 * S.w);
-          loc[p][3] = fmaf(ay[p], wz, loc[p][3]);
-          loc[p][3] = fmaf(-az[p], wy, loc[p][3]);
-          loc[p][4] = fmaf(az[p], wx, loc[p][4]);
-          loc[p][4] = fmaf(-ax, wz, loc[p][4]);
-          loc[p][5] = fmaf(ax, wy, loc[p][5]);
-          loc[p][5] = fmaf(-ay[p], wx, loc[p][5]);
-        }
-      }
+    for (int p = 0; p < P_OBS; p++) {
+      az[p] = kz * (fz0[p] - (float)lz);
+      az2[p] = az[p] * az[p];
     }
+    const uint32_t Kz = K + (uint32_t)(lz * JEFI_TS * JEFI_TS * WP * 16);
+    one_row<WP, SELF, 0>(Kz, ax, ay[0], az, az2, loc);
+    one_row<WP, SELF, 1>(Kz, ax, ay[1], az, az2, loc);
+    one_row<WP, SELF, 2>(Kz, ax, ay[2], az, az2, loc);
+    one_row<WP, SELF, 3>(Kz, ax, ay[3], az, az2, loc);
   }
 #pragma unroll
   for (int p = 0; p < P_OBS; p++)
@@ -160,16 +199,17 @@ __device__ __forceinline__ void tile_pairs(const unsigned char* __restrict__ smS
     for (int a = 0; a < 6; a++) acc[p][a] += loc[p][a];  // second accumulation level: one add per tile
 }
 
+template <int WP>
 __global__ void __launch_bounds__(TILED_THREADS, 2) k_field_tiled(tiled_params P) {
-  extern __shared__ __align__(16) unsigned char smem[];
+  extern __shared__ __align__(128) unsigned char smem[];
+  __shared__ __align__(8) unsigned long long mbar_storage;
   const jefi_dims& d = P.d;
   const int tid = threadIdx.x;
   const int lane = tid & 31, warp = tid >> 5;
   // observation tile of this CTA
   const int obx = blockIdx.x % P.nobx, oby = (blockIdx.x / P.nobx) % P.noby, obz = blockIdx.x / (P.nobx * P.noby);
   const int ox0 = obx * OB, oy0 = oby * OB, oz0 = obz * OB;
-  // lane -> cell of a 4x4x2 warp box; every quarter-warp (8 lanes) is a compact 2x2x2 sub-box so that one
-  // LDS.128 phase touches few distinct slots of the same source cell
+  // lane -> cell of a 4x4x2 warp box; every quarter-warp (8 lanes) is a compact 2x2x2 sub-box
   const int lxo = (lane & 1) + 2 * ((lane >> 3) & 1);
   const int lyo = ((lane >> 1) & 1) + 2 * ((lane >> 4) & 1);
   const int lzo = (lane >> 2) & 1;
@@ -183,10 +223,20 @@ __global__ void __launch_bounds__(TILED_THREADS, 2) k_field_tiled(tiled_params P
 #pragma unroll
     for (int a = 0; a < 6; a++) acc[p][a] = 0.f;
 
-  const uint32_t pitchB = (uint32_t)P.wpitch * 16u;
-  const uint32_t dOff = (uint32_t)JEFI_TCELLS * pitchB;  // D window follows the S window
-  const uint32_t smS_addr = (uint32_t)__cvta_generic_to_shared(smem);
+  constexpr uint32_t PITCHB = WP * 16;
+  constexpr uint32_t DOFFB = JEFI_TCELLS * PITCHB;  // D window follows the S window
+  const uint32_t smS = (uint32_t)__cvta_generic_to_shared(smem);
+  const uint32_t bar = (uint32_t)__cvta_generic_to_shared(&mbar_storage);
+  if (tid == 0) {
+    mbar_init(bar, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  uint32_t phase = 0;
   const int ntiles = d.ntx * d.nty * d.ntz;
+  // thread -> (cell, array) of the bulk copies it issues
+  const int cp_cell = tid & (JEFI_TCELLS - 1);
+  const int cp_arr = tid >> 6;  // 0: S, 1: D, >= 2: no copy
 
   for (int st = 0; st < ntiles; st++) {
     const int stx = st % d.ntx, sty = (st / d.ntx) % d.nty, stz = st / (d.ntx * d.nty);
@@ -199,43 +249,53 @@ __global__ void __launch_bounds__(TILED_THREADS, 2) k_field_tiled(tiled_params P
     const bool self = (mnx == 0 && mny == 0 && mnz == 0);
     const int m_lo = self ? 0 : jefi_delay_fp32(jefi_q_fp32(P.g.kx, P.g.ky, P.g.kz, (float)mnx, (float)mny, (float)mnz));
     const int m_hi = jefi_delay_fp32(jefi_q_fp32(P.g.kx, P.g.ky, P.g.kz, (float)mxx, (float)mxy, (float)mxz));
-    const int W = m_hi - m_lo + 1;
+    const int W = m_hi - m_lo + 1;  // <= WP (jefi_tiled_prepare)
+    // window entry j <-> delay m = m_hi - j <-> absolute step t = t0 + j.  Entries with t < 0 (before t0,
+    // PAPER.md:217) or m > H-2 (not stored, reading A15) are zero: j < jv.
+    const long t0 = P.n - m_hi;
+    long jvl = -t0;
+    if (jvl < m_hi - (d.H - 2)) jvl = m_hi - (d.H - 2);
+    const int jv = jvl < 0 ? 0 : (jvl > W ? W : (int)jvl);
+    const int nvalid = W - jv;  // < H
+    int s0 = (int)((t0 + jv) % d.H);
+    if (s0 < 0) s0 += d.H;
+    const int lenA = min(nvalid, d.H - s0), lenB = nvalid - lenA;  // ring wrap: at most two runs
 
-    __syncthreads();  // everyone is done reading the previous tile
-    {
-      const size_t tile_base = (size_t)st * JEFI_TCELLS * d.H;
-      const unsigned rcp = 0xFFFFFFFFu / (unsigned)W + 1u;  // ceil(2^32 / W): exact quotient for idx < 2^16
-      const int total = JEFI_TCELLS * W;
-      for (int idx = tid; idx < total; idx += TILED_THREADS) {
-        int cell = W == 1 ? idx : (int)__umulhi((unsigned)idx, rcp);
-        int w = idx - cell * W;
-        int m = m_lo + w;
-        long t = P.n - m;
-        bool valid = (t >= 0) && (m <= d.H - 2);
-        int slot = P.nslot - m;
-        slot += slot < 0 ? d.H : 0;
-        slot = valid ? slot : 0;
-        size_t g = tile_base + (size_t)cell * d.H + slot;
-        uint32_t dst = smS_addr + (uint32_t)cell * pitchB + (uint32_t)w * 16u;
-        cp_async16(dst, P.ringS + g, valid);
-        cp_async16(dst + dOff, P.ringD + g, valid);
+    fence_proxy_async();  // order this thread's generic-proxy accesses of the window before the async-proxy writes
+    __syncthreads();      // everyone is done reading the previous tile
+    if (jv > 0) {         // zero part of the window (only in the first steps of a run or with a shallow ring)
+      for (int idx = tid; idx < 2 * JEFI_TCELLS * jv; idx += TILED_THREADS) {
+        int row = idx / jv, j = idx - row * jv;
+        *reinterpret_cast<float4*>(smem + (size_t)row * PITCHB + (size_t)j * 16) = make_float4(0.f, 0.f, 0.f, 0.f);
       }
-      cp_async_wait_all();
     }
-    __syncthreads();
-
-    float fx0[P_OBS], fy0[P_OBS], fz0[P_OBS];
+    if (tid == 0) mbar_expect_tx(bar, (uint32_t)(2 * JEFI_TCELLS * nvalid * 16));
+    if (cp_arr < 2 && nvalid > 0) {
+      const float4* ring = cp_arr == 0 ? P.ringS : P.ringD;
+      const float4* src = ring + ((size_t)st * JEFI_TCELLS + cp_cell) * d.H;
+      const uint32_t dst = smS + (uint32_t)cp_arr * DOFFB + (uint32_t)cp_cell * PITCHB + (uint32_t)jv * 16u;
+      bulk_g2s(dst, src + s0, (uint32_t)lenA * 16u, bar);
+      if (lenB > 0) bulk_g2s(dst + (uint32_t)lenA * 16u, src, (uint32_t)lenB * 16u, bar);
+    }
+    // per-tile geometry while the copies fly: d'_x for the 4 source columns, d'_y for the 4 source rows
+    float ax[JEFI_TS], ay[JEFI_TS], fz0[P_OBS];
 #pragma unroll
-    for (int p = 0; p < P_OBS; p++) {
-      fx0[p] = (float)(oi - sx0);
-      fy0[p] = (float)(oj - sy0);
-      fz0[p] = (float)(ok0 + 4 * p - sz0);
+    for (int l = 0; l < JEFI_TS; l++) {
+      ax[l] = P.g.kx * (float)(oi - sx0 - l);
+      ay[l] = P.g.ky * (float)(oj - sy0 - l);
     }
-    const uint32_t cconst = 0u - (0x4B400000u + (uint32_t)m_lo) * 16u;  // wraps mod 2^32 together with bits*16
+#pragma unroll
+    for (int p = 0; p < P_OBS; p++) fz0[p] = (float)(ok0 + 4 * p - sz0);
+    const uint32_t K = smS + ((uint32_t)m_hi + 0x4B400000u) * 16u;  // wraps mod 2^32 together with bits*16
+
+    mbar_wait(bar, phase);
+    phase ^= 1u;
+    if (jv > 0) __syncthreads();  // the zero fill is generic-proxy: make it visible to all warps
+
     if (self)
-      tile_pairs<true>(smem, dOff, pitchB, P.g.kx, P.g.ky, P.g.kz, fx0, fy0, fz0, cconst, acc);
+      tile_pairs<WP, true>(K, P.g.kz, ax, ay, fz0, acc);
     else
-      tile_pairs<false>(smem, dOff, pitchB, P.g.kx, P.g.ky, P.g.kz, fx0, fy0, fz0, cconst, acc);
+      tile_pairs<WP, false>(K, P.g.kz, ax, ay, fz0, acc);
   }
 
 #pragma unroll
@@ -247,6 +307,18 @@ __global__ void __launch_bounds__(TILED_THREADS, 2) k_field_tiled(tiled_params P
       P.bx[o] = P.g.prefB * acc[p][3]; P.by[o] = P.g.prefB * acc[p][4]; P.bz[o] = P.g.prefB * acc[p][5];
     }
   }
+}
+
+// window pitches the kernel is compiled for (float4 entries per source-cell row)
+static const int kPitches[] = {36, 64, 104};
+typedef void (*tiled_fn)(tiled_params);
+static tiled_fn tiled_kernel_for(int wp) {
+  switch (wp) {
+    case 36: return k_field_tiled<36>;
+    case 64: return k_field_tiled<64>;
+    case 104: return k_field_tiled<104>;
+  }
+  return nullptr;
 }
 
 // Largest slot window over all relative placements of an 8^3 observation tile and a 4^3 source tile (host, fp64).
@@ -274,16 +346,26 @@ int jefi_tiled_prepare(jefi_ctx* c) {
         if (w > wmax) wmax = w;
       }
   c->wmax = wmax;
-  c->tiled_smem = (size_t)2 * JEFI_TCELLS * wmax * sizeof(float4);
+  int wp = 0;
+  for (int cand : kPitches)
+    if (cand >= wmax) { wp = cand; break; }
+  if (wp == 0) {
+    char buf[160];
+    snprintf(buf, sizeof buf, "tiled kernel: slot window of %d exceeds the largest compiled pitch %d", wmax, kPitches[2]);
+    c->err = buf;
+    return JEFI_ESTATE;
+  }
+  c->wpitch = wp;
+  c->tiled_smem = (size_t)2 * JEFI_TCELLS * wp * sizeof(float4);
   int dev = c->cfg.device, max_optin = 0;
   cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
-  if (c->tiled_smem > (size_t)max_optin) {
+  if (c->tiled_smem + 64 > (size_t)max_optin) {
     char buf[160];
     snprintf(buf, sizeof buf, "tiled kernel needs %zu B of shared memory (window %d slots), device allows %d", c->tiled_smem, wmax, max_optin);
     c->err = buf;
     return JEFI_ESTATE;
   }
-  cudaError_t e = cudaFuncSetAttribute(k_field_tiled, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->tiled_smem);
+  cudaError_t e = cudaFuncSetAttribute(tiled_kernel_for(wp), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->tiled_smem);
   if (e != cudaSuccess) { c->err = std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e); return JEFI_ECUDA; }
   return JEFI_OK;
 }
@@ -291,12 +373,12 @@ int jefi_tiled_prepare(jefi_ctx* c) {
 int jefi_launch_field_tiled(jefi_ctx* c, float* ex, float* ey, float* ez, float* bx, float* by, float* bz) {
   const jefi_dims& d = c->dims;
   tiled_params P;
-  P.d = d; P.g = c->geom; P.n = c->step; P.nslot = (int)(c->step % d.H); P.wpitch = c->wmax;
+  P.d = d; P.g = c->geom; P.n = c->step; P.nslot = (int)(c->step % d.H);
   P.nobx = (d.nx + OB - 1) / OB; P.noby = (d.ny + OB - 1) / OB; P.nobz = (d.nz + OB - 1) / OB;
   P.ringS = c->ringS; P.ringD = c->ringD;
   P.ex = ex; P.ey = ey; P.ez = ez; P.bx = bx; P.by = by; P.bz = bz;
   unsigned blocks = (unsigned)(P.nobx * P.noby * P.nobz);
-  k_field_tiled<<<blocks, TILED_THREADS, c->tiled_smem, c->stream>>>(P);
+  tiled_kernel_for(c->wpitch)<<<blocks, TILED_THREADS, c->tiled_smem, c->stream>>>(P);
   JEFI_CUDA_TRY(c, cudaGetLastError());
   c->launches++;
   return JEFI_OK;
