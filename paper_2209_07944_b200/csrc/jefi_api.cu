@@ -48,6 +48,7 @@ extern "C" int jefi_create(const jefi_config* cfg, jefi_ctx** out) {
   c->mtab_dev = nullptr;
   c->mtab_host = nullptr;
   c->src_stage = c->eb_stage = nullptr;
+  c->perm = nullptr;
   c->ev0 = c->ev1 = nullptr;
   c->ev_valid = false;
   c->launches = 0;
@@ -145,6 +146,7 @@ extern "C" void jefi_destroy(jefi_ctx* c) {
   if (c->ringS) cudaFree(c->ringS);
   if (c->ringD) cudaFree(c->ringD);
   if (c->mtab_dev) cudaFree(c->mtab_dev);
+  if (c->perm) cudaFree(c->perm);
   if (c->src_stage) cudaFree(c->src_stage);
   if (c->eb_stage) cudaFree(c->eb_stage);
   if (c->mtab_host) free(c->mtab_host);

@@ -59,6 +59,8 @@ struct jefi_ctx {
   int wmax;             // largest slot window over all (obs tile, source tile) pairs
   int wpitch;           // compiled shared-memory pitch chosen for it
   size_t tiled_smem;
+  unsigned short* perm; // evaluation order of the 512 cells of an observation tile per relative tile offset
+  int ndx, ndy, ndz;
   // particles scratch
   float* src_stage;     // 4N floats, device staging of jefi_field_step_host
   float* eb_stage;      // 6N floats
