@@ -1,0 +1,163 @@
+"""Parity at BASELINE.json's full sizes, in the launch configuration bench.py times.
+
+Configs 1-2: full closed-loop oracle.  Configs 3-5 (6.9e10 .. 4.4e12 pairs per step): the fp64 oracle evaluates E, B
+at seeded sample cells + corners, face centres and the centre, against ALL sources, from the GPU's own history read
+back through jefi_debug_history_slot (per-kernel parity on injected state); deposit and push are
+checked the same way on the GPU's particle state.  Tolerances as in test_gpu_parity.py.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+from oracle import OracleConfig
+from paper_2209_07944_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+
+def sampled_field_err(F, Fo):
+    d = F.astype(np.float64) - Fo
+    nrm = np.linalg.norm(Fo)
+    return np.linalg.norm(d) / nrm, np.abs(d).max() / (nrm / math.sqrt(Fo.size))
+
+
+@pytest.fixture(scope="module")
+def J(cuda_device):
+    from paper_2209_07944_b200 import jefi
+
+    jefi.load_library()
+    return jefi
+
+
+def to_dev(part, device):
+    import torch
+
+    return {k: torch.from_numpy(np.ascontiguousarray(v)).to(device) for k, v in part.items()}
+
+
+def read_ring(J, ctx, w):
+    """The GPU's stored history as the oracle's ring [H][4][N] fp32 (slot = step mod H)."""
+    ring = np.zeros((ctx.H, 4, w.N), dtype=np.float32)
+    step = J.jefi_get_info(ctx.handle)["step"]
+    for back in range(min(ctx.H, step + 1)):
+        ring[(step - back) % ctx.H] = J.jefi_debug_history_slot(ctx.handle, w.N, back, ctx.device).cpu().numpy()
+    return ring, step
+
+
+def check_sampled_fields(J, ctx, w, nsample, tag):
+    cfg = OracleConfig(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt)
+    ring, step = read_ring(J, ctx, w)
+    obs = wl.sample_obs(w.n, nsample, w.seed)
+    Eo, Bo = oracle.field(cfg, step, ring, obs)
+    eb = ctx.EB.cpu().numpy()
+    E, B = eb[:3][:, obs], eb[3:][:, obs]
+    for name, F, Fo in (("E", E, Eo), ("B", B, Bo)):
+        if np.linalg.norm(Fo) == 0.0:  # e.g. step 0: every pair has m >= 2 > n, nothing has arrived yet
+            assert np.all(F == 0.0), f"{tag} {name}: oracle is exactly zero"
+            continue
+        l2, mx = sampled_field_err(F, Fo)
+        assert l2 <= 1e-4, f"{tag} {name}: rel-L2 {l2:.3e}"
+        assert mx <= 1e-3, f"{tag} {name}: max-abs/rms {mx:.3e}"
+
+
+def check_particle_kernels(J, ctx, w, dp, tag):
+    """Deposit and one push of the GPU's current particle state against the oracle (injected state)."""
+    import torch
+
+    cfg = OracleConfig(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt)
+    host = {k: v.cpu().numpy() for k, v in dp.items()}
+    idx = J.jefi_debug_cell_index(ctx.handle, dp["x"], dp["y"], dp["z"]).cpu().numpy()
+    assert np.array_equal(idx, oracle.cell_index(host["x"], host["y"], host["z"])), tag + " cell indices"
+    out = torch.empty((4, w.N), dtype=torch.float32, device=ctx.device)
+    S = ctx.deposit(dp, out).cpu().numpy()
+    So = oracle.deposit(cfg, host["x"], host["y"], host["z"], host["ux"], host["uy"], host["uz"], host["qw"], host["alive"])
+    for a in range(4):
+        assert np.linalg.norm(S[a] - So[a]) <= 1e-5 * max(np.linalg.norm(So[a]), 1e-300), f"{tag} deposit comp {a}"
+    # one push from the same state with the GPU's own fields
+    EB = ctx.EB.cpu().numpy().astype(np.float64)
+    trial = {k: v.clone() for k, v in dp.items()}
+    ctx.push_particles(trial)
+    po = {k: host[k].astype(np.float64) for k in ("x", "y", "z", "ux", "uy", "uz", "qm")}
+    alive_o = host["alive"].copy()
+    oracle.push(cfg, po["x"], po["y"], po["z"], po["ux"], po["uy"], po["uz"], po["qm"], alive_o, EB[:3], EB[3:])
+    got = {k: v.cpu().numpy() for k, v in trial.items()}
+    assert (got["alive"] != alive_o).sum() <= 3, tag + " alive set"
+    was = host["alive"] == 1
+    for k in "xyz":
+        assert np.abs(got[k][was] - po[k][was]).max() / w.n <= 1e-6, f"{tag} push {k}"
+    both = (got["alive"] == 1) & (alive_o == 1)
+    for k in ("ux", "uy", "uz"):
+        assert np.abs(got[k][both] - po[k][both]).max() <= 2e-6 * max(1.0, np.abs(po[k]).max()), f"{tag} push {k}"
+
+
+def test_config2_closed_loop_10_steps_full_oracle(J):
+    """32^3, 2e5 macro-particles: full fp64 closed loop for 10 steps (trajectory bar 1e-5), fields at step 9."""
+    w = wl.WORKLOADS[2]
+    part = wl.particles(2)
+    cfg = OracleConfig(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt)
+    ctx = J.JefiContext(J.GridSpec(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt))
+    assert ctx.H == w.H and ctx.info["field_impl"] == J.JEFI_FIELD_TILED
+    dp = to_dev(part, ctx.device)
+    orc = oracle.OracleJefi(cfg)
+    po = {k: v.astype(np.float64) for k, v in part.items() if k != "alive"}
+    po["alive"] = part["alive"].copy()
+    for s in range(10):
+        ctx.pic_step(dp)
+        So, Eo, Bo = orc.pic_step(po)
+    got = {k: v.cpu().numpy() for k, v in dp.items()}
+    both = (got["alive"] == 1) & (po["alive"] == 1)
+    assert (got["alive"] != po["alive"]).sum() <= 2
+    for k in "xyz":
+        assert np.abs(got[k][both] - po[k][both]).max() / w.n <= 1e-5
+    eb = ctx.EB.cpu().numpy()
+    for name, F, Fo in (("E", eb[:3], Eo), ("B", eb[3:], Bo)):
+        l2, mx = sampled_field_err(F, Fo)
+        assert l2 <= 1e-4 and mx <= 1e-3, (name, l2, mx)
+    ctx.close()
+
+
+@pytest.mark.parametrize("config,steps,nsample", [(3, 10, 2048), (5, 10, 1024)])
+def test_pic_configs_sampled_parity(J, config, steps, nsample):
+    """64^3 / 128^3 PIC configs: run `steps` steps on the GPU, then per-kernel parity on its own state."""
+    w = wl.WORKLOADS[config]
+    part = wl.particles(config)
+    ctx = J.JefiContext(J.GridSpec(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt))
+    assert ctx.H == w.H and ctx.info["field_impl"] == J.JEFI_FIELD_TILED
+    dp = to_dev(part, ctx.device)
+    for s in range(steps):
+        if s == steps - 1:  # state that enters the last step: deposit/push parity on it after the step's fields exist
+            before = {k: v.clone() for k, v in dp.items()}
+        ctx.pic_step(dp)
+        if s in (0, 3):
+            check_sampled_fields(J, ctx, w, nsample // 4, f"cfg{config} step {s}")
+    check_sampled_fields(J, ctx, w, nsample, f"cfg{config} step {steps - 1}")
+    check_particle_kernels(J, ctx, w, before, f"cfg{config}")
+    alive = int(dp["alive"].sum())
+    assert alive > 0.9 * part["x"].shape[0]
+    ctx.close()
+
+
+def test_config4_field_only_sampled_parity(J):
+    """96^3 x 96^3, H = 335, every slot random (J scaled by c so the J-dot term of Eq. 2.4 is visible): one
+    jefi_field_step in bench.py's launch configuration, 8192 sampled cells + 15 special cells against all sources."""
+    import torch
+
+    w = wl.WORKLOADS[4]
+    ctx = J.JefiContext(J.GridSpec(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt))
+    assert ctx.H == w.H == 335 and ctx.info["field_impl"] == J.JEFI_FIELD_TILED
+    ring = np.empty((w.H, 4, w.N), dtype=np.float32)
+    for t in range(w.H):
+        ring[t] = wl.history_slice(w.N, t, w.seed, j_scale=wl.C_SI)
+        ctx.push_sources(torch.from_numpy(ring[t]).to(ctx.device))
+    ctx.field_step()
+    cfg = OracleConfig(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt)
+    obs = wl.sample_obs(w.n, 8192, w.seed)
+    Eo, Bo = oracle.field(cfg, w.H - 1, ring, obs)
+    eb = ctx.EB.cpu().numpy()
+    for name, F, Fo in (("E", eb[:3][:, obs], Eo), ("B", eb[3:][:, obs], Bo)):
+        l2, mx = sampled_field_err(F, Fo)
+        assert l2 <= 1e-4, f"cfg4 {name}: rel-L2 {l2:.3e}"
+        assert mx <= 1e-3, f"cfg4 {name}: max-abs/rms {mx:.3e}"
+    ctx.close()
