@@ -44,7 +44,7 @@ extern "C" int jefi_create(const jefi_config* cfg, jefi_ctx** out) {
   jefi_ctx* c = new (std::nothrow) jefi_ctx();
   if (!c) return fail_create(nullptr, JEFI_ENOMEM, "jefi_create: host allocation failed");
   c->cfg = *cfg;
-  c->ringS = c->ringD = nullptr;
+  c->ring = nullptr;
   c->mtab_dev = nullptr;
   c->mtab_host = nullptr;
   c->src_stage = c->eb_stage = nullptr;
@@ -89,13 +89,11 @@ extern "C" int jefi_create(const jefi_config* cfg, jefi_ctx** out) {
   c->geom.prefB = (float)(-c->mu0 * dV / (4.0 * PI) * c->c / (L0 * L0));
 
   // ---- ring: zero-initialised = "J and rho are simply set to zero" before t0 ----
-  size_t ring_elems = (size_t)d.ncell_pad * H;
-  c->ring_bytes = (long)(2 * ring_elems * sizeof(float4));
-  if ((e = cudaMalloc(&c->ringS, ring_elems * sizeof(float4))) != cudaSuccess ||
-      (e = cudaMalloc(&c->ringD, ring_elems * sizeof(float4))) != cudaSuccess)
+  size_t ring_quads = (size_t)d.ntx * d.nty * d.ntz * H * JEFI_ROW_QUADS;
+  c->ring_bytes = (long)(ring_quads * sizeof(float4));
+  if ((e = cudaMalloc(&c->ring, ring_quads * sizeof(float4))) != cudaSuccess)
     return fail_create(c, JEFI_ENOMEM, std::string("ring allocation (") + std::to_string(c->ring_bytes) + " B): " + cudaGetErrorString(e));
-  cudaMemsetAsync(c->ringS, 0, ring_elems * sizeof(float4), c->stream);
-  cudaMemsetAsync(c->ringD, 0, ring_elems * sizeof(float4), c->stream);
+  cudaMemsetAsync(c->ring, 0, ring_quads * sizeof(float4), c->stream);
 
   // ---- delay table, fp64 on the host: m = floor(R/(c dt) + 1/2) (Eq. 2.6, reading A1) ----
   const int ex = jefi_table_extent(d.nx), ey = jefi_table_extent(d.ny), ez = jefi_table_extent(d.nz);
@@ -143,8 +141,7 @@ extern "C" int jefi_create(const jefi_config* cfg, jefi_ctx** out) {
 extern "C" void jefi_destroy(jefi_ctx* c) {
   if (!c) return;
   cudaStreamSynchronize(c->stream);
-  if (c->ringS) cudaFree(c->ringS);
-  if (c->ringD) cudaFree(c->ringD);
+  if (c->ring) cudaFree(c->ring);
   if (c->mtab_dev) cudaFree(c->mtab_dev);
   if (c->perm) cudaFree(c->perm);
   if (c->src_stage) cudaFree(c->src_stage);
@@ -156,21 +153,27 @@ extern "C" void jefi_destroy(jefi_ctx* c) {
 }
 
 // ------------------------------------------------------------------------------------------------------------
-// Row a1: history push.  One thread per real cell: reads the previous slot, writes value and backward difference.
+// Row a1: history push.  One thread per padded ring cell, in ring order (tile, cell): the 16-byte writes of a tile
+// row are contiguous.  Reads the previous slot, writes value and backward difference.
 // Traffic: 16 B in (4 SoA floats) + 16 B read (previous) + 32 B written per cell.
 // ------------------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) k_push_sources(jefi_dims d, float inv_c, int slot, int prev_slot,
                                                       const float* __restrict__ rho, const float* __restrict__ jx,
                                                       const float* __restrict__ jy, const float* __restrict__ jz,
-                                                      float4* __restrict__ ringS, float4* __restrict__ ringD) {
-  long cidx = (long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (cidx >= d.N) return;
-  int i = (int)(cidx % d.nx), j = (int)((cidx / d.nx) % d.ny), k = (int)(cidx / ((long)d.nx * d.ny));
-  size_t base = (size_t)jefi_ring_cell(d, i, j, k) * d.H;
-  float4 s = make_float4(rho[cidx], jx[cidx] * inv_c, jy[cidx] * inv_c, jz[cidx] * inv_c);
-  float4 p = prev_slot >= 0 ? ringS[base + prev_slot] : make_float4(0.f, 0.f, 0.f, 0.f);
-  ringS[base + slot] = s;
-  ringD[base + slot] = make_float4(s.x - p.x, s.y - p.y, s.z - p.z, s.w - p.w);
+                                                      float4* __restrict__ ring) {
+  long r = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (r >= d.ncell_pad) return;
+  const long tile = r / JEFI_TCELLS;
+  const int cell = (int)(r - tile * JEFI_TCELLS);
+  const int tx = (int)(tile % d.ntx), ty = (int)((tile / d.ntx) % d.nty), tz = (int)(tile / ((long)d.ntx * d.nty));
+  const int i = tx * JEFI_TS + (cell & 3), j = ty * JEFI_TS + ((cell >> 2) & 3), k = tz * JEFI_TS + (cell >> 4);
+  if (i >= d.nx || j >= d.ny || k >= d.nz) return;  // padded cells stay zero
+  const size_t cidx = (size_t)i + (size_t)d.nx * ((size_t)j + (size_t)d.ny * k);
+  const size_t q = jefi_ring_quad(d, tile, slot, cell);
+  const float4 s = make_float4(jx[cidx] * inv_c, jz[cidx] * inv_c, rho[cidx], jy[cidx] * inv_c);
+  const float4 p = prev_slot >= 0 ? ring[jefi_ring_quad(d, tile, prev_slot, cell)] : make_float4(0.f, 0.f, 0.f, 0.f);
+  ring[q] = s;
+  ring[q + JEFI_TCELLS] = make_float4(s.x - p.x, s.y - p.y, s.z - p.z, s.w - p.w);
 }
 
 int jefi_launch_push_sources(jefi_ctx* c, const float* rho, const float* jx, const float* jy, const float* jz) {
@@ -178,8 +181,8 @@ int jefi_launch_push_sources(jefi_ctx* c, const float* rho, const float* jx, con
   long n = c->step + 1;
   int slot = (int)(n % d.H);
   int prev = n >= 1 ? (int)((n - 1) % d.H) : -1;
-  unsigned blocks = (unsigned)((d.N + 255) / 256);
-  k_push_sources<<<blocks, 256, 0, c->stream>>>(d, (float)(1.0 / c->c), slot, prev, rho, jx, jy, jz, c->ringS, c->ringD);
+  unsigned blocks = (unsigned)((d.ncell_pad + 255) / 256);
+  k_push_sources<<<blocks, 256, 0, c->stream>>>(d, (float)(1.0 / c->c), slot, prev, rho, jx, jy, jz, c->ring);
   JEFI_CUDA_TRY(c, cudaGetLastError());
   c->launches++;
   c->step = n;
@@ -257,16 +260,18 @@ extern "C" int jefi_debug_delay_table(jefi_ctx* c, int* m_out_host) {
   return JEFI_OK;
 }
 
-__global__ void __launch_bounds__(256) k_history_slot(jefi_dims d, float cc, int slot, const float4* __restrict__ ringS,
+__global__ void __launch_bounds__(256) k_history_slot(jefi_dims d, float cc, int slot, const float4* __restrict__ ring,
                                                       float* __restrict__ out) {
   long cidx = (long)blockIdx.x * blockDim.x + threadIdx.x;
   if (cidx >= d.N) return;
   int i = (int)(cidx % d.nx), j = (int)((cidx / d.nx) % d.ny), k = (int)(cidx / ((long)d.nx * d.ny));
-  float4 s = ringS[(size_t)jefi_ring_cell(d, i, j, k) * d.H + slot];
-  out[cidx] = s.x;
-  out[d.N + cidx] = s.y * cc;
-  out[2 * d.N + cidx] = s.z * cc;
-  out[3 * d.N + cidx] = s.w * cc;
+  long tile; int cell;
+  jefi_tile_cell(d, i, j, k, tile, cell);
+  float4 s = ring[jefi_ring_quad(d, tile, slot, cell)];  // (Jx/c, Jz/c, rho, Jy/c)
+  out[cidx] = s.z;
+  out[d.N + cidx] = s.x * cc;
+  out[2 * d.N + cidx] = s.w * cc;
+  out[3 * d.N + cidx] = s.y * cc;
 }
 
 extern "C" int jefi_debug_history_slot(jefi_ctx* c, int steps_back, float* out4N) {
@@ -274,7 +279,7 @@ extern "C" int jefi_debug_history_slot(jefi_ctx* c, int steps_back, float* out4N
   const jefi_dims& d = c->dims;
   long t = c->step - steps_back;
   if (steps_back < 0 || steps_back > d.H - 1 || t < 0) { c->err = "jefi_debug_history_slot: step not in the ring"; return JEFI_EINVAL; }
-  k_history_slot<<<(unsigned)((d.N + 255) / 256), 256, 0, c->stream>>>(d, (float)c->c, (int)(t % d.H), c->ringS, out4N);
+  k_history_slot<<<(unsigned)((d.N + 255) / 256), 256, 0, c->stream>>>(d, (float)c->c, (int)(t % d.H), c->ring, out4N);
   JEFI_CUDA_TRY(c, cudaGetLastError());
   JEFI_CUDA_TRY(c, cudaStreamSynchronize(c->stream));
   return JEFI_OK;

@@ -7,13 +7,20 @@
 #include "jefi.h"
 
 // ---- ring geometry -------------------------------------------------------------------------------------
-// Source tile: TS^3 cells.  The ring is stored tile by tile so that the slot window of one source tile is a set
-// of contiguous runs:   ringS[tile][cell_in_tile][slot] = float4(rho, Jx/c, Jy/c, Jz/c)
-//                       ringD[tile][cell_in_tile][slot] = ringS[..][slot(t)] - ringS[..][slot(t-1)]
-// with slot = step mod H, tile = tx + ntx*(ty + nty*tz), cell_in_tile = lx + TS*(ly + TS*lz).
+// Source tile: TS^3 cells.  The ring is stored tile by tile and, inside a tile, slot by slot, so that the slot window
+// of one source tile is ONE contiguous run of rows (two when the ring wraps) = one TMA bulk copy:
+//   ring[tile][slot] = row of JEFI_ROW_QUADS float4:  [0,64)    S(cell) = (Jx/c, Jz/c, rho, Jy/c) of that step
+//                                                     [64,128)  D(cell) = S(step) - S(step-1)   (backward difference)
+//                                                     [128]     pad: makes the row pitch 2064 B, so that the same cell
+//                                                               in consecutive slots falls in consecutive 16-byte bank
+//                                                               groups of shared memory (pitch mod 128 = 16)
+// with slot = step mod H, tile = tx + ntx*(ty + nty*tz), cell = lx + TS*(ly + TS*lz).  The component order
+// (Jx, Jz | rho, Jy) puts the operands of the packed FP32 instructions (FFMA2) in aligned register pairs.
 // The grid is padded to a multiple of TS per axis; padded cells stay zero for ever (they are never written).
 constexpr int JEFI_TS = 4;
 constexpr int JEFI_TCELLS = JEFI_TS * JEFI_TS * JEFI_TS;
+constexpr int JEFI_ROW_QUADS = 2 * JEFI_TCELLS + 1;        // float4 per (tile, slot) row
+constexpr int JEFI_ROW_BYTES = JEFI_ROW_QUADS * 16;        // 2064
 
 struct jefi_dims {
   int nx, ny, nz;     // real cells
@@ -23,11 +30,16 @@ struct jefi_dims {
   long ncell_pad;     // ntx*nty*ntz*TCELLS
 };
 
-__host__ __device__ inline long jefi_ring_cell(const jefi_dims& d, int i, int j, int k) {
+// tile index and cell-in-tile of grid cell (i, j, k)
+__host__ __device__ inline void jefi_tile_cell(const jefi_dims& d, int i, int j, int k, long& tile, int& cell) {
   int tx = i / JEFI_TS, ty = j / JEFI_TS, tz = k / JEFI_TS;
   int lx = i - tx * JEFI_TS, ly = j - ty * JEFI_TS, lz = k - tz * JEFI_TS;
-  long tile = tx + (long)d.ntx * (ty + (long)d.nty * tz);
-  return tile * JEFI_TCELLS + lx + JEFI_TS * (ly + JEFI_TS * lz);
+  tile = tx + (long)d.ntx * (ty + (long)d.nty * tz);
+  cell = lx + JEFI_TS * (ly + JEFI_TS * lz);
+}
+// float4 index of S(cell) in ring row (tile, slot); D(cell) sits JEFI_TCELLS quads further
+__host__ __device__ inline size_t jefi_ring_quad(const jefi_dims& d, long tile, int slot, int cell) {
+  return ((size_t)tile * d.H + (size_t)slot) * JEFI_ROW_QUADS + (size_t)cell;
 }
 
 // Extent of the delay table per axis: it covers every offset the tiled kernel can form, including offsets that
@@ -50,8 +62,7 @@ struct jefi_ctx {
   int field_impl;       // resolved: JEFI_FIELD_REFERENCE or JEFI_FIELD_TILED
   long step;            // n; -1 before the first push
   cudaStream_t stream;
-  float4* ringS;
-  float4* ringD;
+  float4* ring;         // [tile][slot][JEFI_ROW_QUADS]
   long ring_bytes;
   int* mtab_dev;        // [nz][ny][nx] delay table (fp64-built on the host)
   int* mtab_host;
@@ -59,6 +70,7 @@ struct jefi_ctx {
   int wmax;             // largest slot window over all (obs tile, source tile) pairs
   int wpitch;           // compiled shared-memory pitch chosen for it
   size_t tiled_smem;
+  int chunk;            // source tiles per CTA (blockIdx.y splits the source range; > 1 split -> atomic output)
   unsigned short* perm; // evaluation order of the 512 cells of an observation tile per relative tile offset
   int ndx, ndy, ndz;
   // particles scratch

@@ -7,10 +7,11 @@
 //
 // Two kernels:
 //   k_field_reference  one thread per observation cell, all sources, delays from the fp64-built table.
-//   k_field_tiled      256-thread CTA owns an 8x8x8 observation tile (2 cells per thread), walks the 4x4x4 source
-//                      tiles, stages each tile's slot window [m_lo, m_hi] in shared memory with cp.async and
-//                      evaluates pairs with the source cell warp-uniform and the delay per lane.
+//   k_field_tiled      warp-specialised CTA: 8 consumer warps own an 8x8x8 observation tile (2 cells per thread) and
+//                      walk 4x4x4 source tiles; a producer warp stages each tile's slot window [m_lo, m_hi] in a
+//                      two-stage shared-memory ring with TMA bulk copies (mbarrier full/done pipeline).
 #include <stdio.h>
+#include <stdlib.h>
 
 #include "jefi_ctx.h"
 
@@ -18,11 +19,10 @@
 // reference kernel
 // ------------------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(128) k_field_reference(jefi_dims d, jefi_geom g, int ex_, int ey_, long n,
-                                                         const int* __restrict__ mtab, const float4* __restrict__ ringS,
-                                                         const float4* __restrict__ ringD, float* __restrict__ ex,
-                                                         float* __restrict__ ey, float* __restrict__ ez,
-                                                         float* __restrict__ bx, float* __restrict__ by,
-                                                         float* __restrict__ bz) {
+                                                         const int* __restrict__ mtab, const float4* __restrict__ ring,
+                                                         float* __restrict__ ex, float* __restrict__ ey,
+                                                         float* __restrict__ ez, float* __restrict__ bx,
+                                                         float* __restrict__ by, float* __restrict__ bz) {
   long oc = (long)blockIdx.x * blockDim.x + threadIdx.x;
   if (oc >= d.N) return;
   const int I = (int)(oc % d.nx), J = (int)((oc / d.nx) % d.ny), K = (int)(oc / ((long)d.nx * d.ny));
@@ -36,15 +36,17 @@ __global__ void __launch_bounds__(128) k_field_reference(jefi_dims d, jefi_geom 
         int m = mtab[abs(di) + (long)ex_ * (abs(dj) + (long)ey_ * abs(dk))];
         long t = n - m;
         if (m > d.H - 2 || t < 0) continue;  // A15; zero before t0
-        size_t idx = (size_t)jefi_ring_cell(d, i, j, k) * d.H + (size_t)(t % d.H);
-        float4 S = ringS[idx], D = ringD[idx];
+        long tile; int cell;
+        jefi_tile_cell(d, i, j, k, tile, cell);
+        size_t idx = jefi_ring_quad(d, tile, (int)(t % d.H), cell);
+        const float4 S = ring[idx], D = ring[idx + JEFI_TCELLS];  // (Jx, Jz, rho, Jy)/scaled, see jefi_ctx.h
         float ax = g.kx * (float)di, ay = g.ky * (float)dj, az = g.kz * (float)dk;
         float q = fmaf(ax, ax, fmaf(ay, ay, az * az));
         float rs = rsqrtf(q), rs2 = rs * rs, rs3 = rs2 * rs;
-        float qq = fmaf(rs2, D.x, rs3 * S.x);
+        float qq = fmaf(rs2, D.z, rs3 * S.z);
         lex = fmaf(ax, qq, lex); ley = fmaf(ay, qq, ley); lez = fmaf(az, qq, lez);
-        lex = fmaf(-rs, D.y, lex); ley = fmaf(-rs, D.z, ley); lez = fmaf(-rs, D.w, lez);
-        float wx = fmaf(rs2, D.y, rs3 * S.y), wy = fmaf(rs2, D.z, rs3 * S.z), wz = fmaf(rs2, D.w, rs3 * S.w);
+        lex = fmaf(-rs, D.x, lex); ley = fmaf(-rs, D.w, ley); lez = fmaf(-rs, D.y, lez);
+        float wx = fmaf(rs2, D.x, rs3 * S.x), wy = fmaf(rs2, D.w, rs3 * S.w), wz = fmaf(rs2, D.y, rs3 * S.y);
         lbx = fmaf(ay, wz, lbx); lbx = fmaf(-az, wy, lbx);
         lby = fmaf(az, wx, lby); lby = fmaf(-ax, wz, lby);
         lbz = fmaf(ax, wy, lbz); lbz = fmaf(-ay, wx, lbz);
@@ -59,7 +61,7 @@ int jefi_launch_field_reference(jefi_ctx* c, float* ex, float* ey, float* ez, fl
   const jefi_dims& d = c->dims;
   unsigned blocks = (unsigned)((d.N + 127) / 128);
   k_field_reference<<<blocks, 128, 0, c->stream>>>(d, c->geom, jefi_table_extent(d.nx), jefi_table_extent(d.ny), c->step,
-                                                   c->mtab_dev, c->ringS, c->ringD, ex, ey, ez, bx, by, bz);
+                                                   c->mtab_dev, c->ring, ex, ey, ez, bx, by, bz);
   JEFI_CUDA_TRY(c, cudaGetLastError());
   c->launches++;
   return JEFI_OK;
@@ -68,30 +70,43 @@ int jefi_launch_field_reference(jefi_ctx* c, float* ex, float* ey, float* ez, fl
 // ------------------------------------------------------------------------------------------------------------
 // tiled kernel
 //
-// CTA = 256 threads = one 8x8x8 observation tile (512 cells, two per thread); 2 CTAs per SM.
-// For every 4x4x4 source tile the CTA stages, per source cell, the window of ring slots [m_lo, m_hi] that the tile
-// pair can address (m from the extreme offsets), S window and D window, with one TMA bulk copy per (cell, array)
-// (cp.async.bulk + mbarrier; the ring layout [tile][cell][slot] makes each window one contiguous run, two when the
-// ring wraps).  Shared-memory index j = m_hi - m, so that memory order equals slot order.
+// CTA = 8 consumer warps + 1 producer warp, one CTA per SM.  The consumers own one 8x8x8 observation tile (512 cells,
+// two per thread) against the source tiles [t0, t1) of the linear tile order (the whole grid, or one chunk of it when
+// the launch splits the source range over blockIdx.y; partial sums then meet in global memory with fp32 atomics).
+//
+// Staging.  For an (observation tile, source tile) pair the delays lie in [m_lo, m_hi] (from the extreme offsets), and
+// the ring stores a source tile slot by slot (jefi_ctx.h), so the window is one contiguous run of W = m_hi-m_lo+1 ring
+// rows (two runs when the ring wraps).  The producer warp's lane 0 issues it as one or two TMA bulk copies
+// (cp.async.bulk, SASS UBLKCP) into stage `it & 1`, together with the 1 KB evaluation-order row, on the stage's `full`
+// mbarrier; consumers release a stage by arriving (one lane per warp) on its `done` mbarrier.  Row j of a stage
+// holds delay m = m_hi - j.
 //
 // Pair evaluation: the source cell is warp-uniform, the delay per lane:
-//   q = |d'|^2 (1 FFMA), rs = rsqrt(q) (MUFU), t = q*rs + 1.5*2^23 (1 FFMA, integer m in the mantissa),
-//   address = K - 16*bits(t) (1 IMAD), 2 x LDS.128, then 20 FP32 ops:
-//   u = rs*S + D (4), r2 = rs^2 (1), a' = r2*d' (3), E += a'*u.x - rs*D.yzw (6), B += a' x u.yzw (6).
+//   q = |d'|^2 (FFMA), rs = rsqrt(q) (MUFU), t = q*rs + 1.5*2^23 (FFMA; the integer m sits in the mantissa),
+//   address = K - 2064*bits(t) (IMAD), 2 x LDS.128 (S and D quads), then with packed FP32 (fma.rn.f32x2 = SASS FFMA2,
+//   scalar operands broadcast, halves swapped for free):
+//     (wx,wz) = rs*(Jx,Jz) + (DJx,DJz)      (u0,wy) = rs*(rho,Jy) + (Drho,DJy)             2 FFMA2
+//     r2 = rs^2, (a_x,a_z) = (ax,az)*r2, a_y = ay*r2                                       FMUL, FMUL2, FMUL
+//     Exz += (a_x,a_z)*u0   Fxz += rs*(DJx,DJz)   Ey += a_y*u0   Fy += rs*DJy              2 FFMA2 + 2 FFMA
+//     Bxz += a_y*(wz,wx)    Cxz += wy*(a_z,a_x)   By12 += (a_z,a_x)*(wx,wz)                3 FFMA2
+//   E = (Exz - Fxz, Ey - Fy), B = (Bxz.lo - Cxz.lo, By12.lo - By12.hi, Cxz.hi - Bxz.hi):   18 issue slots per pair
+//   (7 scalar FMA-pipe, 8 packed, 1 MUFU, 2 LDS) against 26 for the scalar form.
 //
-// Shared-memory delivery is the scarce resource: measured on B200, an LDS.128 takes 2 cycles when every quarter-warp
-// (8 lanes) touches at most 2 distinct 16-byte words and 4 cycles otherwise.  Which lane evaluates which observation
-// cell is free (any assignment gives the same sums), so for every source tile the 512 cells are taken in the order of
-// their distance to the tile (half-slot buckets): 8 consecutive lanes are then almost equidistant from every source
-// cell of the tile and ~95% of the loads run at the 2-cycle rate.  The order depends only on the relative tile
-// offset; jefi_tiled_prepare tabulates it once (k_build_perm) and the kernel fetches the 1 KB row with the same
-// mbarrier as the windows.  Per-tile partial sums are added to a shared-memory accumulator [6][512] (second level of
-// the two-level accumulation), because a cell is evaluated by a different thread in every tile.
+// Shared-memory delivery is the scarce resource (measured, profiles/): an LDS.128 takes 4 data-pipe cycles, 2 when
+// every lane l reads the same address as lane l^1 (or every l as l^2).  Which lane evaluates which observation cell
+// is free (any assignment gives the same sums), so for every source tile the 512 cells are taken in the order of
+// their distance to the tile: neighbouring lanes then mostly share a slot.  The order depends only on the relative
+// tile offset; jefi_tiled_prepare tabulates it once (k_build_perm).  Per-tile partial sums are added to a
+// shared-memory accumulator [6][512] (second level of the two-level accumulation), because a cell is evaluated by a
+// different thread in every tile; the `done` barrier of tile it-1 orders these updates between tiles.
 // ------------------------------------------------------------------------------------------------------------
 constexpr int OB = 8;            // observation tile edge
 constexpr int OBCELLS = OB * OB * OB;
-constexpr int TILED_THREADS = 256;
-constexpr int P_OBS = OBCELLS / TILED_THREADS;  // observation cells per thread
+constexpr int NCONS = 256;       // consumer threads
+constexpr int NCWARPS = NCONS / 32;
+constexpr int TILED_THREADS = NCONS + 32;  // + producer warp
+constexpr int P_OBS = OBCELLS / NCONS;     // observation cells per consumer thread
+constexpr int HDR_BYTES = 32;
 
 struct tiled_params {
   jefi_dims d;
@@ -100,10 +115,29 @@ struct tiled_params {
   int nslot;       // n mod H
   int nobx, noby, nobz;
   int ndx, ndy;    // extents of the permutation table in relative-offset space
-  const float4* ringS;
-  const float4* ringD;
+  int chunk;       // source tiles per blockIdx.y
+  int atomic_out;  // 1: add into zeroed outputs (source range split over blockIdx.y)
+  const float4* ring;
   const unsigned short* perm;  // [ndz][ndy][ndx][512]
   float *ex, *ey, *ez, *bx, *by, *bz;
+};
+
+struct stage_hdr {  // written by the producer before it arms the stage's full barrier
+  uint32_t K;       // shared address of the stage's row 0 + 2064*(m_hi + 0x4B400000)  (mod 2^32)
+  int self;         // the source tile overlaps the observation tile (contains r' = r)
+  int dx0, dy0, dz0;  // ox0 - sx0, oy0 - sy0, oz0 - sz0
+  int pad[3];
+};
+
+template <int WP>
+struct stage_layout {
+  static constexpr uint32_t ROWS = WP * JEFI_ROW_BYTES;
+  static constexpr uint32_t PERM = ROWS;                       // u16[512]
+  static constexpr uint32_t HDR = PERM + OBCELLS * 2;
+  static constexpr uint32_t BYTES = ((HDR + HDR_BYTES + 127) / 128) * 128;
+  static constexpr uint32_t ACC = 2 * BYTES;                   // float[6][512]
+  static constexpr uint32_t BAR = ACC + 6 * OBCELLS * 4;       // full[2], done[2]
+  static constexpr uint32_t TOTAL = BAR + 4 * 8;
 };
 
 // ---- mbarrier / TMA bulk-copy primitives (PTX ISA: mbarrier, cp.async.bulk) ----
@@ -112,6 +146,9 @@ __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
 }
 __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   asm volatile(
@@ -131,6 +168,35 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t
 }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
+// ---- packed FP32 (sm_100: fma/mul .f32x2 on 64-bit register pairs) ----
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pk(float lo, float hi) {
+  f32x2 r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+  return r;
+}
+__device__ __forceinline__ float lo32(f32x2 v) {
+  float a, b;
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v));
+  return a;
+}
+__device__ __forceinline__ float hi32(f32x2 v) {
+  float a, b;
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v));
+  return b;
+}
+__device__ __forceinline__ f32x2 swap2(f32x2 v) { return pk(hi32(v), lo32(v)); }
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) {
+  f32x2 r;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+  return r;
+}
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) {
+  f32x2 r;
+  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+  return r;
+}
+
 // min / max of |a| over the integer interval [lo, hi]
 __device__ __forceinline__ void abs_range(int lo, int hi, int& mn, int& mx) {
   int alo = abs(lo), ahi = abs(hi);
@@ -138,212 +204,256 @@ __device__ __forceinline__ void abs_range(int lo, int hi, int& mn, int& mx) {
   mn = (lo <= 0 && hi >= 0) ? 0 : min(alo, ahi);
 }
 
+struct quad2 {  // one LDS.128 as two aligned register pairs
+  f32x2 xy, zw;
+};
 template <int IMM>
-__device__ __forceinline__ float4 lds128_imm(uint32_t addr) {
-  float4 v;
-  asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4+%5];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr), "n"(IMM));
+__device__ __forceinline__ quad2 lds128_imm(uint32_t addr) {
+  quad2 v;
+  asm volatile("ld.shared.v2.b64 {%0, %1}, [%2+%3];" : "=l"(v.xy), "=l"(v.zw) : "r"(addr), "n"(IMM));
   return v;
 }
 
-// One observation cell against one source cell.  K = shared address of the cell's S window + 16*(m_hi + MAGICBITS).
-template <int WP, bool SELF, int CELL>
-__device__ __forceinline__ void one_pair(uint32_t K, float ax, float ay, float az, float qyz, float (&loc)[6]) {
-  constexpr int SOFF = CELL * WP * 16;
-  constexpr int DOFF = SOFF + JEFI_TCELLS * WP * 16;
-  float q = fmaf(ax, ax, qyz);
+struct pair_acc {  // per-tile partial sums of one observation cell (first accumulation level)
+  f32x2 Exz, Fxz, Bxz, Cxz, By12;
+  float Ey, Fy;
+};
+
+// One observation cell against one source cell.  Kz = shared address of row m = 0 (i.e. K) + byte offset of the z layer.
+template <bool SELF, int CELL>
+__device__ __forceinline__ void one_pair(uint32_t Kz, f32x2 axz, float ay, float qyz, pair_acc& A) {
+  constexpr int SOFF = CELL * 16;
+  constexpr int DOFF = SOFF + JEFI_TCELLS * 16;
+  const float ax = lo32(axz);
+  const float q = fmaf(ax, ax, qyz);
   float rs = jefi_rsqrt(q);
   if (SELF) rs = q > 0.f ? rs : 0.f;        // the self cell contributes exactly zero
-  float t = fmaf(q, rs, JEFI_MAGIC);        // MAGIC + round(s): m sits in the mantissa
-  uint32_t addr = K - (uint32_t)__float_as_int(t) * 16u;   // window entry j = m_hi - m
-  const float4 S = lds128_imm<SOFF>(addr);
-  const float4 D = lds128_imm<DOFF>(addr);
-  float r2 = rs * rs;
-  float u0 = fmaf(rs, S.x, D.x), u1 = fmaf(rs, S.y, D.y), u2 = fmaf(rs, S.z, D.z), u3 = fmaf(rs, S.w, D.w);
-  float bxr = ax * r2, byr = ay * r2, bzr = az * r2;      // d' rs^2
-  loc[0] = fmaf(bxr, u0, loc[0]); loc[1] = fmaf(byr, u0, loc[1]); loc[2] = fmaf(bzr, u0, loc[2]);
-  loc[0] = fmaf(-rs, D.y, loc[0]); loc[1] = fmaf(-rs, D.z, loc[1]); loc[2] = fmaf(-rs, D.w, loc[2]);
-  loc[3] = fmaf(byr, u3, loc[3]); loc[3] = fmaf(-bzr, u2, loc[3]);
-  loc[4] = fmaf(bzr, u1, loc[4]); loc[4] = fmaf(-bxr, u3, loc[4]);
-  loc[5] = fmaf(bxr, u2, loc[5]); loc[5] = fmaf(-byr, u1, loc[5]);
+  const float t = fmaf(q, rs, JEFI_MAGIC);  // MAGIC + round(s): m sits in the mantissa
+  const uint32_t addr = Kz - (uint32_t)__float_as_int(t) * (uint32_t)JEFI_ROW_BYTES;  // row j = m_hi - m
+  const quad2 S = lds128_imm<SOFF>(addr);   // (Jx, Jz | rho, Jy)
+  const quad2 D = lds128_imm<DOFF>(addr);   // (DJx, DJz | Drho, DJy)
+  const f32x2 rs2 = pk(rs, rs);
+  const f32x2 wxz = fma2(rs2, S.xy, D.xy);  // (wx, wz)
+  const f32x2 u0wy = fma2(rs2, S.zw, D.zw); // (u0, wy)
+  const float r2 = rs * rs;
+  const f32x2 Axz = mul2(axz, pk(r2, r2));  // (a_x, a_z) = d' rs^2
+  const float a_y = ay * r2;
+  const float u0 = lo32(u0wy), wy = hi32(u0wy);
+  const f32x2 Azx = swap2(Axz);
+  A.Exz = fma2(Axz, pk(u0, u0), A.Exz);
+  A.Fxz = fma2(rs2, D.xy, A.Fxz);
+  A.Ey = fmaf(a_y, u0, A.Ey);
+  A.Fy = fmaf(rs, hi32(D.zw), A.Fy);
+  A.Bxz = fma2(pk(a_y, a_y), swap2(wxz), A.Bxz);  // (a_y wz, a_y wx)
+  A.Cxz = fma2(pk(wy, wy), Azx, A.Cxz);           // (wy a_z, wy a_x)
+  A.By12 = fma2(Azx, wxz, A.By12);                // (a_z wx, a_x wz)
 }
 
-template <int WP, bool SELF, int LY>
-__device__ __forceinline__ void one_row(uint32_t Kz, const float (&ax)[JEFI_TS], float ay, float az, float az2, float (&loc)[6]) {
-  float qyz = fmaf(ay, ay, az2);
-  one_pair<WP, SELF, JEFI_TS * LY + 0>(Kz, ax[0], ay, az, qyz, loc);
-  one_pair<WP, SELF, JEFI_TS * LY + 1>(Kz, ax[1], ay, az, qyz, loc);
-  one_pair<WP, SELF, JEFI_TS * LY + 2>(Kz, ax[2], ay, az, qyz, loc);
-  one_pair<WP, SELF, JEFI_TS * LY + 3>(Kz, ax[3], ay, az, qyz, loc);
+template <bool SELF, int LY>
+__device__ __forceinline__ void one_row(uint32_t Kz, const f32x2 (&axz)[JEFI_TS], float ay, float az2, pair_acc& A) {
+  const float qyz = fmaf(ay, ay, az2);
+  one_pair<SELF, JEFI_TS * LY + 0>(Kz, axz[0], ay, qyz, A);
+  one_pair<SELF, JEFI_TS * LY + 1>(Kz, axz[1], ay, qyz, A);
+  one_pair<SELF, JEFI_TS * LY + 2>(Kz, axz[2], ay, qyz, A);
+  one_pair<SELF, JEFI_TS * LY + 3>(Kz, axz[3], ay, qyz, A);
 }
 
 // one observation cell against the 64 cells of the staged source tile
-template <int WP, bool SELF>
+template <bool SELF>
 __device__ __forceinline__ void tile_pairs(uint32_t K, float kz, const float (&ax)[JEFI_TS], const float (&ay)[JEFI_TS], float fz0,
-                                           float (&loc)[6]) {
+                                           pair_acc& A) {
 #pragma unroll 1
   for (int lz = 0; lz < JEFI_TS; lz++) {
     const float az = kz * (fz0 - (float)lz);
     const float az2 = az * az;
-    const uint32_t Kz = K + (uint32_t)(lz * JEFI_TS * JEFI_TS * WP * 16);
-    one_row<WP, SELF, 0>(Kz, ax, ay[0], az, az2, loc);
-    one_row<WP, SELF, 1>(Kz, ax, ay[1], az, az2, loc);
-    one_row<WP, SELF, 2>(Kz, ax, ay[2], az, az2, loc);
-    one_row<WP, SELF, 3>(Kz, ax, ay[3], az, az2, loc);
+    const uint32_t Kz = K + (uint32_t)(lz * JEFI_TS * JEFI_TS * 16);
+    f32x2 axz[JEFI_TS];
+#pragma unroll
+    for (int l = 0; l < JEFI_TS; l++) axz[l] = pk(ax[l], az);
+    one_row<SELF, 0>(Kz, axz, ay[0], az2, A);
+    one_row<SELF, 1>(Kz, axz, ay[1], az2, A);
+    one_row<SELF, 2>(Kz, axz, ay[2], az2, A);
+    one_row<SELF, 3>(Kz, axz, ay[3], az2, A);
   }
 }
 
 template <int WP>
-__global__ void __launch_bounds__(TILED_THREADS, 2) k_field_tiled(tiled_params P) {
+__global__ void __launch_bounds__(TILED_THREADS, 1) k_field_tiled(tiled_params P) {
+  using L = stage_layout<WP>;
   extern __shared__ __align__(128) unsigned char smem[];
-  // dynamic shared memory: [S windows][D windows][accumulators 6 x 512 floats][permutation 512 x u16]
-  constexpr uint32_t PITCHB = WP * 16;
-  constexpr uint32_t DOFFB = JEFI_TCELLS * PITCHB;  // D window follows the S window
-  float* accS = reinterpret_cast<float*>(smem + 2 * DOFFB);
-  unsigned short* permS = reinterpret_cast<unsigned short*>(smem + 2 * DOFFB + 6 * OBCELLS * sizeof(float));
-  __shared__ __align__(8) unsigned long long mbar_storage;
   const jefi_dims& d = P.d;
-  const int tid = threadIdx.x;
-  // observation tile of this CTA
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const uint32_t sm0 = (uint32_t)__cvta_generic_to_shared(smem);
+  float* accS = reinterpret_cast<float*>(smem + L::ACC);
+  const uint32_t barFull = sm0 + L::BAR, barDone = barFull + 16;
+  // observation tile and source-tile range of this CTA
   const int obx = blockIdx.x % P.nobx, oby = (blockIdx.x / P.nobx) % P.noby, obz = blockIdx.x / (P.nobx * P.noby);
   const int ox0 = obx * OB, oy0 = oby * OB, oz0 = obz * OB;
+  const int ntiles = d.ntx * d.nty * d.ntz;
+  const int t0 = blockIdx.y * P.chunk;
+  const int nt = min(P.chunk, ntiles - t0);
 
-  for (int i = tid; i < 6 * OBCELLS; i += TILED_THREADS) accS[i] = 0.f;
-  const uint32_t smS = (uint32_t)__cvta_generic_to_shared(smem);
-  const uint32_t permA = (uint32_t)__cvta_generic_to_shared(permS);
-  const uint32_t bar = (uint32_t)__cvta_generic_to_shared(&mbar_storage);
+  if (tid < NCONS)
+    for (int i = tid; i < 6 * OBCELLS; i += NCONS) accS[i] = 0.f;
   if (tid == 0) {
-    mbar_init(bar, 1);
+    mbar_init(barFull, 1); mbar_init(barFull + 8, 1);
+    mbar_init(barDone, NCWARPS); mbar_init(barDone + 8, NCWARPS);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
-  uint32_t phase = 0;
-  // thread -> (cell, array) of the bulk copies it issues
-  const int cp_cell = tid & (JEFI_TCELLS - 1);
-  const int cp_arr = tid >> 6;  // 0: S, 1: D, 2: permutation row (thread 128), 3: none
 
-  int st = 0;
-  for (int stz = 0; stz < d.ntz; stz++)
-    for (int sty = 0; sty < d.nty; sty++)
-      for (int stx = 0; stx < d.ntx; stx++, st++) {
-        const int sx0 = stx * JEFI_TS, sy0 = sty * JEFI_TS, sz0 = stz * JEFI_TS;
-        // slot window of this (observation tile, source tile) pair from the extreme offsets
-        int mnx, mxx, mny, mxy, mnz, mxz;
-        abs_range(ox0 - (sx0 + JEFI_TS - 1), ox0 + OB - 1 - sx0, mnx, mxx);
-        abs_range(oy0 - (sy0 + JEFI_TS - 1), oy0 + OB - 1 - sy0, mny, mxy);
-        abs_range(oz0 - (sz0 + JEFI_TS - 1), oz0 + OB - 1 - sz0, mnz, mxz);
-        const bool self = (mnx == 0 && mny == 0 && mnz == 0);
-        const int m_lo = self ? 0 : jefi_delay_fp32(jefi_q_fp32(P.g.kx, P.g.ky, P.g.kz, (float)mnx, (float)mny, (float)mnz));
-        const int m_hi = jefi_delay_fp32(jefi_q_fp32(P.g.kx, P.g.ky, P.g.kz, (float)mxx, (float)mxy, (float)mxz));
-        const int W = m_hi - m_lo + 1;  // <= WP (jefi_tiled_prepare)
-        // window entry j <-> delay m = m_hi - j <-> absolute step t = n - m_hi + j.  Entries with t < 0 (before t0,
-        // PAPER.md:217) or m > H-2 (not stored, reading A15) are zero: j < jv.
-        int jv = max(m_hi - P.n, m_hi - (d.H - 2));
-        jv = jv < 0 ? 0 : (jv > W ? W : jv);
-        const int nvalid = W - jv;          // <= H - 1
-        int s0 = P.nslot - (m_hi - jv);     // ring slot of entry jv; m_hi - jv <= H - 2
-        s0 += s0 < 0 ? d.H : 0;
-        const int lenA = min(nvalid, d.H - s0), lenB = nvalid - lenA;  // ring wrap: at most two runs
-
-        fence_proxy_async();  // order this thread's generic-proxy accesses of the window before the async-proxy writes
-        __syncthreads();      // everyone is done with the previous tile (window, permutation, accumulator updates)
-        if (jv > 0) {         // zero part of the window (only in the first steps of a run or with a shallow ring)
-          for (int idx = tid; idx < 2 * JEFI_TCELLS * jv; idx += TILED_THREADS) {
-            int row = idx / jv, j = idx - row * jv;
-            *reinterpret_cast<float4*>(smem + (size_t)row * PITCHB + (size_t)j * 16) = make_float4(0.f, 0.f, 0.f, 0.f);
-          }
-        }
-        if (tid == 0) mbar_expect_tx(bar, (uint32_t)(2 * JEFI_TCELLS * nvalid * 16 + OBCELLS * 2));
-        if (cp_arr < 2) {
-          if (nvalid > 0) {
-            const float4* ring = cp_arr == 0 ? P.ringS : P.ringD;
-            const float4* src = ring + ((size_t)st * JEFI_TCELLS + cp_cell) * d.H;
-            const uint32_t dst = smS + (uint32_t)cp_arr * DOFFB + (uint32_t)cp_cell * PITCHB + (uint32_t)jv * 16u;
-            bulk_g2s(dst, src + s0, (uint32_t)lenA * 16u, bar);
-            if (lenB > 0) bulk_g2s(dst + (uint32_t)lenA * 16u, src, (uint32_t)lenB * 16u, bar);
-          }
-        } else if (tid == 2 * JEFI_TCELLS) {
-          const int ix = 2 * obx - stx + (d.ntx - 1), iy = 2 * oby - sty + (d.nty - 1), iz = 2 * obz - stz + (d.ntz - 1);
-          const size_t row = (size_t)ix + (size_t)P.ndx * ((size_t)iy + (size_t)P.ndy * iz);
-          bulk_g2s(permA, P.perm + row * OBCELLS, OBCELLS * 2, bar);
-        }
-        const uint32_t K = smS + ((uint32_t)m_hi + 0x4B400000u) * 16u;  // wraps mod 2^32 together with bits*16
-
-        mbar_wait(bar, phase);
-        phase ^= 1u;
-        if (jv > 0) __syncthreads();  // the zero fill is generic-proxy: make it visible to all warps
-
-#pragma unroll 1
-        for (int p = 0; p < P_OBS; p++) {
-          // the cell this lane evaluates for this source tile: 8 consecutive lanes are (almost) equidistant from it
-          const int c = permS[p * TILED_THREADS + tid];
-          const int cx = c & 7, cy = (c >> 3) & 7, cz = c >> 6;
-          float ax[JEFI_TS], ay[JEFI_TS];
-#pragma unroll
-          for (int l = 0; l < JEFI_TS; l++) {
-            ax[l] = P.g.kx * (float)(ox0 + cx - sx0 - l);
-            ay[l] = P.g.ky * (float)(oy0 + cy - sy0 - l);
-          }
-          const float fz0 = (float)(oz0 + cz - sz0);
-          float loc[6];
-#pragma unroll
-          for (int a = 0; a < 6; a++) loc[a] = 0.f;
-          if (self)
-            tile_pairs<WP, true>(K, P.g.kz, ax, ay, fz0, loc);
-          else
-            tile_pairs<WP, false>(K, P.g.kz, ax, ay, fz0, loc);
-          // second accumulation level; this tile, cell c belongs to this thread alone
-#pragma unroll
-          for (int a = 0; a < 6; a++) accS[a * OBCELLS + c] += loc[a];
-        }
+  if (warp == NCWARPS) {
+    // ------------------------------------------------ producer warp ------------------------------------------------
+    int stx = t0 % d.ntx, sty = (t0 / d.ntx) % d.nty, stz = t0 / (d.ntx * d.nty);
+    for (int it = 0; it < nt; it++) {
+      const int s = it & 1;
+      if (it >= 2) mbar_wait(barDone + 8 * s, ((it - 2) >> 1) & 1);  // consumers are done with tile it-2 (same stage)
+      const int sx0 = stx * JEFI_TS, sy0 = sty * JEFI_TS, sz0 = stz * JEFI_TS;
+      // slot window of this (observation tile, source tile) pair from the extreme offsets
+      int mnx, mxx, mny, mxy, mnz, mxz;
+      abs_range(ox0 - (sx0 + JEFI_TS - 1), ox0 + OB - 1 - sx0, mnx, mxx);
+      abs_range(oy0 - (sy0 + JEFI_TS - 1), oy0 + OB - 1 - sy0, mny, mxy);
+      abs_range(oz0 - (sz0 + JEFI_TS - 1), oz0 + OB - 1 - sz0, mnz, mxz);
+      const bool self = (mnx == 0 && mny == 0 && mnz == 0);
+      const int m_lo = self ? 0 : jefi_delay_fp32(jefi_q_fp32(P.g.kx, P.g.ky, P.g.kz, (float)mnx, (float)mny, (float)mnz));
+      const int m_hi = jefi_delay_fp32(jefi_q_fp32(P.g.kx, P.g.ky, P.g.kz, (float)mxx, (float)mxy, (float)mxz));
+      const int W = m_hi - m_lo + 1;  // <= WP (jefi_tiled_prepare)
+      // row j <-> delay m = m_hi - j <-> absolute step t = n - m_hi + j.  Rows with t < 0 (before t0)
+      // or m > H-2 (not stored, reading A15) are zero: j < jv.
+      int jv = max(m_hi - P.n, m_hi - (d.H - 2));
+      jv = jv < 0 ? 0 : (jv > W ? W : jv);
+      const int nvalid = W - jv;          // <= H - 1
+      int s0 = P.nslot - (m_hi - jv);     // ring slot of row jv; m_hi - jv <= H - 2
+      s0 += s0 < 0 ? d.H : 0;
+      const int lenA = min(nvalid, d.H - s0), lenB = nvalid - lenA;  // ring wrap: at most two runs
+      const uint32_t sb = sm0 + (uint32_t)s * L::BYTES;
+      if (jv > 0) {  // zero rows (only in the first steps of a run or with a shallow ring)
+        float4* z = reinterpret_cast<float4*>(smem + (size_t)s * L::BYTES);
+        for (int i = lane; i < jv * JEFI_ROW_QUADS; i += 32) z[i] = make_float4(0.f, 0.f, 0.f, 0.f);
       }
+      __syncwarp();
+      if (lane == 0) {
+        stage_hdr h;
+        h.K = sb + ((uint32_t)m_hi + 0x4B400000u) * (uint32_t)JEFI_ROW_BYTES;  // wraps mod 2^32 together with bits*2064
+        h.self = self ? 1 : 0;
+        h.dx0 = ox0 - sx0; h.dy0 = oy0 - sy0; h.dz0 = oz0 - sz0;
+        h.pad[0] = h.pad[1] = h.pad[2] = 0;
+        *reinterpret_cast<stage_hdr*>(smem + (size_t)s * L::BYTES + L::HDR) = h;
+        fence_proxy_async();  // generic-proxy accesses of this stage (zero fill, earlier reads) before the async-proxy writes
+        const uint32_t bar = barFull + 8 * s;
+        mbar_expect_tx(bar, (uint32_t)(nvalid * JEFI_ROW_BYTES + OBCELLS * 2));
+        const size_t tile = (size_t)(t0 + it);
+        const float4* rows = P.ring + tile * d.H * JEFI_ROW_QUADS;
+        if (lenA > 0) bulk_g2s(sb + (uint32_t)(jv * JEFI_ROW_BYTES), rows + (size_t)s0 * JEFI_ROW_QUADS, (uint32_t)(lenA * JEFI_ROW_BYTES), bar);
+        if (lenB > 0) bulk_g2s(sb + (uint32_t)((jv + lenA) * JEFI_ROW_BYTES), rows, (uint32_t)(lenB * JEFI_ROW_BYTES), bar);
+        const int ix = 2 * obx - stx + (d.ntx - 1), iy = 2 * oby - sty + (d.nty - 1), iz = 2 * obz - stz + (d.ntz - 1);
+        const size_t prow = (size_t)ix + (size_t)P.ndx * ((size_t)iy + (size_t)P.ndy * iz);
+        bulk_g2s(sb + L::PERM, P.perm + prow * OBCELLS, OBCELLS * 2, bar);
+      }
+      if (++stx == d.ntx) { stx = 0; if (++sty == d.nty) { sty = 0; ++stz; } }
+    }
+    return;
+  }
 
-  __syncthreads();
+  // -------------------------------------------------- consumer warps --------------------------------------------------
+  for (int it = 0; it < nt; it++) {
+    const int s = it & 1;
+    const unsigned char* st = smem + (size_t)s * L::BYTES;
+    mbar_wait(barFull + 8 * s, (it >> 1) & 1);
+    const stage_hdr h = *reinterpret_cast<const stage_hdr*>(st + L::HDR);
+    const unsigned short* permS = reinterpret_cast<const unsigned short*>(st + L::PERM);
+#pragma unroll 1
+    for (int p = 0; p < P_OBS; p++) {
+      // the cell this lane evaluates for this source tile: neighbouring lanes are (almost) equidistant from it
+      const int c = permS[p * NCONS + tid];
+      const int cx = c & 7, cy = (c >> 3) & 7, cz = c >> 6;
+      float ax[JEFI_TS], ay[JEFI_TS];
+#pragma unroll
+      for (int l = 0; l < JEFI_TS; l++) {
+        ax[l] = P.g.kx * (float)(h.dx0 + cx - l);
+        ay[l] = P.g.ky * (float)(h.dy0 + cy - l);
+      }
+      const float fz0 = (float)(h.dz0 + cz);
+      pair_acc A;
+      A.Exz = A.Fxz = A.Bxz = A.Cxz = A.By12 = pk(0.f, 0.f);
+      A.Ey = A.Fy = 0.f;
+      if (h.self)
+        tile_pairs<true>(h.K, P.g.kz, ax, ay, fz0, A);
+      else
+        tile_pairs<false>(h.K, P.g.kz, ax, ay, fz0, A);
+      // second accumulation level.  Cell c belongs to this thread alone in this tile; the previous tile's updates
+      // (by other threads) are complete once every consumer warp has arrived on that tile's done barrier.
+      if (p == 0 && it > 0) mbar_wait(barDone + 8 * ((it - 1) & 1), ((it - 1) >> 1) & 1);
+      accS[c] += lo32(A.Exz) - lo32(A.Fxz);
+      accS[OBCELLS + c] += A.Ey - A.Fy;
+      accS[2 * OBCELLS + c] += hi32(A.Exz) - hi32(A.Fxz);
+      accS[3 * OBCELLS + c] += lo32(A.Bxz) - lo32(A.Cxz);
+      accS[4 * OBCELLS + c] += lo32(A.By12) - hi32(A.By12);
+      accS[5 * OBCELLS + c] += hi32(A.Cxz) - hi32(A.Bxz);
+    }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(barDone + 8 * s);  // stage s may be refilled; this warp's accumulator updates are done
+  }
+
+  asm volatile("bar.sync 1, %0;" ::"n"(NCONS) : "memory");  // consumers only: all accumulator updates are visible
 #pragma unroll
   for (int p = 0; p < P_OBS; p++) {
-    const int c = p * TILED_THREADS + tid;  // home order: x fastest inside the tile
+    const int c = p * NCONS + tid;  // home order: x fastest inside the tile
     const int oi = ox0 + (c & 7), oj = oy0 + ((c >> 3) & 7), ok = oz0 + (c >> 6);
     if (oi < d.nx && oj < d.ny && ok < d.nz) {
       const size_t o = (size_t)oi + (size_t)d.nx * ((size_t)oj + (size_t)d.ny * ok);
-      P.ex[o] = P.g.prefE * accS[c]; P.ey[o] = P.g.prefE * accS[OBCELLS + c]; P.ez[o] = P.g.prefE * accS[2 * OBCELLS + c];
-      P.bx[o] = P.g.prefB * accS[3 * OBCELLS + c]; P.by[o] = P.g.prefB * accS[4 * OBCELLS + c];
-      P.bz[o] = P.g.prefB * accS[5 * OBCELLS + c];
+      const float vex = P.g.prefE * accS[c], vey = P.g.prefE * accS[OBCELLS + c], vez = P.g.prefE * accS[2 * OBCELLS + c];
+      const float vbx = P.g.prefB * accS[3 * OBCELLS + c], vby = P.g.prefB * accS[4 * OBCELLS + c], vbz = P.g.prefB * accS[5 * OBCELLS + c];
+      if (P.atomic_out) {
+        atomicAdd(P.ex + o, vex); atomicAdd(P.ey + o, vey); atomicAdd(P.ez + o, vez);
+        atomicAdd(P.bx + o, vbx); atomicAdd(P.by + o, vby); atomicAdd(P.bz + o, vbz);
+      } else {
+        P.ex[o] = vex; P.ey[o] = vey; P.ez[o] = vez;
+        P.bx[o] = vbx; P.by[o] = vby; P.bz[o] = vbz;
+      }
     }
   }
 }
 
 // Evaluation order of the 512 cells of an observation tile for one relative tile offset D = (ox0 - sx0, ..):
-// ascending distance to the centre of the source tile in half-slot buckets, ties in home order (x fastest).
+// ascending distance to the centre of the source tile, ties in home order (x fastest).
 // One CTA of 512 threads per offset; rank by counting (a one-off O(512^2) per offset at create time).
 __global__ void __launch_bounds__(OBCELLS) k_build_perm(int ndx, int ndy, int ntx, int nty, int ntz, jefi_geom g,
                                                         unsigned short* __restrict__ perm) {
-  __shared__ int keys[OBCELLS];
+  __shared__ float keys[OBCELLS];
   const int c = threadIdx.x;
   const int ix = blockIdx.x % ndx, iy = (blockIdx.x / ndx) % ndy, iz = blockIdx.x / (ndx * ndy);
   const float Dx = (float)(JEFI_TS * (ix - (ntx - 1))), Dy = (float)(JEFI_TS * (iy - (nty - 1))), Dz = (float)(JEFI_TS * (iz - (ntz - 1)));
   const float half = 0.5f * (float)(JEFI_TS - 1);
   const float rx = g.kx * (Dx + (float)(c & 7) - half), ry = g.ky * (Dy + (float)((c >> 3) & 7) - half),
               rz = g.kz * (Dz + (float)(c >> 6) - half);
-  const int key = (int)(2.f * sqrtf(rx * rx + ry * ry + rz * rz));
+  const float key = rx * rx + ry * ry + rz * rz;
   keys[c] = key;
   __syncthreads();
   int pos = 0;
   for (int j = 0; j < OBCELLS; j++) {
-    int kj = keys[j];
+    float kj = keys[j];
     pos += (kj < key) || (kj == key && j < c);
   }
   perm[(size_t)blockIdx.x * OBCELLS + pos] = (unsigned short)c;
 }
 
-// window pitches the kernel is compiled for (float4 entries per source-cell row)
-static const int kPitches[] = {36, 64, 96};
+// window pitches the kernel is compiled for (ring rows per stage)
+static const int kPitches[] = {36, 48};
 typedef void (*tiled_fn)(tiled_params);
 static tiled_fn tiled_kernel_for(int wp) {
   switch (wp) {
     case 36: return k_field_tiled<36>;
-    case 64: return k_field_tiled<64>;
-    case 96: return k_field_tiled<96>;
+    case 48: return k_field_tiled<48>;
   }
   return nullptr;
+}
+static size_t tiled_smem_for(int wp) {
+  switch (wp) {
+    case 36: return stage_layout<36>::TOTAL;
+    case 48: return stage_layout<48>::TOTAL;
+  }
+  return 0;
 }
 
 // Largest slot window over all relative placements of an 8^3 observation tile and a 4^3 source tile (host, fp64),
@@ -377,15 +487,15 @@ int jefi_tiled_prepare(jefi_ctx* c) {
     if (cand >= wmax) { wp = cand; break; }
   if (wp == 0) {
     char buf[160];
-    snprintf(buf, sizeof buf, "tiled kernel: slot window of %d exceeds the largest compiled pitch %d", wmax, kPitches[2]);
+    snprintf(buf, sizeof buf, "tiled kernel: slot window of %d exceeds the largest compiled pitch %d", wmax, kPitches[1]);
     c->err = buf;
     return JEFI_ESTATE;
   }
   c->wpitch = wp;
-  c->tiled_smem = (size_t)2 * JEFI_TCELLS * wp * sizeof(float4) + 6 * OBCELLS * sizeof(float) + OBCELLS * sizeof(unsigned short);
+  c->tiled_smem = tiled_smem_for(wp);
   int dev = c->cfg.device, max_optin = 0;
   cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
-  if (c->tiled_smem + 64 > (size_t)max_optin) {
+  if (c->tiled_smem > (size_t)max_optin) {
     char buf[160];
     snprintf(buf, sizeof buf, "tiled kernel needs %zu B of shared memory (window %d slots), device allows %d", c->tiled_smem, wmax, max_optin);
     c->err = buf;
@@ -393,6 +503,24 @@ int jefi_tiled_prepare(jefi_ctx* c) {
   }
   cudaError_t e = cudaFuncSetAttribute(tiled_kernel_for(wp), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->tiled_smem);
   if (e != cudaSuccess) { c->err = std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e); return JEFI_ECUDA; }
+  // how the source range is split over blockIdx.y: JEFI_FIELD_CHUNK (source tiles per CTA) overrides the default, which
+  // keeps one CTA per observation tile (deterministic sums) once there are at least four waves of them and otherwise
+  // splits the source tiles so that the grid has about four CTAs per SM (partial sums meet in fp32 atomics).
+  int nsm = 148;
+  cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+  const int nobs = nobx * noby * nobz, ntiles = d.ntx * d.nty * d.ntz;
+  int chunk = ntiles;
+  const char* env = getenv("JEFI_FIELD_CHUNK");
+  if (env && atoi(env) > 0) {
+    chunk = atoi(env);
+  } else if (nobs < 4 * nsm) {
+    int nsplit = (4 * nsm + nobs - 1) / nobs;
+    chunk = (ntiles + nsplit - 1) / nsplit;
+  }
+  if (chunk < 1) chunk = 1;
+  if (chunk > ntiles) chunk = ntiles;
+  if ((ntiles + chunk - 1) / chunk > 65535) chunk = (ntiles + 65534) / 65535;
+  c->chunk = chunk;
   // evaluation-order table over all relative tile offsets
   c->ndx = d.ntx + 2 * nobx - 2; c->ndy = d.nty + 2 * noby - 2; c->ndz = d.ntz + 2 * nobz - 2;
   size_t rows = (size_t)c->ndx * c->ndy * c->ndz;
@@ -412,10 +540,18 @@ int jefi_launch_field_tiled(jefi_ctx* c, float* ex, float* ey, float* ez, float*
   P.d = d; P.g = c->geom; P.n = (int)c->step; P.nslot = (int)(c->step % d.H);
   P.nobx = (d.nx + OB - 1) / OB; P.noby = (d.ny + OB - 1) / OB; P.nobz = (d.nz + OB - 1) / OB;
   P.ndx = c->ndx; P.ndy = c->ndy;
-  P.ringS = c->ringS; P.ringD = c->ringD; P.perm = c->perm;
+  const int ntiles = d.ntx * d.nty * d.ntz;
+  P.chunk = c->chunk;
+  const int nsplit = (ntiles + c->chunk - 1) / c->chunk;
+  P.atomic_out = nsplit > 1 ? 1 : 0;
+  P.ring = c->ring; P.perm = c->perm;
   P.ex = ex; P.ey = ey; P.ez = ez; P.bx = bx; P.by = by; P.bz = bz;
-  unsigned blocks = (unsigned)(P.nobx * P.noby * P.nobz);
-  tiled_kernel_for(c->wpitch)<<<blocks, TILED_THREADS, c->tiled_smem, c->stream>>>(P);
+  if (P.atomic_out) {
+    float* outs[6] = {ex, ey, ez, bx, by, bz};
+    for (float* o : outs) JEFI_CUDA_TRY(c, cudaMemsetAsync(o, 0, (size_t)d.N * sizeof(float), c->stream));
+  }
+  dim3 grid((unsigned)(P.nobx * P.noby * P.nobz), (unsigned)nsplit);
+  tiled_kernel_for(c->wpitch)<<<grid, TILED_THREADS, c->tiled_smem, c->stream>>>(P);
   JEFI_CUDA_TRY(c, cudaGetLastError());
   c->launches++;
   return JEFI_OK;
