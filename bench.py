@@ -141,6 +141,21 @@ def run_reference(args, w: wl.Workload) -> dict:
 
 
 # --------------------------------------------------------------------------------------------------- product arm
+def max_over_ranks(dist, ms: float, device) -> float:
+    """Multi-GPU timing rule: a step takes as long as the slowest rank (all-reduce MAX; identity at world size 1)."""
+    import torch
+
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_rate(world: int, pairs_per_rank: float, ms_max: float) -> float:
+    """Whole-job Gpairs/s: every rank processed pairs_per_rank pairs (replicas) in ms_max."""
+    return world * pairs_per_rank / (ms_max * 1e-3) / 1e9
+
+
 def time_pic(J, torch, device, config: int, steps: int, warmup: int) -> dict:
     w = wl.WORKLOADS[config]
     ctx = J.JefiContext(J.GridSpec(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt), device=device)
@@ -235,11 +250,8 @@ def run_product(args, w: wl.Workload) -> dict:
         ctx.field_step()
         kms.append(ctx.last_field_kernel_ms())
     kernel_ms = float(np.mean(kms))
-    t_ms = torch.tensor([step_ms], dtype=torch.float64, device=device)
-    if dist is not None:
-        dist.all_reduce(t_ms, op=dist.ReduceOp.MAX)
-    step_ms_max = float(t_ms.item())
-    value = world * pairs / (step_ms_max * 1e-3) / 1e9
+    step_ms_max = max_over_ranks(dist, step_ms, device)
+    value = aggregate_rate(world, pairs, step_ms_max)
 
     # ---- end to end through the C-ABI with host buffers ----
     src_pin = torch.empty(4 * N, dtype=torch.float32).pin_memory()
@@ -253,10 +265,8 @@ def run_product(args, w: wl.Workload) -> dict:
         J.jefi_field_step_host(ctx.handle, N, src_pin, eb_pin)
     torch.cuda.synchronize(device)
     e2e_ms = (time.perf_counter() - t0) * 1e3 / e2e_steps
-    t_e = torch.tensor([e2e_ms], dtype=torch.float64, device=device)
-    if dist is not None:
-        dist.all_reduce(t_e, op=dist.ReduceOp.MAX)
-    e2e_val = world * pairs / (float(t_e.item()) * 1e-3) / 1e9
+    e2e_ms_max = max_over_ranks(dist, e2e_ms, device)
+    e2e_val = aggregate_rate(world, pairs, e2e_ms_max)
     checksum = float(eb_pin[:N].double().abs().sum())
 
     impl = ctx.info["field_impl"]
@@ -279,7 +289,7 @@ def run_product(args, w: wl.Workload) -> dict:
                             "kernel_ms": kernel_ms, "flop_per_pair": FLOP_PER_PAIR,
                             "peak_source": "148 SM x 128 FP32 lanes x 2 FLOP x clocks.max.sm (derived, DESIGN.md §7)"},
                "e2e": {"value": e2e_val, "unit": "Gpairs/s", "h2d_bytes_per_step": 16 * N, "d2h_bytes_per_step": 24 * N,
-                       "ms_per_step": float(t_e.item()), "checksum_abs_ex": checksum},
+                       "ms_per_step": e2e_ms_max, "checksum_abs_ex": checksum},
                "gpu_launches": int(launches), "clocks": clocks}
         if not args.no_pic and world == 1:
             out["pic"] = []

@@ -102,7 +102,10 @@ int jefi_launch_field_reference(jefi_ctx* c, float* ex, float* ey, float* ez, fl
 // ------------------------------------------------------------------------------------------------------------
 constexpr int OB = 8;            // observation tile edge
 constexpr int OBCELLS = OB * OB * OB;
-constexpr int NCONS = 256;       // consumer threads
+#ifndef JEFI_NCONS
+#define JEFI_NCONS 512
+#endif
+constexpr int NCONS = JEFI_NCONS;  // consumer threads
 constexpr int NCWARPS = NCONS / 32;
 constexpr int TILED_THREADS = NCONS + 32;  // + producer warp
 constexpr int P_OBS = OBCELLS / NCONS;     // observation cells per consumer thread
