@@ -158,7 +158,7 @@ def aggregate_rate(world: int, pairs_per_rank: float, ms_max: float) -> float:
 
 def time_pic(J, torch, device, config: int, steps: int, warmup: int) -> dict:
     w = wl.WORKLOADS[config]
-    ctx = J.JefiContext(J.GridSpec(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt), device=device)
+    ctx = J.JefiContext(J.GridSpec(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt), device=device, sort_every=8)
     part = {k: torch.from_numpy(v).to(device) for k, v in wl.particles(config).items()}
     for _ in range(warmup):
         ctx.pic_step(part)
@@ -176,6 +176,85 @@ def time_pic(J, torch, device, config: int, steps: int, warmup: int) -> dict:
            "particles": int(part["x"].numel()), "field_kernel_ms": fk, "launches": ctx.launch_count() - l0,
            "field_impl": ctx.info["field_impl"]}
     ctx.close()
+    return out
+
+
+def hbm_peak_gbs():
+    """Measured HBM copy bandwidth of this pool's B200s (MEASURED_PEAKS.json, driver-written), else the guide's fallback."""
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "of measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:  # noqa: BLE001
+        return 6650.0, "of fallback (B200_PROFILING.md, 6.65 TB/s)"
+
+
+def time_particle_kernels(J, torch, device, config: int = 5, reps: int = 5) -> dict:
+    """HBM roofline of the particle kernels: jefi_deposit (direct and cell-sorted) and
+    jefi_push_particles on the particle set of a config (default 5: 8e6 macro-particles on 128^3), each call timed
+    alone with CUDA events.  The context uses H = 2 (these kernels never touch the ring); E, B are seeded random
+    fields scaled so that nothing leaves the grid.  Particle arrays (232 MB) exceed L2; a 512 MB fill between
+    repetitions flushes it anyway.  Algorithmic bytes per call are stated in DESIGN.md §6.3-6.4."""
+    w = wl.WORKLOADS[config]
+    part_h = wl.particles(config)
+    P, N = int(part_h["x"].shape[0]), w.N
+    peak, peak_src = hbm_peak_gbs()
+    flush = torch.empty(128 * 1024 * 1024, dtype=torch.float32, device=device)
+    g = torch.Generator(device=device)
+    g.manual_seed(w.seed)
+    out = {"workload": w.name + "_particles", "particles": P, "grid": [w.n] * 3, "hbm_peak_gbs": peak, "peak_source": peak_src,
+           "l2": "512 MB fill between repetitions", "kernels": {}}
+
+    def timed(fn):
+        ms = []
+        for _ in range(reps + 1):
+            flush.fill_(1.0)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            fn()
+            e1.record()
+            torch.cuda.synchronize(device)
+            ms.append(e0.elapsed_time(e1))
+        return float(np.median(ms[1:]))
+
+    def entry(ms, nbytes, launches):
+        return {"ms": ms, "algorithmic_bytes": nbytes, "gbs": nbytes / (ms * 1e-3) / 1e9, "frac": nbytes / (ms * 1e-3) / 1e9 / peak,
+                "mparticles_per_s": P / (ms * 1e-3) / 1e6, "launches_per_call": launches}
+
+    EB = (torch.rand((6, N), device=device, generator=g) - 0.5)
+    EB[:3] *= 1e3   # V/m: u changes by ~1e-7 per step, nobody leaves
+    EB[3:] *= 1e-3  # tesla
+    dep_bytes = 29.0 * P + 32.0 * N   # 7 floats + alive per particle; zero-fill and final write-back of the four grids
+    push_bytes = 53.0 * P + 24.0 * N  # 29 B read + 24 B written per particle; every field value read at least once
+    ctxs = {m: J.JefiContext(J.GridSpec(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt, H=2), device=device,
+                             field_impl=J.JEFI_FIELD_REFERENCE, deposit_mode=getattr(J, "JEFI_DEPOSIT_" + m))
+            for m in ("DIRECT", "RUNS", "SORTED")}
+    part = {k: torch.from_numpy(v).to(device) for k, v in part_h.items()}
+    for order in ("caller_order", "cell_sorted"):
+        if order == "cell_sorted":
+            c0 = ctxs["RUNS"]
+            scratch = {k: v.clone() for k, v in part.items()}
+            c0.sort_particles(scratch)  # allocates the scratch
+            l0 = c0.launch_count()
+            ms = timed(lambda: c0.sort_particles(part))
+            # keys 13 B in + 8 out; scatter 8 in + 4 out; gather 4 + 37 in, 37 out; copy back 37 in + 37 out
+            out["kernels"]["sort_particles"] = entry(ms, 222.0 * P, (c0.launch_count() - l0) // (reps + 1))
+            del scratch
+        for m, extra in (("DIRECT", 0.0), ("RUNS", 0.0), ("SORTED", 41.0)):
+            if order == "cell_sorted" and m == "SORTED":
+                continue
+            ctx = ctxs[m]
+            l0 = ctx.launch_count()
+            ms = timed(lambda: ctx.deposit(part))
+            out["kernels"][f"deposit_{m.lower()}_{order}"] = entry(ms, dep_bytes + extra * P, (ctx.launch_count() - l0) // (reps + 1))
+        pp = {k: v.clone() for k, v in part.items()}
+        ms = timed(lambda: ctxs["RUNS"].push_particles(pp, EB))
+        out["kernels"][f"push_{order}"] = entry(ms, push_bytes, 1)
+        del pp
+    for ctx in ctxs.values():
+        ctx.close()
+    del part
+    del flush
+    torch.cuda.empty_cache()
     return out
 
 
@@ -293,11 +372,15 @@ def run_product(args, w: wl.Workload) -> dict:
                "gpu_launches": int(launches), "clocks": clocks}
         if not args.no_pic and world == 1:
             out["pic"] = []
-            for cfgno, st, wu in ((1, 64, 5), (2, 20, 3), (3, 10, 3)):
+            for cfgno, st, wu in ((1, 64, 5), (2, 20, 3), (3, 10, 3), (5, 3, 1)):
                 try:
                     out["pic"].append(time_pic(J, torch, device, cfgno, st, wu))
                 except Exception as e:  # noqa: BLE001
                     out["pic"].append({"workload": wl.WORKLOADS[cfgno].name, "error": str(e)})
+            try:
+                out["particle_kernels"] = time_particle_kernels(J, torch, device)
+            except Exception as e:  # noqa: BLE001
+                out["particle_kernels"] = {"error": str(e)}
         if keep_host:
             import oracle
 
@@ -322,13 +405,21 @@ def main():
     ap.add_argument("--workload", type=int, default=4, help="BASELINE.json config number of the field workload (4 = 96^3)")
     ap.add_argument("--no-pic", action="store_true", help="skip the PIC steps/s legs on configs 1-3")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--particles-only", action="store_true", help="only the deposit/push HBM-roofline leg (for ncu captures)")
     ap.add_argument("--cpu-obs", type=int, default=4096, help="observation cells of the cpu_baseline sample")
     ap.add_argument("--ref-obs", type=int, default=1024, help="observation cells per step of --impl reference")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "jefi" else max(args.warmup, 0)
     w = wl.WORKLOADS[args.workload]
     rank = int(os.environ.get("RANK", "0"))
-    if args.impl == "reference":
+    if args.particles_only:
+        import torch
+
+        from paper_2209_07944_b200 import jefi as J
+
+        J.load_library()
+        res = time_particle_kernels(J, torch, torch.device("cuda:0"), reps=max(1, args.steps))
+    elif args.impl == "reference":
         if rank != 0:
             return  # rank 0 alone runs the CPU oracle
         res = run_reference(args, w)

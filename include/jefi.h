@@ -39,6 +39,13 @@ extern "C" {
 #define JEFI_FIELD_REFERENCE 1 /* one thread per observation cell, table-driven delays (slow; the paper's K1 in fp32) */
 #define JEFI_FIELD_TILED 2     /* shared-memory tiled kernel; jefi_create fails with JEFI_ESTATE if not provable */
 
+/* deposit_mode values */
+#define JEFI_DEPOSIT_AUTO 0   /* = JEFI_DEPOSIT_RUNS (the measured best on sorted and unsorted lists) */
+#define JEFI_DEPOSIT_DIRECT 1 /* caller's order; lanes of a warp that hit the same node are combined wherever they sit (match-any) */
+#define JEFI_DEPOSIT_SORTED 2 /* internal counting sort by cell (context scratch, every call), then JEFI_DEPOSIT_RUNS over that order */
+#define JEFI_DEPOSIT_RUNS 3   /* caller's order; runs of neighbouring lanes in the same cell are combined by a segmented shuffle
+                                 reduction: one reduction per (warp, cell, node) when the list is cell-sorted (jefi_sort_particles) */
+
 typedef struct jefi_ctx jefi_ctx; /* opaque */
 
 typedef struct {
@@ -54,6 +61,7 @@ typedef struct {
   int device;           /* CUDA device ordinal */
   void* stream;         /* cudaStream_t; NULL -> default stream */
   int field_impl;       /* JEFI_FIELD_* */
+  int deposit_mode;     /* JEFI_DEPOSIT_* */
 } jefi_config;
 
 /* Create a context: allocates the ring (32*H*N_padded bytes, zeroed = "zero before t0"), builds the
@@ -80,10 +88,20 @@ int jefi_get_info(const jefi_ctx* ctx, int* H, int* ndt, int* field_impl, long* 
  *   rho,jx,jy,jz  OUT, N floats each (C/m^3, A/m^2), overwritten (zeroed by the call).
  * Node (i,j,k) = floor(xi-.5) ... gets q*w/dV with the 8 trilinear weights; nodes outside the grid are virtual
  * and dropped.  Sums are fp32 atomics: the order of equal-cell particles is not defined.
- * The caller's particle arrays are not modified. */
+ * The caller's particle arrays are never modified: with JEFI_DEPOSIT_SORTED the cell order is an index array in
+ * context scratch (12 bytes per particle + 8 bytes per cell, allocated on first use).  np < 2^31. */
 int jefi_deposit(jefi_ctx* ctx, long np, const float* x, const float* y, const float* z, const float* ux,
                  const float* uy, const float* uz, const float* qw, const unsigned char* alive, float* rho,
                  float* jx, float* jy, float* jz);
+
+/* Put the caller's particle arrays in cell order, in place: first the depositing particles (alive, at least one node
+ * inside the grid) grouped by base node (i,j,k) = floor(xi-.5).. with i fastest, then all others.  The order inside a
+ * group is not defined.  Optional for correctness (no call depends on the order), it is what makes the warp-level
+ * combination of jefi_deposit and the field gathers of jefi_push_particles coalesce; particles move at most c dt per
+ * step, so sorting every few steps is enough.  All of x..alive are IN/OUT np-element arrays; tag is an optional
+ * (NULL ok) int array permuted along with them, e.g. particle ids.  Uses context scratch (53 bytes per particle). */
+int jefi_sort_particles(jefi_ctx* ctx, long np, float* x, float* y, float* z, float* ux, float* uy, float* uz,
+                        float* qw, float* q_over_m, unsigned char* alive, int* tag);
 
 /* Store the sources of the next step: n += 1, ring slot n mod H <- (rho, J) and their backward differences
  * against step n-1 (the finite differences of Eqs. 2.4-2.5; zero history before step 0).
@@ -127,6 +145,11 @@ int jefi_debug_delay_table(jefi_ctx* ctx, int* m_out_host);
 /* Node index (i,j,k) = floor(xi - .5) of each particle as the deposit/push kernels compute it:
  * ijk_out = DEVICE int array [np][3]. */
 int jefi_debug_cell_index(jefi_ctx* ctx, long np, const float* x, const float* y, const float* z, int* ijk_out);
+/* The cell order that JEFI_DEPOSIT_SORTED and jefi_sort_particles use for these positions: order_out = DEVICE int
+ * array [np], a permutation of 0..np-1 whose first *n_alive_host entries are the depositing particles grouped by base
+ * node (i fastest, then j, then k); the order inside a group is not defined.  n_alive_host is a HOST long. */
+int jefi_debug_cell_order(jefi_ctx* ctx, long np, const float* x, const float* y, const float* z,
+                          const unsigned char* alive, int* order_out, long* n_alive_host);
 /* The stored sources of step n - steps_back: out4N = DEVICE float array [4][N] = rho, Jx, Jy, Jz (J rescaled
  * back to A/m^2).  JEFI_EINVAL if that step is not in the ring. */
 int jefi_debug_history_slot(jefi_ctx* ctx, int steps_back, float* out4N);

@@ -38,7 +38,7 @@ extern "C" int jefi_create(const jefi_config* cfg, jefi_ctx** out) {
   if (out) *out = nullptr;
   if (!cfg || !out) return fail_create(nullptr, JEFI_EINVAL, "jefi_create: NULL argument");
   if (cfg->nx < 1 || cfg->ny < 1 || cfg->nz < 1 || !(cfg->dx > 0) || !(cfg->dy > 0) || !(cfg->dz > 0) || !(cfg->dt > 0) ||
-      cfg->c < 0 || cfg->eps0 < 0 || cfg->H < 0 || cfg->hist_cap < 0)
+      cfg->c < 0 || cfg->eps0 < 0 || cfg->H < 0 || cfg->hist_cap < 0 || cfg->deposit_mode < 0 || cfg->deposit_mode > 3)
     return fail_create(nullptr, JEFI_EINVAL, "jefi_create: grid sizes, spacings and dt must be positive");
   if ((long)cfg->nx * cfg->ny * cfg->nz > (1L << 30)) return fail_create(nullptr, JEFI_EINVAL, "jefi_create: grid too large");
   jefi_ctx* c = new (std::nothrow) jefi_ctx();
@@ -49,6 +49,10 @@ extern "C" int jefi_create(const jefi_config* cfg, jefi_ctx** out) {
   c->mtab_host = nullptr;
   c->src_stage = c->eb_stage = nullptr;
   c->perm = nullptr;
+  c->sort_count = c->sort_offset = c->sort_sums = nullptr;
+  c->sort_key = c->sort_rank = c->sort_order = nullptr;
+  c->sort_cap = 0;
+  c->sort_buf = nullptr;
   c->ev0 = c->ev1 = nullptr;
   c->ev_valid = false;
   c->launches = 0;
@@ -146,6 +150,13 @@ extern "C" void jefi_destroy(jefi_ctx* c) {
   if (c->perm) cudaFree(c->perm);
   if (c->src_stage) cudaFree(c->src_stage);
   if (c->eb_stage) cudaFree(c->eb_stage);
+  if (c->sort_count) cudaFree(c->sort_count);
+  if (c->sort_offset) cudaFree(c->sort_offset);
+  if (c->sort_sums) cudaFree(c->sort_sums);
+  if (c->sort_key) cudaFree(c->sort_key);
+  if (c->sort_rank) cudaFree(c->sort_rank);
+  if (c->sort_order) cudaFree(c->sort_order);
+  if (c->sort_buf) cudaFree(c->sort_buf);
   if (c->mtab_host) free(c->mtab_host);
   if (c->ev0) cudaEventDestroy(c->ev0);
   if (c->ev1) cudaEventDestroy(c->ev1);

@@ -73,7 +73,12 @@ struct jefi_ctx {
   int chunk;            // source tiles per CTA (blockIdx.y splits the source range; > 1 split -> atomic output)
   unsigned short* perm; // evaluation order of the 512 cells of an observation tile per relative tile offset
   int ndx, ndy, ndz;
-  // particles scratch
+  // cell-sorted deposit scratch (jefi_particles.cu)
+  unsigned *sort_count, *sort_offset, *sort_sums;  // per-bin counts, exclusive offsets, scan tile sums (+ grand total)
+  int *sort_key, *sort_rank, *sort_order;          // per particle
+  long sort_cap;
+  void* sort_buf;                                  // jefi_sort_particles: permuted copies of the caller's arrays
+  // host-variant staging
   float* src_stage;     // 4N floats, device staging of jefi_field_step_host
   float* eb_stage;      // 6N floats
   // bookkeeping

@@ -73,12 +73,205 @@ __global__ void __launch_bounds__(256) k_deposit(int nx, int ny, int nz, float i
   }
 }
 
+// ------------------------------------------------------------------------------------------------------------
+// cell-sorted deposit (internal order; the caller's arrays are never permuted).
+//
+//   k_sort_keys     key = base node (i+1, j+1, k+1) of Eq. (2.15) linearised over (nx+1)(ny+1)(nz+1) bins; an atomic
+//                   counter per bin hands every alive particle its rank inside the bin
+//   exclusive scan  of the bin counts (three small kernels)
+//   k_sort_scatter  order[offset[key] + rank] = particle
+//   k_deposit_sorted  thread t takes particle order[t]; lanes with equal keys are contiguous, so the 8 x 4 node
+//                   contributions are combined with a segmented shuffle reduction (5 steps) and only the first lane
+//                   of every run issues the fp32 reductions: one per (warp, cell, node, quantity).
+// ------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_sort_keys(int nx, int ny, int nz, int nbins, long np, const float* __restrict__ x,
+                                                   const float* __restrict__ y, const float* __restrict__ z,
+                                                   const unsigned char* __restrict__ alive, int* __restrict__ key,
+                                                   int* __restrict__ rank, unsigned* __restrict__ count) {
+  long p = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= np) return;
+  int kk = nbins, r = 0;  // extra last bin: dead particles and particles with no node inside the grid
+  if (alive == nullptr || alive[p] != 0) {
+    int i, j, k;
+    float a;
+    cic_cell(x[p], i, a); cic_cell(y[p], j, a); cic_cell(z[p], k, a);
+    // alive particles have xi in [0, n): i in [-1, n-1].  A particle outside that range has all 8 nodes outside the
+    // grid (virtual): it deposits nothing and is left out of the order.
+    if (i >= -1 && i < nx && j >= -1 && j < ny && k >= -1 && k < nz) kk = (i + 1) + (nx + 1) * ((j + 1) + (ny + 1) * (k + 1));
+  }
+  r = (int)atomicAdd(count + kk, 1u);
+  key[p] = kk;
+  rank[p] = r;
+}
+
+constexpr int SCAN_ITEMS = 8, SCAN_THREADS = 256, SCAN_TILE = SCAN_ITEMS * SCAN_THREADS;
+
+// exclusive scan of one tile of SCAN_TILE counts; tile total -> sums[blockIdx.x]
+__global__ void __launch_bounds__(SCAN_THREADS) k_scan_tiles(const unsigned* __restrict__ in, unsigned* __restrict__ out, long n,
+                                                             unsigned* __restrict__ sums) {
+  __shared__ unsigned warp_tot[SCAN_THREADS / 32];
+  const long base = (long)blockIdx.x * SCAN_TILE + (long)threadIdx.x * SCAN_ITEMS;
+  unsigned v[SCAN_ITEMS], t = 0;
+#pragma unroll
+  for (int i = 0; i < SCAN_ITEMS; i++) { v[i] = base + i < n ? in[base + i] : 0u; t += v[i]; }
+  const unsigned lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  unsigned inc = t;
+#pragma unroll
+  for (int s = 1; s < 32; s <<= 1) { unsigned o = __shfl_up_sync(0xffffffffu, inc, s); if (lane >= (unsigned)s) inc += o; }
+  if (lane == 31) warp_tot[warp] = inc;
+  __syncthreads();
+  unsigned woff = 0;
+  for (unsigned w = 0; w < warp; w++) woff += warp_tot[w];
+  unsigned run = woff + inc - t;
+#pragma unroll
+  for (int i = 0; i < SCAN_ITEMS; i++) { if (base + i < n) out[base + i] = run; run += v[i]; }
+  if (threadIdx.x == SCAN_THREADS - 1) sums[blockIdx.x] = woff + inc;
+}
+// exclusive scan of the tile totals in one block (ntiles <= a few thousand); grand total -> sums[ntiles]
+__global__ void __launch_bounds__(1024) k_scan_sums(unsigned* __restrict__ sums, int ntiles) {
+  __shared__ unsigned warp_tot[32];
+  __shared__ unsigned carry;
+  if (threadIdx.x == 0) carry = 0;
+  __syncthreads();
+  const unsigned lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  for (int b0 = 0; b0 < ntiles; b0 += 1024) {
+    const int i = b0 + threadIdx.x;
+    const unsigned t = i < ntiles ? sums[i] : 0u;
+    unsigned inc = t;
+#pragma unroll
+    for (int s = 1; s < 32; s <<= 1) { unsigned o = __shfl_up_sync(0xffffffffu, inc, s); if (lane >= (unsigned)s) inc += o; }
+    if (lane == 31) warp_tot[warp] = inc;
+    __syncthreads();
+    unsigned woff = 0;
+    for (unsigned w = 0; w < warp; w++) woff += warp_tot[w];
+    const unsigned c0 = carry;
+    if (i < ntiles) sums[i] = c0 + woff + inc - t;
+    __syncthreads();
+    if (threadIdx.x == 1023) carry = c0 + woff + inc;
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) sums[ntiles] = carry;
+}
+__global__ void __launch_bounds__(256) k_scan_add(unsigned* __restrict__ out, long n, const unsigned* __restrict__ sums) {
+  long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) out[i] += sums[i / SCAN_TILE];
+}
+
+__global__ void __launch_bounds__(256) k_sort_scatter(long np, const int* __restrict__ key, const int* __restrict__ rank,
+                                                      const unsigned* __restrict__ offset, int* __restrict__ order) {
+  long p = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= np) return;
+  order[offset[key[p]] + (unsigned)rank[p]] = (int)p;
+}
+
+__global__ void __launch_bounds__(256) k_deposit_sorted(int nx, int ny, int nz, float inv_dV, float cc, long np,
+                                                        const unsigned* __restrict__ n_alive, const int* __restrict__ order,
+                                                        const unsigned char* __restrict__ alive, const float* __restrict__ x,
+                                                        const float* __restrict__ y, const float* __restrict__ z,
+                                                        const float* __restrict__ ux, const float* __restrict__ uy,
+                                                        const float* __restrict__ uz, const float* __restrict__ qw,
+                                                        float* __restrict__ rho, float* __restrict__ jx,
+                                                        float* __restrict__ jy, float* __restrict__ jz) {
+  const long t = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  const long na = order ? (long)*n_alive : np;
+  if (((long)blockIdx.x * blockDim.x + (threadIdx.x & ~31)) >= na) return;  // whole warp beyond the last particle
+  bool live = t < na;
+  const unsigned FULL = 0xffffffffu, lane = threadIdx.x & 31;
+  int i = 0, j = 0, k = 0, kk = -2 - (int)lane;  // padding lanes: unique keys, never merged
+  float al = 0, be = 0, ch = 0, r0 = 0, vx = 0, vy = 0, vz = 0;
+  long p = t;
+  if (live) {
+    if (order) p = order[t];
+    else live = alive == nullptr || alive[p] != 0;
+  }
+  if (live) {
+    cic_cell(x[p], i, al); cic_cell(y[p], j, be); cic_cell(z[p], k, ch);
+    kk = (i + 1) + (nx + 1) * ((j + 1) + (ny + 1) * (k + 1));  // distinct (i,j,k) in [-1, n) give distinct keys; anything
+                                                                // outside that range has no node in the grid (dropped below)
+    float u0 = ux[p], u1 = uy[p], u2 = uz[p];
+    float ig = rsqrtf(1.f + u0 * u0 + u1 * u1 + u2 * u2);
+    vx = cc * u0 * ig; vy = cc * u1 * ig; vz = cc * u2 * ig;
+    r0 = qw[p] * inv_dV;
+  }
+  // run structure of the warp: a run = maximal stretch of neighbouring lanes with the same key (in a cell-sorted list, all
+  // particles of the cell that fall in this warp; in an unsorted list mostly single lanes)
+  const int kprev = __shfl_up_sync(FULL, kk, 1);
+  const bool head = lane == 0 || kprev != kk;
+  const unsigned heads = __ballot_sync(FULL, head);
+  const unsigned above = heads & ~((2u << lane) - 1u);         // run heads strictly above this lane
+  const unsigned run_end = above ? (unsigned)__ffs(above) - 2u : 31u;  // last lane of this lane's run
+  bool same[5];
+#pragma unroll
+  for (int s = 0; s < 5; s++) same[s] = lane + (1u << s) <= run_end;
+#pragma unroll
+  for (int c3 = 0; c3 < 8; c3++) {
+    const int a = c3 & 1, b = (c3 >> 1) & 1, c = c3 >> 2;
+    const float w = (a ? al : 1.f - al) * (b ? be : 1.f - be) * (c ? ch : 1.f - ch);
+    float a0 = r0 * w, a1 = a0 * vx, a2 = a0 * vy, a3 = a0 * vz;
+#pragma unroll
+    for (int s = 0; s < 5; s++) {  // segmented suffix sum: the head of a run ends up with the run total
+      const float b0 = __shfl_down_sync(FULL, a0, 1u << s), b1 = __shfl_down_sync(FULL, a1, 1u << s);
+      const float b2 = __shfl_down_sync(FULL, a2, 1u << s), b3 = __shfl_down_sync(FULL, a3, 1u << s);
+      if (same[s]) { a0 += b0; a1 += b1; a2 += b2; a3 += b3; }
+    }
+    const int ii = i + a, jj = j + b, kz = k + c;
+    if (live && head && ii >= 0 && ii < nx && jj >= 0 && jj < ny && kz >= 0 && kz < nz) {  // virtual nodes dropped
+      const long node = (long)ii + (long)nx * ((long)jj + (long)ny * kz);
+      atomicAdd(rho + node, a0); atomicAdd(jx + node, a1); atomicAdd(jy + node, a2); atomicAdd(jz + node, a3);
+    }
+  }
+}
+
+static inline long sort_bins(const jefi_dims& d) { return (long)(d.nx + 1) * (d.ny + 1) * (d.nz + 1); }
+
+static int ensure_sort_scratch(jefi_ctx* c, long np) {
+  const long nb = sort_bins(c->dims) + 1;  // + the bin of the non-depositing particles
+  const long ntiles = (nb + SCAN_TILE - 1) / SCAN_TILE;
+  if (!c->sort_count) {
+    JEFI_CUDA_TRY(c, cudaMalloc(&c->sort_count, (size_t)nb * sizeof(unsigned)));
+    JEFI_CUDA_TRY(c, cudaMalloc(&c->sort_offset, (size_t)nb * sizeof(unsigned)));
+    JEFI_CUDA_TRY(c, cudaMalloc(&c->sort_sums, (size_t)(ntiles + 1) * sizeof(unsigned)));
+  }
+  if (np > c->sort_cap) {
+    if (c->sort_key) { cudaFree(c->sort_key); cudaFree(c->sort_rank); cudaFree(c->sort_order); }
+    if (c->sort_buf) cudaFree(c->sort_buf);
+    c->sort_key = c->sort_rank = c->sort_order = nullptr;
+    c->sort_buf = nullptr;
+    c->sort_cap = 0;
+    JEFI_CUDA_TRY(c, cudaMalloc(&c->sort_key, (size_t)np * sizeof(int)));
+    JEFI_CUDA_TRY(c, cudaMalloc(&c->sort_rank, (size_t)np * sizeof(int)));
+    JEFI_CUDA_TRY(c, cudaMalloc(&c->sort_order, (size_t)np * sizeof(int)));
+    c->sort_cap = np;
+  }
+  return JEFI_OK;
+}
+
+// Builds c->sort_order: the depositing particles grouped by base node, then everything else (dead, or with no node in
+// the grid).  The number of depositing particles is the offset of the last bin, c->sort_offset[sort_bins].
+static int build_cell_order(jefi_ctx* c, long np, const float* x, const float* y, const float* z, const unsigned char* alive) {
+  const jefi_dims& d = c->dims;
+  int rc = ensure_sort_scratch(c, np);
+  if (rc != JEFI_OK) return rc;
+  const long nbins = sort_bins(d), nb = nbins + 1;
+  const int ntiles = (int)((nb + SCAN_TILE - 1) / SCAN_TILE);
+  const unsigned pb = (unsigned)((np + 255) / 256);
+  JEFI_CUDA_TRY(c, cudaMemsetAsync(c->sort_count, 0, (size_t)nb * sizeof(unsigned), c->stream));
+  k_sort_keys<<<pb, 256, 0, c->stream>>>(d.nx, d.ny, d.nz, (int)nbins, np, x, y, z, alive, c->sort_key, c->sort_rank, c->sort_count);
+  k_scan_tiles<<<ntiles, SCAN_THREADS, 0, c->stream>>>(c->sort_count, c->sort_offset, nb, c->sort_sums);
+  k_scan_sums<<<1, 1024, 0, c->stream>>>(c->sort_sums, ntiles);
+  k_scan_add<<<(unsigned)((nb + 255) / 256), 256, 0, c->stream>>>(c->sort_offset, nb, c->sort_sums);
+  k_sort_scatter<<<pb, 256, 0, c->stream>>>(np, c->sort_key, c->sort_rank, c->sort_offset, c->sort_order);
+  JEFI_CUDA_TRY(c, cudaGetLastError());
+  c->launches += 5;
+  return JEFI_OK;
+}
+
 extern "C" int jefi_deposit(jefi_ctx* c, long np, const float* x, const float* y, const float* z, const float* ux,
                             const float* uy, const float* uz, const float* qw, const unsigned char* alive, float* rho,
                             float* jx, float* jy, float* jz) {
   if (!c) return JEFI_EINVAL;
-  if (np < 0 || !rho || !jx || !jy || !jz || (np > 0 && (!x || !y || !z || !ux || !uy || !uz || !qw))) {
-    c->err = "jefi_deposit: NULL array or negative np";
+  if (np < 0 || np > 0x7fffffffL || !rho || !jx || !jy || !jz || (np > 0 && (!x || !y || !z || !ux || !uy || !uz || !qw))) {
+    c->err = "jefi_deposit: NULL array or np out of range";
     return JEFI_EINVAL;
   }
   const jefi_dims& d = c->dims;
@@ -89,10 +282,92 @@ extern "C" int jefi_deposit(jefi_ctx* c, long np, const float* x, const float* y
   if (np == 0) return JEFI_OK;
   float inv_dV = (float)(1.0 / (c->cfg.dx * c->cfg.dy * c->cfg.dz));
   unsigned blocks = (unsigned)((np + 255) / 256);
-  k_deposit<<<blocks, 256, 0, c->stream>>>(d.nx, d.ny, d.nz, inv_dV, (float)c->c, np, x, y, z, ux, uy, uz, qw, alive, rho, jx,
-                                           jy, jz);
+  int mode = c->cfg.deposit_mode;
+  if (mode == JEFI_DEPOSIT_AUTO) mode = JEFI_DEPOSIT_RUNS;  // cheapest on sorted and unsorted lists alike
+  if (mode == JEFI_DEPOSIT_SORTED) {
+    int rc = build_cell_order(c, np, x, y, z, alive);
+    if (rc != JEFI_OK) return rc;
+    k_deposit_sorted<<<blocks, 256, 0, c->stream>>>(d.nx, d.ny, d.nz, inv_dV, (float)c->c, np, c->sort_offset + sort_bins(d),
+                                                    c->sort_order, alive, x, y, z, ux, uy, uz, qw, rho, jx, jy, jz);
+  } else if (mode == JEFI_DEPOSIT_RUNS) {
+    k_deposit_sorted<<<blocks, 256, 0, c->stream>>>(d.nx, d.ny, d.nz, inv_dV, (float)c->c, np, nullptr, nullptr, alive, x, y, z,
+                                                    ux, uy, uz, qw, rho, jx, jy, jz);
+  } else {
+    k_deposit<<<blocks, 256, 0, c->stream>>>(d.nx, d.ny, d.nz, inv_dV, (float)c->c, np, x, y, z, ux, uy, uz, qw, alive, rho, jx,
+                                             jy, jz);
+  }
   JEFI_CUDA_TRY(c, cudaGetLastError());
   c->launches++;
+  return JEFI_OK;
+}
+
+// The internal cell order for these positions (debug/parity export; synchronises).
+extern "C" int jefi_debug_cell_order(jefi_ctx* c, long np, const float* x, const float* y, const float* z,
+                                     const unsigned char* alive, int* order_out, long* n_alive_host) {
+  if (!c || np < 0 || np > 0x7fffffffL || !n_alive_host || (np > 0 && (!x || !y || !z || !order_out))) return JEFI_EINVAL;
+  *n_alive_host = 0;
+  if (np == 0) return JEFI_OK;
+  int rc = build_cell_order(c, np, x, y, z, alive);
+  if (rc != JEFI_OK) return rc;
+  unsigned na = 0;
+  JEFI_CUDA_TRY(c, cudaMemcpyAsync(&na, c->sort_offset + sort_bins(c->dims), sizeof na, cudaMemcpyDeviceToHost, c->stream));
+  JEFI_CUDA_TRY(c, cudaMemcpyAsync(order_out, c->sort_order, (size_t)np * sizeof(int), cudaMemcpyDeviceToDevice, c->stream));
+  JEFI_CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  *n_alive_host = (long)na;
+  return JEFI_OK;
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// jefi_sort_particles: the caller asks for its own arrays to be put in cell order (gather through the order into
+// context scratch with coalesced writes, then a coalesced copy back).
+// ------------------------------------------------------------------------------------------------------------
+struct perm_arrays {
+  float* f[8];          // x y z ux uy uz qw qm
+  unsigned char* alive;
+  int* tag;             // may be NULL
+};
+__global__ void __launch_bounds__(256) k_permute_gather(long np, const int* __restrict__ order, perm_arrays A, float* __restrict__ buf,
+                                                        unsigned char* __restrict__ abuf, int* __restrict__ tbuf) {
+  long t = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= np) return;
+  const int p = order[t];
+#pragma unroll
+  for (int a = 0; a < 8; a++) buf[(size_t)a * np + t] = A.f[a][p];
+  abuf[t] = A.alive[p];
+  if (A.tag) tbuf[t] = A.tag[p];
+}
+__global__ void __launch_bounds__(256) k_permute_copyback(long np, perm_arrays A, const float* __restrict__ buf,
+                                                          const unsigned char* __restrict__ abuf, const int* __restrict__ tbuf) {
+  long t = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= np) return;
+#pragma unroll
+  for (int a = 0; a < 8; a++) A.f[a][t] = buf[(size_t)a * np + t];
+  A.alive[t] = abuf[t];
+  if (A.tag) A.tag[t] = tbuf[t];
+}
+
+extern "C" int jefi_sort_particles(jefi_ctx* c, long np, float* x, float* y, float* z, float* ux, float* uy, float* uz, float* qw,
+                                   float* q_over_m, unsigned char* alive, int* tag) {
+  if (!c) return JEFI_EINVAL;
+  if (np < 0 || np > 0x7fffffffL || (np > 0 && (!x || !y || !z || !ux || !uy || !uz || !qw || !q_over_m || !alive))) {
+    c->err = "jefi_sort_particles: NULL array or np out of range";
+    return JEFI_EINVAL;
+  }
+  if (np == 0) return JEFI_OK;
+  int rc = build_cell_order(c, np, x, y, z, alive);
+  if (rc != JEFI_OK) return rc;
+  if (!c->sort_buf) JEFI_CUDA_TRY(c, cudaMalloc(&c->sort_buf, (size_t)c->sort_cap * (8 * sizeof(float) + sizeof(int) + 1) + 64));
+  float* buf = (float*)c->sort_buf;
+  int* tbuf = (int*)(buf + (size_t)8 * c->sort_cap);
+  unsigned char* abuf = (unsigned char*)(tbuf + c->sort_cap);
+  perm_arrays A;
+  A.f[0] = x; A.f[1] = y; A.f[2] = z; A.f[3] = ux; A.f[4] = uy; A.f[5] = uz; A.f[6] = qw; A.f[7] = q_over_m;
+  A.alive = alive; A.tag = tag;
+  const unsigned pb = (unsigned)((np + 255) / 256);
+  k_permute_gather<<<pb, 256, 0, c->stream>>>(np, c->sort_order, A, buf, abuf, tbuf);
+  k_permute_copyback<<<pb, 256, 0, c->stream>>>(np, A, buf, abuf, tbuf);
+  JEFI_CUDA_TRY(c, cudaGetLastError());
+  c->launches += 2;
   return JEFI_OK;
 }
 

@@ -16,11 +16,13 @@ LIB_PATH = os.path.join(_HERE, "libjefi.so")
 
 JEFI_OK, JEFI_EINVAL, JEFI_ENOMEM, JEFI_ECUDA, JEFI_ESTATE = 0, -1, -2, -3, -4
 JEFI_FIELD_AUTO, JEFI_FIELD_REFERENCE, JEFI_FIELD_TILED = 0, 1, 2
+JEFI_DEPOSIT_AUTO, JEFI_DEPOSIT_DIRECT, JEFI_DEPOSIT_SORTED, JEFI_DEPOSIT_RUNS = 0, 1, 2, 3
 
 EXPORTS = [
     "jefi_create", "jefi_destroy", "jefi_last_error", "jefi_get_info", "jefi_deposit", "jefi_push_sources",
     "jefi_field_step", "jefi_push_particles", "jefi_field_step_host", "jefi_launch_count",
     "jefi_last_field_kernel_ms", "jefi_debug_delay_table", "jefi_debug_cell_index", "jefi_debug_history_slot",
+    "jefi_debug_cell_order", "jefi_sort_particles",
 ]
 
 
@@ -35,7 +37,7 @@ class jefi_config(C.Structure):
         ("c", C.c_double), ("eps0", C.c_double),
         ("H", C.c_int), ("hist_cap", C.c_int),
         ("Eext", C.c_double * 3), ("Bext", C.c_double * 3),
-        ("device", C.c_int), ("stream", C.c_void_p), ("field_impl", C.c_int),
+        ("device", C.c_int), ("stream", C.c_void_p), ("field_impl", C.c_int), ("deposit_mode", C.c_int),
     ]
 
 
@@ -79,6 +81,10 @@ def load_library() -> C.CDLL:
     lib.jefi_debug_delay_table.restype = C.c_int
     lib.jefi_debug_cell_index.argtypes = [vp, C.c_long, f32p, f32p, f32p, vp]
     lib.jefi_debug_cell_index.restype = C.c_int
+    lib.jefi_sort_particles.argtypes = [vp, C.c_long] + [f32p] * 8 + [u8p, vp]
+    lib.jefi_sort_particles.restype = C.c_int
+    lib.jefi_debug_cell_order.argtypes = [vp, C.c_long, f32p, f32p, f32p, u8p, vp, C.POINTER(C.c_long)]
+    lib.jefi_debug_cell_order.restype = C.c_int
     lib.jefi_debug_history_slot.argtypes = [vp, C.c_int, f32p]
     lib.jefi_debug_history_slot.restype = C.c_int
     _lib = lib
@@ -110,10 +116,10 @@ def _dev(t, dtype, n: Optional[int], name: str) -> int:
 def jefi_create(nx: int, ny: int, nz: int, dx: float, dy: float, dz: float, dt: float, c: float = 0.0,
                 eps0: float = 0.0, H: int = 0, hist_cap: int = 0, Eext: Sequence[float] = (0, 0, 0),
                 Bext: Sequence[float] = (0, 0, 0), device: int = 0, stream: int = 0,
-                field_impl: int = JEFI_FIELD_AUTO) -> int:
+                field_impl: int = JEFI_FIELD_AUTO, deposit_mode: int = JEFI_DEPOSIT_AUTO) -> int:
     lib = load_library()
     cfg = jefi_config(nx, ny, nz, dx, dy, dz, dt, c, eps0, H, hist_cap, (C.c_double * 3)(*Eext),
-                      (C.c_double * 3)(*Bext), device, C.c_void_p(stream), field_impl)
+                      (C.c_double * 3)(*Bext), device, C.c_void_p(stream), field_impl, deposit_mode)
     h = C.c_void_p()
     rc = lib.jefi_create(C.byref(cfg), C.byref(h))
     if rc != JEFI_OK:
@@ -172,6 +178,17 @@ def jefi_push_particles(handle: int, N: int, x, y, z, ux, uy, uz, q_over_m, aliv
     _check(handle, load_library().jefi_push_particles(handle, np_, *pp, pal, *pf), "jefi_push_particles")
 
 
+def jefi_sort_particles(handle: int, x, y, z, ux, uy, uz, qw, q_over_m, alive, tag=None) -> None:
+    import torch
+
+    f = torch.float32
+    np_ = x.numel()
+    pp = [_dev(t, f, np_, n) for t, n in zip((x, y, z, ux, uy, uz, qw, q_over_m), ("x", "y", "z", "ux", "uy", "uz", "qw", "q_over_m"))]
+    rc = load_library().jefi_sort_particles(handle, np_, *pp, _dev(alive, torch.uint8, np_, "alive"),
+                                            _dev(tag, torch.int32, np_, "tag"))
+    _check(handle, rc, "jefi_sort_particles")
+
+
 def jefi_field_step_host(handle: int, N: int, src_host, eb_host) -> None:
     """src_host: CPU float32 tensor [4*N] (pinned recommended); eb_host: CPU float32 tensor [6*N]."""
     import torch
@@ -197,6 +214,20 @@ def jefi_debug_delay_table(handle: int, nx: int, ny: int, nz: int):
     out = np.empty((nz, ny, nx), dtype=np.int32)
     _check(handle, load_library().jefi_debug_delay_table(handle, out.ctypes.data), "jefi_debug_delay_table")
     return out
+
+
+def jefi_debug_cell_order(handle: int, x, y, z, alive=None):
+    """(order, n_alive): int32 CUDA tensor of the depositing particles in the internal cell order."""
+    import torch
+
+    np_ = x.numel()
+    order = torch.empty(max(np_, 1), dtype=torch.int32, device=x.device)[:np_]
+    na = C.c_long(0)
+    f = torch.float32
+    rc = load_library().jefi_debug_cell_order(handle, np_, _dev(x, f, np_, "x"), _dev(y, f, np_, "y"), _dev(z, f, np_, "z"),
+                                              _dev(alive, torch.uint8, np_, "alive"), order.data_ptr(), C.byref(na))
+    _check(handle, rc, "jefi_debug_cell_order")
+    return order, na.value
 
 
 def jefi_debug_cell_index(handle: int, x, y, z):
@@ -243,7 +274,8 @@ class GridSpec:
 class JefiContext:
     """Owns one jefi_ctx and the E/B/rho/J device tensors of a run; every method is one C-ABI call."""
 
-    def __init__(self, grid: GridSpec, device=None, field_impl: int = JEFI_FIELD_AUTO):
+    def __init__(self, grid: GridSpec, device=None, field_impl: int = JEFI_FIELD_AUTO,
+                 deposit_mode: int = JEFI_DEPOSIT_AUTO, sort_every: int = 0):
         import torch
 
         if not torch.cuda.is_available():
@@ -255,9 +287,11 @@ class JefiContext:
         stream = torch.cuda.current_stream(self.device).cuda_stream
         self.handle = jefi_create(grid.nx, grid.ny, grid.nz, grid.dx, grid.dy, grid.dz, grid.dt, grid.c, grid.eps0,
                                   grid.H, grid.hist_cap, grid.Eext, grid.Bext, self.device.index or 0, stream,
-                                  field_impl)
+                                  field_impl, deposit_mode)
         self.info = jefi_get_info(self.handle)
         self.H = self.info["H"]
+        self.sort_every = int(sort_every)  # pic_step calls jefi_sort_particles every sort_every steps (0 = never)
+        self._pic_steps = 0
         z = lambda k: torch.zeros((k, self.N), dtype=torch.float32, device=self.device)
         self.EB = z(6)   # ex ey ez bx by bz
         self.src = z(4)  # rho jx jy jz
@@ -289,8 +323,17 @@ class JefiContext:
         jefi_push_particles(self.handle, self.N, part["x"], part["y"], part["z"], part["ux"], part["uy"], part["uz"],
                             part["qm"], part["alive"], f[0], f[1], f[2], f[3], f[4], f[5])
 
+    def sort_particles(self, part: dict) -> None:
+        """Cell-sort the particle arrays in place (part["tag"], if present, is permuted along)."""
+        jefi_sort_particles(self.handle, part["x"], part["y"], part["z"], part["ux"], part["uy"], part["uz"], part["qw"],
+                            part["qm"], part["alive"], part.get("tag"))
+
     def pic_step(self, part: dict) -> None:
-        """deposit -> push_sources -> field_step -> push_particles, all on one stream."""
+        """deposit -> push_sources -> field_step -> push_particles, all on one stream; with
+        sort_every > 0 the particle arrays are first put in cell order every sort_every steps (jefi_sort_particles)."""
+        if self.sort_every > 0 and self._pic_steps % self.sort_every == 0:
+            self.sort_particles(part)
+        self._pic_steps += 1
         self.deposit(part)
         self.push_sources()
         self.field_step()

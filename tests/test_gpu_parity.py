@@ -240,6 +240,102 @@ def test_deposit_parity_and_indices(J, shape):
     ctx.close()
 
 
+@pytest.mark.parametrize("shape,count", [((16, 16, 16), 20000), ((13, 10, 7), 50000), ((5, 4, 3), 7), ((8, 8, 8), 300000)])
+def test_deposit_sorted_mode_order_and_parity(J, shape, count):
+    """JEFI_DEPOSIT_SORTED: the internal order is a valid cell sort of exactly the depositing particles (keys compared
+    bit-exactly with the oracle's cell indices; the order inside a cell is free), and the sums match the oracle."""
+    dx = 1e-4
+    dt = dx / (2 * C)
+    cfg = OracleConfig(*shape, dx, dx, dx, dt)
+    g = J.GridSpec(*shape, dx, dx, dx, dt)
+    ctx = J.JefiContext(g, field_impl=J.JEFI_FIELD_REFERENCE, deposit_mode=J.JEFI_DEPOSIT_SORTED)
+    part = edge_particles(min(shape), 5, count)
+    for k, lim in zip("xyz", shape):
+        part[k] = (part[k] * (lim / min(shape))).astype(np.float32)
+        part[k] = np.minimum(part[k], np.nextafter(np.float32(lim), np.float32(0)))
+    dp = to_dev(part, ctx.device)
+    order, na = J.jefi_debug_cell_order(ctx.handle, dp["x"], dp["y"], dp["z"], dp["alive"])
+    order = order.cpu().numpy()
+    P = part["x"].shape[0]
+    alive_idx = np.flatnonzero(part["alive"])
+    assert np.array_equal(np.sort(order), np.arange(P))                          # a permutation of all particles
+    assert na == alive_idx.size and np.array_equal(np.sort(order[:na]), alive_idx)  # depositing particles first
+    idx = oracle.cell_index(part["x"], part["y"], part["z"])                    # [P][3], int
+    key = (idx[:, 0] + 1) + (shape[0] + 1) * ((idx[:, 1] + 1) + (shape[1] + 1) * (idx[:, 2] + 1))
+    assert np.all(np.diff(key[order[:na]]) >= 0)                                  # grouped by cell, ascending
+    S = ctx.deposit(dp).cpu().numpy()
+    So = oracle.deposit(cfg, part["x"], part["y"], part["z"], part["ux"], part["uy"], part["uz"], part["qw"], part["alive"])
+    for a in range(4):
+        assert np.linalg.norm(S[a] - So[a]) <= 1e-5 * np.linalg.norm(So[a]), a
+    assert np.array_equal(S[0] != 0, So[0] != 0)
+    # a second call with fewer particles reuses the scratch; a particle marked alive but outside the grid adds nothing
+    sub = {k: v[:1000].copy() for k, v in part.items()}
+    sub["x"][0] = np.float32(shape[0] + 3.0)
+    sub["alive"][0] = 1
+    S2 = ctx.deposit(to_dev(sub, ctx.device)).cpu().numpy()
+    So2 = oracle.deposit(cfg, sub["x"], sub["y"], sub["z"], sub["ux"], sub["uy"], sub["uz"], sub["qw"], sub["alive"])
+    for a in range(4):
+        assert np.linalg.norm(S2[a] - So2[a]) <= 1e-5 * np.linalg.norm(So2[a]), a
+    ctx.close()
+
+
+def test_deposit_modes_agree_on_config3_particles(J):
+    """1e6 beam electrons of config 3 on the 64^3 grid: direct, sorted and auto deposits against the oracle."""
+    w = wl.WORKLOADS[3]
+    part = wl.particles(3)
+    cfg = OracleConfig(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt)
+    So = oracle.deposit(cfg, part["x"], part["y"], part["z"], part["ux"], part["uy"], part["uz"], part["qw"], part["alive"])
+    for mode in (J.JEFI_DEPOSIT_DIRECT, J.JEFI_DEPOSIT_SORTED, J.JEFI_DEPOSIT_RUNS, J.JEFI_DEPOSIT_AUTO):
+        ctx = J.JefiContext(J.GridSpec(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt), field_impl=J.JEFI_FIELD_REFERENCE, deposit_mode=mode)
+        S = ctx.deposit(to_dev(part, ctx.device)).cpu().numpy()
+        for a in range(4):
+            assert np.linalg.norm(S[a] - So[a]) <= 1e-5 * np.linalg.norm(So[a]), (mode, a)
+        ctx.close()
+
+
+@pytest.mark.parametrize("mode", ["DIRECT", "RUNS"])
+def test_sort_particles_in_place(J, mode):
+    """jefi_sort_particles permutes all arrays consistently (checked through the tag), groups the depositing particles
+    by cell, and changes neither the deposit (to summation order) nor any particle's push (bit for bit)."""
+    import torch
+
+    shape, dx = (13, 10, 7), 1e-4
+    dt = dx / (2 * C)
+    cfg = OracleConfig(*shape, dx, dx, dx, dt)
+    ctx = J.JefiContext(J.GridSpec(*shape, dx, dx, dx, dt), field_impl=J.JEFI_FIELD_REFERENCE,
+                        deposit_mode=getattr(J, "JEFI_DEPOSIT_" + mode))
+    part = edge_particles(min(shape), 21, 40000)
+    for k, lim in zip("xyz", shape):
+        part[k] = (part[k] * (lim / min(shape))).astype(np.float32)
+        part[k] = np.minimum(part[k], np.nextafter(np.float32(lim), np.float32(0)))
+    P = part["x"].shape[0]
+    dp = to_dev(part, ctx.device)
+    dp["tag"] = torch.arange(P, dtype=torch.int32, device=ctx.device)
+    ctx.sort_particles(dp)
+    tag = dp["tag"].cpu().numpy()
+    assert np.array_equal(np.sort(tag), np.arange(P))
+    for k, v in part.items():
+        assert np.array_equal(dp[k].cpu().numpy(), v[tag]), k  # every array moved with its particle
+    na = int(part["alive"].sum())
+    assert np.all(dp["alive"].cpu().numpy()[:na] == 1) and np.all(dp["alive"].cpu().numpy()[na:] == 0)
+    idx = oracle.cell_index(part["x"], part["y"], part["z"])
+    key = (idx[:, 0] + 1) + (shape[0] + 1) * ((idx[:, 1] + 1) + (shape[1] + 1) * (idx[:, 2] + 1))
+    assert np.all(np.diff(key[tag[:na]]) >= 0)
+    S = ctx.deposit(dp).cpu().numpy()
+    So = oracle.deposit(cfg, part["x"], part["y"], part["z"], part["ux"], part["uy"], part["uz"], part["qw"], part["alive"])
+    for a in range(4):
+        assert np.linalg.norm(S[a] - So[a]) <= 1e-5 * np.linalg.norm(So[a]), a
+    # push: sorted and unsorted copies give bit-identical particles
+    rng = np.random.default_rng(9)
+    EB = torch.from_numpy(rng.normal(0, 1, (6, cfg.N)).astype(np.float32) * np.array([[1e4]] * 3 + [[1e-2]] * 3, dtype=np.float32)).to(ctx.device)
+    du = to_dev(part, ctx.device)
+    ctx.push_particles(du, EB)
+    ctx.push_particles(dp, EB)
+    for k in ("x", "y", "z", "ux", "uy", "uz", "alive"):
+        assert np.array_equal(dp[k].cpu().numpy(), du[k].cpu().numpy()[tag]), k
+    ctx.close()
+
+
 def test_deposit_empty_and_all_dead(J):
     import torch
 
@@ -289,13 +385,18 @@ def test_push_parity_one_step_with_external_fields(J):
 
 
 # ------------------------------------------------------------------------------------------- closed loop (config 1)
-def run_closed_loop(J, config, steps, scale=1.0, impl=None):
+def run_closed_loop(J, config, steps, scale=1.0, impl=None, sort_every=0):
+    import torch
+
     w = wl.WORKLOADS[config]
     part = wl.particles(config, scale)
     cfg = OracleConfig(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt)
     assert cfg.H == w.H
     ctx = make_ctx(J, (w.n,) * 3, (w.dx,) * 3, w.dt, J.JEFI_FIELD_AUTO if impl is None else impl)
+    ctx.sort_every = sort_every
     dp = to_dev(part, ctx.device)
+    if sort_every:
+        dp["tag"] = torch.arange(part["x"].shape[0], dtype=torch.int32, device=ctx.device)
     orc = oracle.OracleJefi(cfg)
     po = {k: v.astype(np.float64) for k, v in part.items() if k != "alive"}
     po["alive"] = part["alive"].copy()
@@ -307,6 +408,9 @@ def run_closed_loop(J, config, steps, scale=1.0, impl=None):
             eb = ctx.EB.cpu().numpy()
             hist.append((s, eb[:3].copy(), eb[3:].copy(), Eo, Bo, ctx.src.cpu().numpy().copy(), So))
     got = {k: v.cpu().numpy() for k, v in dp.items()}
+    if sort_every:  # back to the oracle's particle numbering
+        inv = np.argsort(got.pop("tag"))
+        got = {k: v[inv] for k, v in got.items()}
     ctx.close()
     return w, got, po, hist
 
@@ -321,6 +425,17 @@ def test_closed_loop_config1_10_steps(J):
         assert_field_parity(E, B, Eo, Bo, f"cfg1 step {s}: ")
         for a in range(4):
             assert np.linalg.norm(S[a] - So[a]) <= 1e-5 * max(np.linalg.norm(So[a]), 1e-300)
+
+
+def test_closed_loop_config1_10_steps_with_periodic_cell_sort(J):
+    """Same loop with jefi_sort_particles every 3 steps: trajectories (matched through the tag) keep the 1e-5 bar."""
+    w, got, po, hist = run_closed_loop(J, 1, 10, sort_every=3)
+    both = (got["alive"] == 1) & (po["alive"] == 1)
+    assert (got["alive"] != po["alive"]).sum() <= 1
+    for k in "xyz":
+        assert np.abs(got[k][both] - po[k][both]).max() / w.n <= 1e-5
+    s, E, B, Eo, Bo, S, So = hist[-1]
+    assert_field_parity(E, B, Eo, Bo, "cfg1 step 9 (sorted): ")
 
 
 def test_closed_loop_config1_full_64_steps(J):
