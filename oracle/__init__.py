@@ -10,6 +10,8 @@ from .jefi_oracle import (  # noqa: F401
     OracleJefi,
     build_oracle,
     delay,
+    RULE_NEAREST,
+    RULE_LINEAR,
     delay_table,
     num_dt,
     num_threads,

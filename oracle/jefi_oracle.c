@@ -18,7 +18,8 @@
  *               steps < 0 are zero, steps older than n-(H-1) are not stored and
  *               contribute zero (reading A15).
  *
- * Parity pins: tests/test_oracle_*.py (P1-P15 of SURVEY.md §8(c)); nothing here is "parity unpinned".
+ * Parity pins: tests/test_oracle_*.py (P1-P15 of SURVEY.md §8(c); L1-L5 for the linear retarded-time rule); nothing
+ * here is "parity unpinned".
  */
 #include <math.h>
 #include <stddef.h>
@@ -72,6 +73,16 @@ void orc_delay_table(int nx, int ny, int nz, double dx, double dy, double dz, do
         m_out[ia + (size_t)nx * (jb + (size_t)ny * kc)] = (int32_t)orc_delay(ia * dx, jb * dy, kc * dz, dt, c);
 }
 
+/* Retarded-time rules.  ORC_RULE_NEAREST is reading A1 (the five BASELINE.json configs): sources and derivatives taken
+ * at the stored step nearest to t_r = t^n - R/c.  ORC_RULE_LINEAR is the second rule of SURVEY.md §8(f) NEXT-1 (reading
+ * A22): the VALUES rho(t_r), J(t_r) of Eqs. (2.4)-(2.5) are taken on the straight line through the same
+ * two samples that A1 uses, S(t_r) = S^{n-m} + (t_r - t^{n-m}) (S^{n-m} - S^{n-m-1})/dt with m the nearest step, i.e.
+ * linear interpolation between steps n-m-1 and n-m when t_r falls between them and its continuation by up to dt/2
+ * beyond step n-m otherwise (second-order accurate in dt); the time derivatives stay the paper's finite difference
+ * (S^{n-m} - S^{n-m-1})/dt. */
+#define ORC_RULE_NEAREST 0
+#define ORC_RULE_LINEAR 1
+
 /* ------------------------------------------------------------------------------------------------
  * Field: Eqs. (2.4)-(2.6); self cell skipped; zero before t0 (:217).
  * obs_idx == NULL -> all N cells (nobs must equal N).  E, B are [3][nobs] doubles.
@@ -110,6 +121,11 @@ void orc_delay_table(int nx, int ny, int nz, double dx, double dy, double dz, do
           }                                                                                                  \
           double drho = (rho0 - rho1) / dt;                      /* backward difference, Eq. (2.4) */        \
           double djx = (jx0 - jx1) / dt, djy = (jy0 - jy1) / dt, djz = (jz0 - jz1) / dt; /* Eq. (2.5) */     \
+          if (rule == ORC_RULE_LINEAR) { /* reading A22: S(t_r) = S^{n-m} + (t_r - t^{n-m}) S_dot^{n-m} */   \
+            double tr_minus_tm = ((double)m - s) * dt;           /* t_r = t^n - s dt, t^{n-m} = t^n - m dt */   \
+            rho0 += tr_minus_tm * drho;                                                                      \
+            jx0 += tr_minus_tm * djx; jy0 += tr_minus_tm * djy; jz0 += tr_minus_tm * djz;                    \
+          }                                                                                                  \
           double R3 = R2 * R;                                                                                \
           /* Eq. (2.4): d rho/R^3 + d rho_dot/(c R^2) - J_dot/(c^2 R)   (reading A2) */                      \
           Ex += ddx * rho0 / R3 + ddx * drho / (c * R2) - djx / (c * c * R);                                 \
@@ -127,12 +143,12 @@ void orc_delay_table(int nx, int ny, int nz, double dx, double dy, double dz, do
     B[o] = prefB * Bx; B[nobs + o] = prefB * By; B[2 * nobs + o] = prefB * Bz;                               \
   }
 
-void orc_field_f64(int nx, int ny, int nz, double dx, double dy, double dz, double dt, double c, double eps0,
+void orc_field_f64(int nx, int ny, int nz, double dx, double dy, double dz, double dt, double c, double eps0, int rule,
                    long n, long H, const double* ring, long nobs, const int64_t* obs_idx, double* E, double* B) {
   ORC_FIELD_BODY(double)
 }
 
-void orc_field_f32(int nx, int ny, int nz, double dx, double dy, double dz, double dt, double c, double eps0,
+void orc_field_f32(int nx, int ny, int nz, double dx, double dy, double dz, double dt, double c, double eps0, int rule,
                    long n, long H, const float* ring, long nobs, const int64_t* obs_idx, double* E, double* B) {
   ORC_FIELD_BODY(float)
 }

@@ -22,6 +22,7 @@ _LIB = os.path.join(_HERE, "libjefi_oracle.so")
 # Reading A18: SI constants used when the config leaves c / eps0 at 0.
 C_SI = 299792458.0
 EPS0_SI = 8.8541878128e-12
+RULE_NEAREST, RULE_LINEAR = 0, 1
 
 
 def build_oracle(force: bool = False) -> str:
@@ -50,7 +51,7 @@ def _L():
         lib.orc_delay.argtypes = [dbl, dbl, dbl, dbl, dbl]
         lib.orc_delay_table.argtypes = [i32, i32, i32, dbl, dbl, dbl, dbl, dbl, p]
         for name in ("orc_field_f64", "orc_field_f32"):
-            getattr(lib, name).argtypes = [i32, i32, i32, dbl, dbl, dbl, dbl, dbl, dbl, i64, i64, p, i64, p, p, p]
+            getattr(lib, name).argtypes = [i32, i32, i32, dbl, dbl, dbl, dbl, dbl, dbl, i32, i64, i64, p, i64, p, p, p]
             getattr(lib, name).restype = None
         lib.orc_cell_index.argtypes = [i64, p, p, p, p]
         lib.orc_deposit.argtypes = [i32, i32, i32, dbl, dbl, dbl, dbl, i64] + [p] * 12
@@ -85,6 +86,7 @@ class OracleConfig:
     hist_cap: int = 10000
     Eext: Sequence[float] = (0.0, 0.0, 0.0)
     Bext: Sequence[float] = (0.0, 0.0, 0.0)
+    delay_rule: int = 0  # RULE_NEAREST (reading A1) or RULE_LINEAR (reading A22)
 
     def __post_init__(self):
         if self.H == 0:
@@ -122,8 +124,9 @@ def delay_table(cfg: OracleConfig) -> np.ndarray:
     return out
 
 
-def field(cfg: OracleConfig, n: int, ring: np.ndarray, obs_idx: Optional[np.ndarray] = None):
+def field(cfg: OracleConfig, n: int, ring: np.ndarray, obs_idx: Optional[np.ndarray] = None, rule: Optional[int] = None):
     """E, B at step n (Eqs. 2.4-2.6).  ring: [H][4][N] float64 or float32, slot = step mod H.
+    rule: RULE_NEAREST / RULE_LINEAR (default: cfg.delay_rule).
 
     Returns (E, B), each float64 [3][nobs]; obs_idx None -> all cells.
     """
@@ -138,7 +141,8 @@ def field(cfg: OracleConfig, n: int, ring: np.ndarray, obs_idx: Optional[np.ndar
     E = np.empty((3, nobs), dtype=np.float64)
     B = np.empty((3, nobs), dtype=np.float64)
     fn = {np.dtype(np.float64): _L().orc_field_f64, np.dtype(np.float32): _L().orc_field_f32}[ring.dtype]
-    fn(cfg.nx, cfg.ny, cfg.nz, cfg.dx, cfg.dy, cfg.dz, cfg.dt, cfg.c, cfg.eps0, int(n), int(H), _ptr(ring),
+    fn(cfg.nx, cfg.ny, cfg.nz, cfg.dx, cfg.dy, cfg.dz, cfg.dt, cfg.c, cfg.eps0, int(cfg.delay_rule if rule is None else rule),
+       int(n), int(H), _ptr(ring),
        int(nobs), _ptr(idx), _ptr(E), _ptr(B))
     return E, B
 
