@@ -46,6 +46,12 @@ extern "C" {
 #define JEFI_DEPOSIT_RUNS 3   /* caller's order; runs of neighbouring lanes in the same cell are combined by a segmented shuffle
                                  reduction: one reduction per (warp, cell, node) when the list is cell-sorted (jefi_sort_particles) */
 
+/* delay_rule values: how the retarded time t_r = t^n - R/c of Eq. (2.6), which is not a stored step, is served */
+#define JEFI_DELAY_NEAREST 0 /* sources and differences at the nearest stored step, m = floor(R/(c dt) + 1/2) (A1) */
+#define JEFI_DELAY_LINEAR 1  /* same m and the same two samples; the VALUES rho, J are taken on the straight line through
+                                them, S(t_r) = S^{n-m} - phi (S^{n-m} - S^{n-m-1}), phi = R/(c dt) - m in [-1/2, 1/2)
+                                (second order in dt); the time derivatives stay (S^{n-m} - S^{n-m-1})/dt (A22) */
+
 typedef struct jefi_ctx jefi_ctx; /* opaque */
 
 typedef struct {
@@ -62,6 +68,7 @@ typedef struct {
   void* stream;         /* cudaStream_t; NULL -> default stream */
   int field_impl;       /* JEFI_FIELD_* */
   int deposit_mode;     /* JEFI_DEPOSIT_* */
+  int delay_rule;       /* JEFI_DELAY_* */
 } jefi_config;
 
 /* Create a context: allocates the ring (32*H*N_padded bytes, zeroed = "zero before t0"), builds the

@@ -38,7 +38,7 @@ extern "C" int jefi_create(const jefi_config* cfg, jefi_ctx** out) {
   if (out) *out = nullptr;
   if (!cfg || !out) return fail_create(nullptr, JEFI_EINVAL, "jefi_create: NULL argument");
   if (cfg->nx < 1 || cfg->ny < 1 || cfg->nz < 1 || !(cfg->dx > 0) || !(cfg->dy > 0) || !(cfg->dz > 0) || !(cfg->dt > 0) ||
-      cfg->c < 0 || cfg->eps0 < 0 || cfg->H < 0 || cfg->hist_cap < 0 || cfg->deposit_mode < 0 || cfg->deposit_mode > 3)
+      cfg->c < 0 || cfg->eps0 < 0 || cfg->H < 0 || cfg->hist_cap < 0 || cfg->deposit_mode < 0 || cfg->deposit_mode > 3 || cfg->delay_rule < 0 || cfg->delay_rule > 1)
     return fail_create(nullptr, JEFI_EINVAL, "jefi_create: grid sizes, spacings and dt must be positive");
   if ((long)cfg->nx * cfg->ny * cfg->nz > (1L << 30)) return fail_create(nullptr, JEFI_EINVAL, "jefi_create: grid too large");
   jefi_ctx* c = new (std::nothrow) jefi_ctx();

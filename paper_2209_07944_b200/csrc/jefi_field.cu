@@ -18,7 +18,7 @@
 // ------------------------------------------------------------------------------------------------------------
 // reference kernel
 // ------------------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(128) k_field_reference(jefi_dims d, jefi_geom g, int ex_, int ey_, long n,
+__global__ void __launch_bounds__(128) k_field_reference(jefi_dims d, jefi_geom g, int ex_, int ey_, long n, int linear,
                                                          const int* __restrict__ mtab, const float4* __restrict__ ring,
                                                          float* __restrict__ ex, float* __restrict__ ey,
                                                          float* __restrict__ ez, float* __restrict__ bx,
@@ -39,10 +39,15 @@ __global__ void __launch_bounds__(128) k_field_reference(jefi_dims d, jefi_geom 
         long tile; int cell;
         jefi_tile_cell(d, i, j, k, tile, cell);
         size_t idx = jefi_ring_quad(d, tile, (int)(t % d.H), cell);
-        const float4 S = ring[idx], D = ring[idx + JEFI_TCELLS];  // (Jx, Jz, rho, Jy)/scaled, see jefi_ctx.h
+        float4 S = ring[idx];
+        const float4 D = ring[idx + JEFI_TCELLS];  // (Jx, Jz, rho, Jy)/scaled, see jefi_ctx.h
         float ax = g.kx * (float)di, ay = g.ky * (float)dj, az = g.kz * (float)dk;
         float q = fmaf(ax, ax, fmaf(ay, ay, az * az));
         float rs = rsqrtf(q), rs2 = rs * rs, rs3 = rs2 * rs;
+        if (linear) {  // JEFI_DELAY_LINEAR: values on the line through the two samples, S(t_r) = S - phi D, phi = s - m
+          const float phi = fmaf(q, rs, -(float)m);
+          S.x = fmaf(-phi, D.x, S.x); S.y = fmaf(-phi, D.y, S.y); S.z = fmaf(-phi, D.z, S.z); S.w = fmaf(-phi, D.w, S.w);
+        }
         float qq = fmaf(rs2, D.z, rs3 * S.z);
         lex = fmaf(ax, qq, lex); ley = fmaf(ay, qq, ley); lez = fmaf(az, qq, lez);
         lex = fmaf(-rs, D.x, lex); ley = fmaf(-rs, D.w, ley); lez = fmaf(-rs, D.y, lez);
@@ -61,7 +66,7 @@ int jefi_launch_field_reference(jefi_ctx* c, float* ex, float* ey, float* ez, fl
   const jefi_dims& d = c->dims;
   unsigned blocks = (unsigned)((d.N + 127) / 128);
   k_field_reference<<<blocks, 128, 0, c->stream>>>(d, c->geom, jefi_table_extent(d.nx), jefi_table_extent(d.ny), c->step,
-                                                   c->mtab_dev, c->ring, ex, ey, ez, bx, by, bz);
+                                                   c->cfg.delay_rule == JEFI_DELAY_LINEAR ? 1 : 0, c->mtab_dev, c->ring, ex, ey, ez, bx, by, bz);
   JEFI_CUDA_TRY(c, cudaGetLastError());
   c->launches++;
   return JEFI_OK;
@@ -223,7 +228,7 @@ struct pair_acc {  // per-tile partial sums of one observation cell (first accum
 };
 
 // One observation cell against one source cell.  Kz = shared address of row m = 0 (i.e. K) + byte offset of the z layer.
-template <bool SELF, int CELL>
+template <bool SELF, bool LINEAR, int CELL>
 __device__ __forceinline__ void one_pair(uint32_t Kz, f32x2 axz, float ay, float qyz, pair_acc& A) {
   constexpr int SOFF = CELL * 16;
   constexpr int DOFF = SOFF + JEFI_TCELLS * 16;
@@ -233,8 +238,14 @@ __device__ __forceinline__ void one_pair(uint32_t Kz, f32x2 axz, float ay, float
   if (SELF) rs = q > 0.f ? rs : 0.f;        // the self cell contributes exactly zero
   const float t = fmaf(q, rs, JEFI_MAGIC);  // MAGIC + round(s): m sits in the mantissa
   const uint32_t addr = Kz - (uint32_t)__float_as_int(t) * (uint32_t)JEFI_ROW_BYTES;  // row j = m_hi - m
-  const quad2 S = lds128_imm<SOFF>(addr);   // (Jx, Jz | rho, Jy)
+  quad2 S = lds128_imm<SOFF>(addr);         // (Jx, Jz | rho, Jy)
   const quad2 D = lds128_imm<DOFF>(addr);   // (DJx, DJz | Drho, DJy)
+  if (LINEAR) {  // JEFI_DELAY_LINEAR: S(t_r) = S - phi D with phi = s - m in [-1/2, 1/2) (3 scalar + 2 packed instructions)
+    const float nphi = fmaf(-q, rs, t - JEFI_MAGIC);  // m - s
+    const f32x2 nphi2 = pk(nphi, nphi);
+    S.xy = fma2(nphi2, D.xy, S.xy);
+    S.zw = fma2(nphi2, D.zw, S.zw);
+  }
   const f32x2 rs2 = pk(rs, rs);
   const f32x2 wxz = fma2(rs2, S.xy, D.xy);  // (wx, wz)
   const f32x2 u0wy = fma2(rs2, S.zw, D.zw); // (u0, wy)
@@ -252,17 +263,17 @@ __device__ __forceinline__ void one_pair(uint32_t Kz, f32x2 axz, float ay, float
   A.By12 = fma2(Azx, wxz, A.By12);                // (a_z wx, a_x wz)
 }
 
-template <bool SELF, int LY>
+template <bool SELF, bool LINEAR, int LY>
 __device__ __forceinline__ void one_row(uint32_t Kz, const f32x2 (&axz)[JEFI_TS], float ay, float az2, pair_acc& A) {
   const float qyz = fmaf(ay, ay, az2);
-  one_pair<SELF, JEFI_TS * LY + 0>(Kz, axz[0], ay, qyz, A);
-  one_pair<SELF, JEFI_TS * LY + 1>(Kz, axz[1], ay, qyz, A);
-  one_pair<SELF, JEFI_TS * LY + 2>(Kz, axz[2], ay, qyz, A);
-  one_pair<SELF, JEFI_TS * LY + 3>(Kz, axz[3], ay, qyz, A);
+  one_pair<SELF, LINEAR, JEFI_TS * LY + 0>(Kz, axz[0], ay, qyz, A);
+  one_pair<SELF, LINEAR, JEFI_TS * LY + 1>(Kz, axz[1], ay, qyz, A);
+  one_pair<SELF, LINEAR, JEFI_TS * LY + 2>(Kz, axz[2], ay, qyz, A);
+  one_pair<SELF, LINEAR, JEFI_TS * LY + 3>(Kz, axz[3], ay, qyz, A);
 }
 
 // one observation cell against the 64 cells of the staged source tile
-template <bool SELF>
+template <bool SELF, bool LINEAR>
 __device__ __forceinline__ void tile_pairs(uint32_t K, float kz, const float (&ax)[JEFI_TS], const float (&ay)[JEFI_TS], float fz0,
                                            pair_acc& A) {
 #pragma unroll 1
@@ -273,14 +284,14 @@ __device__ __forceinline__ void tile_pairs(uint32_t K, float kz, const float (&a
     f32x2 axz[JEFI_TS];
 #pragma unroll
     for (int l = 0; l < JEFI_TS; l++) axz[l] = pk(ax[l], az);
-    one_row<SELF, 0>(Kz, axz, ay[0], az2, A);
-    one_row<SELF, 1>(Kz, axz, ay[1], az2, A);
-    one_row<SELF, 2>(Kz, axz, ay[2], az2, A);
-    one_row<SELF, 3>(Kz, axz, ay[3], az2, A);
+    one_row<SELF, LINEAR, 0>(Kz, axz, ay[0], az2, A);
+    one_row<SELF, LINEAR, 1>(Kz, axz, ay[1], az2, A);
+    one_row<SELF, LINEAR, 2>(Kz, axz, ay[2], az2, A);
+    one_row<SELF, LINEAR, 3>(Kz, axz, ay[3], az2, A);
   }
 }
 
-template <int WP>
+template <int WP, bool LINEAR>
 __global__ void __launch_bounds__(TILED_THREADS, 1) k_field_tiled(tiled_params P) {
   using L = stage_layout<WP>;
   extern __shared__ __align__(128) unsigned char smem[];
@@ -381,9 +392,9 @@ __global__ void __launch_bounds__(TILED_THREADS, 1) k_field_tiled(tiled_params P
       A.Exz = A.Fxz = A.Bxz = A.Cxz = A.By12 = pk(0.f, 0.f);
       A.Ey = A.Fy = 0.f;
       if (h.self)
-        tile_pairs<true>(h.K, P.g.kz, ax, ay, fz0, A);
+        tile_pairs<true, LINEAR>(h.K, P.g.kz, ax, ay, fz0, A);
       else
-        tile_pairs<false>(h.K, P.g.kz, ax, ay, fz0, A);
+        tile_pairs<false, LINEAR>(h.K, P.g.kz, ax, ay, fz0, A);
       // second accumulation level.  Cell c belongs to this thread alone in this tile; the previous tile's updates
       // (by other threads) are complete once every consumer warp has arrived on that tile's done barrier.
       if (p == 0 && it > 0) mbar_wait(barDone + 8 * ((it - 1) & 1), ((it - 1) >> 1) & 1);
@@ -444,10 +455,10 @@ __global__ void __launch_bounds__(OBCELLS) k_build_perm(int ndx, int ndy, int nt
 // window pitches the kernel is compiled for (ring rows per stage)
 static const int kPitches[] = {36, 48};
 typedef void (*tiled_fn)(tiled_params);
-static tiled_fn tiled_kernel_for(int wp) {
+static tiled_fn tiled_kernel_for(int wp, bool linear) {
   switch (wp) {
-    case 36: return k_field_tiled<36>;
-    case 48: return k_field_tiled<48>;
+    case 36: return linear ? k_field_tiled<36, true> : k_field_tiled<36, false>;
+    case 48: return linear ? k_field_tiled<48, true> : k_field_tiled<48, false>;
   }
   return nullptr;
 }
@@ -504,7 +515,7 @@ int jefi_tiled_prepare(jefi_ctx* c) {
     c->err = buf;
     return JEFI_ESTATE;
   }
-  cudaError_t e = cudaFuncSetAttribute(tiled_kernel_for(wp), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->tiled_smem);
+  cudaError_t e = cudaFuncSetAttribute(tiled_kernel_for(wp, c->cfg.delay_rule == JEFI_DELAY_LINEAR), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->tiled_smem);
   if (e != cudaSuccess) { c->err = std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e); return JEFI_ECUDA; }
   // how the source range is split over blockIdx.y: JEFI_FIELD_CHUNK (source tiles per CTA) overrides the default, which
   // keeps one CTA per observation tile (deterministic sums) once there are at least four waves of them and otherwise
@@ -554,7 +565,7 @@ int jefi_launch_field_tiled(jefi_ctx* c, float* ex, float* ey, float* ez, float*
     for (float* o : outs) JEFI_CUDA_TRY(c, cudaMemsetAsync(o, 0, (size_t)d.N * sizeof(float), c->stream));
   }
   dim3 grid((unsigned)(P.nobx * P.noby * P.nobz), (unsigned)nsplit);
-  tiled_kernel_for(c->wpitch)<<<grid, TILED_THREADS, c->tiled_smem, c->stream>>>(P);
+  tiled_kernel_for(c->wpitch, c->cfg.delay_rule == JEFI_DELAY_LINEAR)<<<grid, TILED_THREADS, c->tiled_smem, c->stream>>>(P);
   JEFI_CUDA_TRY(c, cudaGetLastError());
   c->launches++;
   return JEFI_OK;

@@ -17,6 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libjefi.so")
 JEFI_OK, JEFI_EINVAL, JEFI_ENOMEM, JEFI_ECUDA, JEFI_ESTATE = 0, -1, -2, -3, -4
 JEFI_FIELD_AUTO, JEFI_FIELD_REFERENCE, JEFI_FIELD_TILED = 0, 1, 2
 JEFI_DEPOSIT_AUTO, JEFI_DEPOSIT_DIRECT, JEFI_DEPOSIT_SORTED, JEFI_DEPOSIT_RUNS = 0, 1, 2, 3
+JEFI_DELAY_NEAREST, JEFI_DELAY_LINEAR = 0, 1
 
 EXPORTS = [
     "jefi_create", "jefi_destroy", "jefi_last_error", "jefi_get_info", "jefi_deposit", "jefi_push_sources",
@@ -38,6 +39,7 @@ class jefi_config(C.Structure):
         ("H", C.c_int), ("hist_cap", C.c_int),
         ("Eext", C.c_double * 3), ("Bext", C.c_double * 3),
         ("device", C.c_int), ("stream", C.c_void_p), ("field_impl", C.c_int), ("deposit_mode", C.c_int),
+        ("delay_rule", C.c_int),
     ]
 
 
@@ -116,10 +118,11 @@ def _dev(t, dtype, n: Optional[int], name: str) -> int:
 def jefi_create(nx: int, ny: int, nz: int, dx: float, dy: float, dz: float, dt: float, c: float = 0.0,
                 eps0: float = 0.0, H: int = 0, hist_cap: int = 0, Eext: Sequence[float] = (0, 0, 0),
                 Bext: Sequence[float] = (0, 0, 0), device: int = 0, stream: int = 0,
-                field_impl: int = JEFI_FIELD_AUTO, deposit_mode: int = JEFI_DEPOSIT_AUTO) -> int:
+                field_impl: int = JEFI_FIELD_AUTO, deposit_mode: int = JEFI_DEPOSIT_AUTO,
+                delay_rule: int = JEFI_DELAY_NEAREST) -> int:
     lib = load_library()
     cfg = jefi_config(nx, ny, nz, dx, dy, dz, dt, c, eps0, H, hist_cap, (C.c_double * 3)(*Eext),
-                      (C.c_double * 3)(*Bext), device, C.c_void_p(stream), field_impl, deposit_mode)
+                      (C.c_double * 3)(*Bext), device, C.c_void_p(stream), field_impl, deposit_mode, delay_rule)
     h = C.c_void_p()
     rc = lib.jefi_create(C.byref(cfg), C.byref(h))
     if rc != JEFI_OK:
@@ -275,7 +278,7 @@ class JefiContext:
     """Owns one jefi_ctx and the E/B/rho/J device tensors of a run; every method is one C-ABI call."""
 
     def __init__(self, grid: GridSpec, device=None, field_impl: int = JEFI_FIELD_AUTO,
-                 deposit_mode: int = JEFI_DEPOSIT_AUTO, sort_every: int = 0):
+                 deposit_mode: int = JEFI_DEPOSIT_AUTO, sort_every: int = 0, delay_rule: int = JEFI_DELAY_NEAREST):
         import torch
 
         if not torch.cuda.is_available():
@@ -287,7 +290,7 @@ class JefiContext:
         stream = torch.cuda.current_stream(self.device).cuda_stream
         self.handle = jefi_create(grid.nx, grid.ny, grid.nz, grid.dx, grid.dy, grid.dz, grid.dt, grid.c, grid.eps0,
                                   grid.H, grid.hist_cap, grid.Eext, grid.Bext, self.device.index or 0, stream,
-                                  field_impl, deposit_mode)
+                                  field_impl, deposit_mode, delay_rule)
         self.info = jefi_get_info(self.handle)
         self.H = self.info["H"]
         self.sort_every = int(sort_every)  # pic_step calls jefi_sort_particles every sort_every steps (0 = never)

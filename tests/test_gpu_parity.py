@@ -123,6 +123,65 @@ def test_field_parity_random_history(J, impl, shape, h, kappa, fill):
 
 
 @pytest.mark.parametrize("impl", ["reference", "tiled"])
+@pytest.mark.parametrize("shape,h,kappa,fill", [FIELD_CASES[0], FIELD_CASES[1], FIELD_CASES[3], FIELD_CASES[6], FIELD_CASES[7]])
+def test_field_parity_linear_delay_rule(J, impl, shape, h, kappa, fill):
+    """JEFI_DELAY_LINEAR (reading A22) against the oracle's RULE_LINEAR; it must also differ from the nearest rule."""
+    dt = h[0] / (kappa * C)
+    cfg = OracleConfig(*shape, *h, dt, delay_rule=oracle.RULE_LINEAR)
+    nsteps = {"full": cfg.H, "early": max(2, cfg.H // 3), "wrapped": 2 * cfg.H + 3}[fill]
+    slices = [wl.history_slice(cfg.N, t, 777, j_scale=C) for t in range(nsteps)]
+    g = J.GridSpec(*shape, *h, dt)
+    ctx = J.JefiContext(g, field_impl=J.JEFI_FIELD_TILED if impl == "tiled" else J.JEFI_FIELD_REFERENCE,
+                        delay_rule=J.JEFI_DELAY_LINEAR)
+    E, B = run_history(J, ctx, slices)
+    Eo, Bo = oracle_history(cfg, slices)
+    assert_field_parity(E, B, Eo, Bo, f"linear {impl} {shape} {fill}: ")
+    if cfg.N > 8:
+        En, Bn = oracle_history(OracleConfig(*shape, *h, dt), slices)
+        assert field_err(E, En)[0] > 1e-3  # the two rules are visibly different on this input
+    ctx.close()
+
+
+def analytic_sources(cfg, t):
+    """PAPER.md:421-425 Eqs. (3.4)-(3.5): Jx = Jy = Jz = sin(x+y+z) sin(t), rho = 3 (cos(t) - 1) cos(x+y+z) at the cell
+    centres, time t = step * dt; fp32 [4][N] as the C-ABI takes them."""
+    k, j, i = np.meshgrid(np.arange(cfg.nz), np.arange(cfg.ny), np.arange(cfg.nx), indexing="ij")
+    u = ((i + 0.5) * cfg.dx + (j + 0.5) * cfg.dy + (k + 0.5) * cfg.dz).ravel()
+    tt = t * cfg.dt
+    jv = np.sin(u) * math.sin(tt)
+    return np.stack([3.0 * (math.cos(tt) - 1.0) * np.cos(u), jv, jv, jv]).astype(np.float32)
+
+
+@pytest.mark.parametrize("rule", ["NEAREST", "LINEAR"])
+def test_paper_analytic_sources_ndt_scan(J, rule):
+    """The paper's N_dt experiment: 20^3 cells, dx = 0.3, dt = 0.05, c = eps0 = mu0 = 1 (kappa = 6), ring
+    depths below and above the ~207 steps light needs to cross the diagonal.  Every depth is compared with the oracle
+    at the same depth; depths >= N_dt + 2 agree with one another bit for bit on the GPU as they do in the oracle (P9),
+    a truncated history visibly does not."""
+    n = 20
+    base = OracleConfig(n, n, n, 0.3, 0.3, 0.3, 0.05, c=1.0, eps0=1.0)
+    ndt = oracle.num_dt(base)
+    assert ndt == 208
+    step = 260
+    res = {}
+    for depth in (ndt + 2, ndt + 42, 101, 31):
+        cfg = OracleConfig(n, n, n, 0.3, 0.3, 0.3, 0.05, c=1.0, eps0=1.0, H=depth, delay_rule=getattr(oracle, "RULE_" + rule))
+        slices = [analytic_sources(cfg, t) for t in range(step + 1)]
+        ctx = J.JefiContext(J.GridSpec(n, n, n, 0.3, 0.3, 0.3, 0.05, c=1.0, eps0=1.0, H=depth),
+                            delay_rule=getattr(J, "JEFI_DELAY_" + rule))
+        assert ctx.H == depth
+        E, B = run_history(J, ctx, slices)
+        Eo, Bo = oracle_history(cfg, slices)
+        assert_field_parity(E, B, Eo, Bo, f"analytic sources, depth {depth}: ")
+        res[depth] = (E, B, ctx.info["field_impl"])
+        ctx.close()
+    E0, B0, _ = res[ndt + 2]
+    assert np.array_equal(res[ndt + 42][0], E0) and np.array_equal(res[ndt + 42][1], B0)
+    for depth in (101, 31):
+        assert field_err(res[depth][0], E0.astype(np.float64))[0] > 1e-2
+
+
+@pytest.mark.parametrize("impl", ["reference", "tiled"])
 def test_field_light_cone_exact_zero(J, impl):
     """A single source cell switched on at step n0: cells outside the light cone are exactly zero on the GPU too."""
     import torch
