@@ -95,11 +95,11 @@ def visible_gpu_index(local_rank: int) -> int:
 
 
 # --------------------------------------------------------------------------------------------------- reference arm
-def oracle_sample_rate(w: wl.Workload, ring_host: np.ndarray, n_obs: int, seed_tag: int):
+def oracle_sample_rate(w: wl.Workload, ring_host: np.ndarray, n_obs: int, seed_tag: int, rule: int = 0):
     """Oracle pairs/s on n_obs seeded observation cells against all sources (fp64, all host cores)."""
     import oracle
 
-    cfg = oracle.OracleConfig(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt)
+    cfg = oracle.OracleConfig(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt, delay_rule=rule)
     obs = np.random.default_rng([w.seed, seed_tag]).integers(0, w.N, size=n_obs, dtype=np.int64)
     t0 = time.perf_counter()
     oracle.field(cfg, w.H - 1, ring_host, obs)
@@ -123,7 +123,7 @@ def run_reference(args, w: wl.Workload) -> dict:
     n_obs = args.ref_obs
     rates = []
     for i in range(args.warmup + args.steps):
-        r, dt = oracle_sample_rate(w, ring, n_obs, i)
+        r, dt = oracle_sample_rate(w, ring, n_obs, i, 1 if args.delay_rule == "linear" else 0)
         log(f"[reference] step {i}: {n_obs} obs cells x {w.N - 1} sources in {dt:.2f} s -> {r / 1e9:.4f} Gpairs/s")
         if i >= args.warmup:
             rates.append((r, dt))
@@ -134,7 +134,7 @@ def run_reference(args, w: wl.Workload) -> dict:
     return {"impl": "reference", "metric": "jefimenko_source_obs_pairs_per_s", "value": val, "unit": "Gpairs/s",
             "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / len(rates),
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": w.name, "grid": [w.n] * 3, "H": w.H, "dx": w.dx, "dt": w.dt},
+            "config": {"workload": w.name, "grid": [w.n] * 3, "H": w.H, "dx": w.dx, "dt": w.dt, "delay_rule": args.delay_rule},
             "cpu_baseline": {"value": val, "unit": "Gpairs/s", "cores": cores, "kind": "oracle", "sample": sample},
             "e2e": {"value": val, "unit": "Gpairs/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -278,7 +278,8 @@ def run_product(args, w: wl.Workload) -> dict:
         dist.init_process_group("nccl", device_id=device)
     J.load_library()
 
-    ctx = J.JefiContext(J.GridSpec(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt), device=device)
+    ctx = J.JefiContext(J.GridSpec(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt), device=device,
+                        delay_rule=J.JEFI_DELAY_LINEAR if args.delay_rule == "linear" else J.JEFI_DELAY_NEAREST)
     N, H = w.N, ctx.H
     assert H == w.H
     keep_host = (rank == 0 and world == 1 and not args.no_cpu_baseline)
@@ -362,7 +363,8 @@ def run_product(args, w: wl.Workload) -> dict:
                "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                "config": {"workload": w.name, "grid": [w.n] * 3, "H": H, "dx": w.dx, "dt": w.dt,
                           "pairs_per_step": pairs, "l2": "inputs (9.5 GB ring) larger than L2, no flush",
-                          "parallelism": "replicas" if world > 1 else "single", "field_impl": impl},
+                          "parallelism": "replicas" if world > 1 else "single", "field_impl": impl,
+                          "delay_rule": args.delay_rule},
                "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
                             "traffic": None, "kernel": "k_field_tiled" if impl == 2 else "k_field_reference",
                             "kernel_ms": kernel_ms, "flop_per_pair": FLOP_PER_PAIR,
@@ -384,7 +386,7 @@ def run_product(args, w: wl.Workload) -> dict:
         if keep_host:
             import oracle
 
-            r, dt = oracle_sample_rate(w, ring_host, args.cpu_obs, 0)
+            r, dt = oracle_sample_rate(w, ring_host, args.cpu_obs, 0, 1 if args.delay_rule == "linear" else 0)
             out["cpu_baseline"] = {"value": r / 1e9, "unit": "Gpairs/s", "cores": oracle.num_threads(), "kind": "oracle",
                                    "sample": f"{args.cpu_obs} seeded observation cells x all {N - 1} source cells "
                                              f"({dt:.1f} s of fp64 CPU work)"}
@@ -405,6 +407,8 @@ def main():
     ap.add_argument("--workload", type=int, default=4, help="BASELINE.json config number of the field workload (4 = 96^3)")
     ap.add_argument("--no-pic", action="store_true", help="skip the PIC steps/s legs on configs 1-3")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--delay-rule", default="nearest", choices=["nearest", "linear"],
+                    help="retarded-time rule: nearest = BASELINE.json's configs (reading A1); linear = second rule (A22)")
     ap.add_argument("--particles-only", action="store_true", help="only the deposit/push HBM-roofline leg (for ncu captures)")
     ap.add_argument("--cpu-obs", type=int, default=4096, help="observation cells of the cpu_baseline sample")
     ap.add_argument("--ref-obs", type=int, default=1024, help="observation cells per step of --impl reference")

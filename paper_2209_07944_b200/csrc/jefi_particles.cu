@@ -201,8 +201,13 @@ __global__ void __launch_bounds__(256) k_deposit_sorted(int nx, int ny, int nz, 
   const unsigned above = heads & ~((2u << lane) - 1u);         // run heads strictly above this lane
   const unsigned run_end = above ? (unsigned)__ffs(above) - 2u : 31u;  // last lane of this lane's run
   bool same[5];
+  unsigned any_same = 0;  // bit s: some lane of the warp still has a partner at stride 2^s (skips the idle reduction steps of
+                          // short runs: with 4 particles per cell only strides 1 and 2 do any work)
 #pragma unroll
-  for (int s = 0; s < 5; s++) same[s] = lane + (1u << s) <= run_end;
+  for (int s = 0; s < 5; s++) {
+    same[s] = lane + (1u << s) <= run_end;
+    any_same |= (__ballot_sync(FULL, same[s]) != 0u ? 1u : 0u) << s;
+  }
 #pragma unroll
   for (int c3 = 0; c3 < 8; c3++) {
     const int a = c3 & 1, b = (c3 >> 1) & 1, c = c3 >> 2;
@@ -210,6 +215,7 @@ __global__ void __launch_bounds__(256) k_deposit_sorted(int nx, int ny, int nz, 
     float a0 = r0 * w, a1 = a0 * vx, a2 = a0 * vy, a3 = a0 * vz;
 #pragma unroll
     for (int s = 0; s < 5; s++) {  // segmented suffix sum: the head of a run ends up with the run total
+      if (!((any_same >> s) & 1u)) continue;  // warp-uniform
       const float b0 = __shfl_down_sync(FULL, a0, 1u << s), b1 = __shfl_down_sync(FULL, a1, 1u << s);
       const float b2 = __shfl_down_sync(FULL, a2, 1u << s), b3 = __shfl_down_sync(FULL, a3, 1u << s);
       if (same[s]) { a0 += b0; a1 += b1; a2 += b2; a3 += b3; }

@@ -139,21 +139,23 @@ def test_pic_configs_sampled_parity(J, config, steps, nsample):
     ctx.close()
 
 
-def test_config4_field_only_sampled_parity(J):
+@pytest.mark.parametrize("rule,nsample", [("NEAREST", 8192), ("LINEAR", 2048)])
+def test_config4_field_only_sampled_parity(J, rule, nsample):
     """96^3 x 96^3, H = 335, every slot random (J scaled by c so the J-dot term of Eq. 2.4 is visible): one
-    jefi_field_step in bench.py's launch configuration, 8192 sampled cells + 15 special cells against all sources."""
+    jefi_field_step in bench.py's launch configuration, sampled cells + 15 special cells against all sources; the same
+    for the second retarded-time rule (JEFI_DELAY_LINEAR, bench.py --delay-rule linear)."""
     import torch
 
     w = wl.WORKLOADS[4]
-    ctx = J.JefiContext(J.GridSpec(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt))
+    ctx = J.JefiContext(J.GridSpec(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt), delay_rule=getattr(J, "JEFI_DELAY_" + rule))
     assert ctx.H == w.H == 335 and ctx.info["field_impl"] == J.JEFI_FIELD_TILED
     ring = np.empty((w.H, 4, w.N), dtype=np.float32)
     for t in range(w.H):
         ring[t] = wl.history_slice(w.N, t, w.seed, j_scale=wl.C_SI)
         ctx.push_sources(torch.from_numpy(ring[t]).to(ctx.device))
     ctx.field_step()
-    cfg = OracleConfig(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt)
-    obs = wl.sample_obs(w.n, 8192, w.seed)
+    cfg = OracleConfig(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt, delay_rule=getattr(oracle, "RULE_" + rule))
+    obs = wl.sample_obs(w.n, nsample, w.seed)
     Eo, Bo = oracle.field(cfg, w.H - 1, ring, obs)
     eb = ctx.EB.cpu().numpy()
     for name, F, Fo in (("E", eb[:3][:, obs], Eo), ("B", eb[3:][:, obs], Bo)):
