@@ -30,6 +30,9 @@ from paper_2209_07944_b200 import workloads as wl  # noqa: E402
 # FP32 roofline of the field kernel ("bound": "alu"): 148 SMs x 128 FP32 lanes x 2 FLOP x max SM clock.
 N_SM, LANES = 148, 128
 FLOP_PER_PAIR = 48.0  # 24 FMA per source-observation pair
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE k_field_tiled launch, from the committed ncu --set full capture
+# (profiles/r1_v5_field_tiled_ncu_full.md: 121.862 GB + 55.2 MB); the ring itself is 9.56 GB, L2 hit rate 86 %.
+FIELD_DRAM_BYTES = {(4, "nearest"): 121.862e9 + 55.2e6}
 
 
 def log(*a):
@@ -366,7 +369,7 @@ def run_product(args, w: wl.Workload) -> dict:
                           "parallelism": "replicas" if world > 1 else "single", "field_impl": impl,
                           "delay_rule": args.delay_rule},
                "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                            "traffic": None, "kernel": "k_field_tiled" if impl == 2 else "k_field_reference",
+                            "traffic": FIELD_DRAM_BYTES.get((w.config, args.delay_rule)), "kernel": "k_field_tiled" if impl == 2 else "k_field_reference",
                             "kernel_ms": kernel_ms, "flop_per_pair": FLOP_PER_PAIR,
                             "peak_source": "148 SM x 128 FP32 lanes x 2 FLOP x clocks.max.sm (derived, DESIGN.md §7)"},
                "e2e": {"value": e2e_val, "unit": "Gpairs/s", "h2d_bytes_per_step": 16 * N, "d2h_bytes_per_step": 24 * N,
