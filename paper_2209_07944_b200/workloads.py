@@ -151,6 +151,55 @@ def particles(config: int, scale: float = 1.0) -> Dict[str, np.ndarray]:
     raise ValueError(f"config {config} has no particles")
 
 
+# ---------------------------------------------------------------------------------------------------------------
+# The paper's own slab set-ups (PAPER.md:243-250 grid and time step, :262 point emission, :288 zero-velocity column in
+# a 10 T field): non-cubic grids, kappa = dx/(c dt) = 0.334 (neighbouring cells have delay 0),
+# an external field.  The paper's seed and macro-particle count are unknown; these are seeded stand-ins.
+# ---------------------------------------------------------------------------------------------------------------
+@dataclass(frozen=True)
+class SlabWorkload:
+    name: str
+    shape: tuple  # (nx, ny, nz)
+    dx: float
+    dt: float
+    Bext: tuple
+    total_charge: float  # coulomb
+    seed: int
+
+    @property
+    def N(self) -> int:
+        return self.shape[0] * self.shape[1] * self.shape[2]
+
+
+SLABS: Dict[str, SlabWorkload] = {
+    "point_emission": SlabWorkload("slab_1x101x101_point_emission", (1, 101, 101), 1e-5, 1e-13, (0.0, 0.0, 0.0), -5e-14, SEED0 + 11),
+    "column_in_By": SlabWorkload("slab_1x251x111_column_in_By", (1, 251, 111), 1e-5, 1e-13, (0.0, 10.0, 0.0), -5e-14, SEED0 + 12),
+}
+
+
+def slab_particles(which: str, count: int) -> Dict[str, np.ndarray]:
+    """`count` macro-electrons of total charge -5e-14 C.
+    point_emission (Fig. 5): uniform in the cell j = k = 50, velocity in the yz plane, speed Gaussian about
+    v0 (10 eV) with sigma 0.2 v0, direction uniform.  column_in_By (Fig. 8): uniform in the column
+    j = 124, k = 5..105, at rest."""
+    w = SLABS[which]
+    rng = np.random.default_rng(w.seed)
+    wt = w.total_charge / (-E_CHARGE) / count
+    x = rng.uniform(0.0, 1.0, count)
+    if which == "point_emission":
+        y, z = rng.uniform(50.0, 51.0, count), rng.uniform(50.0, 51.0, count)
+        v0 = math.sqrt(2.0 * 10.0 * E_CHARGE / M_E)
+        speed = np.abs(rng.normal(v0, 0.2 * v0, count))
+        ang = rng.uniform(0.0, 2.0 * math.pi, count)
+        beta = speed / C_SI
+        g = 1.0 / np.sqrt(1.0 - beta * beta)
+        mom = [np.zeros(count), g * beta * np.cos(ang), g * beta * np.sin(ang)]
+    else:
+        y, z = rng.uniform(124.0, 125.0, count), rng.uniform(5.0, 106.0, count)
+        mom = [np.zeros(count) for _ in range(3)]
+    return _concat([_species(x, y, z, *mom, -E_CHARGE, M_E, wt)])
+
+
 def history_slices(n_cells: int, H: int, seed: int, j_scale: float = 1.0) -> Iterator[np.ndarray]:
     """Config-4 style source history: H slices of [4][N] fp32, i.i.d. uniform in [-1, 1].
 
