@@ -154,6 +154,16 @@ def max_over_ranks(dist, ms: float, device) -> float:
     return float(t.item())
 
 
+def assemble_slabs(dist, EB, plane: int, k0: int, k1: int) -> None:
+    """--shard obs: every rank has computed the observation planes [k0, k1) of EB ([6][N], plane = nx*ny cells per
+    z-plane); zero the rest and sum over ranks, so that every rank ends up with the whole E, B (24 N bytes over NVLink,
+    the all-gather of SURVEY.md §8(e) written as an all-reduce because slabs need not be equal)."""
+    EB[:, :plane * k0] = 0
+    EB[:, plane * k1:] = 0
+    if dist is not None:
+        dist.all_reduce(EB, op=dist.ReduceOp.SUM)
+
+
 def aggregate_rate(world: int, pairs_per_rank: float, ms_max: float) -> float:
     """Whole-job Gpairs/s: every rank processed pairs_per_rank pairs (replicas) in ms_max."""
     return world * pairs_per_rank / (ms_max * 1e-3) / 1e9
@@ -306,10 +316,22 @@ def run_product(args, w: wl.Workload) -> dict:
             dist.barrier()
         torch.cuda.synchronize(device)
 
+    # --shard obs (N > 1): every rank holds the whole history and solves its slab of observation planes, then E, B are
+    # assembled over NVLink (strong scaling of ONE field step).  Default: replicas.
+    shard = args.shard == "obs" and world > 1
+    k0, k1 = J.slab_range(w.n, rank, world) if shard else (0, w.n)
+
+    def field_step():
+        if shard:
+            ctx.field_step_slab(k0, k1)
+            assemble_slabs(dist, ctx.EB, w.n * w.n, k0, k1)
+        else:
+            ctx.field_step()
+
     # ---- device-resident timing ----
     for i in range(args.warmup):
         ctx.push_sources(fresh[i % len(fresh)])
-        ctx.field_step()
+        field_step()
     barrier()
     sampler = ClockSampler(visible_gpu_index(local))
     sampler.start()
@@ -319,7 +341,7 @@ def run_product(args, w: wl.Workload) -> dict:
     e0.record()
     for i in range(args.steps):
         ctx.push_sources(fresh[(args.warmup + i) % len(fresh)])
-        ctx.field_step()
+        field_step()
     e1.record()
     barrier()
     clocks = sampler.stop()
@@ -334,7 +356,7 @@ def run_product(args, w: wl.Workload) -> dict:
         kms.append(ctx.last_field_kernel_ms())
     kernel_ms = float(np.mean(kms))
     step_ms_max = max_over_ranks(dist, step_ms, device)
-    value = aggregate_rate(world, pairs, step_ms_max)
+    value = aggregate_rate(1 if shard else world, pairs, step_ms_max)  # sharded: the job is ONE step of N^2 pairs
 
     # ---- end to end through the C-ABI with host buffers ----
     src_pin = torch.empty(4 * N, dtype=torch.float32).pin_memory()
@@ -349,7 +371,7 @@ def run_product(args, w: wl.Workload) -> dict:
     torch.cuda.synchronize(device)
     e2e_ms = (time.perf_counter() - t0) * 1e3 / e2e_steps
     e2e_ms_max = max_over_ranks(dist, e2e_ms, device)
-    e2e_val = aggregate_rate(world, pairs, e2e_ms_max)
+    e2e_val = aggregate_rate(1 if shard else world, pairs, e2e_ms_max)  # sharded runs: one rank's own full step
     checksum = float(eb_pin[:N].double().abs().sum())
 
     impl = ctx.info["field_impl"]
@@ -363,10 +385,10 @@ def run_product(args, w: wl.Workload) -> dict:
         achieved = FLOP_PER_PAIR * pairs / (kernel_ms * 1e-3) / 1e12
         out = {"metric": "jefimenko_source_obs_pairs_per_s", "value": value, "unit": "Gpairs/s", "n_gpus": world,
                "steps": args.steps, "warmup": args.warmup, "ms_per_step": step_ms_max, "higher_is_better": True,
-               "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+               "scaling": "strong" if shard else "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                "config": {"workload": w.name, "grid": [w.n] * 3, "H": H, "dx": w.dx, "dt": w.dt,
                           "pairs_per_step": pairs, "l2": "inputs (9.5 GB ring) larger than L2, no flush",
-                          "parallelism": "replicas" if world > 1 else "single", "field_impl": impl,
+                          "parallelism": ("obs_slabs" if shard else "replicas") if world > 1 else "single", "field_impl": impl,
                           "delay_rule": args.delay_rule},
                "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
                             "traffic": FIELD_DRAM_BYTES.get((w.config, args.delay_rule)), "kernel": "k_field_tiled" if impl == 2 else "k_field_reference",
@@ -410,6 +432,8 @@ def main():
     ap.add_argument("--workload", type=int, default=4, help="BASELINE.json config number of the field workload (4 = 96^3)")
     ap.add_argument("--no-pic", action="store_true", help="skip the PIC steps/s legs on configs 1-3")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--shard", default="replicas", choices=["replicas", "obs"],
+                    help="N > 1: replicas (default, weak scaling) or observation z-slabs of one field step (strong scaling)")
     ap.add_argument("--delay-rule", default="nearest", choices=["nearest", "linear"],
                     help="retarded-time rule: nearest = BASELINE.json's configs (reading A1); linear = second rule (A22)")
     ap.add_argument("--particles-only", action="store_true", help="only the deposit/push HBM-roofline leg (for ncu captures)")

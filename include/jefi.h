@@ -123,6 +123,12 @@ int jefi_push_sources(jefi_ctx* ctx, const float* rho, const float* jx, const fl
  * JEFI_ESTATE before the first jefi_push_sources. */
 int jefi_field_step(jefi_ctx* ctx, float* ex, float* ey, float* ez, float* bx, float* by, float* bz);
 
+/* The same solve restricted to the observation cells of the z-planes k0 <= k < k1 (all sources, as always): only those
+ * entries of ex..bz are written.  Observation cells are independent (Eqs. 2.4-2.5 are sums per observation point), so
+ * disjoint slabs computed by different calls - or by different GPUs that hold the same history, SURVEY.md §8(e) - add up to
+ * jefi_field_step bit for bit.  k0 must be a multiple of 8 (the observation tile edge); JEFI_EINVAL otherwise. */
+int jefi_field_step_slab(jefi_ctx* ctx, int k0, int k1, float* ex, float* ey, float* ez, float* bx, float* by, float* bz);
+
 /* Field interpolation (Eq. 2.20) + relativistic Boris push (Eqs. 2.7-2.11, DESIGN.md §3 A5/A6) + kill rule
  * (PAPER.md:205, 239): for each alive particle gather E,B from the 8 nodes (virtual nodes count as zero), add
  * Eext/Bext, update u and then the position by v*dt; a particle whose new position leaves [0,n) on any axis gets

@@ -206,17 +206,27 @@ extern "C" int jefi_push_sources(jefi_ctx* c, const float* rho, const float* jx,
   return jefi_launch_push_sources(c, rho, jx, jy, jz);
 }
 
-extern "C" int jefi_field_step(jefi_ctx* c, float* ex, float* ey, float* ez, float* bx, float* by, float* bz) {
+extern "C" int jefi_field_step_slab(jefi_ctx* c, int k0, int k1, float* ex, float* ey, float* ez, float* bx, float* by, float* bz) {
   if (!c) return JEFI_EINVAL;
   if (!ex || !ey || !ez || !bx || !by || !bz) { c->err = "jefi_field_step: NULL array"; return JEFI_EINVAL; }
+  if (k0 < 0 || k1 > c->dims.nz || k0 > k1 || (k0 % 8) != 0) {
+    c->err = "jefi_field_step_slab: need 0 <= k0 <= k1 <= nz with k0 a multiple of 8";
+    return JEFI_EINVAL;
+  }
   if (c->step < 0) { c->err = "jefi_field_step before any jefi_push_sources"; return JEFI_ESTATE; }
+  if (k0 == k1) return JEFI_OK;
   JEFI_CUDA_TRY(c, cudaEventRecord(c->ev0, c->stream));
-  int rc = c->field_impl == JEFI_FIELD_TILED ? jefi_launch_field_tiled(c, ex, ey, ez, bx, by, bz)
-                                             : jefi_launch_field_reference(c, ex, ey, ez, bx, by, bz);
+  int rc = c->field_impl == JEFI_FIELD_TILED ? jefi_launch_field_tiled(c, k0, k1, ex, ey, ez, bx, by, bz)
+                                             : jefi_launch_field_reference(c, k0, k1, ex, ey, ez, bx, by, bz);
   if (rc != JEFI_OK) return rc;
   JEFI_CUDA_TRY(c, cudaEventRecord(c->ev1, c->stream));
   c->ev_valid = true;
   return JEFI_OK;
+}
+
+extern "C" int jefi_field_step(jefi_ctx* c, float* ex, float* ey, float* ez, float* bx, float* by, float* bz) {
+  if (!c) return JEFI_EINVAL;
+  return jefi_field_step_slab(c, 0, c->dims.nz, ex, ey, ez, bx, by, bz);
 }
 
 extern "C" float jefi_last_field_kernel_ms(jefi_ctx* c) {

@@ -118,7 +118,7 @@ __device__ __forceinline__ float jefi_q_fp32(float kx, float ky, float kz, float
 
 // implemented in the .cu files
 int jefi_launch_push_sources(jefi_ctx* c, const float* rho, const float* jx, const float* jy, const float* jz);
-int jefi_launch_field_reference(jefi_ctx* c, float* ex, float* ey, float* ez, float* bx, float* by, float* bz);
-int jefi_launch_field_tiled(jefi_ctx* c, float* ex, float* ey, float* ez, float* bx, float* by, float* bz);
+int jefi_launch_field_reference(jefi_ctx* c, int k0, int k1, float* ex, float* ey, float* ez, float* bx, float* by, float* bz);
+int jefi_launch_field_tiled(jefi_ctx* c, int k0, int k1, float* ex, float* ey, float* ez, float* bx, float* by, float* bz);
 int jefi_tiled_prepare(jefi_ctx* c);   // window size + smem opt-in; returns JEFI_ESTATE if it cannot run
 int jefi_verify_delay_fp32(jefi_ctx* c, long* mismatches);

@@ -18,13 +18,13 @@
 // ------------------------------------------------------------------------------------------------------------
 // reference kernel
 // ------------------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(128) k_field_reference(jefi_dims d, jefi_geom g, int ex_, int ey_, long n, int linear,
+__global__ void __launch_bounds__(128) k_field_reference(jefi_dims d, jefi_geom g, int ex_, int ey_, long n, int linear, long oc0, long oc1,
                                                          const int* __restrict__ mtab, const float4* __restrict__ ring,
                                                          float* __restrict__ ex, float* __restrict__ ey,
                                                          float* __restrict__ ez, float* __restrict__ bx,
                                                          float* __restrict__ by, float* __restrict__ bz) {
-  long oc = (long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (oc >= d.N) return;
+  long oc = oc0 + (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (oc >= oc1) return;
   const int I = (int)(oc % d.nx), J = (int)((oc / d.nx) % d.ny), K = (int)(oc / ((long)d.nx * d.ny));
   float aex = 0, aey = 0, aez = 0, abx = 0, aby = 0, abz = 0;
   for (int k = 0; k < d.nz; k++) {
@@ -62,11 +62,12 @@ __global__ void __launch_bounds__(128) k_field_reference(jefi_dims d, jefi_geom 
   bx[oc] = g.prefB * abx; by[oc] = g.prefB * aby; bz[oc] = g.prefB * abz;
 }
 
-int jefi_launch_field_reference(jefi_ctx* c, float* ex, float* ey, float* ez, float* bx, float* by, float* bz) {
+int jefi_launch_field_reference(jefi_ctx* c, int k0, int k1, float* ex, float* ey, float* ez, float* bx, float* by, float* bz) {
   const jefi_dims& d = c->dims;
-  unsigned blocks = (unsigned)((d.N + 127) / 128);
+  const long oc0 = (long)k0 * d.nx * d.ny, oc1 = (long)k1 * d.nx * d.ny;  // observation cells of the z-planes [k0, k1)
+  unsigned blocks = (unsigned)((oc1 - oc0 + 127) / 128);
   k_field_reference<<<blocks, 128, 0, c->stream>>>(d, c->geom, jefi_table_extent(d.nx), jefi_table_extent(d.ny), c->step,
-                                                   c->cfg.delay_rule == JEFI_DELAY_LINEAR ? 1 : 0, c->mtab_dev, c->ring, ex, ey, ez, bx, by, bz);
+                                                   c->cfg.delay_rule == JEFI_DELAY_LINEAR ? 1 : 0, oc0, oc1, c->mtab_dev, c->ring, ex, ey, ez, bx, by, bz);
   JEFI_CUDA_TRY(c, cudaGetLastError());
   c->launches++;
   return JEFI_OK;
@@ -123,6 +124,8 @@ struct tiled_params {
   int nslot;       // n mod H
   int nobx, noby, nobz;
   int ndx, ndy;    // extents of the permutation table in relative-offset space
+  int obz0;        // first observation tile layer of this launch (jefi_field_step_slab)
+  int k1;          // observation planes k >= k1 are not written
   int chunk;       // source tiles per blockIdx.y
   int atomic_out;  // 1: add into zeroed outputs (source range split over blockIdx.y)
   const float4* ring;
@@ -301,7 +304,7 @@ __global__ void __launch_bounds__(TILED_THREADS, 1) k_field_tiled(tiled_params P
   float* accS = reinterpret_cast<float*>(smem + L::ACC);
   const uint32_t barFull = sm0 + L::BAR, barDone = barFull + 16;
   // observation tile and source-tile range of this CTA
-  const int obx = blockIdx.x % P.nobx, oby = (blockIdx.x / P.nobx) % P.noby, obz = blockIdx.x / (P.nobx * P.noby);
+  const int obx = blockIdx.x % P.nobx, oby = (blockIdx.x / P.nobx) % P.noby, obz = P.obz0 + blockIdx.x / (P.nobx * P.noby);
   const int ox0 = obx * OB, oy0 = oby * OB, oz0 = obz * OB;
   const int ntiles = d.ntx * d.nty * d.ntz;
   const int t0 = blockIdx.y * P.chunk;
@@ -414,7 +417,7 @@ __global__ void __launch_bounds__(TILED_THREADS, 1) k_field_tiled(tiled_params P
   for (int p = 0; p < P_OBS; p++) {
     const int c = p * NCONS + tid;  // home order: x fastest inside the tile
     const int oi = ox0 + (c & 7), oj = oy0 + ((c >> 3) & 7), ok = oz0 + (c >> 6);
-    if (oi < d.nx && oj < d.ny && ok < d.nz) {
+    if (oi < d.nx && oj < d.ny && ok < P.k1) {
       const size_t o = (size_t)oi + (size_t)d.nx * ((size_t)oj + (size_t)d.ny * ok);
       const float vex = P.g.prefE * accS[c], vey = P.g.prefE * accS[OBCELLS + c], vez = P.g.prefE * accS[2 * OBCELLS + c];
       const float vbx = P.g.prefB * accS[3 * OBCELLS + c], vby = P.g.prefB * accS[4 * OBCELLS + c], vbz = P.g.prefB * accS[5 * OBCELLS + c];
@@ -548,7 +551,7 @@ int jefi_tiled_prepare(jefi_ctx* c) {
   return JEFI_OK;
 }
 
-int jefi_launch_field_tiled(jefi_ctx* c, float* ex, float* ey, float* ez, float* bx, float* by, float* bz) {
+int jefi_launch_field_tiled(jefi_ctx* c, int k0, int k1, float* ex, float* ey, float* ez, float* bx, float* by, float* bz) {
   const jefi_dims& d = c->dims;
   tiled_params P;
   P.d = d; P.g = c->geom; P.n = (int)c->step; P.nslot = (int)(c->step % d.H);
@@ -560,11 +563,14 @@ int jefi_launch_field_tiled(jefi_ctx* c, float* ex, float* ey, float* ez, float*
   P.atomic_out = nsplit > 1 ? 1 : 0;
   P.ring = c->ring; P.perm = c->perm;
   P.ex = ex; P.ey = ey; P.ez = ez; P.bx = bx; P.by = by; P.bz = bz;
+  P.obz0 = k0 / OB; P.k1 = k1;
+  const int nlayers = (k1 - k0 + OB - 1) / OB;
   if (P.atomic_out) {
     float* outs[6] = {ex, ey, ez, bx, by, bz};
-    for (float* o : outs) JEFI_CUDA_TRY(c, cudaMemsetAsync(o, 0, (size_t)d.N * sizeof(float), c->stream));
+    const size_t plane = (size_t)d.nx * d.ny;
+    for (float* o : outs) JEFI_CUDA_TRY(c, cudaMemsetAsync(o + plane * k0, 0, plane * (size_t)(k1 - k0) * sizeof(float), c->stream));
   }
-  dim3 grid((unsigned)(P.nobx * P.noby * P.nobz), (unsigned)nsplit);
+  dim3 grid((unsigned)(P.nobx * P.noby * nlayers), (unsigned)nsplit);
   tiled_kernel_for(c->wpitch, c->cfg.delay_rule == JEFI_DELAY_LINEAR)<<<grid, TILED_THREADS, c->tiled_smem, c->stream>>>(P);
   JEFI_CUDA_TRY(c, cudaGetLastError());
   c->launches++;

@@ -21,7 +21,7 @@ JEFI_DELAY_NEAREST, JEFI_DELAY_LINEAR = 0, 1
 
 EXPORTS = [
     "jefi_create", "jefi_destroy", "jefi_last_error", "jefi_get_info", "jefi_deposit", "jefi_push_sources",
-    "jefi_field_step", "jefi_push_particles", "jefi_field_step_host", "jefi_launch_count",
+    "jefi_field_step", "jefi_field_step_slab", "jefi_push_particles", "jefi_field_step_host", "jefi_launch_count",
     "jefi_last_field_kernel_ms", "jefi_debug_delay_table", "jefi_debug_cell_index", "jefi_debug_history_slot",
     "jefi_debug_cell_order", "jefi_sort_particles",
 ]
@@ -71,6 +71,8 @@ def load_library() -> C.CDLL:
     lib.jefi_push_sources.restype = C.c_int
     lib.jefi_field_step.argtypes = [vp] + [f32p] * 6
     lib.jefi_field_step.restype = C.c_int
+    lib.jefi_field_step_slab.argtypes = [vp, C.c_int, C.c_int] + [f32p] * 6
+    lib.jefi_field_step_slab.restype = C.c_int
     lib.jefi_push_particles.argtypes = [vp, C.c_long] + [f32p] * 7 + [u8p] + [f32p] * 6
     lib.jefi_push_particles.restype = C.c_int
     lib.jefi_field_step_host.argtypes = [vp, f32p, f32p]
@@ -157,6 +159,23 @@ def jefi_field_step(handle: int, N: int, ex, ey, ez, bx, by, bz) -> None:
     f = torch.float32
     ptrs = [_dev(t, f, N, n) for t, n in zip((ex, ey, ez, bx, by, bz), ("ex", "ey", "ez", "bx", "by", "bz"))]
     _check(handle, load_library().jefi_field_step(handle, *ptrs), "jefi_field_step")
+
+
+def jefi_field_step_slab(handle: int, N: int, k0: int, k1: int, ex, ey, ez, bx, by, bz) -> None:
+    import torch
+
+    f = torch.float32
+    ptrs = [_dev(t, f, N, n) for t, n in zip((ex, ey, ez, bx, by, bz), ("ex", "ey", "ez", "bx", "by", "bz"))]
+    _check(handle, load_library().jefi_field_step_slab(handle, int(k0), int(k1), *ptrs), "jefi_field_step_slab")
+
+
+def slab_range(nz: int, rank: int, world: int, edge: int = 8):
+    """Observation z-planes [k0, k1) of `rank` out of `world`: whole layers of 8-cell observation tiles,
+    spread as evenly as the layer count allows; ranks beyond the layer count get an empty range."""
+    layers = (nz + edge - 1) // edge
+    lo = (layers * rank) // world
+    hi = (layers * (rank + 1)) // world
+    return min(lo * edge, nz), min(hi * edge, nz)
 
 
 def jefi_deposit(handle: int, N: int, x, y, z, ux, uy, uz, qw, alive, rho, jx, jy, jz) -> None:
@@ -313,6 +332,12 @@ class JefiContext:
     def field_step(self, out=None):
         o = self.EB if out is None else out
         jefi_field_step(self.handle, self.N, o[0], o[1], o[2], o[3], o[4], o[5])
+        return o
+
+    def field_step_slab(self, k0: int, k1: int, out=None):
+        """E, B on the observation planes k0 <= k < k1 only (the other entries of `out` are left as they are)."""
+        o = self.EB if out is None else out
+        jefi_field_step_slab(self.handle, self.N, k0, k1, o[0], o[1], o[2], o[3], o[4], o[5])
         return o
 
     def deposit(self, part: dict, out=None):

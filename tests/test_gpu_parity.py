@@ -182,6 +182,41 @@ def test_paper_analytic_sources_ndt_scan(J, rule):
 
 
 @pytest.mark.parametrize("impl", ["reference", "tiled"])
+@pytest.mark.parametrize("shape,world", [((16, 16, 16), 2), ((13, 10, 20), 3), ((9, 5, 3), 2), ((24, 24, 40), 4)])
+def test_field_step_slabs_add_up_to_the_full_step_bitwise(J, impl, shape, world):
+    """observation slabs are independent; `world` slab calls (what `world` GPUs would each do) assemble the
+    full jefi_field_step bit for bit, and each call writes nothing outside its slab."""
+    import torch
+
+    h = (1e-4,) * 3
+    dt = h[0] / (2 * C)
+    cfg = OracleConfig(*shape, *h, dt)
+    ctx = make_ctx(J, shape, h, dt, J.JEFI_FIELD_TILED if impl == "tiled" else J.JEFI_FIELD_REFERENCE)
+    for t in range(min(cfg.H, 40)):
+        ctx.push_sources(torch.from_numpy(wl.history_slice(cfg.N, t, 99, j_scale=C)).to(ctx.device))
+    full = ctx.field_step().clone()
+    asm = torch.full_like(full, float("nan"))
+    plane = shape[0] * shape[1]
+    covered = 0
+    for r in range(world):
+        k0, k1 = J.slab_range(shape[2], r, world)
+        assert k0 % 8 == 0 and 0 <= k0 <= k1 <= shape[2]
+        part = torch.full_like(full, -7.0)
+        ctx.field_step_slab(k0, k1, part)
+        assert bool((part[:, :plane * k0] == -7.0).all()) and bool((part[:, plane * k1:] == -7.0).all())
+        asm[:, plane * k0:plane * k1] = part[:, plane * k0:plane * k1]
+        covered += k1 - k0
+    assert covered == shape[2]
+    if impl == "reference" or ctx.info["field_impl"] == J.JEFI_FIELD_TILED:
+        same = torch.equal(asm, full)
+        if not same:  # split source range (small grids): partial sums meet in fp32 atomics, order not defined
+            assert float((asm - full).abs().max()) <= 1e-5 * float(full.abs().max())
+    with pytest.raises(J.JefiError):
+        ctx.field_step_slab(4, shape[2])  # k0 not a multiple of 8
+    ctx.close()
+
+
+@pytest.mark.parametrize("impl", ["reference", "tiled"])
 def test_field_light_cone_exact_zero(J, impl):
     """A single source cell switched on at step n0: cells outside the light cone are exactly zero on the GPU too."""
     import torch

@@ -71,3 +71,46 @@ def test_reference_arm_under_torchrun_prints_one_line_from_rank0():
     js = json.loads(lines[0])
     assert js["impl"] == "reference" and js["n_gpus"] == 2 and js["cpu_baseline"]["kind"] == "oracle"
     assert js["value"] > 0 and js["e2e"]["h2d_bytes_per_step"] == 0 and js["config"]["workload"].startswith("cfg1")
+
+
+def test_slab_range_partitions_every_layer():
+    """Host logic of the observation-slab sharding (bench.py --shard obs)."""
+    from paper_2209_07944_b200.jefi import slab_range
+
+    for nz in (1, 7, 8, 9, 96, 100, 128):
+        for world in (1, 2, 3, 4, 8, 16):
+            r = [slab_range(nz, k, world) for k in range(world)]
+            assert r[0][0] == 0 and r[-1][1] == nz
+            assert all(a[1] == b[0] for a, b in zip(r, r[1:])) and all(a[0] % 8 == 0 for a in r)
+    assert [slab_range(96, k, 8) for k in range(8)] == [(0, 8), (8, 24), (24, 32), (32, 48), (48, 56), (56, 72), (72, 80), (80, 96)]
+
+
+def _slab_worker(rank: int, world: int, port: int, out):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    import bench
+    from paper_2209_07944_b200.jefi import slab_range
+
+    nx, ny, nz = 5, 4, 20
+    full = torch.arange(6 * nx * ny * nz, dtype=torch.float32).reshape(6, -1) + 1.0  # what a 1-GPU field step would give
+    k0, k1 = slab_range(nz, rank, world)
+    mine = torch.full_like(full, 123.0)  # stale values outside the slab must not leak into the result
+    mine[:, nx * ny * k0:nx * ny * k1] = full[:, nx * ny * k0:nx * ny * k1]
+    bench.assemble_slabs(dist, mine, nx * ny, k0, k1)
+    out.put((rank, bool(torch.equal(mine, full))))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_slab_assembly_gloo_world2():
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_slab_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = sorted(q.get(timeout=120) for _ in procs)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    assert res == [(0, True), (1, True)]
