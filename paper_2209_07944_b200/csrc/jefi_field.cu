@@ -432,18 +432,30 @@ __global__ void __launch_bounds__(TILED_THREADS, 1) k_field_tiled(tiled_params P
   }
 }
 
-// Evaluation order of the 512 cells of an observation tile for one relative tile offset D = (ox0 - sx0, ..):
-// ascending distance to the centre of the source tile, ties in home order (x fastest).
-// One CTA of 512 threads per offset; rank by counting (a one-off O(512^2) per offset at create time).
-__global__ void __launch_bounds__(OBCELLS) k_build_perm(int ndx, int ndy, int ntx, int nty, int ntz, jefi_geom g,
+// Evaluation order of the 512 cells of an observation tile for one relative tile offset D = (ox0 - sx0, ..).
+// What it is for: an LDS.128 costs 2 data-pipe cycles instead of 4 when EVERY lane pair (2k, 2k+1) of the warp reads one
+// quad, i.e. when the two observation cells of every pair have the same delay to the source cell being evaluated.
+//   1. rank the cells by their distance to the centre of the source tile (ties in home order, x fastest): neighbours in
+//      this order are almost equidistant from every cell of the tile; consecutive cells form the 256 lane pairs;
+//   2. per pair, the 64-bit set of source cells for which its two delays differ (same fp32 delay arithmetic as the kernel);
+//   3. deal the pairs to the 16 warps greedily: a warp starts from the first free pair of the distance order and then takes,
+//      15 times, the free pair among the next `band` pairs that adds the fewest new cells to the union of its pairs' sets
+//      (a source cell outside the union takes the fast path for that warp).  The band keeps the delays of one warp within
+//      8 slots: rows 8 apart share a 16-byte bank group and would be replayed.
+// Any order gives the same sums; this table only decides how fast.  One CTA of 512 threads per offset, once at create.
+__global__ void __launch_bounds__(OBCELLS) k_build_perm(int ndx, int ndy, int ntx, int nty, int ntz, jefi_geom g, int band,
                                                         unsigned short* __restrict__ perm) {
   __shared__ float keys[OBCELLS];
+  __shared__ unsigned short order[OBCELLS];
+  __shared__ unsigned long long mask[OBCELLS / 2];
+  __shared__ unsigned short picked[OBCELLS / 2];
+  __shared__ unsigned red[2][OBCELLS / 32];
   const int c = threadIdx.x;
   const int ix = blockIdx.x % ndx, iy = (blockIdx.x / ndx) % ndy, iz = blockIdx.x / (ndx * ndy);
-  const float Dx = (float)(JEFI_TS * (ix - (ntx - 1))), Dy = (float)(JEFI_TS * (iy - (nty - 1))), Dz = (float)(JEFI_TS * (iz - (ntz - 1)));
+  const int Dxi = JEFI_TS * (ix - (ntx - 1)), Dyi = JEFI_TS * (iy - (nty - 1)), Dzi = JEFI_TS * (iz - (ntz - 1));
   const float half = 0.5f * (float)(JEFI_TS - 1);
-  const float rx = g.kx * (Dx + (float)(c & 7) - half), ry = g.ky * (Dy + (float)((c >> 3) & 7) - half),
-              rz = g.kz * (Dz + (float)(c >> 6) - half);
+  const float rx = g.kx * ((float)Dxi + (float)(c & 7) - half), ry = g.ky * ((float)Dyi + (float)((c >> 3) & 7) - half),
+              rz = g.kz * ((float)Dzi + (float)(c >> 6) - half);
   const float key = rx * rx + ry * ry + rz * rz;
   keys[c] = key;
   __syncthreads();
@@ -452,7 +464,50 @@ __global__ void __launch_bounds__(OBCELLS) k_build_perm(int ndx, int ndy, int nt
     float kj = keys[j];
     pos += (kj < key) || (kj == key && j < c);
   }
-  perm[(size_t)blockIdx.x * OBCELLS + pos] = (unsigned short)c;
+  order[pos] = (unsigned short)c;
+  __syncthreads();
+  // 2. pair c = cells order[2c], order[2c+1]: source cells whose delay differs between the two
+  unsigned long long mine = 0;
+  bool avail = c < OBCELLS / 2;
+  if (avail) {
+    const int a = order[2 * c], b = order[2 * c + 1];
+    for (int sc = 0; sc < JEFI_TCELLS; sc++) {
+      const int lx = sc & 3, ly = (sc >> 2) & 3, lz = sc >> 4;
+      const float qa = jefi_q_fp32(g.kx, g.ky, g.kz, (float)(Dxi + (a & 7) - lx), (float)(Dyi + ((a >> 3) & 7) - ly), (float)(Dzi + (a >> 6) - lz));
+      const float qb = jefi_q_fp32(g.kx, g.ky, g.kz, (float)(Dxi + (b & 7) - lx), (float)(Dyi + ((b >> 3) & 7) - ly), (float)(Dzi + (b >> 6) - lz));
+      const int ma = qa > 0.f ? jefi_delay_fp32(qa) : 0, mb = qb > 0.f ? jefi_delay_fp32(qb) : 0;
+      mine |= (unsigned long long)(ma != mb) << sc;
+    }
+    mask[c] = mine;
+  }
+  __syncthreads();
+  // 3. greedy deal of the pairs to the warps (block-wide argmin per pick; keys are (cost << 16) | pair, pairs in distance order)
+  const unsigned lane = c & 31, warp = c >> 5;
+  int pick = 0;
+  for (int w = 0; w < OBCELLS / 32; w++) {
+    unsigned long long uni = 0;
+    int lo = 0;  // the warp's first pair = the lowest free pair; the others come from the `band` pairs that follow it
+    for (int i = 0; i < 16; i++, pick++) {
+      unsigned k = 0xffffffffu;
+      if (avail) {
+        const unsigned cost = i == 0 ? 0u : (c < lo + band ? (unsigned)__popcll(uni | mine) : 0x7fffu);
+        k = (cost << 16) | (unsigned)c;
+      }
+      k = __reduce_min_sync(0xffffffffu, k);
+      if (lane == 0) red[pick & 1][warp] = k;
+      __syncthreads();
+      unsigned best = 0xffffffffu;
+#pragma unroll
+      for (int q = 0; q < OBCELLS / 32; q++) best = min(best, red[pick & 1][q]);
+      const int sel = (int)(best & 0xffffu);
+      if (i == 0) lo = sel;
+      if (c == sel) avail = false;
+      if (c == 0) picked[pick] = (unsigned short)sel;
+      uni |= mask[sel];
+    }
+  }
+  __syncthreads();
+  perm[(size_t)blockIdx.x * OBCELLS + c] = order[2 * picked[c >> 1] + (c & 1)];
 }
 
 // window pitches the kernel is compiled for (ring rows per stage)
@@ -545,7 +600,12 @@ int jefi_tiled_prepare(jefi_ctx* c) {
     c->err = std::string("permutation table allocation: ") + cudaGetErrorString(e);
     return JEFI_ENOMEM;
   }
-  k_build_perm<<<(unsigned)rows, OBCELLS, 0, c->stream>>>(c->ndx, c->ndy, d.ntx, d.nty, d.ntz, c->geom, c->perm);
+  // pairs a warp may draw from, counted from its first pair in the distance order: wide enough to find pairs that differ on
+  // the same source cells, narrow enough that the delays of one warp stay within 8 slots (rows 8 apart share a bank group)
+  int band = 64;
+  const char* benv = getenv("JEFI_PERM_BAND");
+  if (benv && atoi(benv) > 0) band = atoi(benv);
+  k_build_perm<<<(unsigned)rows, OBCELLS, 0, c->stream>>>(c->ndx, c->ndy, d.ntx, d.nty, d.ntz, c->geom, band, c->perm);
   if ((e = cudaGetLastError()) != cudaSuccess) { c->err = std::string("k_build_perm: ") + cudaGetErrorString(e); return JEFI_ECUDA; }
   c->launches++;
   return JEFI_OK;
