@@ -31,8 +31,8 @@ from paper_2209_07944_b200 import workloads as wl  # noqa: E402
 N_SM, LANES = 148, 128
 FLOP_PER_PAIR = 48.0  # 24 FMA per source-observation pair
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE k_field_tiled launch, from the committed ncu --set full capture
-# (profiles/r1_v5_field_tiled_ncu_full.md: 121.862 GB + 55.2 MB); the ring itself is 9.56 GB, L2 hit rate 86 %.
-FIELD_DRAM_BYTES = {(4, "nearest"): 121.862e9 + 55.2e6}
+# (profiles/r1_v6_field_tiled_ncu_full.md: 85.259 GB + 52.9 MB); the ring itself is 9.56 GB, L2 hit rate 90 %.
+FIELD_DRAM_BYTES = {(4, "nearest"): 85.259e9 + 52.9e6}
 
 
 def log(*a):

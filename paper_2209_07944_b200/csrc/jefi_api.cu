@@ -53,6 +53,7 @@ extern "C" int jefi_create(const jefi_config* cfg, jefi_ctx** out) {
   c->sort_key = c->sort_rank = c->sort_order = nullptr;
   c->sort_cap = 0;
   c->sort_buf = nullptr;
+  c->eb_pack = nullptr;
   c->ev0 = c->ev1 = nullptr;
   c->ev_valid = false;
   c->launches = 0;
@@ -157,6 +158,7 @@ extern "C" void jefi_destroy(jefi_ctx* c) {
   if (c->sort_rank) cudaFree(c->sort_rank);
   if (c->sort_order) cudaFree(c->sort_order);
   if (c->sort_buf) cudaFree(c->sort_buf);
+  if (c->eb_pack) cudaFree(c->eb_pack);
   if (c->mtab_host) free(c->mtab_host);
   if (c->ev0) cudaEventDestroy(c->ev0);
   if (c->ev1) cudaEventDestroy(c->ev1);

@@ -77,6 +77,7 @@ struct jefi_ctx {
   unsigned *sort_count, *sort_offset, *sort_sums;  // per-bin counts, exclusive offsets, scan tile sums (+ grand total)
   int *sort_key, *sort_rank, *sort_order;          // per particle
   long sort_cap;
+  float4* eb_pack;                                 // jefi_push_particles: E, B packed two float4 per node
   void* sort_buf;                                  // jefi_sort_particles: permuted copies of the caller's arrays
   // host-variant staging
   float* src_stage;     // 4N floats, device staging of jefi_field_step_host

@@ -92,11 +92,11 @@ int jefi_launch_field_reference(jefi_ctx* c, int k0, int k1, float* ex, float* e
 //   address = K - 2064*bits(t) (IMAD), 2 x LDS.128 (S and D quads), then with packed FP32 (fma.rn.f32x2 = SASS FFMA2,
 //   scalar operands broadcast, halves swapped for free):
 //     (wx,wz) = rs*(Jx,Jz) + (DJx,DJz)      (u0,wy) = rs*(rho,Jy) + (Drho,DJy)             2 FFMA2
-//     r2 = rs^2, (a_x,a_z) = (ax,az)*r2, a_y = ay*r2                                       FMUL, FMUL2, FMUL
+//     r2 = rs^2, (a_x,a_z) = (ax,az)*r2, a_y = ay*r2                                       4 FMUL
 //     Exz += (a_x,a_z)*u0   Fxz += rs*(DJx,DJz)   Ey += a_y*u0   Fy += rs*DJy              2 FFMA2 + 2 FFMA
 //     Bxz += a_y*(wz,wx)    Cxz += wy*(a_z,a_x)   By12 += (a_z,a_x)*(wx,wz)                3 FFMA2
-//   E = (Exz - Fxz, Ey - Fy), B = (Bxz.lo - Cxz.lo, By12.lo - By12.hi, Cxz.hi - Bxz.hi):   18 issue slots per pair
-//   (7 scalar FMA-pipe, 8 packed, 1 MUFU, 2 LDS) against 26 for the scalar form.
+//   E = (Exz - Fxz, Ey - Fy), B = (Bxz.lo - Cxz.lo, By12.lo - By12.hi, Cxz.hi - Bxz.hi):   19 issue slots per pair
+//   (9 scalar FMA-pipe, 7 packed, 1 MUFU, 2 LDS) against 26 for the scalar form.
 //
 // Shared-memory delivery is the scarce resource (measured, profiles/): an LDS.128 takes 4 data-pipe cycles, 2 when
 // every lane l reads the same address as lane l^1 (or every l as l^2).  Which lane evaluates which observation cell
@@ -202,12 +202,6 @@ __device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) {
   asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
   return r;
 }
-__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) {
-  f32x2 r;
-  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
-  return r;
-}
-
 // min / max of |a| over the integer interval [lo, hi]
 __device__ __forceinline__ void abs_range(int lo, int hi, int& mn, int& mx) {
   int alo = abs(lo), ahi = abs(hi);
@@ -232,10 +226,9 @@ struct pair_acc {  // per-tile partial sums of one observation cell (first accum
 
 // One observation cell against one source cell.  Kz = shared address of row m = 0 (i.e. K) + byte offset of the z layer.
 template <bool SELF, bool LINEAR, int CELL>
-__device__ __forceinline__ void one_pair(uint32_t Kz, f32x2 axz, float ay, float qyz, pair_acc& A) {
+__device__ __forceinline__ void one_pair(uint32_t Kz, float ax, float ay, float az, float qyz, pair_acc& A) {
   constexpr int SOFF = CELL * 16;
   constexpr int DOFF = SOFF + JEFI_TCELLS * 16;
-  const float ax = lo32(axz);
   const float q = fmaf(ax, ax, qyz);
   float rs = jefi_rsqrt(q);
   if (SELF) rs = q > 0.f ? rs : 0.f;        // the self cell contributes exactly zero
@@ -253,8 +246,8 @@ __device__ __forceinline__ void one_pair(uint32_t Kz, f32x2 axz, float ay, float
   const f32x2 wxz = fma2(rs2, S.xy, D.xy);  // (wx, wz)
   const f32x2 u0wy = fma2(rs2, S.zw, D.zw); // (u0, wy)
   const float r2 = rs * rs;
-  const f32x2 Axz = mul2(axz, pk(r2, r2));  // (a_x, a_z) = d' rs^2
-  const float a_y = ay * r2;
+  const f32x2 Axz = pk(ax * r2, az * r2);   // (a_x, a_z) = d' rs^2: two scalar multiplies, so that no (ax, az) register pair
+  const float a_y = ay * r2;                // has to be kept alive (measured 1.3 % faster than one FMUL2 on kept pairs)
   const float u0 = lo32(u0wy), wy = hi32(u0wy);
   const f32x2 Azx = swap2(Axz);
   A.Exz = fma2(Axz, pk(u0, u0), A.Exz);
@@ -267,12 +260,12 @@ __device__ __forceinline__ void one_pair(uint32_t Kz, f32x2 axz, float ay, float
 }
 
 template <bool SELF, bool LINEAR, int LY>
-__device__ __forceinline__ void one_row(uint32_t Kz, const f32x2 (&axz)[JEFI_TS], float ay, float az2, pair_acc& A) {
+__device__ __forceinline__ void one_row(uint32_t Kz, const float (&ax)[JEFI_TS], float ay, float az, float az2, pair_acc& A) {
   const float qyz = fmaf(ay, ay, az2);
-  one_pair<SELF, LINEAR, JEFI_TS * LY + 0>(Kz, axz[0], ay, qyz, A);
-  one_pair<SELF, LINEAR, JEFI_TS * LY + 1>(Kz, axz[1], ay, qyz, A);
-  one_pair<SELF, LINEAR, JEFI_TS * LY + 2>(Kz, axz[2], ay, qyz, A);
-  one_pair<SELF, LINEAR, JEFI_TS * LY + 3>(Kz, axz[3], ay, qyz, A);
+  one_pair<SELF, LINEAR, JEFI_TS * LY + 0>(Kz, ax[0], ay, az, qyz, A);
+  one_pair<SELF, LINEAR, JEFI_TS * LY + 1>(Kz, ax[1], ay, az, qyz, A);
+  one_pair<SELF, LINEAR, JEFI_TS * LY + 2>(Kz, ax[2], ay, az, qyz, A);
+  one_pair<SELF, LINEAR, JEFI_TS * LY + 3>(Kz, ax[3], ay, az, qyz, A);
 }
 
 // one observation cell against the 64 cells of the staged source tile
@@ -284,13 +277,10 @@ __device__ __forceinline__ void tile_pairs(uint32_t K, float kz, const float (&a
     const float az = kz * (fz0 - (float)lz);
     const float az2 = az * az;
     const uint32_t Kz = K + (uint32_t)(lz * JEFI_TS * JEFI_TS * 16);
-    f32x2 axz[JEFI_TS];
-#pragma unroll
-    for (int l = 0; l < JEFI_TS; l++) axz[l] = pk(ax[l], az);
-    one_row<SELF, LINEAR, 0>(Kz, axz, ay[0], az2, A);
-    one_row<SELF, LINEAR, 1>(Kz, axz, ay[1], az2, A);
-    one_row<SELF, LINEAR, 2>(Kz, axz, ay[2], az2, A);
-    one_row<SELF, LINEAR, 3>(Kz, axz, ay[3], az2, A);
+    one_row<SELF, LINEAR, 0>(Kz, ax, ay[0], az, az2, A);
+    one_row<SELF, LINEAR, 1>(Kz, ax, ay[1], az, az2, A);
+    one_row<SELF, LINEAR, 2>(Kz, ax, ay[2], az, az2, A);
+    one_row<SELF, LINEAR, 3>(Kz, ax, ay[3], az, az2, A);
   }
 }
 

@@ -388,13 +388,26 @@ struct push_consts {
   float Eext[3], Bext[3];
 };
 
+// E, B of a node packed into two float4 (Ex, Ey, Ez, Bx | By, Bz, 0, 0): the push then gathers 16 quads per particle instead
+// of 48 words (one sector per node when the lanes of a warp sit in the same cell).  24 N bytes in, 32 N out per step.
+__global__ void __launch_bounds__(256) k_pack_fields(long N, const float* __restrict__ ex, const float* __restrict__ ey,
+                                                     const float* __restrict__ ez, const float* __restrict__ bx,
+                                                     const float* __restrict__ by, const float* __restrict__ bz,
+                                                     float4* __restrict__ pack) {
+  long n = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (n >= N) return;
+  pack[2 * n] = make_float4(ex[n], ey[n], ez[n], bx[n]);
+  pack[2 * n + 1] = make_float4(by[n], bz[n], 0.f, 0.f);
+}
+
+template <bool PACKED>
 __global__ void __launch_bounds__(256) k_push(push_consts K, long np, float* __restrict__ x, float* __restrict__ y,
                                               float* __restrict__ z, float* __restrict__ ux, float* __restrict__ uy,
                                               float* __restrict__ uz, const float* __restrict__ qm,
                                               unsigned char* __restrict__ alive, const float* __restrict__ ex,
                                               const float* __restrict__ ey, const float* __restrict__ ez,
                                               const float* __restrict__ bx, const float* __restrict__ by,
-                                              const float* __restrict__ bz) {
+                                              const float* __restrict__ bz, const float4* __restrict__ pack) {
   long p = (long)blockIdx.x * blockDim.x + threadIdx.x;
   if (p >= np || alive[p] == 0) return;
   float xp = x[p], yp = y[p], zp = z[p];
@@ -409,8 +422,14 @@ __global__ void __launch_bounds__(256) k_push(push_consts K, long np, float* __r
     if (ii >= 0 && ii < K.nx && jj >= 0 && jj < K.ny && kk >= 0 && kk < K.nz) {
       float w = (a ? al : 1.f - al) * (b ? be : 1.f - be) * (c ? ch : 1.f - ch);
       long node = (long)ii + (long)K.nx * ((long)jj + (long)K.ny * kk);
-      E0 = fmaf(w, __ldg(ex + node), E0); E1 = fmaf(w, __ldg(ey + node), E1); E2 = fmaf(w, __ldg(ez + node), E2);
-      B0 = fmaf(w, __ldg(bx + node), B0); B1 = fmaf(w, __ldg(by + node), B1); B2 = fmaf(w, __ldg(bz + node), B2);
+      if (PACKED) {
+        const float4 f0 = __ldg(pack + 2 * node), f1 = __ldg(pack + 2 * node + 1);
+        E0 = fmaf(w, f0.x, E0); E1 = fmaf(w, f0.y, E1); E2 = fmaf(w, f0.z, E2);
+        B0 = fmaf(w, f0.w, B0); B1 = fmaf(w, f1.x, B1); B2 = fmaf(w, f1.y, B2);
+      } else {
+        E0 = fmaf(w, __ldg(ex + node), E0); E1 = fmaf(w, __ldg(ey + node), E1); E2 = fmaf(w, __ldg(ez + node), E2);
+        B0 = fmaf(w, __ldg(bx + node), B0); B1 = fmaf(w, __ldg(by + node), B1); B2 = fmaf(w, __ldg(bz + node), B2);
+      }
     }
   }
   E0 += K.Eext[0]; E1 += K.Eext[1]; E2 += K.Eext[2];
@@ -457,7 +476,14 @@ extern "C" int jefi_push_particles(jefi_ctx* c, long np, float* x, float* y, flo
   K.sx = (float)(c->c * c->cfg.dt / c->cfg.dx); K.sy = (float)(c->c * c->cfg.dt / c->cfg.dy); K.sz = (float)(c->c * c->cfg.dt / c->cfg.dz);
   for (int a = 0; a < 3; a++) { K.Eext[a] = (float)c->cfg.Eext[a]; K.Bext[a] = (float)c->cfg.Bext[a]; }
   unsigned blocks = (unsigned)((np + 255) / 256);
-  k_push<<<blocks, 256, 0, c->stream>>>(K, np, x, y, z, ux, uy, uz, q_over_m, alive, ex, ey, ez, bx, by, bz);
+  if (np >= d.N) {  // enough particles per node for the packed copy of the fields to pay for itself
+    if (!c->eb_pack) JEFI_CUDA_TRY(c, cudaMalloc(&c->eb_pack, (size_t)d.N * 2 * sizeof(float4)));
+    k_pack_fields<<<(unsigned)((d.N + 255) / 256), 256, 0, c->stream>>>(d.N, ex, ey, ez, bx, by, bz, c->eb_pack);
+    k_push<true><<<blocks, 256, 0, c->stream>>>(K, np, x, y, z, ux, uy, uz, q_over_m, alive, ex, ey, ez, bx, by, bz, c->eb_pack);
+    c->launches++;
+  } else {
+    k_push<false><<<blocks, 256, 0, c->stream>>>(K, np, x, y, z, ux, uy, uz, q_over_m, alive, ex, ey, ez, bx, by, bz, nullptr);
+  }
   JEFI_CUDA_TRY(c, cudaGetLastError());
   c->launches++;
   return JEFI_OK;
