@@ -618,7 +618,13 @@ int jefi_launch_field_tiled(jefi_ctx* c, int k0, int k1, float* ex, float* ey, f
   if (P.atomic_out) {
     float* outs[6] = {ex, ey, ez, bx, by, bz};
     const size_t plane = (size_t)d.nx * d.ny;
-    for (float* o : outs) JEFI_CUDA_TRY(c, cudaMemsetAsync(o + plane * k0, 0, plane * (size_t)(k1 - k0) * sizeof(float), c->stream));
+    bool block = k0 == 0 && k1 == d.nz;  // full step into one [6][N] block (the usual case): one memset node
+    for (int a = 1; a < 6; a++) block = block && outs[a] == outs[a - 1] + d.N;
+    if (block) {
+      JEFI_CUDA_TRY(c, cudaMemsetAsync(ex, 0, (size_t)6 * d.N * sizeof(float), c->stream));
+    } else {
+      for (float* o : outs) JEFI_CUDA_TRY(c, cudaMemsetAsync(o + plane * k0, 0, plane * (size_t)(k1 - k0) * sizeof(float), c->stream));
+    }
   }
   dim3 grid((unsigned)(P.nobx * P.noby * nlayers), (unsigned)nsplit);
   tiled_kernel_for(c->wpitch, c->cfg.delay_rule == JEFI_DELAY_LINEAR)<<<grid, TILED_THREADS, c->tiled_smem, c->stream>>>(P);

@@ -284,10 +284,14 @@ extern "C" int jefi_deposit(jefi_ctx* c, long np, const float* x, const float* y
     return JEFI_EINVAL;
   }
   const jefi_dims& d = c->dims;
-  JEFI_CUDA_TRY(c, cudaMemsetAsync(rho, 0, d.N * sizeof(float), c->stream));
-  JEFI_CUDA_TRY(c, cudaMemsetAsync(jx, 0, d.N * sizeof(float), c->stream));
-  JEFI_CUDA_TRY(c, cudaMemsetAsync(jy, 0, d.N * sizeof(float), c->stream));
-  JEFI_CUDA_TRY(c, cudaMemsetAsync(jz, 0, d.N * sizeof(float), c->stream));
+  if (jx == rho + d.N && jy == jx + d.N && jz == jy + d.N) {  // one [4][N] block (the usual case): one memset node
+    JEFI_CUDA_TRY(c, cudaMemsetAsync(rho, 0, 4 * d.N * sizeof(float), c->stream));
+  } else {
+    JEFI_CUDA_TRY(c, cudaMemsetAsync(rho, 0, d.N * sizeof(float), c->stream));
+    JEFI_CUDA_TRY(c, cudaMemsetAsync(jx, 0, d.N * sizeof(float), c->stream));
+    JEFI_CUDA_TRY(c, cudaMemsetAsync(jy, 0, d.N * sizeof(float), c->stream));
+    JEFI_CUDA_TRY(c, cudaMemsetAsync(jz, 0, d.N * sizeof(float), c->stream));
+  }
   if (np == 0) return JEFI_OK;
   float inv_dV = (float)(1.0 / (c->cfg.dx * c->cfg.dy * c->cfg.dz));
   unsigned blocks = (unsigned)((np + 255) / 256);
