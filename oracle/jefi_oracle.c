@@ -18,8 +18,9 @@
  *               steps < 0 are zero, steps older than n-(H-1) are not stored and
  *               contribute zero (reading A15).
  *
- * Parity pins: tests/test_oracle_*.py (P1-P15 of SURVEY.md §8(c); L1-L5 for the linear retarded-time rule); nothing
- * here is "parity unpinned".
+ * Parity pins: tests/test_oracle_*.py (P1-P15 of SURVEY.md §8(c); P16 = the gamma of the Boris rotation when E and B are
+ * both non-zero, hand-computed 90-degree rotations; L1-L6 for the linear retarded-time rule); nothing here is
+ * "parity unpinned".
  */
 #include <math.h>
 #include <stddef.h>

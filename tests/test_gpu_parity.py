@@ -478,6 +478,40 @@ def test_push_parity_one_step_with_external_fields(J):
     ctx.close()
 
 
+def test_push_parity_strongly_relativistic_crossed_fields(J):
+    """u ~ 1, h E/c ~ 1 and h B/gamma ~ 1 per step (units c = 1): the regime in which the gamma of Eq. (2.10) matters (oracle pin
+    P16: gamma of u^-, reading A6); a push that took gamma from u^{n-1/2} would be off by O(0.1) here."""
+    import torch
+
+    n, dx, dt = 12, 50.0, 1.0
+    kw = dict(c=1.0, eps0=1.0, Eext=(0.3, -0.2, 0.1), Bext=(0.0, 0.5, -0.4))
+    cfg = OracleConfig(n, n, n, dx, dx, dx, dt, **kw)
+    ctx = make_ctx(J, (n, n, n), (dx, dx, dx), dt, J.JEFI_FIELD_REFERENCE, **kw)
+    rng = np.random.default_rng(160)
+    P = 20000
+    part = dict(x=rng.uniform(0, n, P), y=rng.uniform(0, n, P), z=rng.uniform(0, n, P), ux=rng.normal(0, 0.7, P),
+                uy=rng.normal(0, 0.7, P), uz=rng.normal(0, 0.7, P), qw=np.ones(P), qm=np.where(rng.uniform(size=P) < 0.5, -2.0, 2.0))
+    part = {k: v.astype(np.float32) for k, v in part.items()}
+    part["alive"] = np.ones(P, dtype=np.uint8)
+    F = rng.normal(0, 1.0, (6, cfg.N)).astype(np.float32)
+    F[3:] *= 1.5
+    dp = to_dev(part, ctx.device)
+    ctx.push_particles(dp, torch.from_numpy(F).to(ctx.device))
+    po = {k: v.astype(np.float64) for k, v in part.items() if k != "alive"}
+    alive_o = part["alive"].copy()
+    oracle.push(cfg, po["x"], po["y"], po["z"], po["ux"], po["uy"], po["uz"], po["qm"], alive_o, F[:3].astype(np.float64),
+                F[3:].astype(np.float64))
+    got = {k: v.cpu().numpy() for k, v in dp.items()}
+    assert (got["alive"] != alive_o).sum() <= 1
+    umax = max(np.abs(po[k]).max() for k in ("ux", "uy", "uz"))
+    assert umax > 2.0  # strongly relativistic
+    for k in ("ux", "uy", "uz"):
+        assert np.abs(got[k] - po[k]).max() <= 2e-6 * umax, k
+    for k in "xyz":
+        assert np.abs(got[k] - po[k]).max() / n <= 1e-6, k
+    ctx.close()
+
+
 # ------------------------------------------------------------------------------------------- closed loop (config 1)
 def run_closed_loop(J, config, steps, scale=1.0, impl=None, sort_every=0):
     import torch

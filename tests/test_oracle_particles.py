@@ -201,3 +201,65 @@ def test_p15_two_macro_charges_first_step_is_coulomb_between_clouds():
     assert part["uy"][0] == 0.0 and part["uz"][1] == 0.0
     v = C * part["ux"][1] / math.sqrt(1 + part["ux"][1] ** 2)
     assert np.isclose(part["x"][1], pb[0] + v * cfg.dt / cfg.dx, rtol=1e-15)
+
+
+# ---------------------------------------------------------------- P16 which gamma the rotation uses when E != 0 and B != 0
+def _rotated(ux, uy, ang):
+    return ux * math.cos(ang) - uy * math.sin(ang), ux * math.sin(ang) + uy * math.cos(ang)
+
+
+def _p16_case(sign, E, u0, via_grid):
+    """Heaviside-Lorentz-like units c = 1, dt = 2, q/m = sign (h = (q/m) dt/2 = sign), B = (0, 0, 2).  Expected values are
+    written out by hand from Eqs. (2.9)-(2.11) in the relativistic reading A6:
+      u^- = u + h E/c;  gamma^- = sqrt(1 + |u^-|^2);  the rotation of Eq. (2.10) turns the part of u^- perpendicular to B by
+      theta = 2 atan(h B/gamma^-) (clockwise about B for h B > 0, the pinned direction of P11);  u^{n+1/2} = u^+ + h E/c.
+    The numbers are chosen so that |u^-|^2 = 3 exactly: gamma^- = 2, |h| B/gamma^- = 1, theta = 90 degrees, i.e. the
+    perpendicular part goes (a, b) -> (b, -a) for h > 0 and (a, b) -> (-b, a) for h < 0.  Taking gamma from u^{n-1/2}
+    instead (sqrt(2) or sqrt(3) here) turns by 109.5 / 98.2 degrees: every component is then off by > 0.1."""
+    n, dx, dt = 8, 100.0, 2.0
+    kw = dict(c=1.0, eps0=1.0)
+    Bz = 2.0
+    if via_grid:
+        cfg = OracleConfig(n, n, n, dx, dx, dx, dt, **kw)
+        Eg = np.repeat(np.array(E, dtype=np.float64)[:, None], cfg.N, 1)
+        Bg = np.repeat(np.array([0.0, 0.0, Bz])[:, None], cfg.N, 1)
+    else:
+        cfg = OracleConfig(n, n, n, dx, dx, dx, dt, Eext=tuple(E), Bext=(0.0, 0.0, Bz), **kw)
+        Eg = Bg = np.zeros((3, cfg.N))
+    r0 = (4.0, 4.0, 4.0)  # interior: all 8 nodes inside, weights sum to 1 (P14), so a uniform grid field is exact
+    st = one_particle(r0, u0, float(sign))
+    oracle.push(cfg, *st, Eg, Bg)
+    return cfg, r0, np.array([st[0][0], st[1][0], st[2][0]]), np.array([st[3][0], st[4][0], st[5][0]]), st[7][0]
+
+
+def test_p16_boris_gamma_of_u_minus_E_parallel_B():
+    """E || B (both along z), u^{n-1/2} = (0.6, 0.8, 0), h E/c = +-sqrt(2): u^- = (0.6, 0.8, +-sqrt 2), |u^-|^2 = 3."""
+    r2 = math.sqrt(2.0)
+    for sign in (+1.0, -1.0):
+        for via_grid in (False, True):
+            cfg, r0, r1, u1, alive = _p16_case(sign, (0.0, 0.0, r2), (0.6, 0.8, 0.0), via_grid)
+            # perpendicular part (0.6, 0.8) turned by -+90 degrees; parallel part kicked twice by h E/c = sign sqrt 2
+            want_u = np.array([0.8, -0.6, 2 * r2]) if sign > 0 else np.array([-0.8, 0.6, -2 * r2])
+            assert np.allclose(u1, want_u, rtol=0, atol=1e-14), (sign, via_grid, u1)
+            g1 = math.sqrt(1.0 + 1.0 + 8.0)  # |u_new|^2 = 0.64 + 0.36 + 8
+            want_r = np.array(r0) + want_u / g1 * cfg.dt / cfg.dx  # Eq. (2.8), v = c u/gamma, grid units
+            assert np.allclose(r1, want_r, rtol=0, atol=1e-14) and alive == 1
+            # the misreading gamma(u^{n-1/2}) = sqrt 2 would turn by 2 atan(2/sqrt 2) instead: far outside 1e-6
+            bad = _rotated(0.6, 0.8, -sign * 2 * math.atan(2.0 / r2))
+            assert abs(bad[0] - want_u[0]) > 0.1
+
+
+def test_p16_boris_gamma_of_u_minus_E_perpendicular_B():
+    """E along x, B along z, u^{n-1/2} = (0, 1, 1), h E/c = +-1: u^- = (+-1, 1, 1), |u^-|^2 = 3, gamma^- = 2."""
+    for sign in (+1.0, -1.0):
+        for via_grid in (False, True):
+            cfg, r0, r1, u1, alive = _p16_case(sign, (1.0, 0.0, 0.0), (0.0, 1.0, 1.0), via_grid)
+            # h > 0: u^- = (1, 1, 1) -> u^+ = (1, -1, 1) -> + (1, 0, 0);  h < 0: u^- = (-1, 1, 1) -> u^+ = (-1, -1, 1) -> + (-1, 0, 0)
+            want_u = np.array([2.0, -1.0, 1.0]) if sign > 0 else np.array([-2.0, -1.0, 1.0])
+            assert np.allclose(u1, want_u, rtol=0, atol=1e-14), (sign, via_grid, u1)
+            g1 = math.sqrt(7.0)
+            want_r = np.array(r0) + want_u / g1 * cfg.dt / cfg.dx
+            assert np.allclose(r1, want_r, rtol=0, atol=1e-14) and alive == 1
+            # gamma(u^{n-1/2}) = sqrt 3 would give tan(theta/2) = 2/sqrt 3
+            bad = _rotated(sign * 1.0, 1.0, -sign * 2 * math.atan(2.0 / math.sqrt(3.0)))
+            assert abs(bad[1] - (-1.0)) > 0.1
