@@ -19,8 +19,8 @@
  *               contribute zero (reading A15).
  *
  * Parity pins: tests/test_oracle_*.py (P1-P15 of SURVEY.md §8(c); P16 = the gamma of the Boris rotation when E and B are
- * both non-zero, hand-computed 90-degree rotations; L1-L6 for the linear retarded-time rule); nothing here is
- * "parity unpinned".
+ * both non-zero, hand-computed 90-degree rotations; L1-L6 for the linear retarded-time rule; Q1-Q7 in
+ * tests/test_oracle_shape2.py for the S^(2) deposit / interpolation); nothing here is "parity unpinned".
  */
 #include <math.h>
 #include <stddef.h>
@@ -223,6 +223,87 @@ static void orc_gather(int nx, int ny, int nz, double xi, double eta, double zet
       }
 }
 
+/* ------------------------------------------------------------------------------------------------
+ * Second-order shape function S^(2), Eq. (2.14) with reading A11: the printed
+ * first range "0 <= |x| <= Delta" overlaps the second and must read 0 <= |x| <= Delta/2 (the two branches then meet at
+ * |x| = Delta/2 with value 1/2 and S^(2) is the quadratic B-spline):
+ *     S2(x) = (1/Delta^2) (-x^2 + 3/4 Delta^2)          for        |x| <= Delta/2
+ *           = (1/(8 Delta^2)) (2|x| - 3 Delta)^2        for Delta/2 <= |x| <= 3/2 Delta,      0 beyond.
+ * the same allocation as Eqs. (2.16)-(2.20) with S^(2) in place of the linear weights.
+ * A particle at xi (grid units, Delta = 1) lies in cell ic = floor(xi) whose centre is at ic + 1/2; the centres within
+ * 3/2 of it are ic-1, ic, ic+1, so 3 nodes per axis (27 in 3-D) get weight S2(xi - (node + 1/2)); the weight of node
+ * (a, b, c) is the product of the three axis weights, as for the volume weighting of Eq. (2.16).  Nodes outside the region
+ * are virtual and dropped / count as zero exactly as for first order (readings A8, A12).
+ * ---------------------------------------------------------------------------------------------- */
+static double orc_s2(double x) {
+  double ax = fabs(x);
+  if (ax <= 0.5) return -x * x + 0.75;
+  if (ax <= 1.5) return (2.0 * ax - 3.0) * (2.0 * ax - 3.0) / 8.0;
+  return 0.0;
+}
+
+/* the three nodes ic-1, ic, ic+1 of one axis and their weights */
+static inline void orc_cell_s2(double xi, long* ic, double w[3]) {
+  double f = floor(xi);
+  *ic = (long)f;
+  for (int a = -1; a <= 1; a++) w[a + 1] = orc_s2(xi - ((double)(*ic + a) + 0.5));
+}
+
+void orc_cell_index_s2(long np, const double* x, const double* y, const double* z, int32_t* ijk /* [np][3], centre node */) {
+  for (long p = 0; p < np; p++) {
+    ijk[3 * p] = (int32_t)floor(x[p]); ijk[3 * p + 1] = (int32_t)floor(y[p]); ijk[3 * p + 2] = (int32_t)floor(z[p]);
+  }
+}
+
+void orc_deposit_s2(int nx, int ny, int nz, double dx, double dy, double dz, double c, long np,
+                    const double* x, const double* y, const double* z,
+                    const double* ux, const double* uy, const double* uz,
+                    const double* qw, const uint8_t* alive,
+                    double* rho, double* jx, double* jy, double* jz) {
+  const size_t N = (size_t)nx * ny * nz;
+  const double dV = dx * dy * dz;
+  for (size_t cidx = 0; cidx < N; cidx++) { rho[cidx] = 0; jx[cidx] = 0; jy[cidx] = 0; jz[cidx] = 0; }
+  for (long p = 0; p < np; p++) {
+    if (alive && !alive[p]) continue;
+    long i, j, k; double wx[3], wy[3], wz[3];
+    orc_cell_s2(x[p], &i, wx); orc_cell_s2(y[p], &j, wy); orc_cell_s2(z[p], &k, wz);
+    double g = sqrt(1.0 + ux[p] * ux[p] + uy[p] * uy[p] + uz[p] * uz[p]);
+    double vx = c * ux[p] / g, vy = c * uy[p] / g, vz = c * uz[p] / g;
+    for (int cc = -1; cc <= 1; cc++)
+      for (int bb = -1; bb <= 1; bb++)
+        for (int aa = -1; aa <= 1; aa++) {
+          long ii = i + aa, jj = j + bb, kk = k + cc;
+          if (ii < 0 || ii >= nx || jj < 0 || jj >= ny || kk < 0 || kk >= nz) continue; /* virtual node */
+          double w = wx[aa + 1] * wy[bb + 1] * wz[cc + 1];
+          double r = qw[p] * w / dV;                                                    /* Eq. (2.18) */
+          size_t cidx = ii + (size_t)nx * (jj + (size_t)ny * kk);
+          rho[cidx] += r;
+          jx[cidx] += r * vx; jy[cidx] += r * vy; jz[cidx] += r * vz;                    /* Eq. (2.19) */
+        }
+  }
+}
+
+static void orc_gather_s2(int nx, int ny, int nz, double xi, double eta, double zeta,
+                          const double* fx, const double* fy, const double* fz, double out[3]) {
+  long i, j, k; double wx[3], wy[3], wz[3];
+  orc_cell_s2(xi, &i, wx); orc_cell_s2(eta, &j, wy); orc_cell_s2(zeta, &k, wz);
+  out[0] = out[1] = out[2] = 0;
+  for (int cc = -1; cc <= 1; cc++)
+    for (int bb = -1; bb <= 1; bb++)
+      for (int aa = -1; aa <= 1; aa++) {
+        long ii = i + aa, jj = j + bb, kk = k + cc;
+        if (ii < 0 || ii >= nx || jj < 0 || jj >= ny || kk < 0 || kk >= nz) continue;
+        double w = wx[aa + 1] * wy[bb + 1] * wz[cc + 1];
+        size_t cidx = ii + (size_t)nx * (jj + (size_t)ny * kk);
+        out[0] += w * fx[cidx]; out[1] += w * fy[cidx]; out[2] += w * fz[cidx];
+      }
+}
+
+void orc_interp_s2(int nx, int ny, int nz, long np, const double* x, const double* y, const double* z,
+                   const double* fx, const double* fy, const double* fz, double* out /* [np][3] */) {
+  for (long p = 0; p < np; p++) orc_gather_s2(nx, ny, nz, x[p], y[p], z[p], fx, fy, fz, out + 3 * p);
+}
+
 void orc_interp(int nx, int ny, int nz, long np, const double* x, const double* y, const double* z,
                 const double* fx, const double* fy, const double* fz, double* out /* [np][3] */) {
   for (long p = 0; p < np; p++) orc_gather(nx, ny, nz, x[p], y[p], z[p], fx, fy, fz, out + 3 * p);
@@ -232,18 +313,24 @@ void orc_interp(int nx, int ny, int nz, long np, const double* x, const double* 
  * readings A5/A6 (u = gamma v/c; identical to the paper's printed form as gamma -> 1), position update
  * Eq. (2.8), kill rule PAPER.md:205, 239 (reading A13).  Given momenta are u^{n-1/2} (reading A7).
  * Eext/Bext are uniform background fields added at the particle.
- * Positions in grid units, updated in place; alive[p] cleared when the particle leaves [0,n) on any axis. */
+ * Positions in grid units, updated in place; alive[p] cleared when the particle leaves [0,n) on any axis.
+ * shape_order: 1 = the paper's linear weights (Eq. 2.20), 2 = S^(2) (Eq. 2.14). */
 void orc_push(int nx, int ny, int nz, double dx, double dy, double dz, double dt, double c, long np,
               double* x, double* y, double* z, double* ux, double* uy, double* uz,
               const double* q_over_m, uint8_t* alive,
               const double* ex, const double* ey, const double* ez,
               const double* bx, const double* by, const double* bz,
-              const double* Eext, const double* Bext) {
+              const double* Eext, const double* Bext, int shape_order) {
   for (long p = 0; p < np; p++) {
     if (!alive[p]) continue;
     double Ep[3], Bp[3];
-    orc_gather(nx, ny, nz, x[p], y[p], z[p], ex, ey, ez, Ep);   /* Eq. (2.20) */
-    orc_gather(nx, ny, nz, x[p], y[p], z[p], bx, by, bz, Bp);
+    if (shape_order == 2) {                                        /* S^(2) weights, Eq. (2.14) */
+      orc_gather_s2(nx, ny, nz, x[p], y[p], z[p], ex, ey, ez, Ep);
+      orc_gather_s2(nx, ny, nz, x[p], y[p], z[p], bx, by, bz, Bp);
+    } else {
+      orc_gather(nx, ny, nz, x[p], y[p], z[p], ex, ey, ez, Ep);   /* Eq. (2.20) */
+      orc_gather(nx, ny, nz, x[p], y[p], z[p], bx, by, bz, Bp);
+    }
     for (int a = 0; a < 3; a++) { Ep[a] += Eext[a]; Bp[a] += Bext[a]; }
     double h = q_over_m[p] * dt / 2.0;
     /* Eq. (2.9): half electric kick */

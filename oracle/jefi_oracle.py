@@ -56,7 +56,10 @@ def _L():
         lib.orc_cell_index.argtypes = [i64, p, p, p, p]
         lib.orc_deposit.argtypes = [i32, i32, i32, dbl, dbl, dbl, dbl, i64] + [p] * 12
         lib.orc_interp.argtypes = [i32, i32, i32, i64] + [p] * 7
-        lib.orc_push.argtypes = [i32, i32, i32, dbl, dbl, dbl, dbl, dbl, i64] + [p] * 16
+        lib.orc_push.argtypes = [i32, i32, i32, dbl, dbl, dbl, dbl, dbl, i64] + [p] * 16 + [i32]
+        lib.orc_cell_index_s2.argtypes = [i64, p, p, p, p]
+        lib.orc_deposit_s2.argtypes = lib.orc_deposit.argtypes
+        lib.orc_interp_s2.argtypes = lib.orc_interp.argtypes
         _lib = lib
     return _lib
 
@@ -87,6 +90,7 @@ class OracleConfig:
     Eext: Sequence[float] = (0.0, 0.0, 0.0)
     Bext: Sequence[float] = (0.0, 0.0, 0.0)
     delay_rule: int = 0  # RULE_NEAREST (reading A1) or RULE_LINEAR (reading A22)
+    shape_order: int = 1  # 1 = linear / CIC weights (Eqs. 2.16, 2.20, what the paper uses); 2 = S^(2), Eq. (2.14) (NEXT-4)
 
     def __post_init__(self):
         if self.H == 0:
@@ -147,19 +151,24 @@ def field(cfg: OracleConfig, n: int, ring: np.ndarray, obs_idx: Optional[np.ndar
     return E, B
 
 
-def cell_index(x, y, z) -> np.ndarray:
+def cell_index(x, y, z, shape_order: int = 1) -> np.ndarray:
+    """Base node floor(xi - 1/2) of the 8 linear weights (Eq. 2.15), or for shape_order 2 the centre node floor(xi) of the
+    27 S^(2) weights."""
     x, y, z = _f64(x), _f64(y), _f64(z)
     out = np.empty((x.shape[0], 3), dtype=np.int32)
-    _L().orc_cell_index(x.shape[0], _ptr(x), _ptr(y), _ptr(z), _ptr(out))
+    fn = _L().orc_cell_index_s2 if shape_order == 2 else _L().orc_cell_index
+    fn(x.shape[0], _ptr(x), _ptr(y), _ptr(z), _ptr(out))
     return out
 
 
 def deposit(cfg: OracleConfig, x, y, z, ux, uy, uz, qw, alive=None):
-    """CIC deposit (Eqs. 2.15-2.19).  Positions in grid units, u = gamma v / c.  Returns [4][N] float64."""
+    """CIC deposit (Eqs. 2.15-2.19; 27-node S^(2) weights of Eq. 2.14 when cfg.shape_order == 2).  Positions in grid
+    units, u = gamma v / c.  Returns [4][N] float64."""
     x, y, z, ux, uy, uz, qw = map(_f64, (x, y, z, ux, uy, uz, qw))
     al = None if alive is None else np.ascontiguousarray(alive, dtype=np.uint8)
     out = np.empty((4, cfg.N), dtype=np.float64)
-    _L().orc_deposit(cfg.nx, cfg.ny, cfg.nz, cfg.dx, cfg.dy, cfg.dz, cfg.c, x.shape[0], _ptr(x), _ptr(y), _ptr(z),
+    fn = _L().orc_deposit_s2 if cfg.shape_order == 2 else _L().orc_deposit
+    fn(cfg.nx, cfg.ny, cfg.nz, cfg.dx, cfg.dy, cfg.dz, cfg.c, x.shape[0], _ptr(x), _ptr(y), _ptr(z),
                      _ptr(ux), _ptr(uy), _ptr(uz), _ptr(qw), _ptr(al), _ptr(out[0]), _ptr(out[1]), _ptr(out[2]),
                      _ptr(out[3]))
     return out
@@ -170,7 +179,8 @@ def interp(cfg: OracleConfig, x, y, z, F):
     x, y, z = map(_f64, (x, y, z))
     F = _f64(F)
     out = np.empty((x.shape[0], 3), dtype=np.float64)
-    _L().orc_interp(cfg.nx, cfg.ny, cfg.nz, x.shape[0], _ptr(x), _ptr(y), _ptr(z), _ptr(F[0]), _ptr(F[1]), _ptr(F[2]),
+    fn = _L().orc_interp_s2 if cfg.shape_order == 2 else _L().orc_interp
+    fn(cfg.nx, cfg.ny, cfg.nz, x.shape[0], _ptr(x), _ptr(y), _ptr(z), _ptr(F[0]), _ptr(F[1]), _ptr(F[2]),
                     _ptr(out))
     return out
 
@@ -184,7 +194,7 @@ def push(cfg: OracleConfig, x, y, z, ux, uy, uz, q_over_m, alive, E, B):
     Eext, Bext = _f64(cfg.Eext), _f64(cfg.Bext)
     _L().orc_push(cfg.nx, cfg.ny, cfg.nz, cfg.dx, cfg.dy, cfg.dz, cfg.dt, cfg.c, x.shape[0], _ptr(x), _ptr(y), _ptr(z),
                   _ptr(ux), _ptr(uy), _ptr(uz), _ptr(q_over_m), _ptr(alive), _ptr(E[0]), _ptr(E[1]), _ptr(E[2]),
-                  _ptr(B[0]), _ptr(B[1]), _ptr(B[2]), _ptr(Eext), _ptr(Bext))
+                  _ptr(B[0]), _ptr(B[1]), _ptr(B[2]), _ptr(Eext), _ptr(Bext), int(cfg.shape_order))
 
 
 class OracleJefi:
