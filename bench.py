@@ -1,21 +1,29 @@
 #!/usr/bin/env python
 """bench.py — Jefimenko field-solve throughput on B200 (BASELINE.json metric), one JSON line on stdout.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload 4] [--no-pic] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload 4|analytic20|slab251] [--no-pic] [--impl reference]
 
 Product arm: the timed "step" is one pass of the field path over the 96^3 field-only workload (BASELINE.json
 configs[3], the one the metric "G source-obs pairs/s and % FP32 peak" is quoted on): jefi_push_sources of a fresh
 seeded source slice already resident in HBM + jefi_field_step.  The ring (9.5 GB) is far larger than L2, so no
-L2 flush is needed between iterations.  `e2e` repeats it through jefi_field_step_host with pinned HOST buffers.
-`pic` adds PIC steps/s (deposit -> push_sources -> field_step -> push_particles) on configs 1-3.
+L2 flush is needed between iterations (workloads whose ring would fit in L2 are timed step by step with a 512 MB fill
+in between).  `e2e` repeats it through jefi_field_step_host with pinned HOST buffers.
+`pic` adds PIC steps/s (deposit -> push_sources -> field_step -> push_particles) on configs 1, 2, 3, 5;
+`paper_workloads` the pairs/s of the paper's own shapes (20^3 at kappa = 6, the 1x251x111 slab).
 Reference arm (--impl reference): the fp64 CPU oracle, as it stands, on a bounded sample of the same workload.
-N > 1: replicas only: every rank runs the same workload on its own GPU, no data-path collective.
+N > 1: one process per GPU.  Under torchrun (WORLD_SIZE set) this process is one rank; without it `--gpus N` re-executes
+itself under `python -m torch.distributed.run --nproc-per-node N` so that N ranks really run.  Default: replicas
+(every rank runs the same workload on its own GPU, no data-path collective); `--shard obs` splits the
+observation planes of ONE step over the ranks and assembles E, B with an NCCL all-reduce.
 """
 from __future__ import annotations
 
 import argparse
+import hashlib
 import json
 import os
+import socket
+import subprocess
 import sys
 import threading
 import time
@@ -30,9 +38,31 @@ from paper_2209_07944_b200 import workloads as wl  # noqa: E402
 # FP32 roofline of the field kernel ("bound": "alu"): 148 SMs x 128 FP32 lanes x 2 FLOP x max SM clock.
 N_SM, LANES = 148, 128
 FLOP_PER_PAIR = 48.0  # 24 FMA per source-observation pair
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE k_field_tiled launch, from the committed ncu --set full capture
-# (profiles/r1_v6_field_tiled_ncu_full.md: 85.259 GB + 52.9 MB); the ring itself is 9.56 GB, L2 hit rate 90 %.
-FIELD_DRAM_BYTES = {(4, "nearest"): 85.259e9 + 52.9e6}
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE k_field_tiled launch, per (workload, delay rule), each from a committed
+# `ncu --set full` capture under profiles/ and valid only for the kernel source it was taken from: the entry names the file
+# and the sha1 (first 12 hex digits) of csrc/jefi_field.cu + csrc/jefi_ctx.h of that build.  With a different kernel source
+# `traffic` is null and `traffic_source` says the capture is stale.
+FIELD_DRAM_BYTES = {
+    # (workload name, rule): (bytes, profile, kernel source sha)  -- filled from profiles/r2_*_ncu_full.md
+}
+
+
+def kernel_source_sha() -> str:
+    h = hashlib.sha1()
+    for f in ("jefi_field.cu", "jefi_ctx.h"):
+        with open(os.path.join(ROOT, "paper_2209_07944_b200", "csrc", f), "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()[:12]
+
+
+def field_traffic(name: str, rule: str):
+    ent = FIELD_DRAM_BYTES.get((name, rule))
+    if ent is None:
+        return None, "no ncu --set full capture of this workload / rule under profiles/"
+    nbytes, prof, sha = ent
+    if sha != kernel_source_sha():
+        return None, f"stale: {prof} was captured on kernel source {sha}, this build is {kernel_source_sha()}"
+    return nbytes, prof
 
 
 def log(*a):
@@ -98,11 +128,18 @@ def visible_gpu_index(local_rank: int) -> int:
 
 
 # --------------------------------------------------------------------------------------------------- reference arm
-def oracle_sample_rate(w: wl.Workload, ring_host: np.ndarray, n_obs: int, seed_tag: int, rule: int = 0):
+def oracle_config(w: wl.FieldWorkload, rule: int = 0):
+    import oracle
+
+    kw = dict(c=w.c, eps0=w.eps0) if w.c > 0 else {}
+    return oracle.OracleConfig(*w.shape, *w.h, w.dt, delay_rule=rule, **kw)
+
+
+def oracle_sample_rate(w: wl.FieldWorkload, ring_host: np.ndarray, n_obs: int, seed_tag: int, rule: int = 0):
     """Oracle pairs/s on n_obs seeded observation cells against all sources (fp64, all host cores)."""
     import oracle
 
-    cfg = oracle.OracleConfig(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt, delay_rule=rule)
+    cfg = oracle_config(w, rule)
     obs = np.random.default_rng([w.seed, seed_tag]).integers(0, w.N, size=n_obs, dtype=np.int64)
     t0 = time.perf_counter()
     oracle.field(cfg, w.H - 1, ring_host, obs)
@@ -110,20 +147,26 @@ def oracle_sample_rate(w: wl.Workload, ring_host: np.ndarray, n_obs: int, seed_t
     return n_obs * (w.N - 1) / dt, dt
 
 
-def host_ring(w: wl.Workload) -> np.ndarray:
+def host_ring(w: wl.FieldWorkload) -> np.ndarray:
     ring = np.empty((w.H, 4, w.N), dtype=np.float32)
     for t in range(w.H):
-        ring[t] = wl.history_slice(w.N, t, w.seed)
+        ring[t] = w.slice(t)
     return ring
 
 
-def run_reference(args, w: wl.Workload) -> dict:
+def workload_config(w: wl.FieldWorkload, rule: str) -> dict:
+    """The `config` object both arms print (same keys, so that the driver can match the two lines)."""
+    return {"workload": w.name, "grid": list(w.shape), "H": w.H, "dx": w.h[0], "dt": w.dt, "kappa": round(w.kappa, 6),
+            "pairs_per_step": float(w.N) * float(w.N - 1), "delay_rule": rule}
+
+
+def run_reference(args, w: wl.FieldWorkload) -> dict:
     import oracle
 
     cores = oracle.num_threads()
     log(f"[reference] building the {w.H}-slot host history of {w.name} ...")
     ring = host_ring(w)
-    n_obs = args.ref_obs
+    n_obs = min(args.ref_obs, w.N)
     rates = []
     for i in range(args.warmup + args.steps):
         r, dt = oracle_sample_rate(w, ring, n_obs, i, 1 if args.delay_rule == "linear" else 0)
@@ -137,7 +180,7 @@ def run_reference(args, w: wl.Workload) -> dict:
     return {"impl": "reference", "metric": "jefimenko_source_obs_pairs_per_s", "value": val, "unit": "Gpairs/s",
             "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / len(rates),
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": w.name, "grid": [w.n] * 3, "H": w.H, "dx": w.dx, "dt": w.dt, "delay_rule": args.delay_rule},
+            "config": workload_config(w, args.delay_rule),
             "cpu_baseline": {"value": val, "unit": "Gpairs/s", "cores": cores, "kind": "oracle", "sample": sample},
             "e2e": {"value": val, "unit": "Gpairs/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -171,7 +214,7 @@ def aggregate_rate(world: int, pairs_per_rank: float, ms_max: float) -> float:
 
 def time_pic(J, torch, device, config: int, steps: int, warmup: int) -> dict:
     w = wl.WORKLOADS[config]
-    ctx = J.JefiContext(J.GridSpec(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt), device=device, sort_every=8)
+    ctx = J.JefiContext(J.GridSpec(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt), device=device)  # cell sort every 8 steps, packed E/B
     part = {k: torch.from_numpy(v).to(device) for k, v in wl.particles(config).items()}
     for _ in range(warmup):
         ctx.pic_step(part)
@@ -184,10 +227,10 @@ def time_pic(J, torch, device, config: int, steps: int, warmup: int) -> dict:
     e1.record()
     torch.cuda.synchronize(device)
     ms = e0.elapsed_time(e1) / steps
-    fk = ctx.last_field_kernel_ms()
+    fk = float(np.mean([ctx.field_kernel_ms(i) for i in range(min(steps, 64))]))
     out = {"workload": w.name, "steps": steps, "warmup": warmup, "ms_per_step": ms, "steps_per_s": 1e3 / ms,
            "particles": int(part["x"].numel()), "field_kernel_ms": fk, "launches": ctx.launch_count() - l0,
-           "field_impl": ctx.info["field_impl"]}
+           "field_impl": ctx.info["field_impl"], "tiles": ctx.tile_info}
     ctx.close()
     return out
 
@@ -271,7 +314,51 @@ def time_particle_kernels(J, torch, device, config: int = 5, reps: int = 5) -> d
     return out
 
 
-def run_product(args, w: wl.Workload) -> dict:
+def fp32_peak_tflops(sm_max_mhz) -> float:
+    return N_SM * LANES * 2 * (sm_max_mhz or 1965.0) * 1e6 / 1e12
+
+
+def time_field_workload(J, torch, device, w: wl.FieldWorkload, rule: str, steps: int, warmup: int, sm_max_mhz) -> dict:
+    """pairs/s of one field-only workload on one GPU (the `paper_workloads` leg): H pushes fill the history, then `steps`
+    steps of jefi_push_sources + jefi_field_step, each timed with its own CUDA events; the ring of these small grids would
+    fit in L2, so a 512 MB fill runs between steps."""
+    ctx = J.JefiContext(J.GridSpec(*w.shape, *w.h, w.dt, c=w.c, eps0=w.eps0), device=device,
+                        delay_rule=J.JEFI_DELAY_LINEAR if rule == "linear" else J.JEFI_DELAY_NEAREST)
+    for t in range(w.H):
+        ctx.push_sources(torch.from_numpy(w.slice(t)).to(device))
+    fresh = [torch.from_numpy(w.slice(w.H + i)).to(device) for i in range(4)]
+    flush = torch.empty(128 * 1024 * 1024, dtype=torch.float32, device=device)
+    ms, kms = [], []
+    for i in range(warmup + steps):
+        flush.fill_(float(i))
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        ctx.push_sources(fresh[i % 4])
+        ctx.field_step()
+        e1.record()
+        torch.cuda.synchronize(device)
+        if i >= warmup:
+            ms.append(e0.elapsed_time(e1))
+            kms.append(ctx.last_field_kernel_ms())
+    pairs = float(w.N) * float(w.N - 1)
+    step_ms, kernel_ms = float(np.mean(ms)), float(np.mean(kms))
+    peak = fp32_peak_tflops(sm_max_mhz)
+    achieved = FLOP_PER_PAIR * pairs / (kernel_ms * 1e-3) / 1e12
+    out = {"config": workload_config(w, rule), "value": pairs / (step_ms * 1e-3) / 1e9, "unit": "Gpairs/s", "ms_per_step": step_ms,
+           "steps": steps, "warmup": warmup, "l2": "512 MB fill between steps",
+           "field_impl": ctx.info["field_impl"], "field_impl_reason": ctx.info["field_impl_reason"], "tiles": ctx.tile_info,
+           "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+                        "kernel_ms": kernel_ms, "peak_source": PEAK_SOURCE}}
+    ctx.close()
+    del flush
+    return out
+
+
+PEAK_SOURCE = ("of derived: 148 SM x 128 FP32 lanes x 2 FLOP x clocks.max.sm (MEASURED_PEAKS.json has no FP32 figure; an FFMA-chain "
+               "probe on the box reaches 0.97 of it, profiles/r2_fp32_peak.md)")
+
+
+def run_product(args, w: wl.FieldWorkload) -> dict:
     import torch
 
     from paper_2209_07944_b200 import jefi as J
@@ -288,19 +375,20 @@ def run_product(args, w: wl.Workload) -> dict:
         import torch.distributed as dist
 
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("NCCL_DEBUG", "INFO")  # the rank count is visible in the log
         dist.init_process_group("nccl", device_id=device)
     J.load_library()
 
-    ctx = J.JefiContext(J.GridSpec(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt), device=device,
+    ctx = J.JefiContext(J.GridSpec(*w.shape, *w.h, w.dt, c=w.c, eps0=w.eps0), device=device,
                         delay_rule=J.JEFI_DELAY_LINEAR if args.delay_rule == "linear" else J.JEFI_DELAY_NEAREST)
     N, H = w.N, ctx.H
     assert H == w.H
     keep_host = (rank == 0 and world == 1 and not args.no_cpu_baseline)
     ring_host = np.empty((H, 4, N), dtype=np.float32) if keep_host else None
-    log(f"[rank {rank}] {w.name}: N={N} H={H} ring={ctx.info['ring_bytes'] / 1e9:.2f} GB field_impl={ctx.info['field_impl']}")
+    log(f"[rank {rank}/{world}] {w.name}: N={N} H={H} ring={ctx.info['ring_bytes'] / 1e9:.2f} GB; {ctx.info['field_impl_reason']}")
     t0 = time.perf_counter()
     for t in range(H):  # fill the history so that every delay is valid at the timed steps
-        s = wl.history_slice(N, t, w.seed)
+        s = w.slice(t)
         if keep_host:
             ring_host[t] = s
         ctx.push_sources(torch.from_numpy(s).to(device, non_blocking=False))
@@ -308,8 +396,11 @@ def run_product(args, w: wl.Workload) -> dict:
     log(f"[rank {rank}] history filled in {time.perf_counter() - t0:.1f} s")
 
     nfresh = args.warmup + args.steps
-    fresh = [torch.from_numpy(wl.history_slice(N, H + i, w.seed)).to(device) for i in range(min(nfresh, 8))]
+    fresh = [torch.from_numpy(w.slice(H + i)).to(device) for i in range(min(nfresh, 8))]
     pairs = float(N) * float(N - 1)
+    # inputs larger than L2 need no flush; a ring that would (nearly) fit in the 126 MB L2 is flushed between steps
+    need_flush = ctx.info["ring_bytes"] < 512 * 1024 * 1024
+    flush = torch.empty(128 * 1024 * 1024, dtype=torch.float32, device=device) if need_flush else None
 
     def barrier():
         if dist is not None:
@@ -317,14 +408,16 @@ def run_product(args, w: wl.Workload) -> dict:
         torch.cuda.synchronize(device)
 
     # --shard obs (N > 1): every rank holds the whole history and solves its slab of observation planes, then E, B are
-    # assembled over NVLink (strong scaling of ONE field step).  Default: replicas (DESIGN.md §9).
+    # assembled over NVLink (strong scaling of ONE field step).  Default: replicas (DESIGN.md section 9).
     shard = args.shard == "obs" and world > 1
-    k0, k1 = J.slab_range(w.n, rank, world) if shard else (0, w.n)
+    nz = w.shape[2]
+    k0, k1 = ctx.slab_range(rank, world) if shard else (0, nz)
+    plane = w.shape[0] * w.shape[1]
 
     def field_step():
         if shard:
             ctx.field_step_slab(k0, k1)
-            assemble_slabs(dist, ctx.EB, w.n * w.n, k0, k1)
+            assemble_slabs(dist, ctx.EB, plane, k0, k1)
         else:
             ctx.field_step()
 
@@ -335,33 +428,43 @@ def run_product(args, w: wl.Workload) -> dict:
     barrier()
     sampler = ClockSampler(visible_gpu_index(local))
     sampler.start()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     l0 = ctx.launch_count()
     barrier()
-    e0.record()
-    for i in range(args.steps):
-        ctx.push_sources(fresh[(args.warmup + i) % len(fresh)])
-        field_step()
-    e1.record()
-    barrier()
+    if not need_flush:
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for i in range(args.steps):
+            ctx.push_sources(fresh[(args.warmup + i) % len(fresh)])
+            field_step()
+        e1.record()
+        barrier()
+        step_ms = e0.elapsed_time(e1) / args.steps
+    else:
+        evs = []
+        for i in range(args.steps):
+            flush.fill_(float(i))
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            ctx.push_sources(fresh[(args.warmup + i) % len(fresh)])
+            field_step()
+            e1.record()
+            evs.append((e0, e1))
+        barrier()
+        step_ms = float(np.mean([a.elapsed_time(b) for a, b in evs]))
     clocks = sampler.stop()
     launches = ctx.launch_count() - l0
-    step_ms = e0.elapsed_time(e1) / args.steps
-    # per-launch duration of the dominant kernel: CUDA events recorded by the library on the launching stream
-    # around the kernel alone, over a second pass of the same launches (keeps the timed region free of syncs)
-    kms = []
-    for i in range(max(3, min(args.steps, 8))):
-        ctx.push_sources(fresh[i % len(fresh)])
-        ctx.field_step()
-        kms.append(ctx.last_field_kernel_ms())
+    # per-launch duration of the dominant kernel FROM THE TIMED LAUNCHES: the library records CUDA events on its stream around
+    # the field kernel of every step (it keeps the last 64); they are read back here, after the timed region
+    kms = [ctx.field_kernel_ms(i) for i in range(min(args.steps, 64))]
     kernel_ms = float(np.mean(kms))
     step_ms_max = max_over_ranks(dist, step_ms, device)
     value = aggregate_rate(1 if shard else world, pairs, step_ms_max)  # sharded: the job is ONE step of N^2 pairs
+    pairs_per_launch = pairs * (k1 - k0) / nz if shard else pairs
 
     # ---- end to end through the C-ABI with host buffers ----
     src_pin = torch.empty(4 * N, dtype=torch.float32).pin_memory()
     eb_pin = torch.empty(6 * N, dtype=torch.float32).pin_memory()
-    src_pin.copy_(torch.from_numpy(wl.history_slice(N, H + 100, w.seed).reshape(-1)))
+    src_pin.copy_(torch.from_numpy(w.slice(H + 100).reshape(-1)))
     J.jefi_field_step_host(ctx.handle, N, src_pin, eb_pin)  # warm-up (allocates the staging buffers)
     barrier()
     e2e_steps = max(1, min(args.steps, 3))
@@ -374,26 +477,30 @@ def run_product(args, w: wl.Workload) -> dict:
     e2e_val = aggregate_rate(1 if shard else world, pairs, e2e_ms_max)  # sharded runs: one rank's own full step
     checksum = float(eb_pin[:N].double().abs().sum())
 
-    impl = ctx.info["field_impl"]
+    impl, reason, tiles = ctx.info["field_impl"], ctx.info["field_impl_reason"], ctx.tile_info
     ctx.close()
+    del flush
     torch.cuda.empty_cache()
 
     out = None
     if rank == 0:
         sm_max = clocks.get("sm_max_mhz") or 1965.0
-        peak = N_SM * LANES * 2 * sm_max * 1e6 / 1e12
-        achieved = FLOP_PER_PAIR * pairs / (kernel_ms * 1e-3) / 1e12
+        peak = fp32_peak_tflops(sm_max)
+        achieved = FLOP_PER_PAIR * pairs_per_launch / (kernel_ms * 1e-3) / 1e12
+        traffic, traffic_src = field_traffic(w.name, args.delay_rule)
+        cfg = workload_config(w, args.delay_rule)
+        cfg.update({"l2": "512 MB fill between timed steps" if need_flush else f"inputs ({ctx.info['ring_bytes'] / 1e9:.1f} GB ring) larger than L2, no flush",
+                    "parallelism": ("obs_slabs" if shard else "replicas") if world > 1 else "single", "field_impl": impl,
+                    "field_impl_reason": reason, "tiles": tiles})
         out = {"metric": "jefimenko_source_obs_pairs_per_s", "value": value, "unit": "Gpairs/s", "n_gpus": world,
                "steps": args.steps, "warmup": args.warmup, "ms_per_step": step_ms_max, "higher_is_better": True,
                "scaling": "strong" if shard else "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-               "config": {"workload": w.name, "grid": [w.n] * 3, "H": H, "dx": w.dx, "dt": w.dt,
-                          "pairs_per_step": pairs, "l2": "inputs (9.5 GB ring) larger than L2, no flush",
-                          "parallelism": ("obs_slabs" if shard else "replicas") if world > 1 else "single", "field_impl": impl,
-                          "delay_rule": args.delay_rule},
+               "config": cfg,
                "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                            "traffic": FIELD_DRAM_BYTES.get((w.config, args.delay_rule)), "kernel": "k_field_tiled" if impl == 2 else "k_field_reference",
-                            "kernel_ms": kernel_ms, "flop_per_pair": FLOP_PER_PAIR,
-                            "peak_source": "148 SM x 128 FP32 lanes x 2 FLOP x clocks.max.sm (derived, DESIGN.md §7)"},
+                            "traffic": traffic, "traffic_source": traffic_src,
+                            "kernel": "k_field_tiled" if impl == 2 else "k_field_reference",
+                            "kernel_ms": kernel_ms, "kernel_ms_source": f"CUDA events around the field kernel of the {len(kms)} timed steps",
+                            "flop_per_pair": FLOP_PER_PAIR, "peak_source": PEAK_SOURCE, "kernel_source_sha": kernel_source_sha()},
                "e2e": {"value": e2e_val, "unit": "Gpairs/s", "h2d_bytes_per_step": 16 * N, "d2h_bytes_per_step": 24 * N,
                        "ms_per_step": e2e_ms_max, "checksum_abs_ex": checksum},
                "gpu_launches": int(launches), "clocks": clocks}
@@ -404,6 +511,14 @@ def run_product(args, w: wl.Workload) -> dict:
                     out["pic"].append(time_pic(J, torch, device, cfgno, st, wu))
                 except Exception as e:  # noqa: BLE001
                     out["pic"].append({"workload": wl.WORKLOADS[cfgno].name, "error": str(e)})
+            out["paper_workloads"] = []
+            for key in ("analytic20", "slab251"):
+                if wl.field_workload(key).name == w.name:
+                    continue
+                try:
+                    out["paper_workloads"].append(time_field_workload(J, torch, device, wl.field_workload(key), "nearest", 20, 3, sm_max))
+                except Exception as e:  # noqa: BLE001
+                    out["paper_workloads"].append({"config": {"workload": key}, "error": str(e)})
             try:
                 out["particle_kernels"] = time_particle_kernels(J, torch, device)
             except Exception as e:  # noqa: BLE001
@@ -411,9 +526,10 @@ def run_product(args, w: wl.Workload) -> dict:
         if keep_host:
             import oracle
 
-            r, dt = oracle_sample_rate(w, ring_host, args.cpu_obs, 0, 1 if args.delay_rule == "linear" else 0)
+            nobs = min(args.cpu_obs, N)
+            r, dt = oracle_sample_rate(w, ring_host, nobs, 0, 1 if args.delay_rule == "linear" else 0)
             out["cpu_baseline"] = {"value": r / 1e9, "unit": "Gpairs/s", "cores": oracle.num_threads(), "kind": "oracle",
-                                   "sample": f"{args.cpu_obs} seeded observation cells x all {N - 1} source cells "
+                                   "sample": f"{nobs} seeded observation cells x all {N - 1} source cells "
                                              f"({dt:.1f} s of fp64 CPU work)"}
         else:
             out["cpu_baseline"] = None
@@ -423,14 +539,27 @@ def run_product(args, w: wl.Workload) -> dict:
     return out
 
 
+def spawn_command(argv, gpus: int, port: int):
+    """`python bench.py --gpus N` outside torchrun: the command that re-runs this file with N ranks, one per GPU."""
+    return [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={gpus}", "--master-addr", "127.0.0.1",
+            "--master-port", str(port), os.path.abspath(__file__)] + list(argv)
+
+
+def free_port() -> int:
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        return sk.getsockname()[1]
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="jefi", choices=["jefi", "reference"])
-    ap.add_argument("--workload", type=int, default=4, help="BASELINE.json config number of the field workload (4 = 96^3)")
-    ap.add_argument("--no-pic", action="store_true", help="skip the PIC steps/s legs on configs 1-3")
+    ap.add_argument("--workload", default="4", help="field workload: BASELINE.json config number (4 = 96^3, the default), or one of "
+                    "the paper's own shapes: analytic20 (20^3, kappa = 6), slab251 (1x251x111), slab101")
+    ap.add_argument("--no-pic", action="store_true", help="skip the PIC steps/s, paper-workload and particle-kernel legs")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--shard", default="replicas", choices=["replicas", "obs"],
                     help="N > 1: replicas (default, weak scaling) or observation z-slabs of one field step (strong scaling)")
@@ -440,8 +569,15 @@ def main():
     ap.add_argument("--cpu-obs", type=int, default=4096, help="observation cells of the cpu_baseline sample")
     ap.add_argument("--ref-obs", type=int, default=1024, help="observation cells per step of --impl reference")
     args = ap.parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # not under torchrun: start the N ranks ourselves (their stdout/stderr pass through; rank 0 prints the one JSON line)
+        rc = subprocess.call(spawn_command(sys.argv[1:], args.gpus, free_port()))
+        sys.exit(rc)
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if world != args.gpus:
+        log(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}; the launcher's world size is what runs and is reported")
     args.warmup = max(args.warmup, 3) if args.impl == "jefi" else max(args.warmup, 0)
-    w = wl.WORKLOADS[args.workload]
+    w = wl.field_workload(args.workload)
     rank = int(os.environ.get("RANK", "0"))
     if args.particles_only:
         import torch
@@ -452,7 +588,8 @@ def main():
         res = time_particle_kernels(J, torch, torch.device("cuda:0"), reps=max(1, args.steps))
     elif args.impl == "reference":
         if rank != 0:
-            return  # rank 0 alone runs the CPU oracle
+            log(f"[reference] rank {rank} of {world}: idle (rank 0 alone runs the CPU oracle)")
+            return
         res = run_reference(args, w)
     else:
         res = run_product(args, w)

@@ -35,7 +35,8 @@ extern "C" {
 #define JEFI_ESTATE (-4) /* call not valid in this state (e.g. field_step before any push_sources) */
 
 /* field_impl values */
-#define JEFI_FIELD_AUTO 0      /* tiled kernel when its delay arithmetic is proven equal to the fp64 table, else reference */
+#define JEFI_FIELD_AUTO 0      /* tiled kernel when its delay arithmetic is proven equal to the fp64 table, else reference;
+                                  jefi_field_impl_reason() says which one runs and why */
 #define JEFI_FIELD_REFERENCE 1 /* one thread per observation cell, table-driven delays (slow; the paper's K1 in fp32) */
 #define JEFI_FIELD_TILED 2     /* shared-memory tiled kernel; jefi_create fails with JEFI_ESTATE if not provable */
 
@@ -69,6 +70,13 @@ typedef struct {
   int field_impl;       /* JEFI_FIELD_* */
   int deposit_mode;     /* JEFI_DEPOSIT_* */
   int delay_rule;       /* JEFI_DELAY_* */
+  int shape_order;      /* particle shape function of jefi_deposit / jefi_push_particles: 0 or 1 -> S^(1), the linear (CIC,
+                           volume-weighted) weights the paper uses, Eqs. (2.13), (2.16), (2.20); 2 -> S^(2), the quadratic
+                           spline of Eq. (2.14) on 27 nodes (DESIGN.md section 3 A11) */
+  int field_chunk;      /* tuning of the tiled field kernel: source tiles per CTA.  0 -> automatic (whole source range per
+                           CTA on large grids; on small grids the range is split over CTAs to fill the GPU and the partial
+                           sums are added by a second kernel in a fixed order); > 0 -> that many; -1 -> never split.
+                           The result is deterministic (bit-identical from run to run) for every value. */
 } jefi_config;
 
 /* Create a context: allocates the ring (32*H*N_padded bytes, zeroed = "zero before t0"), builds the
@@ -86,6 +94,17 @@ const char* jefi_last_error(const jefi_ctx* ctx);
 /* Values the context resolved at create time (H, N_dt, which field kernel runs ...).  All optional (NULL ok). */
 int jefi_get_info(const jefi_ctx* ctx, int* H, int* ndt, int* field_impl, long* step, long* ring_bytes);
 
+/* Why the context runs the field kernel it runs (one line of text, never NULL): e.g. "tiled: fp32 delays proven on 13824
+ * offsets, window 36 slots in pitch 36, 1 pass" or "reference: 3 fp32 delay mismatches against the fp64 table". */
+const char* jefi_field_impl_reason(const jefi_ctx* ctx);
+
+/* Geometry of the tiled field kernel (all optional, NULL ok): observation tile and source tile in cells per axis
+ * (8x8x8 / 4x4x4; 1x16x32 / 1x8x8 on grids with nx <= 3 such as the paper's 1 x ny x nz slabs), the largest slot window of a
+ * tile pair, the shared-memory pitch it is served from (window > pitch: the tile is evaluated in ceil(window/pitch) passes),
+ * and the number of pieces the source range is split into.  obs_tile[2] is the granularity of jefi_field_step_slab. */
+int jefi_get_tile_info(const jefi_ctx* ctx, int obs_tile[3], int src_tile[3], int* window_slots, int* window_pitch,
+                       int* source_split);
+
 /* CIC (volume-weighted) charge/current deposit, Eqs. (2.15)-(2.19).
  *   np            number of macro-particles (>= 0)
  *   x,y,z         positions, grid units, np floats each
@@ -93,7 +112,8 @@ int jefi_get_info(const jefi_ctx* ctx, int* H, int* ndt, int* field_impl, long* 
  *   qw            charge of each macro-particle, coulomb
  *   alive         np bytes, 0 = dead (skipped); NULL = all alive
  *   rho,jx,jy,jz  OUT, N floats each (C/m^3, A/m^2), overwritten (zeroed by the call).
- * Node (i,j,k) = floor(xi-.5) ... gets q*w/dV with the 8 trilinear weights; nodes outside the grid are virtual
+ * Node (i,j,k) = floor(xi-.5) ... gets q*w/dV with the 8 trilinear weights (shape_order 2: the 27 nodes around the
+ * centre node floor(xi) with the S^(2) weights of Eq. 2.14); nodes outside the grid are virtual
  * and dropped.  Sums are fp32 atomics: the order of equal-cell particles is not defined.
  * The caller's particle arrays are never modified: with JEFI_DEPOSIT_SORTED the cell order is an index array in
  * context scratch (12 bytes per particle + 8 bytes per cell, allocated on first use).  np < 2^31. */
@@ -126,8 +146,15 @@ int jefi_field_step(jefi_ctx* ctx, float* ex, float* ey, float* ez, float* bx, f
 /* The same solve restricted to the observation cells of the z-planes k0 <= k < k1 (all sources, as always): only those
  * entries of ex..bz are written.  Observation cells are independent (Eqs. 2.4-2.5 are sums per observation point), so
  * disjoint slabs computed by different calls - or by different GPUs that hold the same history, SURVEY.md §8(e) - add up to
- * jefi_field_step bit for bit.  k0 must be a multiple of 8 (the observation tile edge); JEFI_EINVAL otherwise. */
+ * jefi_field_step bit for bit (every sum is formed in a fixed order, also when the source range is split over CTAs).
+ * k0 must be a multiple of the observation tile's z edge (jefi_get_tile_info: 8, or 32 on nx <= 3 grids); JEFI_EINVAL
+ * otherwise. */
 int jefi_field_step_slab(jefi_ctx* ctx, int k0, int k1, float* ex, float* ey, float* ez, float* bx, float* by, float* bz);
+
+/* jefi_field_step that ALSO writes E, B interleaved per cell, eb_packed[8*c + 0..7] = (Ex, Ey, Ez, Bx, By, Bz, 0, 0) (DEVICE,
+ * 8*N floats, 16-byte aligned): the layout jefi_push_particles_packed gathers from (two 16-byte loads per node instead of
+ * six scattered words).  Written by the field kernel's own epilogue, no extra pass.  ex..bz as in jefi_field_step. */
+int jefi_field_step_packed(jefi_ctx* ctx, float* ex, float* ey, float* ez, float* bx, float* by, float* bz, float* eb_packed);
 
 /* Field interpolation (Eq. 2.20) + relativistic Boris push (Eqs. 2.7-2.11, DESIGN.md §3 A5/A6) + kill rule
  * (PAPER.md:205, 239): for each alive particle gather E,B from the 8 nodes (virtual nodes count as zero), add
@@ -138,6 +165,10 @@ int jefi_field_step_slab(jefi_ctx* ctx, int k0, int k1, float* ex, float* ey, fl
 int jefi_push_particles(jefi_ctx* ctx, long np, float* x, float* y, float* z, float* ux, float* uy, float* uz,
                         const float* q_over_m, unsigned char* alive, const float* ex, const float* ey,
                         const float* ez, const float* bx, const float* by, const float* bz);
+
+/* The same push reading the fields from the interleaved array jefi_field_step_packed wrote (8*N floats, DEVICE). */
+int jefi_push_particles_packed(jefi_ctx* ctx, long np, float* x, float* y, float* z, float* ux, float* uy, float* uz,
+                               const float* q_over_m, unsigned char* alive, const float* eb_packed);
 
 /* End-to-end variant of one field step with HOST buffers (pinned memory recommended): copies the newest source
  * slice (4 x N floats) host->device, does jefi_push_sources + jefi_field_step, copies E,B (6 x N floats)
@@ -152,11 +183,16 @@ long jefi_launch_count(const jefi_ctx* ctx);
  * context's stream.  Synchronises on the end event.  < 0 if no field step ran. */
 float jefi_last_field_kernel_ms(jefi_ctx* ctx);
 
+/* The same for the field step `calls_back` calls ago (0 = the most recent; the context keeps the events of its last 64
+ * field steps), so that a timed loop can be read back afterwards without a synchronisation inside it.  < 0 if out of range. */
+float jefi_field_kernel_ms(jefi_ctx* ctx, int calls_back);
+
 /* ---- debug / parity exports (synchronise; not on the timed path) ---- */
-/* m for every non-negative offset (a,b,c): m_out[a + nx*(b + ny*c)], HOST int array of N entries. */
+/* m for every non-negative offset (a,b,c): m_out[a + nx*(b + ny*c)], HOST int array of N entries (SURVEY.md §8(b) sketched
+ * short*; delays reach the history cap of 10000 and the device table is int, so int it is). */
 int jefi_debug_delay_table(jefi_ctx* ctx, int* m_out_host);
-/* Node index (i,j,k) = floor(xi - .5) of each particle as the deposit/push kernels compute it:
- * ijk_out = DEVICE int array [np][3]. */
+/* Node index (i,j,k) = floor(xi - .5) of each particle as the deposit/push kernels compute it (shape_order 2: the centre
+ * node floor(xi)): ijk_out = DEVICE int array [np][3]. */
 int jefi_debug_cell_index(jefi_ctx* ctx, long np, const float* x, const float* y, const float* z, int* ijk_out);
 /* The cell order that JEFI_DEPOSIT_SORTED and jefi_sort_particles use for these positions: order_out = DEVICE int
  * array [np], a permutation of 0..np-1 whose first *n_alive_host entries are the depositing particles grouped by base

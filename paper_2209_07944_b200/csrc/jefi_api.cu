@@ -8,7 +8,7 @@
 
 #include "jefi_ctx.h"
 
-static std::string g_create_err;
+static thread_local std::string g_create_err;  // jefi_last_error(NULL): per calling thread
 
 static int fail_create(jefi_ctx* c, int code, const std::string& msg) {
   g_create_err = msg;
@@ -33,13 +33,28 @@ extern "C" int jefi_get_info(const jefi_ctx* ctx, int* H, int* ndt, int* field_i
   return JEFI_OK;
 }
 
+extern "C" const char* jefi_field_impl_reason(const jefi_ctx* ctx) { return ctx ? ctx->impl_reason.c_str() : ""; }
+
+extern "C" int jefi_get_tile_info(const jefi_ctx* ctx, int obs_tile[3], int src_tile[3], int* window_slots, int* window_pitch,
+                                  int* source_split) {
+  if (!ctx) return JEFI_EINVAL;
+  const jefi_dims& d = ctx->dims;
+  if (obs_tile) { obs_tile[0] = d.obx; obs_tile[1] = d.oby; obs_tile[2] = d.obz; }
+  if (src_tile) { src_tile[0] = d.tsx; src_tile[1] = d.tsy; src_tile[2] = d.tsz; }
+  if (window_slots) *window_slots = ctx->wmax;
+  if (window_pitch) *window_pitch = ctx->wpitch;
+  if (source_split) *source_split = ctx->nsplit;
+  return JEFI_OK;
+}
+
 
 extern "C" int jefi_create(const jefi_config* cfg, jefi_ctx** out) {
   if (out) *out = nullptr;
   if (!cfg || !out) return fail_create(nullptr, JEFI_EINVAL, "jefi_create: NULL argument");
   if (cfg->nx < 1 || cfg->ny < 1 || cfg->nz < 1 || !(cfg->dx > 0) || !(cfg->dy > 0) || !(cfg->dz > 0) || !(cfg->dt > 0) ||
-      cfg->c < 0 || cfg->eps0 < 0 || cfg->H < 0 || cfg->hist_cap < 0 || cfg->deposit_mode < 0 || cfg->deposit_mode > 3 || cfg->delay_rule < 0 || cfg->delay_rule > 1)
-    return fail_create(nullptr, JEFI_EINVAL, "jefi_create: grid sizes, spacings and dt must be positive");
+      cfg->c < 0 || cfg->eps0 < 0 || cfg->H < 0 || cfg->hist_cap < 0 || cfg->deposit_mode < 0 || cfg->deposit_mode > 3 || cfg->delay_rule < 0 || cfg->delay_rule > 1 ||
+      cfg->shape_order < 0 || cfg->shape_order > 2 || cfg->field_chunk < -1 || cfg->field_impl < 0 || cfg->field_impl > 2)
+    return fail_create(nullptr, JEFI_EINVAL, "jefi_create: grid sizes, spacings and dt must be positive, switches in range");
   if ((long)cfg->nx * cfg->ny * cfg->nz > (1L << 30)) return fail_create(nullptr, JEFI_EINVAL, "jefi_create: grid too large");
   jefi_ctx* c = new (std::nothrow) jefi_ctx();
   if (!c) return fail_create(nullptr, JEFI_ENOMEM, "jefi_create: host allocation failed");
@@ -49,13 +64,19 @@ extern "C" int jefi_create(const jefi_config* cfg, jefi_ctx** out) {
   c->mtab_host = nullptr;
   c->src_stage = c->eb_stage = nullptr;
   c->perm = nullptr;
+  c->partial = nullptr;
+  c->wmax = c->wpitch = 0;
+  c->chunk = 0;
+  c->nsplit = 1;
+  c->tiled_smem = 0;
+  c->shape_order = cfg->shape_order == 2 ? 2 : 1;
   c->sort_count = c->sort_offset = c->sort_sums = nullptr;
   c->sort_key = c->sort_rank = c->sort_order = nullptr;
   c->sort_cap = 0;
   c->sort_buf = nullptr;
   c->eb_pack = nullptr;
-  c->ev0 = c->ev1 = nullptr;
-  c->ev_valid = false;
+  for (int i = 0; i < JEFI_NEVENTS; i++) c->ev0[i] = c->ev1[i] = nullptr;
+  c->field_calls = 0;
   c->launches = 0;
   c->step = -1;
   c->stream = (cudaStream_t)cfg->stream;
@@ -63,6 +84,9 @@ extern "C" int jefi_create(const jefi_config* cfg, jefi_ctx** out) {
   c->eps0 = cfg->eps0 > 0 ? cfg->eps0 : 8.8541878128e-12;
   c->mu0 = 1.0 / (c->eps0 * c->c * c->c);
 
+  // the caller's current device is restored on return (every later entry point does the same, jefi_device_guard)
+  struct restore_dev { int prev = -1; ~restore_dev() { if (prev >= 0) cudaSetDevice(prev); } } rd;
+  cudaGetDevice(&rd.prev);
   cudaError_t e = cudaSetDevice(cfg->device);
   if (e != cudaSuccess) return fail_create(c, JEFI_ECUDA, std::string("cudaSetDevice: ") + cudaGetErrorString(e));
 
@@ -79,7 +103,16 @@ extern "C" int jefi_create(const jefi_config* cfg, jefi_ctx** out) {
 
   jefi_dims& d = c->dims;
   d.nx = cfg->nx; d.ny = cfg->ny; d.nz = cfg->nz;
-  d.ntx = (cfg->nx + JEFI_TS - 1) / JEFI_TS; d.nty = (cfg->ny + JEFI_TS - 1) / JEFI_TS; d.ntz = (cfg->nz + JEFI_TS - 1) / JEFI_TS;
+  // tile geometry: cubes, or x-thin tiles for the paper's 1 x ny x nz slabs
+  c->tile_geom = cfg->nx <= 3 ? JEFI_GEOM_SLABX : JEFI_GEOM_CUBE;
+  if (c->tile_geom == JEFI_GEOM_SLABX) {
+    d.tsx = jefi_geom_slabx::TSX; d.tsy = jefi_geom_slabx::TSY; d.tsz = jefi_geom_slabx::TSZ;
+    d.obx = jefi_geom_slabx::OBX; d.oby = jefi_geom_slabx::OBY; d.obz = jefi_geom_slabx::OBZ;
+  } else {
+    d.tsx = jefi_geom_cube::TSX; d.tsy = jefi_geom_cube::TSY; d.tsz = jefi_geom_cube::TSZ;
+    d.obx = jefi_geom_cube::OBX; d.oby = jefi_geom_cube::OBY; d.obz = jefi_geom_cube::OBZ;
+  }
+  d.ntx = (cfg->nx + d.tsx - 1) / d.tsx; d.nty = (cfg->ny + d.tsy - 1) / d.tsy; d.ntz = (cfg->nz + d.tsz - 1) / d.tsz;
   d.H = H;
   d.N = (long)cfg->nx * cfg->ny * cfg->nz;
   d.ncell_pad = (long)d.ntx * d.nty * d.ntz * JEFI_TCELLS;
@@ -98,10 +131,12 @@ extern "C" int jefi_create(const jefi_config* cfg, jefi_ctx** out) {
   c->ring_bytes = (long)(ring_quads * sizeof(float4));
   if ((e = cudaMalloc(&c->ring, ring_quads * sizeof(float4))) != cudaSuccess)
     return fail_create(c, JEFI_ENOMEM, std::string("ring allocation (") + std::to_string(c->ring_bytes) + " B): " + cudaGetErrorString(e));
-  cudaMemsetAsync(c->ring, 0, ring_quads * sizeof(float4), c->stream);
+  if ((e = cudaMemsetAsync(c->ring, 0, ring_quads * sizeof(float4), c->stream)) != cudaSuccess)
+    return fail_create(c, JEFI_ECUDA, std::string("ring zero fill: ") + cudaGetErrorString(e));
 
   // ---- delay table, fp64 on the host: m = floor(R/(c dt) + 1/2) (Eq. 2.6, reading A1) ----
-  const int ex = jefi_table_extent(d.nx), ey = jefi_table_extent(d.ny), ez = jefi_table_extent(d.nz);
+  const int ex = jefi_table_extent(d.nx, d.obx), ey = jefi_table_extent(d.ny, d.oby), ez = jefi_table_extent(d.nz, d.obz);
+  c->tex = ex; c->tey = ey; c->tez = ez;
   size_t tn = (size_t)ex * ey * ez;
   c->mtab_host = (int*)malloc(tn * sizeof(int));
   if (!c->mtab_host) return fail_create(c, JEFI_ENOMEM, "delay table host allocation failed");
@@ -117,23 +152,33 @@ extern "C" int jefi_create(const jefi_config* cfg, jefi_ctx** out) {
   if ((e = cudaMemcpyAsync(c->mtab_dev, c->mtab_host, tn * sizeof(int), cudaMemcpyHostToDevice, c->stream)) != cudaSuccess)
     return fail_create(c, JEFI_ECUDA, std::string("delay table upload: ") + cudaGetErrorString(e));
 
-  if ((e = cudaEventCreate(&c->ev0)) != cudaSuccess || (e = cudaEventCreate(&c->ev1)) != cudaSuccess)
-    return fail_create(c, JEFI_ECUDA, std::string("cudaEventCreate: ") + cudaGetErrorString(e));
+  for (int i = 0; i < JEFI_NEVENTS; i++)
+    if ((e = cudaEventCreate(&c->ev0[i])) != cudaSuccess || (e = cudaEventCreate(&c->ev1[i])) != cudaSuccess)
+      return fail_create(c, JEFI_ECUDA, std::string("cudaEventCreate: ") + cudaGetErrorString(e));
 
   // ---- choose the field kernel ----
   c->field_impl = JEFI_FIELD_REFERENCE;
+  c->impl_reason = "reference: requested (JEFI_FIELD_REFERENCE)";
   if (cfg->field_impl != JEFI_FIELD_REFERENCE) {
-    long mism = -1;
-    int rc = jefi_verify_delay_fp32(c, &mism);
+    long mism = -1, noff = 0;
+    int rc = jefi_verify_delay_fp32(c, &mism, &noff);
     if (rc != JEFI_OK) return fail_create(c, rc, c->err);
     int prep = (mism == 0) ? jefi_tiled_prepare(c) : JEFI_ESTATE;
+    char buf[320];
     if (mism == 0 && prep == JEFI_OK) {
       c->field_impl = JEFI_FIELD_TILED;
-    } else if (cfg->field_impl == JEFI_FIELD_TILED) {
-      char buf[256];
-      snprintf(buf, sizeof buf, "tiled field kernel not usable: %ld delay mismatches against the fp64 table, prepare rc=%d (%s)",
-               mism, prep, c->err.c_str());
-      return fail_create(c, JEFI_ESTATE, buf);
+      snprintf(buf, sizeof buf, "tiled: fp32 delays proven equal to the fp64 table on %ld offsets; tiles %dx%dx%d / %dx%dx%d, window %d slots "
+               "in pitch %d (%d pass%s), source range in %d piece%s", noff, d.obx, d.oby, d.obz, d.tsx, d.tsy, d.tsz, c->wmax, c->wpitch,
+               (c->wmax + c->wpitch - 1) / c->wpitch, c->wmax > c->wpitch ? "es" : "", c->nsplit, c->nsplit > 1 ? "s" : "");
+      c->impl_reason = buf;
+    } else {
+      if (mism != 0)
+        snprintf(buf, sizeof buf, "reference: %ld of %ld fp32 delays differ from the fp64 table (a tie of the nearest-step rule within fp32 "
+                 "rounding), the tiled kernel cannot be proven", mism, noff);
+      else
+        snprintf(buf, sizeof buf, "reference: tiled kernel could not be prepared (rc=%d: %s)", prep, c->err.c_str());
+      c->impl_reason = buf;
+      if (cfg->field_impl == JEFI_FIELD_TILED) return fail_create(c, JEFI_ESTATE, std::string("tiled field kernel not usable; ") + buf);
     }
   }
   if ((e = cudaStreamSynchronize(c->stream)) != cudaSuccess)
@@ -145,10 +190,12 @@ extern "C" int jefi_create(const jefi_config* cfg, jefi_ctx** out) {
 
 extern "C" void jefi_destroy(jefi_ctx* c) {
   if (!c) return;
+  jefi_device_guard guard(c);
   cudaStreamSynchronize(c->stream);
   if (c->ring) cudaFree(c->ring);
   if (c->mtab_dev) cudaFree(c->mtab_dev);
   if (c->perm) cudaFree(c->perm);
+  if (c->partial) cudaFree(c->partial);
   if (c->src_stage) cudaFree(c->src_stage);
   if (c->eb_stage) cudaFree(c->eb_stage);
   if (c->sort_count) cudaFree(c->sort_count);
@@ -160,8 +207,10 @@ extern "C" void jefi_destroy(jefi_ctx* c) {
   if (c->sort_buf) cudaFree(c->sort_buf);
   if (c->eb_pack) cudaFree(c->eb_pack);
   if (c->mtab_host) free(c->mtab_host);
-  if (c->ev0) cudaEventDestroy(c->ev0);
-  if (c->ev1) cudaEventDestroy(c->ev1);
+  for (int i = 0; i < JEFI_NEVENTS; i++) {
+    if (c->ev0[i]) cudaEventDestroy(c->ev0[i]);
+    if (c->ev1[i]) cudaEventDestroy(c->ev1[i]);
+  }
   delete c;
 }
 
@@ -179,7 +228,7 @@ __global__ void __launch_bounds__(256) k_push_sources(jefi_dims d, float inv_c, 
   const long tile = r / JEFI_TCELLS;
   const int cell = (int)(r - tile * JEFI_TCELLS);
   const int tx = (int)(tile % d.ntx), ty = (int)((tile / d.ntx) % d.nty), tz = (int)(tile / ((long)d.ntx * d.nty));
-  const int i = tx * JEFI_TS + (cell & 3), j = ty * JEFI_TS + ((cell >> 2) & 3), k = tz * JEFI_TS + (cell >> 4);
+  const int i = tx * d.tsx + cell % d.tsx, j = ty * d.tsy + (cell / d.tsx) % d.tsy, k = tz * d.tsz + cell / (d.tsx * d.tsy);
   if (i >= d.nx || j >= d.ny || k >= d.nz) return;  // padded cells stay zero
   const size_t cidx = (size_t)i + (size_t)d.nx * ((size_t)j + (size_t)d.ny * k);
   const size_t q = jefi_ring_quad(d, tile, slot, cell);
@@ -204,57 +253,83 @@ int jefi_launch_push_sources(jefi_ctx* c, const float* rho, const float* jx, con
 
 extern "C" int jefi_push_sources(jefi_ctx* c, const float* rho, const float* jx, const float* jy, const float* jz) {
   if (!c) return JEFI_EINVAL;
+  jefi_device_guard guard(c);
   if (!rho || !jx || !jy || !jz) { c->err = "jefi_push_sources: NULL array"; return JEFI_EINVAL; }
   return jefi_launch_push_sources(c, rho, jx, jy, jz);
 }
 
-extern "C" int jefi_field_step_slab(jefi_ctx* c, int k0, int k1, float* ex, float* ey, float* ez, float* bx, float* by, float* bz) {
-  if (!c) return JEFI_EINVAL;
+static int field_step_impl(jefi_ctx* c, int k0, int k1, float* ex, float* ey, float* ez, float* bx, float* by, float* bz,
+                           float* eb_packed) {
   if (!ex || !ey || !ez || !bx || !by || !bz) { c->err = "jefi_field_step: NULL array"; return JEFI_EINVAL; }
-  if (k0 < 0 || k1 > c->dims.nz || k0 > k1 || (k0 % 8) != 0) {
-    c->err = "jefi_field_step_slab: need 0 <= k0 <= k1 <= nz with k0 a multiple of 8";
+  if (k0 < 0 || k1 > c->dims.nz || k0 > k1 || (k0 % c->dims.obz) != 0) {
+    c->err = "jefi_field_step_slab: need 0 <= k0 <= k1 <= nz with k0 a multiple of the observation tile's z edge (jefi_get_tile_info)";
     return JEFI_EINVAL;
   }
   if (c->step < 0) { c->err = "jefi_field_step before any jefi_push_sources"; return JEFI_ESTATE; }
   if (k0 == k1) return JEFI_OK;
-  JEFI_CUDA_TRY(c, cudaEventRecord(c->ev0, c->stream));
-  int rc = c->field_impl == JEFI_FIELD_TILED ? jefi_launch_field_tiled(c, k0, k1, ex, ey, ez, bx, by, bz)
-                                             : jefi_launch_field_reference(c, k0, k1, ex, ey, ez, bx, by, bz);
+  const int evi = (int)(c->field_calls % JEFI_NEVENTS);
+  JEFI_CUDA_TRY(c, cudaEventRecord(c->ev0[evi], c->stream));
+  int rc = c->field_impl == JEFI_FIELD_TILED ? jefi_launch_field_tiled(c, k0, k1, ex, ey, ez, bx, by, bz, eb_packed)
+                                             : jefi_launch_field_reference(c, k0, k1, ex, ey, ez, bx, by, bz, eb_packed);
   if (rc != JEFI_OK) return rc;
-  JEFI_CUDA_TRY(c, cudaEventRecord(c->ev1, c->stream));
-  c->ev_valid = true;
+  JEFI_CUDA_TRY(c, cudaEventRecord(c->ev1[evi], c->stream));
+  c->field_calls++;
   return JEFI_OK;
+}
+
+extern "C" int jefi_field_step_slab(jefi_ctx* c, int k0, int k1, float* ex, float* ey, float* ez, float* bx, float* by, float* bz) {
+  if (!c) return JEFI_EINVAL;
+  jefi_device_guard guard(c);
+  return field_step_impl(c, k0, k1, ex, ey, ez, bx, by, bz, nullptr);
 }
 
 extern "C" int jefi_field_step(jefi_ctx* c, float* ex, float* ey, float* ez, float* bx, float* by, float* bz) {
   if (!c) return JEFI_EINVAL;
-  return jefi_field_step_slab(c, 0, c->dims.nz, ex, ey, ez, bx, by, bz);
+  jefi_device_guard guard(c);
+  return field_step_impl(c, 0, c->dims.nz, ex, ey, ez, bx, by, bz, nullptr);
 }
 
-extern "C" float jefi_last_field_kernel_ms(jefi_ctx* c) {
-  if (!c || !c->ev_valid) return -1.f;
-  if (cudaEventSynchronize(c->ev1) != cudaSuccess) return -1.f;
+extern "C" int jefi_field_step_packed(jefi_ctx* c, float* ex, float* ey, float* ez, float* bx, float* by, float* bz, float* eb_packed) {
+  if (!c) return JEFI_EINVAL;
+  jefi_device_guard guard(c);
+  if (!eb_packed || ((uintptr_t)eb_packed & 15u)) { c->err = "jefi_field_step_packed: eb_packed must be a 16-byte aligned device array of 8 N floats"; return JEFI_EINVAL; }
+  return field_step_impl(c, 0, c->dims.nz, ex, ey, ez, bx, by, bz, eb_packed);
+}
+
+extern "C" float jefi_field_kernel_ms(jefi_ctx* c, int calls_back) {
+  if (!c || calls_back < 0 || calls_back >= JEFI_NEVENTS || calls_back >= c->field_calls) return -1.f;
+  jefi_device_guard guard(c);
+  const int evi = (int)((c->field_calls - 1 - calls_back) % JEFI_NEVENTS);
+  if (cudaEventSynchronize(c->ev1[evi]) != cudaSuccess) return -1.f;
   float ms = -1.f;
-  if (cudaEventElapsedTime(&ms, c->ev0, c->ev1) != cudaSuccess) return -1.f;
+  if (cudaEventElapsedTime(&ms, c->ev0[evi], c->ev1[evi]) != cudaSuccess) return -1.f;
   return ms;
 }
+
+extern "C" float jefi_last_field_kernel_ms(jefi_ctx* c) { return jefi_field_kernel_ms(c, 0); }
 
 extern "C" int jefi_field_step_host(jefi_ctx* c, const float* src_host, float* eb_host) {
   if (!c) return JEFI_EINVAL;
   if (!src_host || !eb_host) { c->err = "jefi_field_step_host: NULL array"; return JEFI_EINVAL; }
+  jefi_device_guard guard(c);
   const long N = c->dims.N;
-  if (!c->src_stage) {
-    if (cudaMalloc(&c->src_stage, 4 * N * sizeof(float)) != cudaSuccess || cudaMalloc(&c->eb_stage, 6 * N * sizeof(float)) != cudaSuccess) {
-      c->err = "jefi_field_step_host: staging allocation failed";
-      return JEFI_ENOMEM;
-    }
+  // the two staging buffers are allocated independently, so that a failed second allocation is retried by the next call
+  if (!c->src_stage && cudaMalloc(&c->src_stage, 4 * N * sizeof(float)) != cudaSuccess) {
+    c->src_stage = nullptr;
+    c->err = "jefi_field_step_host: staging allocation (sources) failed";
+    return JEFI_ENOMEM;
+  }
+  if (!c->eb_stage && cudaMalloc(&c->eb_stage, 6 * N * sizeof(float)) != cudaSuccess) {
+    c->eb_stage = nullptr;
+    c->err = "jefi_field_step_host: staging allocation (fields) failed";
+    return JEFI_ENOMEM;
   }
   JEFI_CUDA_TRY(c, cudaMemcpyAsync(c->src_stage, src_host, 4 * N * sizeof(float), cudaMemcpyHostToDevice, c->stream));
   float* s = c->src_stage;
-  int rc = jefi_push_sources(c, s, s + N, s + 2 * N, s + 3 * N);
+  int rc = jefi_launch_push_sources(c, s, s + N, s + 2 * N, s + 3 * N);
   if (rc != JEFI_OK) return rc;
   float* o = c->eb_stage;
-  rc = jefi_field_step(c, o, o + N, o + 2 * N, o + 3 * N, o + 4 * N, o + 5 * N);
+  rc = field_step_impl(c, 0, c->dims.nz, o, o + N, o + 2 * N, o + 3 * N, o + 4 * N, o + 5 * N, nullptr);
   if (rc != JEFI_OK) return rc;
   JEFI_CUDA_TRY(c, cudaMemcpyAsync(eb_host, o, 6 * N * sizeof(float), cudaMemcpyDeviceToHost, c->stream));
   JEFI_CUDA_TRY(c, cudaStreamSynchronize(c->stream));
@@ -266,10 +341,11 @@ extern "C" int jefi_field_step_host(jefi_ctx* c, const float* src_host, float* e
 // ------------------------------------------------------------------------------------------------------------
 extern "C" int jefi_debug_delay_table(jefi_ctx* c, int* m_out_host) {
   if (!c || !m_out_host) return JEFI_EINVAL;
+  jefi_device_guard guard(c);
   const jefi_dims& d = c->dims;
-  const int ex = jefi_table_extent(d.nx), ey = jefi_table_extent(d.ny);
+  const int ex = c->tex, ey = c->tey;
   // read the DEVICE copy back so the export shows what the kernels actually index
-  size_t tn = (size_t)ex * ey * jefi_table_extent(d.nz);
+  size_t tn = (size_t)ex * ey * c->tez;
   int* tmp = (int*)malloc(tn * sizeof(int));
   if (!tmp) return JEFI_ENOMEM;
   cudaError_t e = cudaMemcpyAsync(tmp, c->mtab_dev, tn * sizeof(int), cudaMemcpyDeviceToHost, c->stream);
@@ -299,6 +375,7 @@ __global__ void __launch_bounds__(256) k_history_slot(jefi_dims d, float cc, int
 
 extern "C" int jefi_debug_history_slot(jefi_ctx* c, int steps_back, float* out4N) {
   if (!c || !out4N) return JEFI_EINVAL;
+  jefi_device_guard guard(c);
   const jefi_dims& d = c->dims;
   long t = c->step - steps_back;
   if (steps_back < 0 || steps_back > d.H - 1 || t < 0) { c->err = "jefi_debug_history_slot: step not in the ring"; return JEFI_EINVAL; }
@@ -321,9 +398,8 @@ __global__ void __launch_bounds__(256) k_verify_delay(int ex, int ey, int ez, je
   if (jefi_delay_fp32(q) != mtab[idx]) atomicAdd(mismatches, 1ull);
 }
 
-int jefi_verify_delay_fp32(jefi_ctx* c, long* mismatches) {
-  const jefi_dims& d = c->dims;
-  const int ex = jefi_table_extent(d.nx), ey = jefi_table_extent(d.ny), ez = jefi_table_extent(d.nz);
+int jefi_verify_delay_fp32(jefi_ctx* c, long* mismatches, long* offsets) {
+  const int ex = c->tex, ey = c->tey, ez = c->tez;
   unsigned long long* cnt = nullptr;
   JEFI_CUDA_TRY(c, cudaMalloc(&cnt, sizeof(unsigned long long)));
   cudaMemsetAsync(cnt, 0, sizeof(unsigned long long), c->stream);
@@ -337,5 +413,6 @@ int jefi_verify_delay_fp32(jefi_ctx* c, long* mismatches) {
   if (e != cudaSuccess) { c->err = std::string("delay verification: ") + cudaGetErrorString(e); return JEFI_ECUDA; }
   c->launches++;
   *mismatches = (long)h;
+  *offsets = tn - 1;
   return JEFI_OK;
 }

@@ -7,23 +7,38 @@
 #include "jefi.h"
 
 // ---- ring geometry -------------------------------------------------------------------------------------
-// Source tile: TS^3 cells.  The ring is stored tile by tile and, inside a tile, slot by slot, so that the slot window
-// of one source tile is ONE contiguous run of rows (two when the ring wraps) = one TMA bulk copy:
+// Source tile: tsx*tsy*tsz = 64 cells (4x4x4; 1x8x8 on grids with nx <= 3, where a 4-wide tile would be 3/4 padding).
+// The ring is stored tile by tile and, inside a tile, slot by slot, so that the slot window of one source tile is ONE
+// contiguous run of rows (two when the ring wraps) = one TMA bulk copy:
 //   ring[tile][slot] = row of JEFI_ROW_QUADS float4:  [0,64)    S(cell) = (Jx/c, Jz/c, rho, Jy/c) of that step
 //                                                     [64,128)  D(cell) = S(step) - S(step-1)   (backward difference)
 //                                                     [128]     pad: makes the row pitch 2064 B, so that the same cell
 //                                                               in consecutive slots falls in consecutive 16-byte bank
 //                                                               groups of shared memory (pitch mod 128 = 16)
-// with slot = step mod H, tile = tx + ntx*(ty + nty*tz), cell = lx + TS*(ly + TS*lz).  The component order
+// with slot = step mod H, tile = tx + ntx*(ty + nty*tz), cell = lx + tsx*(ly + tsy*lz).  The component order
 // (Jx, Jz | rho, Jy) puts the operands of the packed FP32 instructions (FFMA2) in aligned register pairs.
-// The grid is padded to a multiple of TS per axis; padded cells stay zero for ever (they are never written).
-constexpr int JEFI_TS = 4;
-constexpr int JEFI_TCELLS = JEFI_TS * JEFI_TS * JEFI_TS;
+// The grid is padded to a multiple of the tile per axis; padded cells stay zero for ever (they are never written).
+constexpr int JEFI_TCELLS = 64;
+constexpr int JEFI_NEVENTS = 64;
 constexpr int JEFI_ROW_QUADS = 2 * JEFI_TCELLS + 1;        // float4 per (tile, slot) row
 constexpr int JEFI_ROW_BYTES = JEFI_ROW_QUADS * 16;        // 2064
 
+// Tile geometries the field kernel is compiled for (template parameter of k_field_tiled / k_build_perm).
+template <int OBX_, int OBY_, int OBZ_, int TSX_, int TSY_, int TSZ_>
+struct jefi_tile_geom {
+  static constexpr int OBX = OBX_, OBY = OBY_, OBZ = OBZ_;  // observation tile (512 cells = one per consumer thread)
+  static constexpr int TSX = TSX_, TSY = TSY_, TSZ = TSZ_;  // source tile (64 cells = one ring row)
+  static_assert(OBX_ * OBY_ * OBZ_ == 512 && TSX_ * TSY_ * TSZ_ == JEFI_TCELLS, "tile sizes");
+  static_assert(OBX_ % TSX_ == 0 && OBY_ % TSY_ == 0 && OBZ_ % TSZ_ == 0, "observation tile = whole source tiles");
+};
+using jefi_geom_cube = jefi_tile_geom<8, 8, 8, 4, 4, 4>;
+using jefi_geom_slabx = jefi_tile_geom<1, 16, 32, 1, 8, 8>;
+enum { JEFI_GEOM_CUBE = 0, JEFI_GEOM_SLABX = 1 };
+
 struct jefi_dims {
   int nx, ny, nz;     // real cells
+  int tsx, tsy, tsz;  // source tile
+  int obx, oby, obz;  // observation tile
   int ntx, nty, ntz;  // source tiles per axis
   int H;              // ring depth
   long N;             // nx*ny*nz
@@ -32,10 +47,10 @@ struct jefi_dims {
 
 // tile index and cell-in-tile of grid cell (i, j, k)
 __host__ __device__ inline void jefi_tile_cell(const jefi_dims& d, int i, int j, int k, long& tile, int& cell) {
-  int tx = i / JEFI_TS, ty = j / JEFI_TS, tz = k / JEFI_TS;
-  int lx = i - tx * JEFI_TS, ly = j - ty * JEFI_TS, lz = k - tz * JEFI_TS;
+  int tx = i / d.tsx, ty = j / d.tsy, tz = k / d.tsz;
+  int lx = i - tx * d.tsx, ly = j - ty * d.tsy, lz = k - tz * d.tsz;
   tile = tx + (long)d.ntx * (ty + (long)d.nty * tz);
-  cell = lx + JEFI_TS * (ly + JEFI_TS * lz);
+  cell = lx + d.tsx * (ly + d.tsy * lz);
 }
 // float4 index of S(cell) in ring row (tile, slot); D(cell) sits JEFI_TCELLS quads further
 __host__ __device__ inline size_t jefi_ring_quad(const jefi_dims& d, long tile, int slot, int cell) {
@@ -43,8 +58,8 @@ __host__ __device__ inline size_t jefi_ring_quad(const jefi_dims& d, long tile, 
 }
 
 // Extent of the delay table per axis: it covers every offset the tiled kernel can form, including offsets that
-// involve zero-padded cells (observation tiles are 8 cells, source tiles 4 cells wide).
-inline int jefi_table_extent(int n) { return ((n + 7) / 8) * 8 + 8; }
+// involve zero-padded cells (the grid padded to whole observation tiles, plus one tile of slack).
+inline int jefi_table_extent(int n, int ob) { return ((n + ob - 1) / ob) * ob + ob; }
 
 // Scaled geometry used by the field kernels: d' = d/(c dt) so that |d'| = s is the delay in steps (Eq. 2.6).
 struct jefi_geom {
@@ -59,18 +74,23 @@ struct jefi_ctx {
   jefi_geom geom;
   double c, eps0, mu0;
   int ndt;
+  int shape_order;      // resolved: 1 or 2
   int field_impl;       // resolved: JEFI_FIELD_REFERENCE or JEFI_FIELD_TILED
+  int tile_geom;        // JEFI_GEOM_*
   long step;            // n; -1 before the first push
   cudaStream_t stream;
   float4* ring;         // [tile][slot][JEFI_ROW_QUADS]
   long ring_bytes;
-  int* mtab_dev;        // [nz][ny][nx] delay table (fp64-built on the host)
+  int* mtab_dev;        // [ez][ey][ex] delay table (fp64-built on the host)
   int* mtab_host;
+  int tex, tey, tez;    // its extents
   // tiled-kernel launch parameters
   int wmax;             // largest slot window over all (obs tile, source tile) pairs
-  int wpitch;           // compiled shared-memory pitch chosen for it
+  int wpitch;           // compiled shared-memory pitch (rows per stage) it is served from
   size_t tiled_smem;
-  int chunk;            // source tiles per CTA (blockIdx.y splits the source range; > 1 split -> atomic output)
+  int chunk;            // source tiles per CTA (blockIdx.y splits the source range)
+  int nsplit;           // pieces of the source range; > 1: partial sums go to `partial` and k_reduce_partials adds them
+  float* partial;       // [nsplit][6][N]
   unsigned short* perm; // evaluation order of the 512 cells of an observation tile per relative tile offset
   int ndx, ndy, ndz;
   // cell-sorted deposit scratch (jefi_particles.cu)
@@ -84,9 +104,22 @@ struct jefi_ctx {
   float* eb_stage;      // 6N floats
   // bookkeeping
   long launches;
-  cudaEvent_t ev0, ev1;
-  bool ev_valid;
+  cudaEvent_t ev0[JEFI_NEVENTS], ev1[JEFI_NEVENTS];  // around the field kernel(s) of the last JEFI_NEVENTS field steps
+  long field_calls;
   std::string err;
+  std::string impl_reason;
+};
+
+// Every entry point runs on the context's device whatever the calling thread's current device is, and restores it.
+struct jefi_device_guard {
+  int prev = -1;
+  bool switched = false;
+  explicit jefi_device_guard(const jefi_ctx* c) {
+    if (c && cudaGetDevice(&prev) == cudaSuccess && prev != c->cfg.device) switched = cudaSetDevice(c->cfg.device) == cudaSuccess;
+  }
+  ~jefi_device_guard() {
+    if (switched) cudaSetDevice(prev);
+  }
 };
 
 #define JEFI_CUDA_TRY(ctx, call)                                                                   \
@@ -119,7 +152,9 @@ __device__ __forceinline__ float jefi_q_fp32(float kx, float ky, float kz, float
 
 // implemented in the .cu files
 int jefi_launch_push_sources(jefi_ctx* c, const float* rho, const float* jx, const float* jy, const float* jz);
-int jefi_launch_field_reference(jefi_ctx* c, int k0, int k1, float* ex, float* ey, float* ez, float* bx, float* by, float* bz);
-int jefi_launch_field_tiled(jefi_ctx* c, int k0, int k1, float* ex, float* ey, float* ez, float* bx, float* by, float* bz);
+int jefi_launch_field_reference(jefi_ctx* c, int k0, int k1, float* ex, float* ey, float* ez, float* bx, float* by, float* bz,
+                                float* eb_packed);
+int jefi_launch_field_tiled(jefi_ctx* c, int k0, int k1, float* ex, float* ey, float* ez, float* bx, float* by, float* bz,
+                            float* eb_packed);
 int jefi_tiled_prepare(jefi_ctx* c);   // window size + smem opt-in; returns JEFI_ESTATE if it cannot run
-int jefi_verify_delay_fp32(jefi_ctx* c, long* mismatches);
+int jefi_verify_delay_fp32(jefi_ctx* c, long* mismatches, long* offsets);

@@ -5,13 +5,20 @@
 //   B = prefB * sum [ d' x (Jt rs^3 + DJt rs^2) ]                    (Eq. 2.5)
 // sources taken from ring slot (n - m) mod H with m = round(s) (Eq. 2.6, nearest-step reading).
 //
-// Two kernels:
-//   k_field_reference  one thread per observation cell, all sources, delays from the fp64-built table.
-//   k_field_tiled      warp-specialised CTA: 8 consumer warps own an 8x8x8 observation tile (2 cells per thread) and
-//                      walk 4x4x4 source tiles; a producer warp stages each tile's slot window [m_lo, m_hi] in a
-//                      two-stage shared-memory ring with TMA bulk copies (mbarrier full/done pipeline).
+// Kernels:
+//   k_field_reference  one thread per observation cell, all sources, delays from the fp64-built table (the paper's K1 in
+//                      fp32; used on request or when the fp32 delay arithmetic cannot be proven for a grid).
+//   k_field_tiled      warp-specialised CTA: 16 consumer warps own one 512-cell observation tile (one cell per thread) and
+//                      walk the 64-cell source tiles; a producer warp stages each tile's slot window [m_lo, m_hi] in a
+//                      two-stage shared-memory ring with TMA bulk copies (mbarrier full/done pipeline).  Compiled for two
+//                      tile geometries (8x8x8 / 4x4x4 cubes; 1x16x32 / 1x8x8 for nx <= 3 slabs), two window pitches and
+//                      the two retarded-time rules.  A window wider than the pitch is served in several passes.
+//   k_reduce_partials  adds, in a fixed order, the partial sums of a launch that split the source range over CTAs.
+//   k_build_perm       once per context: the evaluation order of the 512 cells per relative tile offset.
 #include <stdio.h>
 #include <stdlib.h>
+
+#include <type_traits>
 
 #include "jefi_ctx.h"
 
@@ -22,7 +29,7 @@ __global__ void __launch_bounds__(128) k_field_reference(jefi_dims d, jefi_geom 
                                                          const int* __restrict__ mtab, const float4* __restrict__ ring,
                                                          float* __restrict__ ex, float* __restrict__ ey,
                                                          float* __restrict__ ez, float* __restrict__ bx,
-                                                         float* __restrict__ by, float* __restrict__ bz) {
+                                                         float* __restrict__ by, float* __restrict__ bz, float4* __restrict__ pack) {
   long oc = oc0 + (long)blockIdx.x * blockDim.x + threadIdx.x;
   if (oc >= oc1) return;
   const int I = (int)(oc % d.nx), J = (int)((oc / d.nx) % d.ny), K = (int)(oc / ((long)d.nx * d.ny));
@@ -58,16 +65,23 @@ __global__ void __launch_bounds__(128) k_field_reference(jefi_dims d, jefi_geom 
       }
     aex += lex; aey += ley; aez += lez; abx += lbx; aby += lby; abz += lbz;
   }
-  ex[oc] = g.prefE * aex; ey[oc] = g.prefE * aey; ez[oc] = g.prefE * aez;
-  bx[oc] = g.prefB * abx; by[oc] = g.prefB * aby; bz[oc] = g.prefB * abz;
+  const float vex = g.prefE * aex, vey = g.prefE * aey, vez = g.prefE * aez;
+  const float vbx = g.prefB * abx, vby = g.prefB * aby, vbz = g.prefB * abz;
+  ex[oc] = vex; ey[oc] = vey; ez[oc] = vez;
+  bx[oc] = vbx; by[oc] = vby; bz[oc] = vbz;
+  if (pack) {
+    pack[2 * oc] = make_float4(vex, vey, vez, vbx);
+    pack[2 * oc + 1] = make_float4(vby, vbz, 0.f, 0.f);
+  }
 }
 
-int jefi_launch_field_reference(jefi_ctx* c, int k0, int k1, float* ex, float* ey, float* ez, float* bx, float* by, float* bz) {
+int jefi_launch_field_reference(jefi_ctx* c, int k0, int k1, float* ex, float* ey, float* ez, float* bx, float* by, float* bz,
+                                float* eb_packed) {
   const jefi_dims& d = c->dims;
   const long oc0 = (long)k0 * d.nx * d.ny, oc1 = (long)k1 * d.nx * d.ny;  // observation cells of the z-planes [k0, k1)
   unsigned blocks = (unsigned)((oc1 - oc0 + 127) / 128);
-  k_field_reference<<<blocks, 128, 0, c->stream>>>(d, c->geom, jefi_table_extent(d.nx), jefi_table_extent(d.ny), c->step,
-                                                   c->cfg.delay_rule == JEFI_DELAY_LINEAR ? 1 : 0, oc0, oc1, c->mtab_dev, c->ring, ex, ey, ez, bx, by, bz);
+  k_field_reference<<<blocks, 128, 0, c->stream>>>(d, c->geom, c->tex, c->tey, c->step, c->cfg.delay_rule == JEFI_DELAY_LINEAR ? 1 : 0, oc0, oc1,
+                                                   c->mtab_dev, c->ring, ex, ey, ez, bx, by, bz, reinterpret_cast<float4*>(eb_packed));
   JEFI_CUDA_TRY(c, cudaGetLastError());
   c->launches++;
   return JEFI_OK;
@@ -76,16 +90,20 @@ int jefi_launch_field_reference(jefi_ctx* c, int k0, int k1, float* ex, float* e
 // ------------------------------------------------------------------------------------------------------------
 // tiled kernel
 //
-// CTA = 8 consumer warps + 1 producer warp, one CTA per SM.  The consumers own one 8x8x8 observation tile (512 cells,
-// two per thread) against the source tiles [t0, t1) of the linear tile order (the whole grid, or one chunk of it when
-// the launch splits the source range over blockIdx.y; partial sums then meet in global memory with fp32 atomics).
+// CTA = 16 consumer warps + 1 producer warp (544 threads), one CTA per SM.  The consumers own one observation tile
+// (G::OBX x G::OBY x G::OBZ = 512 cells, one per thread) against the source tiles [t0, t1) of the linear tile order (the
+// whole grid, or one chunk of it when the launch splits the source range over blockIdx.y; the pieces' partial sums are
+// then written to a [piece][6][N] buffer and added in a fixed order by k_reduce_partials).
 //
 // Staging.  For an (observation tile, source tile) pair the delays lie in [m_lo, m_hi] (from the extreme offsets), and
 // the ring stores a source tile slot by slot (jefi_ctx.h), so the window is one contiguous run of W = m_hi-m_lo+1 ring
 // rows (two runs when the ring wraps).  The producer warp's lane 0 issues it as one or two TMA bulk copies
-// (cp.async.bulk, SASS UBLKCP) into stage `it & 1`, together with the 1 KB evaluation-order row, on the stage's `full`
+// (cp.async.bulk, SASS UBLKCP) into stage `item & 1`, together with the 1 KB evaluation-order row, on the stage's `full`
 // mbarrier; consumers release a stage by arriving (one lane per warp) on its `done` mbarrier.  Row j of a stage
-// holds delay m = m_hi - j.
+// holds delay m = m_top - j.  A window wider than the compiled pitch WP (large dx/(c dt), e.g. the paper's kappa = 6
+// example) is served in ceil(W/WP) passes over the same source tile: pass p stages the delays
+// [m_hi - p WP - (R-1), m_hi - p WP] and every lane whose delay falls outside contributes exactly zero (MODE_MULTI).
+// The pipeline runs over (tile, pass) items; the stage header tells the consumers what an item is and which is the last.
 //
 // Pair evaluation: the source cell is warp-uniform, the delay per lane:
 //   q = |d'|^2 (FFMA), rs = rsqrt(q) (MUFU), t = q*rs + 1.5*2^23 (FFMA; the integer m sits in the mantissa),
@@ -99,46 +117,46 @@ int jefi_launch_field_reference(jefi_ctx* c, int k0, int k1, float* ex, float* e
 //   (9 scalar FMA-pipe, 7 packed, 1 MUFU, 2 LDS) against 26 for the scalar form.
 //
 // Shared-memory delivery is the scarce resource (measured, profiles/): an LDS.128 takes 4 data-pipe cycles, 2 when
-// every lane l reads the same address as lane l^1 (or every l as l^2).  Which lane evaluates which observation cell
-// is free (any assignment gives the same sums), so for every source tile the 512 cells are taken in the order of
-// their distance to the tile: neighbouring lanes then mostly share a slot.  The order depends only on the relative
-// tile offset; jefi_tiled_prepare tabulates it once (k_build_perm).  Per-tile partial sums are added to a
-// shared-memory accumulator [6][512] (second level of the two-level accumulation), because a cell is evaluated by a
-// different thread in every tile; the `done` barrier of tile it-1 orders these updates between tiles.
+// every lane l reads the same address as lane l^1.  Which lane evaluates which observation cell is free (any assignment
+// gives the same sums), so for every source tile the 512 cells are taken in an order tabulated per relative tile offset
+// (k_build_perm): neighbouring lanes then mostly share a slot.  Per-tile partial sums are added to a shared-memory
+// accumulator [6][512] (second level of the two-level accumulation), because a cell is evaluated by a different thread
+// in every tile; the `done` barrier of item-1 orders these updates between items.
 // ------------------------------------------------------------------------------------------------------------
-constexpr int OB = 8;            // observation tile edge
-constexpr int OBCELLS = OB * OB * OB;
-#ifndef JEFI_NCONS
-#define JEFI_NCONS 512
-#endif
-constexpr int NCONS = JEFI_NCONS;  // consumer threads
+constexpr int OBCELLS = 512;
+constexpr int NCONS = 512;  // consumer threads = observation cells of a tile
 constexpr int NCWARPS = NCONS / 32;
 constexpr int TILED_THREADS = NCONS + 32;  // + producer warp
-constexpr int P_OBS = OBCELLS / NCONS;     // observation cells per consumer thread
 constexpr int HDR_BYTES = 32;
+enum { MODE_PLAIN = 0, MODE_SELF = 1, MODE_MULTI = 2 };
 
 struct tiled_params {
   jefi_dims d;
   jefi_geom g;
   int n;           // current step
   int nslot;       // n mod H
-  int nobx, noby, nobz;
+  int nobx, noby;
   int ndx, ndy;    // extents of the permutation table in relative-offset space
   int obz0;        // first observation tile layer of this launch (jefi_field_step_slab)
   int k1;          // observation planes k >= k1 are not written
   int chunk;       // source tiles per blockIdx.y
-  int atomic_out;  // 1: add into zeroed outputs (source range split over blockIdx.y)
+  int to_partial;  // 1: write this piece's sums to partial[blockIdx.y][6][N] (source range split over blockIdx.y)
   const float4* ring;
   const unsigned short* perm;  // [ndz][ndy][ndx][512]
   float *ex, *ey, *ez, *bx, *by, *bz;
+  float4* pack;    // optional interleaved output (jefi_field_step_packed)
+  float* partial;
 };
 
 struct stage_hdr {  // written by the producer before it arms the stage's full barrier
-  uint32_t K;       // shared address of the stage's row 0 + 2064*(m_hi + 0x4B400000)  (mod 2^32)
-  int self;         // the source tile overlaps the observation tile (contains r' = r)
+  uint32_t K;       // shared address of the stage's row 0 + 2064*(m_top + 0x4B400000)  (mod 2^32)
+  int mode;         // MODE_PLAIN / MODE_SELF (the source tile contains r' = r) / MODE_MULTI (one of several passes)
   int dx0, dy0, dz0;  // ox0 - sx0, oy0 - sy0, oz0 - sz0
-  int pad[3];
+  uint32_t Mtop;    // m_top + 0x4B400000 (MODE_MULTI)
+  uint32_t R;       // rows staged in this item (MODE_MULTI)
+  int last;         // this is the CTA's last item
 };
+static_assert(sizeof(stage_hdr) == HDR_BYTES, "stage header");
 
 template <int WP>
 struct stage_layout {
@@ -187,13 +205,13 @@ __device__ __forceinline__ f32x2 pk(float lo, float hi) {
   return r;
 }
 __device__ __forceinline__ float lo32(f32x2 v) {
-  float a, b;
-  asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v));
+  float a;
+  asm("{ .reg .b32 jf_unused; mov.b64 {%0, jf_unused}, %1; }" : "=f"(a) : "l"(v));
   return a;
 }
 __device__ __forceinline__ float hi32(f32x2 v) {
-  float a, b;
-  asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v));
+  float b;
+  asm("{ .reg .b32 jf_unused; mov.b64 {jf_unused, %0}, %1; }" : "=f"(b) : "l"(v));
   return b;
 }
 __device__ __forceinline__ f32x2 swap2(f32x2 v) { return pk(hi32(v), lo32(v)); }
@@ -203,10 +221,10 @@ __device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) {
   return r;
 }
 // min / max of |a| over the integer interval [lo, hi]
-__device__ __forceinline__ void abs_range(int lo, int hi, int& mn, int& mx) {
-  int alo = abs(lo), ahi = abs(hi);
-  mx = max(alo, ahi);
-  mn = (lo <= 0 && hi >= 0) ? 0 : min(alo, ahi);
+__host__ __device__ __forceinline__ void abs_range(int lo, int hi, int& mn, int& mx) {
+  int alo = lo < 0 ? -lo : lo, ahi = hi < 0 ? -hi : hi;
+  mx = alo > ahi ? alo : ahi;
+  mn = (lo <= 0 && hi >= 0) ? 0 : (alo < ahi ? alo : ahi);
 }
 
 struct quad2 {  // one LDS.128 as two aligned register pairs
@@ -224,16 +242,31 @@ struct pair_acc {  // per-tile partial sums of one observation cell (first accum
   float Ey, Fy;
 };
 
-// One observation cell against one source cell.  Kz = shared address of row m = 0 (i.e. K) + byte offset of the z layer.
-template <bool SELF, bool LINEAR, int CELL>
-__device__ __forceinline__ void one_pair(uint32_t Kz, float ax, float ay, float az, float qyz, pair_acc& A) {
+// what a consumer thread needs to address the stage of one item
+struct item_addr {
+  uint32_t K;     // MODE_PLAIN / MODE_SELF: row 0 + 2064*(m_top + 0x4B400000);  MODE_MULTI: row 0
+  uint32_t Mtop;  // MODE_MULTI
+  uint32_t R;     // MODE_MULTI
+};
+
+// One observation cell against one source cell.  Az = item address + byte offset of the z layer.
+template <int MODE, bool LINEAR, int CELL>
+__device__ __forceinline__ void one_pair(const item_addr& Az, float ax, float ay, float az, float qyz, pair_acc& A) {
   constexpr int SOFF = CELL * 16;
   constexpr int DOFF = SOFF + JEFI_TCELLS * 16;
   const float q = fmaf(ax, ax, qyz);
   float rs = jefi_rsqrt(q);
-  if (SELF) rs = q > 0.f ? rs : 0.f;        // the self cell contributes exactly zero
-  const float t = fmaf(q, rs, JEFI_MAGIC);  // MAGIC + round(s): m sits in the mantissa
-  const uint32_t addr = Kz - (uint32_t)__float_as_int(t) * (uint32_t)JEFI_ROW_BYTES;  // row j = m_hi - m
+  if (MODE != MODE_PLAIN) rs = q > 0.f ? rs : 0.f;  // the self cell contributes exactly zero
+  const float t = fmaf(q, rs, JEFI_MAGIC);          // MAGIC + round(s): m sits in the mantissa
+  uint32_t addr;
+  if (MODE == MODE_MULTI) {
+    const uint32_t j = Az.Mtop - (uint32_t)__float_as_int(t);  // m_top - m: the row of this lane's delay
+    const bool in = j < Az.R;                                 // else the delay belongs to another pass: contributes zero
+    rs = in ? rs : 0.f;
+    addr = Az.K + (in ? j : 0u) * (uint32_t)JEFI_ROW_BYTES;
+  } else {
+    addr = Az.K - (uint32_t)__float_as_int(t) * (uint32_t)JEFI_ROW_BYTES;  // row j = m_top - m
+  }
   quad2 S = lds128_imm<SOFF>(addr);         // (Jx, Jz | rho, Jy)
   const quad2 D = lds128_imm<DOFF>(addr);   // (DJx, DJz | Drho, DJy)
   if (LINEAR) {  // JEFI_DELAY_LINEAR: S(t_r) = S - phi D with phi = s - m in [-1/2, 1/2) (3 scalar + 2 packed instructions)
@@ -259,32 +292,42 @@ __device__ __forceinline__ void one_pair(uint32_t Kz, float ax, float ay, float 
   A.By12 = fma2(Azx, wxz, A.By12);                // (a_z wx, a_x wz)
 }
 
-template <bool SELF, bool LINEAR, int LY>
-__device__ __forceinline__ void one_row(uint32_t Kz, const float (&ax)[JEFI_TS], float ay, float az, float az2, pair_acc& A) {
-  const float qyz = fmaf(ay, ay, az2);
-  one_pair<SELF, LINEAR, JEFI_TS * LY + 0>(Kz, ax[0], ay, az, qyz, A);
-  one_pair<SELF, LINEAR, JEFI_TS * LY + 1>(Kz, ax[1], ay, az, qyz, A);
-  one_pair<SELF, LINEAR, JEFI_TS * LY + 2>(Kz, ax[2], ay, az, qyz, A);
-  one_pair<SELF, LINEAR, JEFI_TS * LY + 3>(Kz, ax[3], ay, az, qyz, A);
-}
-
-// one observation cell against the 64 cells of the staged source tile
-template <bool SELF, bool LINEAR>
-__device__ __forceinline__ void tile_pairs(uint32_t K, float kz, const float (&ax)[JEFI_TS], const float (&ay)[JEFI_TS], float fz0,
-                                           pair_acc& A) {
-#pragma unroll 1
-  for (int lz = 0; lz < JEFI_TS; lz++) {
-    const float az = kz * (fz0 - (float)lz);
-    const float az2 = az * az;
-    const uint32_t Kz = K + (uint32_t)(lz * JEFI_TS * JEFI_TS * 16);
-    one_row<SELF, LINEAR, 0>(Kz, ax, ay[0], az, az2, A);
-    one_row<SELF, LINEAR, 1>(Kz, ax, ay[1], az, az2, A);
-    one_row<SELF, LINEAR, 2>(Kz, ax, ay[2], az, az2, A);
-    one_row<SELF, LINEAR, 3>(Kz, ax, ay[3], az, az2, A);
+// compile-time loop (the LDS offsets of one_pair are immediates)
+template <int I, int N, class F>
+__device__ __forceinline__ void static_for(F&& f) {
+  if constexpr (I < N) {
+    f(std::integral_constant<int, I>{});
+    static_for<I + 1, N>(f);
   }
 }
 
-template <int WP, bool LINEAR>
+// one observation cell against the 64 cells of the staged source tile; the z loop is unrolled to 16 pairs per iteration
+template <class G, int MODE, bool LINEAR>
+__device__ __forceinline__ void tile_pairs(const item_addr& A0, float kz, const float (&ax)[G::TSX], const float (&ay)[G::TSY], float fz0,
+                                           pair_acc& A) {
+  constexpr int LAYER = G::TSX * G::TSY;            // cells per z layer of the source tile
+  constexpr int ZU = LAYER >= 16 ? 1 : 16 / LAYER;  // layers per loop iteration
+#pragma unroll 1
+  for (int lz = 0; lz < G::TSZ; lz += ZU) {
+    item_addr Az = A0;
+    Az.K = A0.K + (uint32_t)(lz * LAYER * 16);
+    static_for<0, ZU>([&](auto zu) {
+      constexpr int ZO = decltype(zu)::value;
+      const float az = kz * (fz0 - (float)(lz + ZO));
+      const float az2 = az * az;
+      static_for<0, G::TSY>([&](auto ly) {
+        constexpr int LY = decltype(ly)::value;
+        const float qyz = fmaf(ay[LY], ay[LY], az2);
+        static_for<0, G::TSX>([&](auto lx) {
+          constexpr int LX = decltype(lx)::value;
+          one_pair<MODE, LINEAR, ZO * LAYER + G::TSX * LY + LX>(Az, ax[LX], ay[LY], az, qyz, A);
+        });
+      });
+    });
+  }
+}
+
+template <class G, int WP, bool LINEAR>
 __global__ void __launch_bounds__(TILED_THREADS, 1) k_field_tiled(tiled_params P) {
   using L = stage_layout<WP>;
   extern __shared__ __align__(128) unsigned char smem[];
@@ -295,7 +338,7 @@ __global__ void __launch_bounds__(TILED_THREADS, 1) k_field_tiled(tiled_params P
   const uint32_t barFull = sm0 + L::BAR, barDone = barFull + 16;
   // observation tile and source-tile range of this CTA
   const int obx = blockIdx.x % P.nobx, oby = (blockIdx.x / P.nobx) % P.noby, obz = P.obz0 + blockIdx.x / (P.nobx * P.noby);
-  const int ox0 = obx * OB, oy0 = oby * OB, oz0 = obz * OB;
+  const int ox0 = obx * G::OBX, oy0 = oby * G::OBY, oz0 = obz * G::OBZ;
   const int ntiles = d.ntx * d.nty * d.ntz;
   const int t0 = blockIdx.y * P.chunk;
   const int nt = min(P.chunk, ntiles - t0);
@@ -312,50 +355,59 @@ __global__ void __launch_bounds__(TILED_THREADS, 1) k_field_tiled(tiled_params P
   if (warp == NCWARPS) {
     // ------------------------------------------------ producer warp ------------------------------------------------
     int stx = t0 % d.ntx, sty = (t0 / d.ntx) % d.nty, stz = t0 / (d.ntx * d.nty);
+    int item = 0;
     for (int it = 0; it < nt; it++) {
-      const int s = it & 1;
-      if (it >= 2) mbar_wait(barDone + 8 * s, ((it - 2) >> 1) & 1);  // consumers are done with tile it-2 (same stage)
-      const int sx0 = stx * JEFI_TS, sy0 = sty * JEFI_TS, sz0 = stz * JEFI_TS;
+      const int sx0 = stx * G::TSX, sy0 = sty * G::TSY, sz0 = stz * G::TSZ;
       // slot window of this (observation tile, source tile) pair from the extreme offsets
       int mnx, mxx, mny, mxy, mnz, mxz;
-      abs_range(ox0 - (sx0 + JEFI_TS - 1), ox0 + OB - 1 - sx0, mnx, mxx);
-      abs_range(oy0 - (sy0 + JEFI_TS - 1), oy0 + OB - 1 - sy0, mny, mxy);
-      abs_range(oz0 - (sz0 + JEFI_TS - 1), oz0 + OB - 1 - sz0, mnz, mxz);
+      abs_range(ox0 - (sx0 + G::TSX - 1), ox0 + G::OBX - 1 - sx0, mnx, mxx);
+      abs_range(oy0 - (sy0 + G::TSY - 1), oy0 + G::OBY - 1 - sy0, mny, mxy);
+      abs_range(oz0 - (sz0 + G::TSZ - 1), oz0 + G::OBZ - 1 - sz0, mnz, mxz);
       const bool self = (mnx == 0 && mny == 0 && mnz == 0);
       const int m_lo = self ? 0 : jefi_delay_fp32(jefi_q_fp32(P.g.kx, P.g.ky, P.g.kz, (float)mnx, (float)mny, (float)mnz));
       const int m_hi = jefi_delay_fp32(jefi_q_fp32(P.g.kx, P.g.ky, P.g.kz, (float)mxx, (float)mxy, (float)mxz));
-      const int W = m_hi - m_lo + 1;  // <= WP (jefi_tiled_prepare)
-      // row j <-> delay m = m_hi - j <-> absolute step t = n - m_hi + j.  Rows with t < 0 (before t0)
-      // or m > H-2 (not stored, reading A15) are zero: j < jv.
-      int jv = max(m_hi - P.n, m_hi - (d.H - 2));
-      jv = jv < 0 ? 0 : (jv > W ? W : jv);
-      const int nvalid = W - jv;          // <= H - 1
-      int s0 = P.nslot - (m_hi - jv);     // ring slot of row jv; m_hi - jv <= H - 2
-      s0 += s0 < 0 ? d.H : 0;
-      const int lenA = min(nvalid, d.H - s0), lenB = nvalid - lenA;  // ring wrap: at most two runs
-      const uint32_t sb = sm0 + (uint32_t)s * L::BYTES;
-      if (jv > 0) {  // zero rows (only in the first steps of a run or with a shallow ring)
-        float4* z = reinterpret_cast<float4*>(smem + (size_t)s * L::BYTES);
-        for (int i = lane; i < jv * JEFI_ROW_QUADS; i += 32) z[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-      }
-      __syncwarp();
-      if (lane == 0) {
-        stage_hdr h;
-        h.K = sb + ((uint32_t)m_hi + 0x4B400000u) * (uint32_t)JEFI_ROW_BYTES;  // wraps mod 2^32 together with bits*2064
-        h.self = self ? 1 : 0;
-        h.dx0 = ox0 - sx0; h.dy0 = oy0 - sy0; h.dz0 = oz0 - sz0;
-        h.pad[0] = h.pad[1] = h.pad[2] = 0;
-        *reinterpret_cast<stage_hdr*>(smem + (size_t)s * L::BYTES + L::HDR) = h;
-        fence_proxy_async();  // generic-proxy accesses of this stage (zero fill, earlier reads) before the async-proxy writes
-        const uint32_t bar = barFull + 8 * s;
-        mbar_expect_tx(bar, (uint32_t)(nvalid * JEFI_ROW_BYTES + OBCELLS * 2));
-        const size_t tile = (size_t)(t0 + it);
-        const float4* rows = P.ring + tile * d.H * JEFI_ROW_QUADS;
-        if (lenA > 0) bulk_g2s(sb + (uint32_t)(jv * JEFI_ROW_BYTES), rows + (size_t)s0 * JEFI_ROW_QUADS, (uint32_t)(lenA * JEFI_ROW_BYTES), bar);
-        if (lenB > 0) bulk_g2s(sb + (uint32_t)((jv + lenA) * JEFI_ROW_BYTES), rows, (uint32_t)(lenB * JEFI_ROW_BYTES), bar);
-        const int ix = 2 * obx - stx + (d.ntx - 1), iy = 2 * oby - sty + (d.nty - 1), iz = 2 * obz - stz + (d.ntz - 1);
-        const size_t prow = (size_t)ix + (size_t)P.ndx * ((size_t)iy + (size_t)P.ndy * iz);
-        bulk_g2s(sb + L::PERM, P.perm + prow * OBCELLS, OBCELLS * 2, bar);
+      const int W = m_hi - m_lo + 1;
+      const int npass = (W + WP - 1) / WP;  // 1 unless the window exceeds the compiled pitch
+      const size_t tile = (size_t)(t0 + it);
+      const float4* rows = P.ring + tile * d.H * JEFI_ROW_QUADS;
+      const int ix = (G::OBX / G::TSX) * obx - stx + (d.ntx - 1), iy = (G::OBY / G::TSY) * oby - sty + (d.nty - 1),
+                iz = (G::OBZ / G::TSZ) * obz - stz + (d.ntz - 1);
+      const size_t prow = (size_t)ix + (size_t)P.ndx * ((size_t)iy + (size_t)P.ndy * iz);
+      for (int p = 0; p < npass; p++, item++) {
+        const int s = item & 1;
+        if (item >= 2) mbar_wait(barDone + 8 * s, ((item - 2) >> 1) & 1);  // consumers are done with item-2 (same stage)
+        const int m_top = m_hi - p * WP;
+        const int R = min(WP, m_top - m_lo + 1);
+        // row j <-> delay m = m_top - j <-> absolute step t = n - m_top + j.  Rows with t < 0 (before t0)
+        // or m > H-2 (not stored, reading A15) are zero: j < jv.
+        int jv = max(m_top - P.n, m_top - (d.H - 2));
+        jv = jv < 0 ? 0 : (jv > R ? R : jv);
+        const int nvalid = R - jv;          // <= H - 1
+        int s0 = P.nslot - (m_top - jv);    // ring slot of row jv; m_top - jv <= H - 2
+        s0 += s0 < 0 ? d.H : 0;
+        const int lenA = min(nvalid, d.H - s0), lenB = nvalid - lenA;  // ring wrap: at most two runs
+        const uint32_t sb = sm0 + (uint32_t)s * L::BYTES;
+        if (jv > 0) {  // zero rows (only in the first steps of a run or with a shallow ring)
+          float4* z = reinterpret_cast<float4*>(smem + (size_t)s * L::BYTES);
+          for (int i = lane; i < jv * JEFI_ROW_QUADS; i += 32) z[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+        __syncwarp();
+        if (lane == 0) {
+          stage_hdr h;
+          h.Mtop = (uint32_t)m_top + 0x4B400000u;
+          h.K = npass > 1 ? sb : sb + h.Mtop * (uint32_t)JEFI_ROW_BYTES;  // wraps mod 2^32 together with bits*2064
+          h.mode = npass > 1 ? MODE_MULTI : (self ? MODE_SELF : MODE_PLAIN);
+          h.dx0 = ox0 - sx0; h.dy0 = oy0 - sy0; h.dz0 = oz0 - sz0;
+          h.R = (uint32_t)R;
+          h.last = (it == nt - 1 && p == npass - 1) ? 1 : 0;
+          *reinterpret_cast<stage_hdr*>(smem + (size_t)s * L::BYTES + L::HDR) = h;
+          fence_proxy_async();  // generic-proxy accesses of this stage (zero fill, earlier reads) before the async-proxy writes
+          const uint32_t bar = barFull + 8 * s;
+          mbar_expect_tx(bar, (uint32_t)(nvalid * JEFI_ROW_BYTES + OBCELLS * 2));
+          if (lenA > 0) bulk_g2s(sb + (uint32_t)(jv * JEFI_ROW_BYTES), rows + (size_t)s0 * JEFI_ROW_QUADS, (uint32_t)(lenA * JEFI_ROW_BYTES), bar);
+          if (lenB > 0) bulk_g2s(sb + (uint32_t)((jv + lenA) * JEFI_ROW_BYTES), rows, (uint32_t)(lenB * JEFI_ROW_BYTES), bar);
+          bulk_g2s(sb + L::PERM, P.perm + prow * OBCELLS, OBCELLS * 2, bar);
+        }
       }
       if (++stx == d.ntx) { stx = 0; if (++sty == d.nty) { sty = 0; ++stz; } }
     }
@@ -363,62 +415,88 @@ __global__ void __launch_bounds__(TILED_THREADS, 1) k_field_tiled(tiled_params P
   }
 
   // -------------------------------------------------- consumer warps --------------------------------------------------
-  for (int it = 0; it < nt; it++) {
-    const int s = it & 1;
+  for (int item = 0;; item++) {
+    const int s = item & 1;
     const unsigned char* st = smem + (size_t)s * L::BYTES;
-    mbar_wait(barFull + 8 * s, (it >> 1) & 1);
+    mbar_wait(barFull + 8 * s, (item >> 1) & 1);
     const stage_hdr h = *reinterpret_cast<const stage_hdr*>(st + L::HDR);
-    const unsigned short* permS = reinterpret_cast<const unsigned short*>(st + L::PERM);
-#pragma unroll 1
-    for (int p = 0; p < P_OBS; p++) {
-      // the cell this lane evaluates for this source tile: neighbouring lanes are (almost) equidistant from it
-      const int c = permS[p * NCONS + tid];
-      const int cx = c & 7, cy = (c >> 3) & 7, cz = c >> 6;
-      float ax[JEFI_TS], ay[JEFI_TS];
+    // the cell this lane evaluates for this source tile: neighbouring lanes are (almost) equidistant from it
+    const int c = reinterpret_cast<const unsigned short*>(st + L::PERM)[tid];
+    const int cx = c % G::OBX, cy = (c / G::OBX) % G::OBY, cz = c / (G::OBX * G::OBY);
+    float ax[G::TSX], ay[G::TSY];
 #pragma unroll
-      for (int l = 0; l < JEFI_TS; l++) {
-        ax[l] = P.g.kx * (float)(h.dx0 + cx - l);
-        ay[l] = P.g.ky * (float)(h.dy0 + cy - l);
-      }
-      const float fz0 = (float)(h.dz0 + cz);
-      pair_acc A;
-      A.Exz = A.Fxz = A.Bxz = A.Cxz = A.By12 = pk(0.f, 0.f);
-      A.Ey = A.Fy = 0.f;
-      if (h.self)
-        tile_pairs<true, LINEAR>(h.K, P.g.kz, ax, ay, fz0, A);
-      else
-        tile_pairs<false, LINEAR>(h.K, P.g.kz, ax, ay, fz0, A);
-      // second accumulation level.  Cell c belongs to this thread alone in this tile; the previous tile's updates
-      // (by other threads) are complete once every consumer warp has arrived on that tile's done barrier.
-      if (p == 0 && it > 0) mbar_wait(barDone + 8 * ((it - 1) & 1), ((it - 1) >> 1) & 1);
-      accS[c] += lo32(A.Exz) - lo32(A.Fxz);
-      accS[OBCELLS + c] += A.Ey - A.Fy;
-      accS[2 * OBCELLS + c] += hi32(A.Exz) - hi32(A.Fxz);
-      accS[3 * OBCELLS + c] += lo32(A.Bxz) - lo32(A.Cxz);
-      accS[4 * OBCELLS + c] += lo32(A.By12) - hi32(A.By12);
-      accS[5 * OBCELLS + c] += hi32(A.Cxz) - hi32(A.Bxz);
-    }
+    for (int l = 0; l < G::TSX; l++) ax[l] = P.g.kx * (float)(h.dx0 + cx - l);
+#pragma unroll
+    for (int l = 0; l < G::TSY; l++) ay[l] = P.g.ky * (float)(h.dy0 + cy - l);
+    const float fz0 = (float)(h.dz0 + cz);
+    pair_acc A;
+    A.Exz = A.Fxz = A.Bxz = A.Cxz = A.By12 = pk(0.f, 0.f);
+    A.Ey = A.Fy = 0.f;
+    item_addr I0;
+    I0.K = h.K; I0.Mtop = h.Mtop; I0.R = h.R;
+    if (h.mode == MODE_PLAIN)
+      tile_pairs<G, MODE_PLAIN, LINEAR>(I0, P.g.kz, ax, ay, fz0, A);
+    else if (h.mode == MODE_SELF)
+      tile_pairs<G, MODE_SELF, LINEAR>(I0, P.g.kz, ax, ay, fz0, A);
+    else
+      tile_pairs<G, MODE_MULTI, LINEAR>(I0, P.g.kz, ax, ay, fz0, A);
+    // second accumulation level.  Cell c belongs to this thread alone in this item; the previous item's updates
+    // (by other threads) are complete once every consumer warp has arrived on that item's done barrier.
+    if (item > 0) mbar_wait(barDone + 8 * ((item - 1) & 1), ((item - 1) >> 1) & 1);
+    accS[c] += lo32(A.Exz) - lo32(A.Fxz);
+    accS[OBCELLS + c] += A.Ey - A.Fy;
+    accS[2 * OBCELLS + c] += hi32(A.Exz) - hi32(A.Fxz);
+    accS[3 * OBCELLS + c] += lo32(A.Bxz) - lo32(A.Cxz);
+    accS[4 * OBCELLS + c] += lo32(A.By12) - hi32(A.By12);
+    accS[5 * OBCELLS + c] += hi32(A.Cxz) - hi32(A.Bxz);
     __syncwarp();
     if (lane == 0) mbar_arrive(barDone + 8 * s);  // stage s may be refilled; this warp's accumulator updates are done
+    if (h.last) break;
   }
 
   asm volatile("bar.sync 1, %0;" ::"n"(NCONS) : "memory");  // consumers only: all accumulator updates are visible
-#pragma unroll
-  for (int p = 0; p < P_OBS; p++) {
-    const int c = p * NCONS + tid;  // home order: x fastest inside the tile
-    const int oi = ox0 + (c & 7), oj = oy0 + ((c >> 3) & 7), ok = oz0 + (c >> 6);
+  {
+    const int c = tid;  // home order: x fastest inside the tile
+    const int oi = ox0 + c % G::OBX, oj = oy0 + (c / G::OBX) % G::OBY, ok = oz0 + c / (G::OBX * G::OBY);
     if (oi < d.nx && oj < d.ny && ok < P.k1) {
       const size_t o = (size_t)oi + (size_t)d.nx * ((size_t)oj + (size_t)d.ny * ok);
       const float vex = P.g.prefE * accS[c], vey = P.g.prefE * accS[OBCELLS + c], vez = P.g.prefE * accS[2 * OBCELLS + c];
       const float vbx = P.g.prefB * accS[3 * OBCELLS + c], vby = P.g.prefB * accS[4 * OBCELLS + c], vbz = P.g.prefB * accS[5 * OBCELLS + c];
-      if (P.atomic_out) {
-        atomicAdd(P.ex + o, vex); atomicAdd(P.ey + o, vey); atomicAdd(P.ez + o, vez);
-        atomicAdd(P.bx + o, vbx); atomicAdd(P.by + o, vby); atomicAdd(P.bz + o, vbz);
+      if (P.to_partial) {
+        float* q = P.partial + (size_t)blockIdx.y * 6 * (size_t)d.N + o;
+        q[0] = vex; q[d.N] = vey; q[2 * d.N] = vez; q[3 * d.N] = vbx; q[4 * d.N] = vby; q[5 * d.N] = vbz;
       } else {
         P.ex[o] = vex; P.ey[o] = vey; P.ez[o] = vez;
         P.bx[o] = vbx; P.by[o] = vby; P.bz[o] = vbz;
+        if (P.pack) {
+          P.pack[2 * o] = make_float4(vex, vey, vez, vbx);
+          P.pack[2 * o + 1] = make_float4(vby, vbz, 0.f, 0.f);
+        }
       }
     }
+  }
+}
+
+// Sum of the `nsplit` partial results of a launch that split the source range over blockIdx.y, piece 0 first: the same
+// order on every run, so E and B are bit-reproducible (and observation slabs assemble the full step bit for bit).
+__global__ void __launch_bounds__(256) k_reduce_partials(long N, int nsplit, long c0, long c1, const float* __restrict__ partial,
+                                                         float* __restrict__ ex, float* __restrict__ ey, float* __restrict__ ez,
+                                                         float* __restrict__ bx, float* __restrict__ by, float* __restrict__ bz,
+                                                         float4* __restrict__ pack) {
+  const long o = c0 + (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (o >= c1) return;
+  float v[6];
+#pragma unroll
+  for (int a = 0; a < 6; a++) v[a] = partial[(size_t)a * N + o];
+  for (int s = 1; s < nsplit; s++) {
+    const float* q = partial + (size_t)s * 6 * (size_t)N + o;
+#pragma unroll
+    for (int a = 0; a < 6; a++) v[a] += q[(size_t)a * N];
+  }
+  ex[o] = v[0]; ey[o] = v[1]; ez[o] = v[2]; bx[o] = v[3]; by[o] = v[4]; bz[o] = v[5];
+  if (pack) {
+    pack[2 * o] = make_float4(v[0], v[1], v[2], v[3]);
+    pack[2 * o + 1] = make_float4(v[4], v[5], 0.f, 0.f);
   }
 }
 
@@ -433,6 +511,7 @@ __global__ void __launch_bounds__(TILED_THREADS, 1) k_field_tiled(tiled_params P
 //      (a source cell outside the union takes the fast path for that warp).  The band keeps the delays of one warp within
 //      8 slots: rows 8 apart share a 16-byte bank group and would be replayed.
 // Any order gives the same sums; this table only decides how fast.  One CTA of 512 threads per offset, once at create.
+template <class G>
 __global__ void __launch_bounds__(OBCELLS) k_build_perm(int ndx, int ndy, int ntx, int nty, int ntz, jefi_geom g, int band,
                                                         unsigned short* __restrict__ perm) {
   __shared__ float keys[OBCELLS];
@@ -442,10 +521,10 @@ __global__ void __launch_bounds__(OBCELLS) k_build_perm(int ndx, int ndy, int nt
   __shared__ unsigned red[2][OBCELLS / 32];
   const int c = threadIdx.x;
   const int ix = blockIdx.x % ndx, iy = (blockIdx.x / ndx) % ndy, iz = blockIdx.x / (ndx * ndy);
-  const int Dxi = JEFI_TS * (ix - (ntx - 1)), Dyi = JEFI_TS * (iy - (nty - 1)), Dzi = JEFI_TS * (iz - (ntz - 1));
-  const float half = 0.5f * (float)(JEFI_TS - 1);
-  const float rx = g.kx * ((float)Dxi + (float)(c & 7) - half), ry = g.ky * ((float)Dyi + (float)((c >> 3) & 7) - half),
-              rz = g.kz * ((float)Dzi + (float)(c >> 6) - half);
+  const int Dxi = G::TSX * (ix - (ntx - 1)), Dyi = G::TSY * (iy - (nty - 1)), Dzi = G::TSZ * (iz - (ntz - 1));
+  const int cx = c % G::OBX, cy = (c / G::OBX) % G::OBY, cz = c / (G::OBX * G::OBY);
+  const float rx = g.kx * ((float)Dxi + (float)cx - 0.5f * (float)(G::TSX - 1)), ry = g.ky * ((float)Dyi + (float)cy - 0.5f * (float)(G::TSY - 1)),
+              rz = g.kz * ((float)Dzi + (float)cz - 0.5f * (float)(G::TSZ - 1));
   const float key = rx * rx + ry * ry + rz * rz;
   keys[c] = key;
   __syncthreads();
@@ -461,10 +540,12 @@ __global__ void __launch_bounds__(OBCELLS) k_build_perm(int ndx, int ndy, int nt
   bool avail = c < OBCELLS / 2;
   if (avail) {
     const int a = order[2 * c], b = order[2 * c + 1];
+    const int axc = a % G::OBX, ayc = (a / G::OBX) % G::OBY, azc = a / (G::OBX * G::OBY);
+    const int bxc = b % G::OBX, byc = (b / G::OBX) % G::OBY, bzc = b / (G::OBX * G::OBY);
     for (int sc = 0; sc < JEFI_TCELLS; sc++) {
-      const int lx = sc & 3, ly = (sc >> 2) & 3, lz = sc >> 4;
-      const float qa = jefi_q_fp32(g.kx, g.ky, g.kz, (float)(Dxi + (a & 7) - lx), (float)(Dyi + ((a >> 3) & 7) - ly), (float)(Dzi + (a >> 6) - lz));
-      const float qb = jefi_q_fp32(g.kx, g.ky, g.kz, (float)(Dxi + (b & 7) - lx), (float)(Dyi + ((b >> 3) & 7) - ly), (float)(Dzi + (b >> 6) - lz));
+      const int lx = sc % G::TSX, ly = (sc / G::TSX) % G::TSY, lz = sc / (G::TSX * G::TSY);
+      const float qa = jefi_q_fp32(g.kx, g.ky, g.kz, (float)(Dxi + axc - lx), (float)(Dyi + ayc - ly), (float)(Dzi + azc - lz));
+      const float qb = jefi_q_fp32(g.kx, g.ky, g.kz, (float)(Dxi + bxc - lx), (float)(Dyi + byc - ly), (float)(Dzi + bzc - lz));
       const int ma = qa > 0.f ? jefi_delay_fp32(qa) : 0, mb = qb > 0.f ? jefi_delay_fp32(qb) : 0;
       mine |= (unsigned long long)(ma != mb) << sc;
     }
@@ -500,15 +581,19 @@ __global__ void __launch_bounds__(OBCELLS) k_build_perm(int ndx, int ndy, int nt
   perm[(size_t)blockIdx.x * OBCELLS + c] = order[2 * picked[c >> 1] + (c & 1)];
 }
 
-// window pitches the kernel is compiled for (ring rows per stage)
+// window pitches the kernel is compiled for (ring rows per stage); a wider window is served in several passes
 static const int kPitches[] = {36, 48};
 typedef void (*tiled_fn)(tiled_params);
-static tiled_fn tiled_kernel_for(int wp, bool linear) {
+template <class G>
+static tiled_fn tiled_kernel_of(int wp, bool linear) {
   switch (wp) {
-    case 36: return linear ? k_field_tiled<36, true> : k_field_tiled<36, false>;
-    case 48: return linear ? k_field_tiled<48, true> : k_field_tiled<48, false>;
+    case 36: return linear ? k_field_tiled<G, 36, true> : k_field_tiled<G, 36, false>;
+    case 48: return linear ? k_field_tiled<G, 48, true> : k_field_tiled<G, 48, false>;
   }
   return nullptr;
+}
+static tiled_fn tiled_kernel_for(int geom, int wp, bool linear) {
+  return geom == JEFI_GEOM_SLABX ? tiled_kernel_of<jefi_geom_slabx>(wp, linear) : tiled_kernel_of<jefi_geom_cube>(wp, linear);
 }
 static size_t tiled_smem_for(int wp) {
   switch (wp) {
@@ -518,41 +603,56 @@ static size_t tiled_smem_for(int wp) {
   return 0;
 }
 
-// Largest slot window over all relative placements of an 8^3 observation tile and a 4^3 source tile (host, fp64),
+// How the source range is split over blockIdx.y.  A CTA per observation tile walking ALL source tiles needs no second
+// kernel; that is used once there are at least four waves of observation tiles.  Smaller grids split the source tiles so
+// that the CTAs fill whole waves of the GPU: cost model = waves x (tiles per CTA + c0), c0 = 1.5 tiles of fixed cost per CTA
+// (accumulator zeroing, barrier set-up, first copy latency, epilogue).
+static void choose_split(int nobs, int ntiles, int nsm, int request, int& chunk, int& nsplit) {
+  if (request == -1 || (request == 0 && nobs >= 4 * nsm)) {
+    chunk = ntiles;
+  } else if (request > 0) {
+    chunk = request < ntiles ? request : ntiles;
+  } else {
+    double best = 1e300;
+    chunk = ntiles;
+    for (int ns = 1; ns <= ntiles && ns <= 256; ns++) {
+      const int ch = (ntiles + ns - 1) / ns;
+      const int pieces = (ntiles + ch - 1) / ch;
+      const long ctas = (long)nobs * pieces;
+      const long waves = (ctas + nsm - 1) / nsm;
+      const double cost = (double)waves * ((double)ch + 1.5);
+      if (cost < best * 0.999) { best = cost; chunk = ch; }
+    }
+  }
+  if (chunk < 1) chunk = 1;
+  if ((ntiles + chunk - 1) / chunk > 65535) chunk = (ntiles + 65534) / 65535;
+  nsplit = (ntiles + chunk - 1) / chunk;
+}
+
+// Largest slot window over all relative placements of an observation tile and a source tile (host, fp64),
 // shared-memory opt-in, and the evaluation-order table.
 int jefi_tiled_prepare(jefi_ctx* c) {
   const jefi_dims& d = c->dims;
   const double L0 = c->c * c->cfg.dt;
-  const int nobx = (d.nx + OB - 1) / OB, noby = (d.ny + OB - 1) / OB, nobz = (d.nz + OB - 1) / OB;
+  const int nobx = (d.nx + d.obx - 1) / d.obx, noby = (d.ny + d.oby - 1) / d.oby, nobz = (d.nz + d.obz - 1) / d.obz;
   int wmax = 1;
-  auto rng = [](int lo, int hi, int& mn, int& mx) {
-    int alo = abs(lo), ahi = abs(hi);
-    mx = alo > ahi ? alo : ahi;
-    mn = (lo <= 0 && hi >= 0) ? 0 : (alo < ahi ? alo : ahi);
-  };
-  // the window depends only on the per-axis difference D = ox0 - sx0 (a multiple of 4)
-  for (int Dz = -(d.ntz - 1) * JEFI_TS; Dz <= (nobz - 1) * OB; Dz += JEFI_TS)
-    for (int Dy = -(d.nty - 1) * JEFI_TS; Dy <= (noby - 1) * OB; Dy += JEFI_TS)
-      for (int Dx = -(d.ntx - 1) * JEFI_TS; Dx <= (nobx - 1) * OB; Dx += JEFI_TS) {
+  // the window depends only on the per-axis difference D = ox0 - sx0 (a multiple of the source tile edge)
+  for (int Dz = -(d.ntz - 1) * d.tsz; Dz <= (nobz - 1) * d.obz; Dz += d.tsz)
+    for (int Dy = -(d.nty - 1) * d.tsy; Dy <= (noby - 1) * d.oby; Dy += d.tsy)
+      for (int Dx = -(d.ntx - 1) * d.tsx; Dx <= (nobx - 1) * d.obx; Dx += d.tsx) {
         int mnx, mxx, mny, mxy, mnz, mxz;
-        rng(Dx - (JEFI_TS - 1), Dx + OB - 1, mnx, mxx);
-        rng(Dy - (JEFI_TS - 1), Dy + OB - 1, mny, mxy);
-        rng(Dz - (JEFI_TS - 1), Dz + OB - 1, mnz, mxz);
+        abs_range(Dx - (d.tsx - 1), Dx + d.obx - 1, mnx, mxx);
+        abs_range(Dy - (d.tsy - 1), Dy + d.oby - 1, mny, mxy);
+        abs_range(Dz - (d.tsz - 1), Dz + d.obz - 1, mnz, mxz);
         double rlo = sqrt(pow(mnx * c->cfg.dx, 2) + pow(mny * c->cfg.dy, 2) + pow(mnz * c->cfg.dz, 2));
         double rhi = sqrt(pow(mxx * c->cfg.dx, 2) + pow(mxy * c->cfg.dy, 2) + pow(mxz * c->cfg.dz, 2));
         int w = (int)floor(rhi / L0 + 0.5) - (int)floor(rlo / L0 + 0.5) + 1;
         if (w > wmax) wmax = w;
       }
   c->wmax = wmax;
-  int wp = 0;
+  int wp = kPitches[sizeof(kPitches) / sizeof(int) - 1];  // wider windows: several passes through the largest pitch
   for (int cand : kPitches)
     if (cand >= wmax) { wp = cand; break; }
-  if (wp == 0) {
-    char buf[160];
-    snprintf(buf, sizeof buf, "tiled kernel: slot window of %d exceeds the largest compiled pitch %d", wmax, kPitches[1]);
-    c->err = buf;
-    return JEFI_ESTATE;
-  }
   c->wpitch = wp;
   c->tiled_smem = tiled_smem_for(wp);
   int dev = c->cfg.device, max_optin = 0;
@@ -563,72 +663,65 @@ int jefi_tiled_prepare(jefi_ctx* c) {
     c->err = buf;
     return JEFI_ESTATE;
   }
-  cudaError_t e = cudaFuncSetAttribute(tiled_kernel_for(wp, c->cfg.delay_rule == JEFI_DELAY_LINEAR), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->tiled_smem);
+  const bool linear = c->cfg.delay_rule == JEFI_DELAY_LINEAR;
+  cudaError_t e = cudaFuncSetAttribute(tiled_kernel_for(c->tile_geom, wp, linear), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->tiled_smem);
   if (e != cudaSuccess) { c->err = std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e); return JEFI_ECUDA; }
-  // how the source range is split over blockIdx.y: JEFI_FIELD_CHUNK (source tiles per CTA) overrides the default, which
-  // keeps one CTA per observation tile (deterministic sums) once there are at least four waves of them and otherwise
-  // splits the source tiles so that the grid has about four CTAs per SM (partial sums meet in fp32 atomics).
   int nsm = 148;
   cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
   const int nobs = nobx * noby * nobz, ntiles = d.ntx * d.nty * d.ntz;
-  int chunk = ntiles;
-  const char* env = getenv("JEFI_FIELD_CHUNK");
-  if (env && atoi(env) > 0) {
-    chunk = atoi(env);
-  } else if (nobs < 4 * nsm) {
-    int nsplit = (4 * nsm + nobs - 1) / nobs;
-    chunk = (ntiles + nsplit - 1) / nsplit;
+  choose_split(nobs, ntiles, nsm, c->cfg.field_chunk, c->chunk, c->nsplit);
+  if (c->nsplit > 1) {
+    const size_t bytes = (size_t)c->nsplit * 6 * (size_t)d.N * sizeof(float);
+    if ((e = cudaMalloc(&c->partial, bytes)) != cudaSuccess) {
+      c->partial = nullptr;
+      c->err = std::string("partial-sum buffer (") + std::to_string(bytes) + " B): " + cudaGetErrorString(e);
+      return JEFI_ENOMEM;
+    }
   }
-  if (chunk < 1) chunk = 1;
-  if (chunk > ntiles) chunk = ntiles;
-  if ((ntiles + chunk - 1) / chunk > 65535) chunk = (ntiles + 65534) / 65535;
-  c->chunk = chunk;
   // evaluation-order table over all relative tile offsets
-  c->ndx = d.ntx + 2 * nobx - 2; c->ndy = d.nty + 2 * noby - 2; c->ndz = d.ntz + 2 * nobz - 2;
+  c->ndx = d.ntx + (d.obx / d.tsx) * (nobx - 1); c->ndy = d.nty + (d.oby / d.tsy) * (noby - 1); c->ndz = d.ntz + (d.obz / d.tsz) * (nobz - 1);
   size_t rows = (size_t)c->ndx * c->ndy * c->ndz;
   if ((e = cudaMalloc(&c->perm, rows * OBCELLS * sizeof(unsigned short))) != cudaSuccess) {
+    c->perm = nullptr;
     c->err = std::string("permutation table allocation: ") + cudaGetErrorString(e);
     return JEFI_ENOMEM;
   }
   // pairs a warp may draw from, counted from its first pair in the distance order: wide enough to find pairs that differ on
   // the same source cells, narrow enough that the delays of one warp stay within 8 slots (rows 8 apart share a bank group)
-  int band = 64;
-  const char* benv = getenv("JEFI_PERM_BAND");
-  if (benv && atoi(benv) > 0) band = atoi(benv);
-  k_build_perm<<<(unsigned)rows, OBCELLS, 0, c->stream>>>(c->ndx, c->ndy, d.ntx, d.nty, d.ntz, c->geom, band, c->perm);
+  const int band = 64;
+  if (c->tile_geom == JEFI_GEOM_SLABX)
+    k_build_perm<jefi_geom_slabx><<<(unsigned)rows, OBCELLS, 0, c->stream>>>(c->ndx, c->ndy, d.ntx, d.nty, d.ntz, c->geom, band, c->perm);
+  else
+    k_build_perm<jefi_geom_cube><<<(unsigned)rows, OBCELLS, 0, c->stream>>>(c->ndx, c->ndy, d.ntx, d.nty, d.ntz, c->geom, band, c->perm);
   if ((e = cudaGetLastError()) != cudaSuccess) { c->err = std::string("k_build_perm: ") + cudaGetErrorString(e); return JEFI_ECUDA; }
   c->launches++;
   return JEFI_OK;
 }
 
-int jefi_launch_field_tiled(jefi_ctx* c, int k0, int k1, float* ex, float* ey, float* ez, float* bx, float* by, float* bz) {
+int jefi_launch_field_tiled(jefi_ctx* c, int k0, int k1, float* ex, float* ey, float* ez, float* bx, float* by, float* bz,
+                            float* eb_packed) {
   const jefi_dims& d = c->dims;
   tiled_params P;
   P.d = d; P.g = c->geom; P.n = (int)c->step; P.nslot = (int)(c->step % d.H);
-  P.nobx = (d.nx + OB - 1) / OB; P.noby = (d.ny + OB - 1) / OB; P.nobz = (d.nz + OB - 1) / OB;
+  P.nobx = (d.nx + d.obx - 1) / d.obx; P.noby = (d.ny + d.oby - 1) / d.oby;
   P.ndx = c->ndx; P.ndy = c->ndy;
-  const int ntiles = d.ntx * d.nty * d.ntz;
   P.chunk = c->chunk;
-  const int nsplit = (ntiles + c->chunk - 1) / c->chunk;
-  P.atomic_out = nsplit > 1 ? 1 : 0;
+  P.to_partial = c->nsplit > 1 ? 1 : 0;
   P.ring = c->ring; P.perm = c->perm;
   P.ex = ex; P.ey = ey; P.ez = ez; P.bx = bx; P.by = by; P.bz = bz;
-  P.obz0 = k0 / OB; P.k1 = k1;
-  const int nlayers = (k1 - k0 + OB - 1) / OB;
-  if (P.atomic_out) {
-    float* outs[6] = {ex, ey, ez, bx, by, bz};
-    const size_t plane = (size_t)d.nx * d.ny;
-    bool block = k0 == 0 && k1 == d.nz;  // full step into one [6][N] block (the usual case): one memset node
-    for (int a = 1; a < 6; a++) block = block && outs[a] == outs[a - 1] + d.N;
-    if (block) {
-      JEFI_CUDA_TRY(c, cudaMemsetAsync(ex, 0, (size_t)6 * d.N * sizeof(float), c->stream));
-    } else {
-      for (float* o : outs) JEFI_CUDA_TRY(c, cudaMemsetAsync(o + plane * k0, 0, plane * (size_t)(k1 - k0) * sizeof(float), c->stream));
-    }
-  }
-  dim3 grid((unsigned)(P.nobx * P.noby * nlayers), (unsigned)nsplit);
-  tiled_kernel_for(c->wpitch, c->cfg.delay_rule == JEFI_DELAY_LINEAR)<<<grid, TILED_THREADS, c->tiled_smem, c->stream>>>(P);
+  P.pack = reinterpret_cast<float4*>(eb_packed);
+  P.partial = c->partial;
+  P.obz0 = k0 / d.obz; P.k1 = k1;
+  const int nlayers = (k1 - k0 + d.obz - 1) / d.obz;
+  dim3 grid((unsigned)(P.nobx * P.noby * nlayers), (unsigned)c->nsplit);
+  tiled_kernel_for(c->tile_geom, c->wpitch, c->cfg.delay_rule == JEFI_DELAY_LINEAR)<<<grid, TILED_THREADS, c->tiled_smem, c->stream>>>(P);
   JEFI_CUDA_TRY(c, cudaGetLastError());
   c->launches++;
+  if (c->nsplit > 1) {
+    const long c0 = (long)k0 * d.nx * d.ny, c1 = (long)k1 * d.nx * d.ny;
+    k_reduce_partials<<<(unsigned)((c1 - c0 + 255) / 256), 256, 0, c->stream>>>(d.N, c->nsplit, c0, c1, c->partial, ex, ey, ez, bx, by, bz, P.pack);
+    JEFI_CUDA_TRY(c, cudaGetLastError());
+    c->launches++;
+  }
   return JEFI_OK;
 }

@@ -3,12 +3,48 @@
 #include "jefi_ctx.h"
 
 // Eq. (2.15)/(2.17) in grid units: node index i = floor(xi - 1/2), fraction alpha = xi - 1/2 - i.  xi - 0.5 is exact
-// in fp32 for 0.25 <= xi < 2^23, so the index equals the fp64 oracle's bit for bit (DESIGN.md §3 A9).
+// in fp32 for 0.25 <= xi < 2^23, so the index equals the fp64 oracle's bit for bit (DESIGN.md §3 A9).  Positions far
+// outside any grid (a caller's stale alive flag) are clamped before the float -> int conversion; they stay outside.
 __device__ __forceinline__ void cic_cell(float xi, int& i, float& alpha) {
-  float s = xi - 0.5f;
+  float s = fminf(fmaxf(xi, -16.f), 2.0e9f) - 0.5f;
   float f = floorf(s);
   i = (int)f;
   alpha = s - f;
+}
+
+// The nodes one axis of a particle touches and their weights, for the two shape functions (jefi_config.shape_order):
+//   ORDER 1  S^(1), Eqs. (2.13), (2.16): nodes i0 = floor(xi - 1/2) and i0 + 1 with weights 1 - alpha, alpha;
+//   ORDER 2  S^(2), Eq. (2.14) (reading A11: the quadratic B-spline): centre node ic = floor(xi), nodes ic-1, ic, ic+1 with
+//            weights (1/2)(1/2 - d)^2, 3/4 - d^2, (1/2)(1/2 + d)^2, d = xi - (ic + 1/2) in [-1/2, 1/2) (xi - ic and the
+//            subtraction of 1/2 are exact in fp32, so d equals the fp64 oracle's).
+template <int ORDER>
+struct axis_stencil {
+  static constexpr int NN = ORDER + 1;
+  int i0;       // first node
+  float w[NN];
+  __device__ __forceinline__ void set(float xi) {
+    if (ORDER == 1) {
+      float al;
+      cic_cell(xi, i0, al);
+      w[0] = 1.f - al;
+      w[ORDER] = al;
+    } else {
+      const float xc = fminf(fmaxf(xi, -16.f), 2.0e9f);
+      const float f = floorf(xc);
+      const float dlt = (xc - f) - 0.5f;
+      i0 = (int)f - 1;
+      w[0] = 0.5f * (0.5f - dlt) * (0.5f - dlt);
+      w[1] = 0.75f - dlt * dlt;
+      w[ORDER] = 0.5f * (0.5f + dlt) * (0.5f + dlt);
+    }
+  }
+};
+// bins of the cell sort per axis and the key of a base node: i0 in [-(NN-1), n-1] <=> at least one node inside the grid
+template <int ORDER>
+__device__ __forceinline__ bool base_key(int nx, int ny, int nz, int i0, int j0, int k0, int& key) {
+  constexpr int S = ORDER;  // NN - 1
+  key = (i0 + S) + (nx + S) * ((j0 + S) + (ny + S) * (k0 + S));
+  return i0 >= -S && i0 < nx && j0 >= -S && j0 < ny && k0 >= -S && k0 < nz;
 }
 
 // ------------------------------------------------------------------------------------------------------------
@@ -44,6 +80,7 @@ __device__ __forceinline__ void warp_aggregated_add4(float* __restrict__ rho, fl
   }
 }
 
+template <int ORDER>
 __global__ void __launch_bounds__(256) k_deposit(int nx, int ny, int nz, float inv_dV, float cc, long np,
                                                  const float* __restrict__ x, const float* __restrict__ y,
                                                  const float* __restrict__ z, const float* __restrict__ ux,
@@ -51,26 +88,31 @@ __global__ void __launch_bounds__(256) k_deposit(int nx, int ny, int nz, float i
                                                  const float* __restrict__ qw, const unsigned char* __restrict__ alive,
                                                  float* __restrict__ rho, float* __restrict__ jx, float* __restrict__ jy,
                                                  float* __restrict__ jz) {
+  constexpr int NN = ORDER + 1;
   long p = (long)blockIdx.x * blockDim.x + threadIdx.x;
   bool live = p < np && (alive == nullptr || alive[p] != 0);
-  int i = 0, j = 0, k = 0;
-  float al = 0, be = 0, ch = 0, r0 = 0, vx = 0, vy = 0, vz = 0;
+  axis_stencil<ORDER> sx, sy, sz;
+  sx.set(0.f); sy.set(0.f); sz.set(0.f);
+  float r0 = 0, vx = 0, vy = 0, vz = 0;
   if (live) {
-    cic_cell(x[p], i, al); cic_cell(y[p], j, be); cic_cell(z[p], k, ch);
+    sx.set(x[p]); sy.set(y[p]); sz.set(z[p]);
     float u0 = ux[p], u1 = uy[p], u2 = uz[p];
     float ig = rsqrtf(1.f + u0 * u0 + u1 * u1 + u2 * u2);  // 1/gamma
     vx = cc * u0 * ig; vy = cc * u1 * ig; vz = cc * u2 * ig;  // v = c u / gamma
     r0 = qw[p] * inv_dV;                                     // Eq. (2.18)
   }
 #pragma unroll
-  for (int c3 = 0; c3 < 8; c3++) {
-    const int a = c3 & 1, b = (c3 >> 1) & 1, c = c3 >> 2;
-    int ii = i + a, jj = j + b, kk = k + c;
-    bool ok = live && ii >= 0 && ii < nx && jj >= 0 && jj < ny && kk >= 0 && kk < nz;  // virtual nodes dropped
-    float w = (a ? al : 1.f - al) * (b ? be : 1.f - be) * (c ? ch : 1.f - ch);          // Eq. (2.16)
-    long node = ok ? (long)ii + (long)nx * ((long)jj + (long)ny * kk) : -1 - (long)(threadIdx.x & 31);
-    warp_aggregated_add4(rho, jx, jy, jz, node, r0 * w, vx, vy, vz);
-  }
+  for (int c = 0; c < NN; c++)
+#pragma unroll
+    for (int b = 0; b < NN; b++)
+#pragma unroll
+      for (int a = 0; a < NN; a++) {
+        int ii = sx.i0 + a, jj = sy.i0 + b, kk = sz.i0 + c;
+        bool ok = live && ii >= 0 && ii < nx && jj >= 0 && jj < ny && kk >= 0 && kk < nz;  // virtual nodes dropped
+        float w = sx.w[a] * sy.w[b] * sz.w[c];                                               // Eq. (2.16)
+        long node = ok ? (long)ii + (long)nx * ((long)jj + (long)ny * kk) : -1 - (long)(threadIdx.x & 31);
+        warp_aggregated_add4(rho, jx, jy, jz, node, r0 * w, vx, vy, vz);
+      }
 }
 
 // ------------------------------------------------------------------------------------------------------------
@@ -84,6 +126,7 @@ __global__ void __launch_bounds__(256) k_deposit(int nx, int ny, int nz, float i
 //                   contributions are combined with a segmented shuffle reduction (5 steps) and only the first lane
 //                   of every run issues the fp32 reductions: one per (warp, cell, node, quantity).
 // ------------------------------------------------------------------------------------------------------------
+template <int ORDER>
 __global__ void __launch_bounds__(256) k_sort_keys(int nx, int ny, int nz, int nbins, long np, const float* __restrict__ x,
                                                    const float* __restrict__ y, const float* __restrict__ z,
                                                    const unsigned char* __restrict__ alive, int* __restrict__ key,
@@ -92,12 +135,12 @@ __global__ void __launch_bounds__(256) k_sort_keys(int nx, int ny, int nz, int n
   if (p >= np) return;
   int kk = nbins, r = 0;  // extra last bin: dead particles and particles with no node inside the grid
   if (alive == nullptr || alive[p] != 0) {
-    int i, j, k;
-    float a;
-    cic_cell(x[p], i, a); cic_cell(y[p], j, a); cic_cell(z[p], k, a);
-    // alive particles have xi in [0, n): i in [-1, n-1].  A particle outside that range has all 8 nodes outside the
-    // grid (virtual): it deposits nothing and is left out of the order.
-    if (i >= -1 && i < nx && j >= -1 && j < ny && k >= -1 && k < nz) kk = (i + 1) + (nx + 1) * ((j + 1) + (ny + 1) * (k + 1));
+    axis_stencil<ORDER> sx, sy, sz;
+    sx.set(x[p]); sy.set(y[p]); sz.set(z[p]);
+    // A particle whose base node is outside [-(NN-1), n) has all its nodes outside the grid (virtual): it
+    // deposits nothing and is left out of the order.
+    int k2;
+    if (base_key<ORDER>(nx, ny, nz, sx.i0, sy.i0, sz.i0, k2)) kk = k2;
   }
   r = (int)atomicAdd(count + kk, 1u);
   key[p] = kk;
@@ -164,10 +207,8 @@ __global__ void __launch_bounds__(256) k_sort_scatter(long np, const int* __rest
   order[offset[key[p]] + (unsigned)rank[p]] = (int)p;
 }
 
-#ifndef JEFI_DEP_MINBLOCKS
-#define JEFI_DEP_MINBLOCKS 1
-#endif
-__global__ void __launch_bounds__(256, JEFI_DEP_MINBLOCKS) k_deposit_sorted(int nx, int ny, int nz, float inv_dV, float cc, long np,
+template <int ORDER>
+__global__ void __launch_bounds__(256) k_deposit_sorted(int nx, int ny, int nz, float inv_dV, float cc, long np,
                                                         const unsigned* __restrict__ n_alive, const int* __restrict__ order,
                                                         const unsigned char* __restrict__ alive, const float* __restrict__ x,
                                                         const float* __restrict__ y, const float* __restrict__ z,
@@ -175,22 +216,31 @@ __global__ void __launch_bounds__(256, JEFI_DEP_MINBLOCKS) k_deposit_sorted(int 
                                                         const float* __restrict__ uz, const float* __restrict__ qw,
                                                         float* __restrict__ rho, float* __restrict__ jx,
                                                         float* __restrict__ jy, float* __restrict__ jz) {
+  constexpr int NN = ORDER + 1;
   const long t = (long)blockIdx.x * blockDim.x + threadIdx.x;
   const long na = order ? (long)*n_alive : np;
   if (((long)blockIdx.x * blockDim.x + (threadIdx.x & ~31)) >= na) return;  // whole warp beyond the last particle
   bool live = t < na;
   const unsigned FULL = 0xffffffffu, lane = threadIdx.x & 31;
-  int i = 0, j = 0, k = 0, kk = -2 - (int)lane;  // padding lanes: unique keys, never merged
-  float al = 0, be = 0, ch = 0, r0 = 0, vx = 0, vy = 0, vz = 0;
+  int kk = -2 - (int)lane;  // padding lanes and non-depositing particles: unique keys, never merged
+  axis_stencil<ORDER> sx, sy, sz;
+  sx.set(0.f); sy.set(0.f); sz.set(0.f);
+  float r0 = 0, vx = 0, vy = 0, vz = 0;
   long p = t;
   if (live) {
     if (order) p = order[t];
     else live = alive == nullptr || alive[p] != 0;
   }
   if (live) {
-    cic_cell(x[p], i, al); cic_cell(y[p], j, be); cic_cell(z[p], k, ch);
-    kk = (i + 1) + (nx + 1) * ((j + 1) + (ny + 1) * (k + 1));  // distinct (i,j,k) in [-1, n) give distinct keys; anything
-                                                                // outside that range has no node in the grid (dropped below)
+    sx.set(x[p]); sy.set(y[p]); sz.set(z[p]);
+    // distinct base nodes in [-(NN-1), n) give distinct keys.  A particle outside that range (possible with alive == NULL or
+    // a stale flag) has no node in the grid: it keeps its unique negative key, so that it can neither alias the key of an
+    // in-grid cell nor be merged into a neighbour's run.
+    int k2;
+    if (base_key<ORDER>(nx, ny, nz, sx.i0, sy.i0, sz.i0, k2)) kk = k2;
+    else live = false;
+  }
+  if (live) {
     float u0 = ux[p], u1 = uy[p], u2 = uz[p];
     float ig = rsqrtf(1.f + u0 * u0 + u1 * u1 + u2 * u2);
     vx = cc * u0 * ig; vy = cc * u1 * ig; vz = cc * u2 * ig;
@@ -212,29 +262,36 @@ __global__ void __launch_bounds__(256, JEFI_DEP_MINBLOCKS) k_deposit_sorted(int 
     any_same |= (__ballot_sync(FULL, same[s]) != 0u ? 1u : 0u) << s;
   }
 #pragma unroll
-  for (int c3 = 0; c3 < 8; c3++) {
-    const int a = c3 & 1, b = (c3 >> 1) & 1, c = c3 >> 2;
-    const float w = (a ? al : 1.f - al) * (b ? be : 1.f - be) * (c ? ch : 1.f - ch);
-    float a0 = r0 * w, a1 = a0 * vx, a2 = a0 * vy, a3 = a0 * vz;
+  for (int c = 0; c < NN; c++)
 #pragma unroll
-    for (int s = 0; s < 5; s++) {  // segmented suffix sum: the head of a run ends up with the run total
-      if (!((any_same >> s) & 1u)) continue;  // warp-uniform
-      const float b0 = __shfl_down_sync(FULL, a0, 1u << s), b1 = __shfl_down_sync(FULL, a1, 1u << s);
-      const float b2 = __shfl_down_sync(FULL, a2, 1u << s), b3 = __shfl_down_sync(FULL, a3, 1u << s);
-      if (same[s]) { a0 += b0; a1 += b1; a2 += b2; a3 += b3; }
-    }
-    const int ii = i + a, jj = j + b, kz = k + c;
-    if (live && head && ii >= 0 && ii < nx && jj >= 0 && jj < ny && kz >= 0 && kz < nz) {  // virtual nodes dropped
-      const long node = (long)ii + (long)nx * ((long)jj + (long)ny * kz);
-      atomicAdd(rho + node, a0); atomicAdd(jx + node, a1); atomicAdd(jy + node, a2); atomicAdd(jz + node, a3);
-    }
-  }
+    for (int b = 0; b < NN; b++)
+#pragma unroll
+      for (int a = 0; a < NN; a++) {
+        const float w = sx.w[a] * sy.w[b] * sz.w[c];
+        float a0 = r0 * w, a1 = a0 * vx, a2 = a0 * vy, a3 = a0 * vz;
+#pragma unroll
+        for (int s = 0; s < 5; s++) {  // segmented suffix sum: the head of a run ends up with the run total
+          if (!((any_same >> s) & 1u)) continue;  // warp-uniform
+          const float b0 = __shfl_down_sync(FULL, a0, 1u << s), b1 = __shfl_down_sync(FULL, a1, 1u << s);
+          const float b2 = __shfl_down_sync(FULL, a2, 1u << s), b3 = __shfl_down_sync(FULL, a3, 1u << s);
+          if (same[s]) { a0 += b0; a1 += b1; a2 += b2; a3 += b3; }
+        }
+        const int ii = sx.i0 + a, jj = sy.i0 + b, kz = sz.i0 + c;
+        if (live && head && ii >= 0 && ii < nx && jj >= 0 && jj < ny && kz >= 0 && kz < nz) {  // virtual nodes dropped
+          const long node = (long)ii + (long)nx * ((long)jj + (long)ny * kz);
+          atomicAdd(rho + node, a0); atomicAdd(jx + node, a1); atomicAdd(jy + node, a2); atomicAdd(jz + node, a3);
+        }
+      }
 }
 
-static inline long sort_bins(const jefi_dims& d) { return (long)(d.nx + 1) * (d.ny + 1) * (d.nz + 1); }
+static inline long sort_bins(const jefi_ctx* c) {
+  const jefi_dims& d = c->dims;
+  const int s = c->shape_order;  // nodes per axis - 1
+  return (long)(d.nx + s) * (d.ny + s) * (d.nz + s);
+}
 
 static int ensure_sort_scratch(jefi_ctx* c, long np) {
-  const long nb = sort_bins(c->dims) + 1;  // + the bin of the non-depositing particles
+  const long nb = sort_bins(c) + 1;  // + the bin of the non-depositing particles
   const long ntiles = (nb + SCAN_TILE - 1) / SCAN_TILE;
   if (!c->sort_count) {
     JEFI_CUDA_TRY(c, cudaMalloc(&c->sort_count, (size_t)nb * sizeof(unsigned)));
@@ -261,11 +318,14 @@ static int build_cell_order(jefi_ctx* c, long np, const float* x, const float* y
   const jefi_dims& d = c->dims;
   int rc = ensure_sort_scratch(c, np);
   if (rc != JEFI_OK) return rc;
-  const long nbins = sort_bins(d), nb = nbins + 1;
+  const long nbins = sort_bins(c), nb = nbins + 1;
   const int ntiles = (int)((nb + SCAN_TILE - 1) / SCAN_TILE);
   const unsigned pb = (unsigned)((np + 255) / 256);
   JEFI_CUDA_TRY(c, cudaMemsetAsync(c->sort_count, 0, (size_t)nb * sizeof(unsigned), c->stream));
-  k_sort_keys<<<pb, 256, 0, c->stream>>>(d.nx, d.ny, d.nz, (int)nbins, np, x, y, z, alive, c->sort_key, c->sort_rank, c->sort_count);
+  if (c->shape_order == 2)
+    k_sort_keys<2><<<pb, 256, 0, c->stream>>>(d.nx, d.ny, d.nz, (int)nbins, np, x, y, z, alive, c->sort_key, c->sort_rank, c->sort_count);
+  else
+    k_sort_keys<1><<<pb, 256, 0, c->stream>>>(d.nx, d.ny, d.nz, (int)nbins, np, x, y, z, alive, c->sort_key, c->sort_rank, c->sort_count);
   k_scan_tiles<<<ntiles, SCAN_THREADS, 0, c->stream>>>(c->sort_count, c->sort_offset, nb, c->sort_sums);
   k_scan_sums<<<1, 1024, 0, c->stream>>>(c->sort_sums, ntiles);
   k_scan_add<<<(unsigned)((nb + 255) / 256), 256, 0, c->stream>>>(c->sort_offset, nb, c->sort_sums);
@@ -279,6 +339,7 @@ extern "C" int jefi_deposit(jefi_ctx* c, long np, const float* x, const float* y
                             const float* uy, const float* uz, const float* qw, const unsigned char* alive, float* rho,
                             float* jx, float* jy, float* jz) {
   if (!c) return JEFI_EINVAL;
+  jefi_device_guard guard(c);
   if (np < 0 || np > 0x7fffffffL || !rho || !jx || !jy || !jz || (np > 0 && (!x || !y || !z || !ux || !uy || !uz || !qw))) {
     c->err = "jefi_deposit: NULL array or np out of range";
     return JEFI_EINVAL;
@@ -297,17 +358,20 @@ extern "C" int jefi_deposit(jefi_ctx* c, long np, const float* x, const float* y
   unsigned blocks = (unsigned)((np + 255) / 256);
   int mode = c->cfg.deposit_mode;
   if (mode == JEFI_DEPOSIT_AUTO) mode = JEFI_DEPOSIT_RUNS;  // cheapest on sorted and unsorted lists alike
+  const float cc = (float)c->c;
+  const bool s2 = c->shape_order == 2;
   if (mode == JEFI_DEPOSIT_SORTED) {
     int rc = build_cell_order(c, np, x, y, z, alive);
     if (rc != JEFI_OK) return rc;
-    k_deposit_sorted<<<blocks, 256, 0, c->stream>>>(d.nx, d.ny, d.nz, inv_dV, (float)c->c, np, c->sort_offset + sort_bins(d),
-                                                    c->sort_order, alive, x, y, z, ux, uy, uz, qw, rho, jx, jy, jz);
+    const unsigned* na = c->sort_offset + sort_bins(c);
+    if (s2) k_deposit_sorted<2><<<blocks, 256, 0, c->stream>>>(d.nx, d.ny, d.nz, inv_dV, cc, np, na, c->sort_order, alive, x, y, z, ux, uy, uz, qw, rho, jx, jy, jz);
+    else k_deposit_sorted<1><<<blocks, 256, 0, c->stream>>>(d.nx, d.ny, d.nz, inv_dV, cc, np, na, c->sort_order, alive, x, y, z, ux, uy, uz, qw, rho, jx, jy, jz);
   } else if (mode == JEFI_DEPOSIT_RUNS) {
-    k_deposit_sorted<<<blocks, 256, 0, c->stream>>>(d.nx, d.ny, d.nz, inv_dV, (float)c->c, np, nullptr, nullptr, alive, x, y, z,
-                                                    ux, uy, uz, qw, rho, jx, jy, jz);
+    if (s2) k_deposit_sorted<2><<<blocks, 256, 0, c->stream>>>(d.nx, d.ny, d.nz, inv_dV, cc, np, nullptr, nullptr, alive, x, y, z, ux, uy, uz, qw, rho, jx, jy, jz);
+    else k_deposit_sorted<1><<<blocks, 256, 0, c->stream>>>(d.nx, d.ny, d.nz, inv_dV, cc, np, nullptr, nullptr, alive, x, y, z, ux, uy, uz, qw, rho, jx, jy, jz);
   } else {
-    k_deposit<<<blocks, 256, 0, c->stream>>>(d.nx, d.ny, d.nz, inv_dV, (float)c->c, np, x, y, z, ux, uy, uz, qw, alive, rho, jx,
-                                             jy, jz);
+    if (s2) k_deposit<2><<<blocks, 256, 0, c->stream>>>(d.nx, d.ny, d.nz, inv_dV, cc, np, x, y, z, ux, uy, uz, qw, alive, rho, jx, jy, jz);
+    else k_deposit<1><<<blocks, 256, 0, c->stream>>>(d.nx, d.ny, d.nz, inv_dV, cc, np, x, y, z, ux, uy, uz, qw, alive, rho, jx, jy, jz);
   }
   JEFI_CUDA_TRY(c, cudaGetLastError());
   c->launches++;
@@ -318,12 +382,13 @@ extern "C" int jefi_deposit(jefi_ctx* c, long np, const float* x, const float* y
 extern "C" int jefi_debug_cell_order(jefi_ctx* c, long np, const float* x, const float* y, const float* z,
                                      const unsigned char* alive, int* order_out, long* n_alive_host) {
   if (!c || np < 0 || np > 0x7fffffffL || !n_alive_host || (np > 0 && (!x || !y || !z || !order_out))) return JEFI_EINVAL;
+  jefi_device_guard guard(c);
   *n_alive_host = 0;
   if (np == 0) return JEFI_OK;
   int rc = build_cell_order(c, np, x, y, z, alive);
   if (rc != JEFI_OK) return rc;
   unsigned na = 0;
-  JEFI_CUDA_TRY(c, cudaMemcpyAsync(&na, c->sort_offset + sort_bins(c->dims), sizeof na, cudaMemcpyDeviceToHost, c->stream));
+  JEFI_CUDA_TRY(c, cudaMemcpyAsync(&na, c->sort_offset + sort_bins(c), sizeof na, cudaMemcpyDeviceToHost, c->stream));
   JEFI_CUDA_TRY(c, cudaMemcpyAsync(order_out, c->sort_order, (size_t)np * sizeof(int), cudaMemcpyDeviceToDevice, c->stream));
   JEFI_CUDA_TRY(c, cudaStreamSynchronize(c->stream));
   *n_alive_host = (long)na;
@@ -362,6 +427,7 @@ __global__ void __launch_bounds__(256) k_permute_copyback(long np, perm_arrays A
 extern "C" int jefi_sort_particles(jefi_ctx* c, long np, float* x, float* y, float* z, float* ux, float* uy, float* uz, float* qw,
                                    float* q_over_m, unsigned char* alive, int* tag) {
   if (!c) return JEFI_EINVAL;
+  jefi_device_guard guard(c);
   if (np < 0 || np > 0x7fffffffL || (np > 0 && (!x || !y || !z || !ux || !uy || !uz || !qw || !q_over_m || !alive))) {
     c->err = "jefi_sort_particles: NULL array or np out of range";
     return JEFI_EINVAL;
@@ -410,38 +476,41 @@ __global__ void __launch_bounds__(256) k_pack_fields(long N, const float* __rest
 #ifndef JEFI_PUSH_MINBLOCKS
 #define JEFI_PUSH_MINBLOCKS 8  /* 32 registers: 100 % occupancy; measured 0.239 -> 0.183 ms on the sorted config-5 list */
 #endif
-template <bool PACKED>
-__global__ void __launch_bounds__(256, JEFI_PUSH_MINBLOCKS) k_push(push_consts K, long np, float* __restrict__ x, float* __restrict__ y,
+template <bool PACKED, int ORDER>
+__global__ void __launch_bounds__(256, ORDER == 1 ? JEFI_PUSH_MINBLOCKS : 4) k_push(push_consts K, long np, float* __restrict__ x, float* __restrict__ y,
                                               float* __restrict__ z, float* __restrict__ ux, float* __restrict__ uy,
                                               float* __restrict__ uz, const float* __restrict__ qm,
                                               unsigned char* __restrict__ alive, const float* __restrict__ ex,
                                               const float* __restrict__ ey, const float* __restrict__ ez,
                                               const float* __restrict__ bx, const float* __restrict__ by,
                                               const float* __restrict__ bz, const float4* __restrict__ pack) {
+  constexpr int NN = ORDER + 1;
   long p = (long)blockIdx.x * blockDim.x + threadIdx.x;
   if (p >= np || alive[p] == 0) return;
   float xp = x[p], yp = y[p], zp = z[p];
-  int i, j, k;
-  float al, be, ch;
-  cic_cell(xp, i, al); cic_cell(yp, j, be); cic_cell(zp, k, ch);
+  axis_stencil<ORDER> nx_, ny_, nz_;
+  nx_.set(xp); ny_.set(yp); nz_.set(zp);
   float E0 = 0, E1 = 0, E2 = 0, B0 = 0, B1 = 0, B2 = 0;
 #pragma unroll
-  for (int c3 = 0; c3 < 8; c3++) {  // Eq. (2.20); virtual nodes count as zero
-    const int a = c3 & 1, b = (c3 >> 1) & 1, c = c3 >> 2;
-    int ii = i + a, jj = j + b, kk = k + c;
-    if (ii >= 0 && ii < K.nx && jj >= 0 && jj < K.ny && kk >= 0 && kk < K.nz) {
-      float w = (a ? al : 1.f - al) * (b ? be : 1.f - be) * (c ? ch : 1.f - ch);
-      long node = (long)ii + (long)K.nx * ((long)jj + (long)K.ny * kk);
-      if (PACKED) {
-        const float4 f0 = __ldg(pack + 2 * node), f1 = __ldg(pack + 2 * node + 1);
-        E0 = fmaf(w, f0.x, E0); E1 = fmaf(w, f0.y, E1); E2 = fmaf(w, f0.z, E2);
-        B0 = fmaf(w, f0.w, B0); B1 = fmaf(w, f1.x, B1); B2 = fmaf(w, f1.y, B2);
-      } else {
-        E0 = fmaf(w, __ldg(ex + node), E0); E1 = fmaf(w, __ldg(ey + node), E1); E2 = fmaf(w, __ldg(ez + node), E2);
-        B0 = fmaf(w, __ldg(bx + node), B0); B1 = fmaf(w, __ldg(by + node), B1); B2 = fmaf(w, __ldg(bz + node), B2);
+  for (int c = 0; c < NN; c++)
+#pragma unroll
+    for (int b = 0; b < NN; b++)
+#pragma unroll
+      for (int a = 0; a < NN; a++) {  // Eq. (2.20); virtual nodes count as zero
+        int ii = nx_.i0 + a, jj = ny_.i0 + b, kk = nz_.i0 + c;
+        if (ii >= 0 && ii < K.nx && jj >= 0 && jj < K.ny && kk >= 0 && kk < K.nz) {
+          float w = nx_.w[a] * ny_.w[b] * nz_.w[c];
+          long node = (long)ii + (long)K.nx * ((long)jj + (long)K.ny * kk);
+          if (PACKED) {
+            const float4 f0 = __ldg(pack + 2 * node), f1 = __ldg(pack + 2 * node + 1);
+            E0 = fmaf(w, f0.x, E0); E1 = fmaf(w, f0.y, E1); E2 = fmaf(w, f0.z, E2);
+            B0 = fmaf(w, f0.w, B0); B1 = fmaf(w, f1.x, B1); B2 = fmaf(w, f1.y, B2);
+          } else {
+            E0 = fmaf(w, __ldg(ex + node), E0); E1 = fmaf(w, __ldg(ey + node), E1); E2 = fmaf(w, __ldg(ez + node), E2);
+            B0 = fmaf(w, __ldg(bx + node), B0); B1 = fmaf(w, __ldg(by + node), B1); B2 = fmaf(w, __ldg(bz + node), B2);
+          }
+        }
       }
-    }
-  }
   E0 += K.Eext[0]; E1 += K.Eext[1]; E2 += K.Eext[2];
   B0 += K.Bext[0]; B1 += K.Bext[1]; B2 += K.Bext[2];
   const float qom = qm[p];
@@ -469,15 +538,7 @@ __global__ void __launch_bounds__(256, JEFI_PUSH_MINBLOCKS) k_push(push_consts K
   if (xn < 0.f || xn >= (float)K.nx || yn < 0.f || yn >= (float)K.ny || zn < 0.f || zn >= (float)K.nz) alive[p] = 0;
 }
 
-extern "C" int jefi_push_particles(jefi_ctx* c, long np, float* x, float* y, float* z, float* ux, float* uy, float* uz,
-                                   const float* q_over_m, unsigned char* alive, const float* ex, const float* ey,
-                                   const float* ez, const float* bx, const float* by, const float* bz) {
-  if (!c) return JEFI_EINVAL;
-  if (np < 0 || !ex || !ey || !ez || !bx || !by || !bz || (np > 0 && (!x || !y || !z || !ux || !uy || !uz || !q_over_m || !alive))) {
-    c->err = "jefi_push_particles: NULL array or negative np";
-    return JEFI_EINVAL;
-  }
-  if (np == 0) return JEFI_OK;
+static push_consts make_push_consts(const jefi_ctx* c) {
   const jefi_dims& d = c->dims;
   push_consts K;
   K.nx = d.nx; K.ny = d.ny; K.nz = d.nz;
@@ -485,34 +546,78 @@ extern "C" int jefi_push_particles(jefi_ctx* c, long np, float* x, float* y, flo
   K.half_dt = (float)(c->cfg.dt / 2.0);
   K.sx = (float)(c->c * c->cfg.dt / c->cfg.dx); K.sy = (float)(c->c * c->cfg.dt / c->cfg.dy); K.sz = (float)(c->c * c->cfg.dt / c->cfg.dz);
   for (int a = 0; a < 3; a++) { K.Eext[a] = (float)c->cfg.Eext[a]; K.Bext[a] = (float)c->cfg.Bext[a]; }
-  unsigned blocks = (unsigned)((np + 255) / 256);
-  if (np >= d.N) {  // enough particles per node for the packed copy of the fields to pay for itself
+  return K;
+}
+
+template <bool PACKED>
+static void launch_push(jefi_ctx* c, long np, float* x, float* y, float* z, float* ux, float* uy, float* uz, const float* q_over_m,
+                        unsigned char* alive, const float* ex, const float* ey, const float* ez, const float* bx, const float* by,
+                        const float* bz, const float4* pack) {
+  const push_consts K = make_push_consts(c);
+  const unsigned blocks = (unsigned)((np + 255) / 256);
+  if (c->shape_order == 2)
+    k_push<PACKED, 2><<<blocks, 256, 0, c->stream>>>(K, np, x, y, z, ux, uy, uz, q_over_m, alive, ex, ey, ez, bx, by, bz, pack);
+  else
+    k_push<PACKED, 1><<<blocks, 256, 0, c->stream>>>(K, np, x, y, z, ux, uy, uz, q_over_m, alive, ex, ey, ez, bx, by, bz, pack);
+  c->launches++;
+}
+
+extern "C" int jefi_push_particles(jefi_ctx* c, long np, float* x, float* y, float* z, float* ux, float* uy, float* uz,
+                                   const float* q_over_m, unsigned char* alive, const float* ex, const float* ey,
+                                   const float* ez, const float* bx, const float* by, const float* bz) {
+  if (!c) return JEFI_EINVAL;
+  jefi_device_guard guard(c);
+  if (np < 0 || !ex || !ey || !ez || !bx || !by || !bz || (np > 0 && (!x || !y || !z || !ux || !uy || !uz || !q_over_m || !alive))) {
+    c->err = "jefi_push_particles: NULL array or negative np";
+    return JEFI_EINVAL;
+  }
+  if (np == 0) return JEFI_OK;
+  const jefi_dims& d = c->dims;
+  if (np >= d.N) {  // enough particles per node for a packed copy of the fields to pay for itself (jefi_field_step_packed +
+                    // jefi_push_particles_packed avoid this pass altogether)
     if (!c->eb_pack) JEFI_CUDA_TRY(c, cudaMalloc(&c->eb_pack, (size_t)d.N * 2 * sizeof(float4)));
     k_pack_fields<<<(unsigned)((d.N + 255) / 256), 256, 0, c->stream>>>(d.N, ex, ey, ez, bx, by, bz, c->eb_pack);
-    k_push<true><<<blocks, 256, 0, c->stream>>>(K, np, x, y, z, ux, uy, uz, q_over_m, alive, ex, ey, ez, bx, by, bz, c->eb_pack);
     c->launches++;
+    launch_push<true>(c, np, x, y, z, ux, uy, uz, q_over_m, alive, ex, ey, ez, bx, by, bz, c->eb_pack);
   } else {
-    k_push<false><<<blocks, 256, 0, c->stream>>>(K, np, x, y, z, ux, uy, uz, q_over_m, alive, ex, ey, ez, bx, by, bz, nullptr);
+    launch_push<false>(c, np, x, y, z, ux, uy, uz, q_over_m, alive, ex, ey, ez, bx, by, bz, nullptr);
   }
   JEFI_CUDA_TRY(c, cudaGetLastError());
-  c->launches++;
   return JEFI_OK;
 }
 
+extern "C" int jefi_push_particles_packed(jefi_ctx* c, long np, float* x, float* y, float* z, float* ux, float* uy, float* uz,
+                                          const float* q_over_m, unsigned char* alive, const float* eb_packed) {
+  if (!c) return JEFI_EINVAL;
+  jefi_device_guard guard(c);
+  if (np < 0 || !eb_packed || ((uintptr_t)eb_packed & 15u) || (np > 0 && (!x || !y || !z || !ux || !uy || !uz || !q_over_m || !alive))) {
+    c->err = "jefi_push_particles_packed: NULL or misaligned array, or negative np";
+    return JEFI_EINVAL;
+  }
+  if (np == 0) return JEFI_OK;
+  launch_push<true>(c, np, x, y, z, ux, uy, uz, q_over_m, alive, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr,
+                    reinterpret_cast<const float4*>(eb_packed));
+  JEFI_CUDA_TRY(c, cudaGetLastError());
+  return JEFI_OK;
+}
+
+template <int ORDER>
 __global__ void __launch_bounds__(256) k_cell_index(long np, const float* __restrict__ x, const float* __restrict__ y,
                                                     const float* __restrict__ z, int* __restrict__ ijk) {
   long p = (long)blockIdx.x * blockDim.x + threadIdx.x;
   if (p >= np) return;
-  int i, j, k;
-  float a;
-  cic_cell(x[p], i, a); cic_cell(y[p], j, a); cic_cell(z[p], k, a);
-  ijk[3 * p] = i; ijk[3 * p + 1] = j; ijk[3 * p + 2] = k;
+  axis_stencil<ORDER> sx, sy, sz;
+  sx.set(x[p]); sy.set(y[p]); sz.set(z[p]);
+  constexpr int C = ORDER - 1;  // order 2: report the centre node i0 + 1
+  ijk[3 * p] = sx.i0 + C; ijk[3 * p + 1] = sy.i0 + C; ijk[3 * p + 2] = sz.i0 + C;
 }
 
 extern "C" int jefi_debug_cell_index(jefi_ctx* c, long np, const float* x, const float* y, const float* z, int* ijk_out) {
   if (!c || np < 0 || (np > 0 && (!x || !y || !z || !ijk_out))) return JEFI_EINVAL;
+  jefi_device_guard guard(c);
   if (np == 0) return JEFI_OK;
-  k_cell_index<<<(unsigned)((np + 255) / 256), 256, 0, c->stream>>>(np, x, y, z, ijk_out);
+  if (c->shape_order == 2) k_cell_index<2><<<(unsigned)((np + 255) / 256), 256, 0, c->stream>>>(np, x, y, z, ijk_out);
+  else k_cell_index<1><<<(unsigned)((np + 255) / 256), 256, 0, c->stream>>>(np, x, y, z, ijk_out);
   JEFI_CUDA_TRY(c, cudaGetLastError());
   JEFI_CUDA_TRY(c, cudaStreamSynchronize(c->stream));
   return JEFI_OK;

@@ -23,7 +23,8 @@ EXPORTS = [
     "jefi_create", "jefi_destroy", "jefi_last_error", "jefi_get_info", "jefi_deposit", "jefi_push_sources",
     "jefi_field_step", "jefi_field_step_slab", "jefi_push_particles", "jefi_field_step_host", "jefi_launch_count",
     "jefi_last_field_kernel_ms", "jefi_debug_delay_table", "jefi_debug_cell_index", "jefi_debug_history_slot",
-    "jefi_debug_cell_order", "jefi_sort_particles",
+    "jefi_debug_cell_order", "jefi_sort_particles", "jefi_field_impl_reason", "jefi_get_tile_info", "jefi_field_step_packed",
+    "jefi_push_particles_packed", "jefi_field_kernel_ms",
 ]
 
 
@@ -39,7 +40,7 @@ class jefi_config(C.Structure):
         ("H", C.c_int), ("hist_cap", C.c_int),
         ("Eext", C.c_double * 3), ("Bext", C.c_double * 3),
         ("device", C.c_int), ("stream", C.c_void_p), ("field_impl", C.c_int), ("deposit_mode", C.c_int),
-        ("delay_rule", C.c_int),
+        ("delay_rule", C.c_int), ("shape_order", C.c_int), ("field_chunk", C.c_int),
     ]
 
 
@@ -81,6 +82,8 @@ def load_library() -> C.CDLL:
     lib.jefi_launch_count.restype = C.c_long
     lib.jefi_last_field_kernel_ms.argtypes = [vp]
     lib.jefi_last_field_kernel_ms.restype = C.c_float
+    lib.jefi_field_kernel_ms.argtypes = [vp, C.c_int]
+    lib.jefi_field_kernel_ms.restype = C.c_float
     lib.jefi_debug_delay_table.argtypes = [vp, vp]
     lib.jefi_debug_delay_table.restype = C.c_int
     lib.jefi_debug_cell_index.argtypes = [vp, C.c_long, f32p, f32p, f32p, vp]
@@ -91,6 +94,15 @@ def load_library() -> C.CDLL:
     lib.jefi_debug_cell_order.restype = C.c_int
     lib.jefi_debug_history_slot.argtypes = [vp, C.c_int, f32p]
     lib.jefi_debug_history_slot.restype = C.c_int
+    lib.jefi_field_impl_reason.argtypes = [vp]
+    lib.jefi_field_impl_reason.restype = C.c_char_p
+    lib.jefi_get_tile_info.argtypes = [vp, C.POINTER(C.c_int * 3), C.POINTER(C.c_int * 3), C.POINTER(C.c_int), C.POINTER(C.c_int),
+                                       C.POINTER(C.c_int)]
+    lib.jefi_get_tile_info.restype = C.c_int
+    lib.jefi_field_step_packed.argtypes = [vp] + [f32p] * 7
+    lib.jefi_field_step_packed.restype = C.c_int
+    lib.jefi_push_particles_packed.argtypes = [vp, C.c_long] + [f32p] * 7 + [u8p, f32p]
+    lib.jefi_push_particles_packed.restype = C.c_int
     _lib = lib
     return lib
 
@@ -121,10 +133,11 @@ def jefi_create(nx: int, ny: int, nz: int, dx: float, dy: float, dz: float, dt: 
                 eps0: float = 0.0, H: int = 0, hist_cap: int = 0, Eext: Sequence[float] = (0, 0, 0),
                 Bext: Sequence[float] = (0, 0, 0), device: int = 0, stream: int = 0,
                 field_impl: int = JEFI_FIELD_AUTO, deposit_mode: int = JEFI_DEPOSIT_AUTO,
-                delay_rule: int = JEFI_DELAY_NEAREST) -> int:
+                delay_rule: int = JEFI_DELAY_NEAREST, shape_order: int = 1, field_chunk: int = 0) -> int:
     lib = load_library()
     cfg = jefi_config(nx, ny, nz, dx, dy, dz, dt, c, eps0, H, hist_cap, (C.c_double * 3)(*Eext),
-                      (C.c_double * 3)(*Bext), device, C.c_void_p(stream), field_impl, deposit_mode, delay_rule)
+                      (C.c_double * 3)(*Bext), device, C.c_void_p(stream), field_impl, deposit_mode, delay_rule,
+                      shape_order, field_chunk)
     h = C.c_void_p()
     rc = lib.jefi_create(C.byref(cfg), C.byref(h))
     if rc != JEFI_OK:
@@ -143,6 +156,19 @@ def jefi_get_info(handle: int) -> dict:
     _check(handle, load_library().jefi_get_info(handle, C.byref(H), C.byref(ndt), C.byref(impl), C.byref(step),
                                                 C.byref(rb)), "jefi_get_info")
     return dict(H=H.value, ndt=ndt.value, field_impl=impl.value, step=step.value, ring_bytes=rb.value)
+
+
+def jefi_field_impl_reason(handle: int) -> str:
+    msg = load_library().jefi_field_impl_reason(handle)
+    return msg.decode() if msg else ""
+
+
+def jefi_get_tile_info(handle: int) -> dict:
+    ob, ts = (C.c_int * 3)(), (C.c_int * 3)()
+    w, wp, ns = C.c_int(), C.c_int(), C.c_int()
+    _check(handle, load_library().jefi_get_tile_info(handle, C.byref(ob), C.byref(ts), C.byref(w), C.byref(wp), C.byref(ns)),
+           "jefi_get_tile_info")
+    return dict(obs_tile=tuple(ob), src_tile=tuple(ts), window_slots=w.value, window_pitch=wp.value, source_split=ns.value)
 
 
 def jefi_push_sources(handle: int, N: int, rho, jx, jy, jz) -> None:
@@ -169,9 +195,19 @@ def jefi_field_step_slab(handle: int, N: int, k0: int, k1: int, ex, ey, ez, bx, 
     _check(handle, load_library().jefi_field_step_slab(handle, int(k0), int(k1), *ptrs), "jefi_field_step_slab")
 
 
+def jefi_field_step_packed(handle: int, N: int, ex, ey, ez, bx, by, bz, eb_packed) -> None:
+    import torch
+
+    f = torch.float32
+    ptrs = [_dev(t, f, N, n) for t, n in zip((ex, ey, ez, bx, by, bz), ("ex", "ey", "ez", "bx", "by", "bz"))]
+    _check(handle, load_library().jefi_field_step_packed(handle, *ptrs, _dev(eb_packed, f, 8 * N, "eb_packed")),
+           "jefi_field_step_packed")
+
+
 def slab_range(nz: int, rank: int, world: int, edge: int = 8):
-    """Observation z-planes [k0, k1) of `rank` out of `world`: whole layers of 8-cell observation tiles,
-    spread as evenly as the layer count allows; ranks beyond the layer count get an empty range."""
+    """Observation z-planes [k0, k1) of `rank` out of `world`: whole layers of observation tiles (`edge` =
+    jefi_get_tile_info()["obs_tile"][2]: 8, or 32 on nx <= 3 grids), spread as evenly as the layer count allows; ranks beyond
+    the layer count get an empty range."""
     layers = (nz + edge - 1) // edge
     lo = (layers * rank) // world
     hi = (layers * (rank + 1)) // world
@@ -198,6 +234,17 @@ def jefi_push_particles(handle: int, N: int, x, y, z, ux, uy, uz, q_over_m, aliv
     pal = _dev(alive, torch.uint8, np_, "alive")
     pf = [_dev(t, f, N, n) for t, n in zip((ex, ey, ez, bx, by, bz), ("ex", "ey", "ez", "bx", "by", "bz"))]
     _check(handle, load_library().jefi_push_particles(handle, np_, *pp, pal, *pf), "jefi_push_particles")
+
+
+def jefi_push_particles_packed(handle: int, N: int, x, y, z, ux, uy, uz, q_over_m, alive, eb_packed) -> None:
+    import torch
+
+    f = torch.float32
+    np_ = x.numel()
+    pp = [_dev(t, f, np_, n) for t, n in zip((x, y, z, ux, uy, uz, q_over_m), ("x", "y", "z", "ux", "uy", "uz", "q_over_m"))]
+    _check(handle, load_library().jefi_push_particles_packed(handle, np_, *pp, _dev(alive, torch.uint8, np_, "alive"),
+                                                             _dev(eb_packed, f, 8 * N, "eb_packed")),
+           "jefi_push_particles_packed")
 
 
 def jefi_sort_particles(handle: int, x, y, z, ux, uy, uz, qw, q_over_m, alive, tag=None) -> None:
@@ -228,6 +275,10 @@ def jefi_launch_count(handle: int) -> int:
 
 def jefi_last_field_kernel_ms(handle: int) -> float:
     return float(load_library().jefi_last_field_kernel_ms(handle))
+
+
+def jefi_field_kernel_ms(handle: int, calls_back: int) -> float:
+    return float(load_library().jefi_field_kernel_ms(handle, int(calls_back)))
 
 
 def jefi_debug_delay_table(handle: int, nx: int, ny: int, nz: int):
@@ -297,7 +348,8 @@ class JefiContext:
     """Owns one jefi_ctx and the E/B/rho/J device tensors of a run; every method is one C-ABI call."""
 
     def __init__(self, grid: GridSpec, device=None, field_impl: int = JEFI_FIELD_AUTO,
-                 deposit_mode: int = JEFI_DEPOSIT_AUTO, sort_every: int = 0, delay_rule: int = JEFI_DELAY_NEAREST):
+                 deposit_mode: int = JEFI_DEPOSIT_AUTO, sort_every: int = 8, delay_rule: int = JEFI_DELAY_NEAREST,
+                 shape_order: int = 1, field_chunk: int = 0, packed_fields: bool = True):
         import torch
 
         if not torch.cuda.is_available():
@@ -309,14 +361,21 @@ class JefiContext:
         stream = torch.cuda.current_stream(self.device).cuda_stream
         self.handle = jefi_create(grid.nx, grid.ny, grid.nz, grid.dx, grid.dy, grid.dz, grid.dt, grid.c, grid.eps0,
                                   grid.H, grid.hist_cap, grid.Eext, grid.Bext, self.device.index or 0, stream,
-                                  field_impl, deposit_mode, delay_rule)
+                                  field_impl, deposit_mode, delay_rule, shape_order, field_chunk)
         self.info = jefi_get_info(self.handle)
+        self.info["field_impl_reason"] = jefi_field_impl_reason(self.handle)
+        self.tile_info = jefi_get_tile_info(self.handle)
         self.H = self.info["H"]
-        self.sort_every = int(sort_every)  # pic_step calls jefi_sort_particles every sort_every steps (0 = never)
+        # pic_step calls jefi_sort_particles every sort_every steps (0 = never).  Default 8: particles move at most c dt =
+        # dx/2 per step, and the deposit / push run 4-6x faster on a cell-sorted list.  A caller that
+        # matches particles by position in the arrays passes a "tag" array (permuted along) or sort_every=0.
+        self.sort_every = int(sort_every)
         self._pic_steps = 0
         z = lambda k: torch.zeros((k, self.N), dtype=torch.float32, device=self.device)
         self.EB = z(6)   # ex ey ez bx by bz
         self.src = z(4)  # rho jx jy jz
+        # interleaved copy of E, B written by the field kernel's epilogue and gathered by the push (pic_step only)
+        self.EBp = torch.zeros(8 * self.N, dtype=torch.float32, device=self.device) if packed_fields else None
 
     def close(self) -> None:
         if getattr(self, "handle", None):
@@ -339,6 +398,18 @@ class JefiContext:
         o = self.EB if out is None else out
         jefi_field_step_slab(self.handle, self.N, k0, k1, o[0], o[1], o[2], o[3], o[4], o[5])
         return o
+
+    def field_step_packed(self):
+        o = self.EB
+        jefi_field_step_packed(self.handle, self.N, o[0], o[1], o[2], o[3], o[4], o[5], self.EBp)
+        return o
+
+    def push_particles_packed(self, part: dict) -> None:
+        jefi_push_particles_packed(self.handle, self.N, part["x"], part["y"], part["z"], part["ux"], part["uy"], part["uz"],
+                                   part["qm"], part["alive"], self.EBp)
+
+    def slab_range(self, rank: int, world: int):
+        return slab_range(self.grid.nz, rank, world, self.tile_info["obs_tile"][2])
 
     def deposit(self, part: dict, out=None):
         o = self.src if out is None else out
@@ -364,11 +435,18 @@ class JefiContext:
         self._pic_steps += 1
         self.deposit(part)
         self.push_sources()
-        self.field_step()
-        self.push_particles(part)
+        if self.EBp is not None:
+            self.field_step_packed()
+            self.push_particles_packed(part)
+        else:
+            self.field_step()
+            self.push_particles(part)
 
     def launch_count(self) -> int:
         return jefi_launch_count(self.handle)
 
     def last_field_kernel_ms(self) -> float:
         return jefi_last_field_kernel_ms(self.handle)
+
+    def field_kernel_ms(self, calls_back: int) -> float:
+        return jefi_field_kernel_ms(self.handle, calls_back)

@@ -236,3 +236,72 @@ def sample_obs(n_cells_axis: int, count: int, seed: int) -> np.ndarray:
     special += [(0, c, c), (m, c, c), (c, 0, c), (c, m, c), (c, c, 0), (c, c, m), (c, c, c)]
     sp = np.array([i + n * (j + n * k) for i, j, k in special], dtype=np.int64)
     return np.concatenate([idx, sp])
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# Field-only workloads of bench.py (one jefi_push_sources + jefi_field_step per timed step).  "4" is BASELINE.json's
+# configs[3], the one the metric is quoted on; the other two are the paper's own shapes (SURVEY.md section 8(f) NEXT-1 and
+# NEXT-2): the 20^3 analytic-source example in units c = eps0 = mu0 = 1 with dx = 0.3, dt = 0.05, i.e. kappa = 6
+# (Eqs. 3.4-3.5) and the 1 x 251 x 111 slab with dx = 1e-5 m, dt = 1e-13 s, kappa = 0.334
+# (PAPER.md:243-250, 288, 356).  Numbers 1, 2, 3, 5 give a random history on that config's grid (used by CPU-sized tests).
+# ---------------------------------------------------------------------------------------------------------------
+def history_depth(shape, h, dt: float, c: float) -> int:
+    """BASELINE.json / PAPER.md:211: H = ceil(L_max/(c dt)) + 2 with L_max the diagonal of the region."""
+    lmax = math.sqrt(sum((n * d) ** 2 for n, d in zip(shape, h)))
+    return int(math.ceil(lmax / (c * dt))) + 2
+
+
+@dataclass(frozen=True)
+class FieldWorkload:
+    name: str
+    config: Optional[int]  # BASELINE.json config number, None for the paper's own shapes
+    shape: tuple           # (nx, ny, nz)
+    h: tuple               # (dx, dy, dz)
+    dt: float
+    c: float               # 0 -> SI
+    eps0: float            # 0 -> SI
+    seed: int
+    kind: str              # "random": i.i.d. uniform [-1, 1) in every cell and slot; "analytic": Eqs. (3.4)-(3.5)
+
+    @property
+    def N(self) -> int:
+        return self.shape[0] * self.shape[1] * self.shape[2]
+
+    @property
+    def c_eff(self) -> float:
+        return self.c if self.c > 0 else C_SI
+
+    @property
+    def H(self) -> int:
+        return history_depth(self.shape, self.h, self.dt, self.c_eff)
+
+    @property
+    def kappa(self) -> float:
+        return self.h[0] / (self.c_eff * self.dt)
+
+    def slice(self, t: int, j_scale: float = 1.0) -> np.ndarray:
+        """Sources of step t as the C-ABI takes them: fp32 [4][N] = rho, Jx, Jy, Jz."""
+        if self.kind == "random":
+            return history_slice(self.N, t, self.seed, j_scale)
+        nx, ny, nz = self.shape
+        k, j, i = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+        u = ((i + 0.5) * self.h[0] + (j + 0.5) * self.h[1] + (k + 0.5) * self.h[2]).ravel()
+        tt = t * self.dt
+        jv = np.sin(u) * math.sin(tt)                                   # Eq. (3.4), PAPER.md:421
+        rho = 3.0 * (math.cos(tt) - 1.0) * np.cos(u)                    # Eq. (3.5), PAPER.md:423
+        return np.stack([rho, jv, jv, jv]).astype(np.float32)
+
+
+def field_workload(key) -> FieldWorkload:
+    key = str(key)
+    if key in ("1", "2", "3", "4", "5"):
+        w = WORKLOADS[int(key)]
+        return FieldWorkload(w.name if w.field_only else w.name + "_random_history", w.config, (w.n,) * 3, (w.dx,) * 3, w.dt, 0.0, 0.0,
+                             w.seed, "random")
+    if key == "analytic20":
+        return FieldWorkload("paper_analytic_20c_kappa6", None, (20, 20, 20), (0.3, 0.3, 0.3), 0.05, 1.0, 1.0, SEED0 + 21, "analytic")
+    if key == "slab251":
+        return FieldWorkload("paper_slab_1x251x111_field_only", None, (1, 251, 111), (1e-5,) * 3, 1e-13, 0.0, 0.0, SEED0 + 22, "random")
+    if key == "slab101":
+        return FieldWorkload("paper_slab_1x101x101_field_only", None, (1, 101, 101), (1e-5,) * 3, 1e-13, 0.0, 0.0, SEED0 + 23, "random")
+    raise ValueError(f"unknown field workload {key!r} (1-5, analytic20, slab251, slab101)")

@@ -97,9 +97,12 @@ def test_config2_closed_loop_10_steps_full_oracle(J):
     w = wl.WORKLOADS[2]
     part = wl.particles(2)
     cfg = OracleConfig(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt)
-    ctx = J.JefiContext(J.GridSpec(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt))
+    import torch
+
+    ctx = J.JefiContext(J.GridSpec(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt))  # default: cell sort every 8 steps
     assert ctx.H == w.H and ctx.info["field_impl"] == J.JEFI_FIELD_TILED
     dp = to_dev(part, ctx.device)
+    dp["tag"] = torch.arange(part["x"].shape[0], dtype=torch.int32, device=ctx.device)
     orc = oracle.OracleJefi(cfg)
     po = {k: v.astype(np.float64) for k, v in part.items() if k != "alive"}
     po["alive"] = part["alive"].copy()
@@ -107,6 +110,8 @@ def test_config2_closed_loop_10_steps_full_oracle(J):
         ctx.pic_step(dp)
         So, Eo, Bo = orc.pic_step(po)
     got = {k: v.cpu().numpy() for k, v in dp.items()}
+    inv = np.argsort(got.pop("tag"))
+    got = {k: v[inv] for k, v in got.items()}
     both = (got["alive"] == 1) & (po["alive"] == 1)
     assert (got["alive"] != po["alive"]).sum() <= 2
     for k in "xyz":
@@ -176,6 +181,9 @@ def test_paper_slab_workloads_closed_loop(J, which, count, steps):
     cfg = OracleConfig(nx, ny, nz, w.dx, w.dx, w.dx, w.dt, Bext=w.Bext)
     ctx = J.JefiContext(J.GridSpec(nx, ny, nz, w.dx, w.dx, w.dx, w.dt, Bext=w.Bext), sort_every=4)
     assert ctx.H == cfg.H
+    # nx = 1: x-thin tiles (1x16x32 observation cells against 1x8x8 source tiles), and kappa = 0.334 passes the fp32 delay proof
+    assert ctx.info["field_impl"] == J.JEFI_FIELD_TILED, ctx.info["field_impl_reason"]
+    assert ctx.tile_info["obs_tile"] == (1, 16, 32) and ctx.tile_info["src_tile"] == (1, 8, 8)
     import torch
 
     dp = to_dev(part, ctx.device)
@@ -195,11 +203,14 @@ def test_paper_slab_workloads_closed_loop(J, which, count, steps):
         assert np.abs(got[k][both] - po[k][both]).max() / max(w.shape) <= 1e-5, k
     eb = ctx.EB.cpu().numpy()
     for name, F, Fo in (("E", eb[:3], Eo), ("B", eb[3:], Bo)):
-        # The fields of these set-ups live in a handful of cells around the charge (peak/RMS ~ 100), so the max-abs bound
-        # is taken against the peak, "1e-3 of the field norm" in the max norm, instead of reading A20's RMS.
-        l2, _ = sampled_field_err(F, Fo)
-        mx = np.abs(F - Fo).max() / np.abs(Fo).max()
-        assert l2 <= 1e-4 and mx <= 1e-3, (which, name, l2, mx, ctx.info["field_impl"])
+        # Reading A20 bounds max|d| by 1e-3 of the RMS of the field.  The fields of these set-ups live in a handful of cells
+        # around the charge (peak/RMS ~ 100), so here the bound is taken against the peak ("1e-3 of the field norm" in the max
+        # norm, reading A20b in DESIGN.md section 3, which records the measured values of both forms: the RMS form reads
+        # 1e-4 for E and 5e-3 for B of the point emission, whose B is confined to the few cells around the ring).
+        l2, mx_rms = sampled_field_err(F, Fo)
+        mx_peak = np.abs(F - Fo).max() / np.abs(Fo).max()
+        print(f"{which} {name}: rel-L2 {l2:.2e}  max-abs/RMS {mx_rms:.2e}  max-abs/peak {mx_peak:.2e}  peak/RMS {np.abs(Fo).max() / (np.linalg.norm(Fo) / np.sqrt(Fo.size)):.1f}")
+        assert l2 <= 1e-4 and mx_peak <= 1e-3, (which, name, l2, mx_peak, ctx.info["field_impl"])
     S = ctx.src.cpu().numpy()
     for a in range(4):
         assert np.linalg.norm(S[a] - So[a]) <= 1e-5 * max(np.linalg.norm(So[a]), 1e-300), a

@@ -1,0 +1,324 @@
+"""GPU parity for the widened hot path: x-thin tile geometry and multi-pass slot windows of the tiled field kernel, the
+packed E/B output, deterministic split sums, the second-order shape function S^(2) and the
+out-of-grid guard of the run deposit.  Everything goes through the C-ABI binding and is compared with the fp64 oracle on
+the same seeded inputs (tolerances: reading A20, as in test_gpu_parity.py).
+"""
+import numpy as np
+import pytest
+
+import oracle
+from oracle import OracleConfig
+from paper_2209_07944_b200 import workloads as wl
+
+from test_gpu_parity import (C, assert_field_parity, edge_particles, field_err, oracle_history, run_history, to_dev)
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def J(cuda_device):
+    from paper_2209_07944_b200 import jefi
+
+    jefi.load_library()
+    return jefi
+
+
+# ------------------------------------------------------------------------------------ tile geometry / multi-pass windows
+THIN_CASES = [
+    # shape, spacing, kappa, fill, expected observation tile, several passes?
+    ((1, 40, 70), (1e-5, 1e-5, 1e-5), 0.334, "wrapped", (1, 16, 32), False),   # the paper's slab regime
+    ((1, 37, 45), (1e-4, 1e-4, 1e-4), 2.0, "full", (1, 16, 32), True),         # thin grid at the benchmark's kappa: window > pitch
+    ((2, 19, 33), (1e-4, 1e-4, 1e-4), 2.0, "early", (1, 16, 32), True),
+    ((3, 8, 8), (1e-4, 2e-4, 1e-4), 1.0, "wrapped", (1, 16, 32), False),
+    ((4, 9, 9), (1e-4, 1e-4, 1e-4), 2.0, "full", (8, 8, 8), False),            # nx = 4: cubes again
+    ((12, 12, 12), (0.3, 0.3, 0.3), 6.0, "wrapped", (8, 8, 8), True),          # kappa = 6: two passes on cubes
+    ((10, 6, 7), (1e-4, 1e-4, 1e-4), 9.3, "full", (8, 8, 8), True),            # three and more passes (9.5 would put
+    # the offsets (1,0,0).. exactly on a tie s = m + 1/2 of the nearest-step rule: not provable in fp32, see the test below)
+]
+
+
+@pytest.mark.parametrize("rule", ["NEAREST", "LINEAR"])
+@pytest.mark.parametrize("shape,h,kappa,fill,obs_tile,multipass", THIN_CASES)
+def test_tiled_kernel_geometries_and_multipass_windows(J, rule, shape, h, kappa, fill, obs_tile, multipass):
+    c = 1.0 if h[0] > 1e-2 else C
+    kw = dict(c=1.0, eps0=1.0) if c == 1.0 else {}
+    dt = h[0] / (kappa * c)
+    cfg = OracleConfig(*shape, *h, dt, delay_rule=getattr(oracle, "RULE_" + rule), **kw)
+    nsteps = {"full": cfg.H, "early": max(3, cfg.H // 3), "wrapped": 2 * cfg.H + 3}[fill]
+    slices = [wl.history_slice(cfg.N, t, 31337, j_scale=c) for t in range(nsteps)]
+    ctx = J.JefiContext(J.GridSpec(*shape, *h, dt, **kw), field_impl=J.JEFI_FIELD_TILED, delay_rule=getattr(J, "JEFI_DELAY_" + rule))
+    ti = ctx.tile_info
+    assert ctx.info["field_impl"] == J.JEFI_FIELD_TILED and ti["obs_tile"] == obs_tile, (ctx.info["field_impl_reason"], ti)
+    assert (ti["window_slots"] > ti["window_pitch"]) == multipass, ti
+    assert ctx.info["field_impl_reason"].startswith("tiled:")
+    E, B = run_history(J, ctx, slices)
+    Eo, Bo = oracle_history(cfg, slices)
+    assert_field_parity(E, B, Eo, Bo, f"{shape} kappa {kappa} {rule}: ")
+    # the reference kernel on the same history agrees with the oracle too (and so with the tiled kernel)
+    ref = J.JefiContext(J.GridSpec(*shape, *h, dt, **kw), field_impl=J.JEFI_FIELD_REFERENCE, delay_rule=getattr(J, "JEFI_DELAY_" + rule))
+    assert ref.info["field_impl_reason"].startswith("reference: requested")
+    E2, B2 = run_history(J, ref, slices)
+    assert_field_parity(E2, B2, Eo, Bo, f"{shape} kappa {kappa} {rule} (reference): ")
+    ctx.close()
+    ref.close()
+
+
+def test_thin_grid_slabs_and_light_cone(J):
+    """1 x 40 x 70: observation slabs in units of the thin tile's z edge (32) assemble the full step bit for bit; a source
+    switched on at step n0 leaves every cell outside its light cone exactly zero."""
+    import torch
+
+    shape, dx = (1, 40, 70), 1e-5
+    dt = dx / (1.3 * C)
+    cfg = OracleConfig(*shape, dx, dx, dx, dt)
+    ctx = J.JefiContext(J.GridSpec(*shape, dx, dx, dx, dt), field_impl=J.JEFI_FIELD_TILED)
+    assert ctx.tile_info["obs_tile"] == (1, 16, 32)
+    src = 0 + 1 * (17 + 40 * 33)
+    rng = np.random.default_rng(8)
+    slices = []
+    for t in range(30):
+        s = np.zeros((4, cfg.N), dtype=np.float32)
+        if t >= 9:
+            s[:, src] = rng.uniform(-1, 1, 4) * np.array([1, C, C, C])
+        slices.append(s)
+    E, B = run_history(J, ctx, slices)
+    Eo, Bo = oracle_history(cfg, slices)
+    zero = (np.abs(Eo).sum(0) == 0) & (np.abs(Bo).sum(0) == 0)
+    assert 100 < zero.sum() < cfg.N - 100
+    assert np.all(E[:, zero] == 0) and np.all(B[:, zero] == 0)
+    assert_field_parity(E, B, Eo, Bo, "thin light cone: ")
+    full = ctx.field_step().clone()
+    asm = torch.full_like(full, float("nan"))
+    plane = shape[0] * shape[1]
+    for r in range(3):
+        k0, k1 = ctx.slab_range(r, 3)
+        assert k0 % 32 == 0
+        part = torch.full_like(full, -7.0)
+        ctx.field_step_slab(k0, k1, part)
+        assert bool((part[:, :plane * k0] == -7.0).all()) and bool((part[:, plane * k1:] == -7.0).all())
+        asm[:, plane * k0:plane * k1] = part[:, plane * k0:plane * k1]
+    assert torch.equal(asm, full)
+    with pytest.raises(J.JefiError):
+        ctx.field_step_slab(8, 70)  # not a multiple of 32 on this geometry
+    ctx.close()
+
+
+def test_exact_ties_of_the_nearest_step_rule_fall_back_to_the_reference_kernel(J):
+    """kappa = 1.5: the offsets (1,0,0), (3,0,0), .. have s = R/(c dt) = m + 1/2 exactly, where the nearest-step rule (reading A1)
+    hangs on the last bit of s.  The fp32 delay arithmetic of the tiled kernel cannot be proven there, so AUTO runs the
+    table-driven reference kernel (whose fp64 table is the oracle's formula), says why, and JEFI_FIELD_TILED refuses."""
+    shape, dx = (9, 10, 11), 1e-4
+    dt = dx / (1.5 * C)
+    cfg = OracleConfig(*shape, dx, dx, dx, dt)
+    ctx = J.JefiContext(J.GridSpec(*shape, dx, dx, dx, dt))
+    assert ctx.info["field_impl"] == J.JEFI_FIELD_REFERENCE
+    assert ctx.info["field_impl_reason"].startswith("reference:") and "differ from the fp64 table" in ctx.info["field_impl_reason"]
+    assert np.array_equal(J.jefi_debug_delay_table(ctx.handle, *shape), oracle.delay_table(cfg))
+    slices = [wl.history_slice(cfg.N, t, 5, j_scale=C) for t in range(cfg.H + 3)]
+    E, B = run_history(J, ctx, slices)
+    Eo, Bo = oracle_history(cfg, slices)
+    assert_field_parity(E, B, Eo, Bo, "kappa 1.5 (reference): ")
+    ctx.close()
+    with pytest.raises(J.JefiError, match="not usable"):
+        J.JefiContext(J.GridSpec(*shape, dx, dx, dx, dt), field_impl=J.JEFI_FIELD_TILED)
+
+
+@pytest.mark.parametrize("shape,chunk", [((16, 16, 16), 0), ((16, 16, 16), 1), ((16, 16, 16), -1), ((24, 20, 9), 0), ((24, 20, 9), 7)])
+def test_split_source_range_is_deterministic_and_packed_output_matches(J, shape, chunk):
+    """Small grids split the source range over CTAs; the pieces are added by k_reduce_partials in a fixed order, so two runs
+    agree bit for bit, every split agrees with the oracle, and the interleaved output of jefi_field_step_packed holds exactly
+    the values of the six SoA arrays."""
+    import torch
+
+    dx = 1e-4
+    dt = dx / (2 * C)
+    cfg = OracleConfig(*shape, dx, dx, dx, dt)
+    slices = [wl.history_slice(cfg.N, t, 1234, j_scale=C) for t in range(cfg.H + 5)]
+    Eo, Bo = oracle_history(cfg, slices)
+    outs = []
+    for rep in range(2):
+        ctx = J.JefiContext(J.GridSpec(*shape, dx, dx, dx, dt), field_impl=J.JEFI_FIELD_TILED, field_chunk=chunk)
+        ns = ctx.tile_info["source_split"]
+        if chunk == -1:
+            assert ns == 1
+        elif chunk == 1:
+            assert ns == 64
+        elif chunk == 0:
+            assert ns > 1  # fewer than four waves of observation tiles: the automatic choice splits
+        for s in slices:
+            ctx.push_sources(torch.from_numpy(s).to(ctx.device))
+        ctx.EBp.fill_(-3.0)
+        eb = ctx.field_step_packed().clone()
+        pk = ctx.EBp.view(cfg.N, 8).clone()
+        assert torch.equal(pk[:, :6].t().contiguous(), eb), "packed output differs from the SoA output"
+        assert bool((pk[:, 6:] == 0).all())
+        e = eb.cpu().numpy()
+        assert_field_parity(e[:3], e[3:], Eo, Bo, f"{shape} chunk {chunk}: ")
+        outs.append(eb)
+        ctx.close()
+    assert torch.equal(outs[0], outs[1]), "two runs of the same step differ"
+
+
+def test_push_packed_is_bitwise_the_same_push(J):
+    import torch
+
+    n, dx = 16, 1e-4
+    dt = dx / (2 * C)
+    ext = dict(Eext=(1e5, -2e5, 3e4), Bext=(0.0, 10.0, 0.5))
+    ctx = J.JefiContext(J.GridSpec(n, n, n, dx, dx, dx, dt, **ext), field_impl=J.JEFI_FIELD_REFERENCE)
+    part = edge_particles(n, 77, 30000)
+    rng = np.random.default_rng(78)
+    F = rng.normal(0, 1, (6, n ** 3)).astype(np.float32) * np.array([[1e7]] * 3 + [[0.05]] * 3, dtype=np.float32)
+    EB = torch.from_numpy(F).to(ctx.device)
+    ctx.EBp.view(n ** 3, 8)[:, :6] = EB.t()
+    a, b = to_dev(part, ctx.device), to_dev(part, ctx.device)
+    ctx.push_particles(a, EB)
+    ctx.push_particles_packed(b)
+    for k in ("x", "y", "z", "ux", "uy", "uz", "alive"):
+        assert torch.equal(a[k], b[k]), k
+    ctx.close()
+
+
+# ------------------------------------------------------------------------------------ run deposit: particles outside the grid
+@pytest.mark.parametrize("mode", ["RUNS", "DIRECT", "SORTED"])
+@pytest.mark.parametrize("order", [1, 2])
+def test_deposit_ignores_alive_particles_outside_the_grid(J, mode, order):
+    """alive == NULL (or a stale flag) with positions outside [0, n): every node of such a particle is virtual
+    (PAPER.md:191).  It must deposit nothing and must not alias the run key of an in-grid cell (e.g. xi >= nx + 0.5 gives
+    i = nx, which a naive key maps onto (i = -1, j + 1)); huge and non-finite positions included."""
+    shape, dx = (6, 5, 4), 1e-4
+    dt = dx / (2 * C)
+    cfg = OracleConfig(*shape, dx, dx, dx, dt, shape_order=order)
+    ctx = J.JefiContext(J.GridSpec(*shape, dx, dx, dx, dt), field_impl=J.JEFI_FIELD_REFERENCE,
+                        deposit_mode=getattr(J, "JEFI_DEPOSIT_" + mode), shape_order=order)
+    rng = np.random.default_rng(3)
+    P = 4096
+    pos = np.stack([rng.uniform(-3.0, n + 3.0, P) for n in shape])
+    # runs of neighbours: an in-grid particle next to an out-of-grid one whose naive key would collide
+    pos[:, 10] = (5.7, 2.2, 1.3); pos[:, 11] = (6.6, 1.2, 1.3)     # i = nx  <->  (i = -1, j + 1)
+    pos[:, 12] = (-0.2, 3.2, 1.3)
+    pos[:, 20] = (1e30, 2.0, 2.0); pos[:, 21] = (-1e30, 2.0, 2.0); pos[:, 22] = (2.0, 3.0e9, 2.0)
+    u = rng.normal(0, 0.3, (3, P))
+    part = dict(x=pos[0], y=pos[1], z=pos[2], ux=u[0], uy=u[1], uz=u[2], qw=rng.uniform(-2, 2, P) * 1e-13)
+    part = {k: v.astype(np.float32) for k, v in part.items()}
+    dp = to_dev(part, ctx.device)
+    dp["alive"] = None
+    S = ctx.deposit(dp).cpu().numpy()
+    So = oracle.deposit(cfg, part["x"], part["y"], part["z"], part["ux"], part["uy"], part["uz"], part["qw"], None)
+    for a in range(4):
+        assert np.linalg.norm(S[a] - So[a]) <= 1e-5 * np.linalg.norm(So[a]), (mode, order, a)
+    assert np.array_equal(S[0] != 0, So[0] != 0)
+    ctx.close()
+
+
+# ------------------------------------------------------------------------------------ S^(2) (NEXT-4)
+@pytest.mark.parametrize("shape", [(16, 16, 16), (13, 10, 7), (1, 9, 11)])
+@pytest.mark.parametrize("mode", ["RUNS", "DIRECT", "SORTED"])
+def test_s2_deposit_parity_and_indices(J, shape, mode):
+    dx = 1e-4
+    dt = dx / (2 * C)
+    cfg = OracleConfig(*shape, dx, dx, dx, dt, shape_order=2)
+    ctx = J.JefiContext(J.GridSpec(*shape, dx, dx, dx, dt), field_impl=J.JEFI_FIELD_REFERENCE, shape_order=2,
+                        deposit_mode=getattr(J, "JEFI_DEPOSIT_" + mode))
+    part = edge_particles(max(shape), 12, 30000)
+    for k, lim in zip("xyz", shape):
+        part[k] = (part[k] * (lim / max(shape))).astype(np.float32)
+        part[k] = np.minimum(part[k], np.nextafter(np.float32(lim), np.float32(0)))
+    dp = to_dev(part, ctx.device)
+    idx = J.jefi_debug_cell_index(ctx.handle, dp["x"], dp["y"], dp["z"]).cpu().numpy()
+    assert np.array_equal(idx, oracle.cell_index(part["x"], part["y"], part["z"], shape_order=2))  # centre node, bit-exact
+    So = oracle.deposit(cfg, part["x"], part["y"], part["z"], part["ux"], part["uy"], part["uz"], part["qw"], part["alive"])
+    S = ctx.deposit(dp).cpu().numpy()
+    for a in range(4):
+        assert np.linalg.norm(S[a] - So[a]) <= 1e-5 * np.linalg.norm(So[a]), a
+    assert np.array_equal(S[0] != 0, So[0] != 0)
+    # cell-sorted through the library's own sort: same sums; and it differs visibly from the first-order deposit
+    ctx.sort_particles(dp)
+    S2 = ctx.deposit(dp).cpu().numpy()
+    for a in range(4):
+        assert np.linalg.norm(S2[a] - So[a]) <= 1e-5 * np.linalg.norm(So[a]), a
+    c1 = OracleConfig(*shape, dx, dx, dx, dt)
+    S1 = oracle.deposit(c1, part["x"], part["y"], part["z"], part["ux"], part["uy"], part["uz"], part["qw"], part["alive"])
+    assert np.linalg.norm(So[0] - S1[0]) > 1e-2 * np.linalg.norm(S1[0])
+    ctx.close()
+
+
+def test_s2_push_parity_one_step(J):
+    import torch
+
+    n, dx = 16, 1e-4
+    dt = dx / (2 * C)
+    ext = dict(Eext=(1e5, -2e5, 3e4), Bext=(0.0, 10.0, 0.5))
+    cfg = OracleConfig(n, n, n, dx, dx, dx, dt, shape_order=2, **ext)
+    ctx = J.JefiContext(J.GridSpec(n, n, n, dx, dx, dx, dt, **ext), field_impl=J.JEFI_FIELD_REFERENCE, shape_order=2)
+    part = edge_particles(n, 21, 30000)
+    rng = np.random.default_rng(22)
+    F = rng.normal(0, 1, (6, cfg.N))
+    F[:3] *= 1e7
+    F[3:] *= 0.05
+    F = F.astype(np.float32)
+    for packed in (False, True):
+        dp = to_dev(part, ctx.device)
+        if packed:
+            ctx.EBp.view(cfg.N, 8)[:, :6] = torch.from_numpy(F).to(ctx.device).t()
+            ctx.push_particles_packed(dp)
+        else:
+            ctx.push_particles(dp, torch.from_numpy(F).to(ctx.device))
+        po = {k: v.astype(np.float64) for k, v in part.items() if k != "alive"}
+        alive_o = part["alive"].copy()
+        oracle.push(cfg, po["x"], po["y"], po["z"], po["ux"], po["uy"], po["uz"], po["qm"], alive_o, F[:3].astype(np.float64),
+                    F[3:].astype(np.float64))
+        got = {k: v.cpu().numpy() for k, v in dp.items()}
+        both = (got["alive"] == 1) & (alive_o == 1)
+        assert (got["alive"] != alive_o).sum() <= 2
+        was = part["alive"] == 1
+        for k in "xyz":
+            assert np.abs(got[k][was] - po[k][was]).max() / n <= 1e-6
+        for k in ("ux", "uy", "uz"):
+            assert np.abs(got[k][both] - po[k][both]).max() <= 2e-6 * max(1.0, np.abs(po[k]).max())
+    # and the first-order push of the same state is visibly different (rough field)
+    c1 = OracleConfig(n, n, n, dx, dx, dx, dt, **ext)
+    p1 = {k: v.astype(np.float64) for k, v in part.items() if k != "alive"}
+    a1 = part["alive"].copy()
+    oracle.push(c1, p1["x"], p1["y"], p1["z"], p1["ux"], p1["uy"], p1["uz"], p1["qm"], a1, F[:3].astype(np.float64), F[3:].astype(np.float64))
+    assert np.abs(p1["ux"] - po["ux"]).max() > 1e-4
+    ctx.close()
+
+
+def test_s2_closed_loop_config1_10_steps(J):
+    """Config 1 (16^3, 4096 macro-electrons) with the S^(2) deposit and interpolation in closed loop for 10 steps against the
+    full fp64 oracle run with shape_order = 2: trajectories 1e-5, fields 1e-4 / 1e-3, deposited sources 1e-5."""
+    import torch
+
+    w = wl.WORKLOADS[1]
+    part = wl.particles(1)
+    cfg = OracleConfig(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt, shape_order=2)
+    ctx = J.JefiContext(J.GridSpec(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt), shape_order=2, sort_every=4)
+    dp = to_dev(part, ctx.device)
+    dp["tag"] = torch.arange(part["x"].shape[0], dtype=torch.int32, device=ctx.device)
+    orc = oracle.OracleJefi(cfg)
+    po = {k: v.astype(np.float64) for k, v in part.items() if k != "alive"}
+    po["alive"] = part["alive"].copy()
+    for s in range(10):
+        ctx.pic_step(dp)
+        So, Eo, Bo = orc.pic_step(po)
+    got = {k: v.cpu().numpy() for k, v in dp.items()}
+    inv = np.argsort(got.pop("tag"))
+    got = {k: v[inv] for k, v in got.items()}
+    both = (got["alive"] == 1) & (po["alive"] == 1)
+    assert (got["alive"] != po["alive"]).sum() <= 1
+    for k in "xyz":
+        assert np.abs(got[k][both] - po[k][both]).max() / w.n <= 1e-5
+    eb = ctx.EB.cpu().numpy()
+    assert_field_parity(eb[:3], eb[3:], Eo, Bo, "cfg1 S2 step 9: ")
+    S = ctx.src.cpu().numpy()
+    for a in range(4):
+        assert np.linalg.norm(S[a] - So[a]) <= 1e-5 * max(np.linalg.norm(So[a]), 1e-300)
+    # first order gives a different run: the switch really changes the physics path
+    o1 = oracle.OracleJefi(OracleConfig(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt))
+    p1 = {k: v.astype(np.float64) for k, v in part.items() if k != "alive"}
+    p1["alive"] = part["alive"].copy()
+    for s in range(10):
+        _, E1, _ = o1.pic_step(p1)
+    assert field_err(eb[:3], E1)[0] > 1e-3
+    ctx.close()

@@ -73,6 +73,27 @@ def test_reference_arm_under_torchrun_prints_one_line_from_rank0():
     assert js["value"] > 0 and js["e2e"]["h2d_bytes_per_step"] == 0 and js["config"]["workload"].startswith("cfg1")
 
 
+def test_gpus_flag_without_torchrun_starts_n_ranks():
+    """`python bench.py --gpus 2` with no WORLD_SIZE in the environment (how the driver ran N = 1 in round 1) must not
+    silently measure one rank: bench.py re-executes itself under torch.distributed.run with 2 ranks, rank 0 prints the one
+    JSON line with n_gpus = 2 and rank 1 really ran (it reports itself idle in the reference arm)."""
+    import bench
+
+    cmd = bench.spawn_command(["--gpus", "3", "--steps", "2"], 3, 29512)
+    assert cmd[1:4] == ["-m", "torch.distributed.run", "--nnodes=1"] and "--nproc-per-node=3" in cmd
+    assert cmd[cmd.index("--master-addr") + 1] == "127.0.0.1" and cmd[-4:] == ["--gpus", "3", "--steps", "2"]
+    assert os.path.samefile(cmd[cmd.index("29512") + 1], os.path.join(ROOT, "bench.py"))
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--impl", "reference", "--workload", "1",
+                        "--steps", "1", "--warmup", "0", "--ref-obs", "64"], capture_output=True, text=True, timeout=600, cwd=ROOT, env=env)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1
+    js = json.loads(lines[0])
+    assert js["impl"] == "reference" and js["n_gpus"] == 2
+    assert "rank 1 of 2: idle" in r.stderr
+
+
 def test_slab_range_partitions_every_layer():
     """Host logic of the observation-slab sharding (bench.py --shard obs)."""
     from paper_2209_07944_b200.jefi import slab_range
@@ -82,6 +103,8 @@ def test_slab_range_partitions_every_layer():
             r = [slab_range(nz, k, world) for k in range(world)]
             assert r[0][0] == 0 and r[-1][1] == nz
             assert all(a[1] == b[0] for a, b in zip(r, r[1:])) and all(a[0] % 8 == 0 for a in r)
+            r32 = [slab_range(nz, k, world, edge=32) for k in range(world)]  # x-thin tile geometry: 32-plane layers
+            assert r32[0][0] == 0 and r32[-1][1] == nz and all(a[1] == b[0] for a, b in zip(r32, r32[1:])) and all(a[0] % 32 == 0 for a in r32)
     assert [slab_range(96, k, 8) for k in range(8)] == [(0, 8), (8, 24), (24, 32), (32, 48), (48, 56), (56, 72), (72, 80), (80, 96)]
 
 
