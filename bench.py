@@ -354,8 +354,8 @@ def time_field_workload(J, torch, device, w: wl.FieldWorkload, rule: str, steps:
     return out
 
 
-PEAK_SOURCE = ("of derived: 148 SM x 128 FP32 lanes x 2 FLOP x clocks.max.sm (MEASURED_PEAKS.json has no FP32 figure; an FFMA-chain "
-               "probe on the box reaches 0.97 of it, profiles/r2_fp32_peak.md)")
+PEAK_SOURCE = ("of derived: 148 SM x 128 FP32 lanes x 2 FLOP x clocks.max.sm (MEASURED_PEAKS.json has no FP32 figure; the FFMA-chain "
+               "probe of this run is in peak_measured, the derived figure is the larger, i.e. conservative, denominator)")
 
 
 def run_product(args, w: wl.FieldWorkload) -> dict:
@@ -477,6 +477,8 @@ def run_product(args, w: wl.FieldWorkload) -> dict:
     e2e_val = aggregate_rate(1 if shard else world, pairs, e2e_ms_max)  # sharded runs: one rank's own full step
     checksum = float(eb_pin[:N].double().abs().sum())
 
+    # measured FP32 pipe throughput of this GPU, in this run (scalar FFMA chains and packed FFMA2 chains)
+    probe = {"ffma": J.jefi_debug_fp32_peak(ctx.handle, False), "ffma2": J.jefi_debug_fp32_peak(ctx.handle, True)} if rank == 0 else None
     impl, reason, tiles = ctx.info["field_impl"], ctx.info["field_impl_reason"], ctx.tile_info
     ctx.close()
     del flush
@@ -500,7 +502,11 @@ def run_product(args, w: wl.FieldWorkload) -> dict:
                             "traffic": traffic, "traffic_source": traffic_src,
                             "kernel": "k_field_tiled" if impl == 2 else "k_field_reference",
                             "kernel_ms": kernel_ms, "kernel_ms_source": f"CUDA events around the field kernel of the {len(kms)} timed steps",
-                            "flop_per_pair": FLOP_PER_PAIR, "peak_source": PEAK_SOURCE, "kernel_source_sha": kernel_source_sha()},
+                            "flop_per_pair": FLOP_PER_PAIR, "peak_source": PEAK_SOURCE, "kernel_source_sha": kernel_source_sha(),
+                            "peak_measured": {"ffma_tflops": probe["ffma"]["tflops"], "ffma2_tflops": probe["ffma2"]["tflops"],
+                                              "sm_count": probe["ffma"]["sm_count"],
+                                              "how": "jefi_debug_fp32_peak: 2048 threads/SM x 16 independent FMA chains, CUDA events, best of 3",
+                                              "frac_of_measured": achieved / max(probe["ffma"]["tflops"], probe["ffma2"]["tflops"])}},
                "e2e": {"value": e2e_val, "unit": "Gpairs/s", "h2d_bytes_per_step": 16 * N, "d2h_bytes_per_step": 24 * N,
                        "ms_per_step": e2e_ms_max, "checksum_abs_ex": checksum},
                "gpu_launches": int(launches), "clocks": clocks}

@@ -188,6 +188,16 @@ float jefi_last_field_kernel_ms(jefi_ctx* ctx);
 float jefi_field_kernel_ms(jefi_ctx* ctx, int calls_back);
 
 /* ---- debug / parity exports (synchronise; not on the timed path) ---- */
+/* The library's own memory checks.  A build with -DJEFI_CHECKED (libjefi_checked.so, `python -m paper_2209_07944_b200.build
+ * --checked`) verifies on the device that every shared-memory address of the field kernel lies inside the rows staged for its
+ * item [0], that pipeline stages are read in sequence [1], that the cell sort scatters inside the list [2], and poisons
+ * stages with NaN before refilling them.  errors_host = HOST long[4] of violation counts since the library was loaded;
+ * returns 1 in a checked build, 0 (JEFI_OK, counters always zero) in the normal one, < 0 on error.  Synchronises. */
+int jefi_debug_check_errors(jefi_ctx* ctx, long errors_host[4]);
+/* FP32 roofline probe: all SMs run independent register-resident FMA chains (packed = 0: scalar fma.rn.f32, 1: fma.rn.f32x2),
+ * timed with CUDA events on the context's stream; *tflops_out = 2 * FMAs / time (HOST double), *sm_count_out the SM count
+ * (optional).  This is the measured denominator next to the derived 148 x 128 x 2 x clock figure. */
+int jefi_debug_fp32_peak(jefi_ctx* ctx, int packed, double* tflops_out, int* sm_count_out);
 /* m for every non-negative offset (a,b,c): m_out[a + nx*(b + ny*c)], HOST int array of N entries (SURVEY.md §8(b) sketched
  * short*; delays reach the history cap of 10000 and the device table is int, so int it is). */
 int jefi_debug_delay_table(jefi_ctx* ctx, int* m_out_host);

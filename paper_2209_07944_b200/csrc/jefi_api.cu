@@ -339,6 +339,21 @@ extern "C" int jefi_field_step_host(jefi_ctx* c, const float* src_host, float* e
 // ------------------------------------------------------------------------------------------------------------
 // debug exports
 // ------------------------------------------------------------------------------------------------------------
+extern "C" int jefi_debug_check_errors(jefi_ctx* c, long errors_host[4]) {
+  if (!c || !errors_host) return JEFI_EINVAL;
+  jefi_device_guard guard(c);
+  unsigned long long h[4] = {0, 0, 0, 0};
+  JEFI_CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  JEFI_CUDA_TRY(c, jefi_field_check_errors(h));      // [0] address outside the staged rows, [1] item sequence
+  JEFI_CUDA_TRY(c, jefi_particle_check_errors(h + 2));  // [2] sort scatter index outside the list
+  for (int i = 0; i < 4; i++) errors_host[i] = (long)h[i];
+#ifdef JEFI_CHECKED
+  return 1;  // a checked build: the counters are live
+#else
+  return JEFI_OK;
+#endif
+}
+
 extern "C" int jefi_debug_delay_table(jefi_ctx* c, int* m_out_host) {
   if (!c || !m_out_host) return JEFI_EINVAL;
   jefi_device_guard guard(c);

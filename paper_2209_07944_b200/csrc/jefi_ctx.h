@@ -158,3 +158,5 @@ int jefi_launch_field_tiled(jefi_ctx* c, int k0, int k1, float* ex, float* ey, f
                             float* eb_packed);
 int jefi_tiled_prepare(jefi_ctx* c);   // window size + smem opt-in; returns JEFI_ESTATE if it cannot run
 int jefi_verify_delay_fp32(jefi_ctx* c, long* mismatches, long* offsets);
+cudaError_t jefi_field_check_errors(unsigned long long out[2]);     // -DJEFI_CHECKED counters (zero in normal builds)
+cudaError_t jefi_particle_check_errors(unsigned long long out[2]);

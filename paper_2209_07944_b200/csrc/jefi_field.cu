@@ -18,8 +18,6 @@
 #include <stdio.h>
 #include <stdlib.h>
 
-#include <type_traits>
-
 #include "jefi_ctx.h"
 
 // ------------------------------------------------------------------------------------------------------------
@@ -205,13 +203,15 @@ __device__ __forceinline__ f32x2 pk(float lo, float hi) {
   return r;
 }
 __device__ __forceinline__ float lo32(f32x2 v) {
-  float a;
-  asm("{ .reg .b32 jf_unused; mov.b64 {%0, jf_unused}, %1; }" : "=f"(a) : "l"(v));
+  float a, b;
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v));
+  (void)b;
   return a;
 }
 __device__ __forceinline__ float hi32(f32x2 v) {
-  float b;
-  asm("{ .reg .b32 jf_unused; mov.b64 {jf_unused, %0}, %1; }" : "=f"(b) : "l"(v));
+  float a, b;
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v));
+  (void)a;
   return b;
 }
 __device__ __forceinline__ f32x2 swap2(f32x2 v) { return pk(hi32(v), lo32(v)); }
@@ -247,7 +247,22 @@ struct item_addr {
   uint32_t K;     // MODE_PLAIN / MODE_SELF: row 0 + 2064*(m_top + 0x4B400000);  MODE_MULTI: row 0
   uint32_t Mtop;  // MODE_MULTI
   uint32_t R;     // MODE_MULTI
+#ifdef JEFI_CHECKED
+  uint32_t lo, hi;  // shared-memory byte range of the rows staged for this item (+ the z-layer offset)
+#endif
 };
+
+// -DJEFI_CHECKED (libjefi_checked.so, paper_2209_07944_b200/build.py --checked): the library's own memory checks, run under the
+// whole GPU test-suite in place of compute-sanitizer (closed on this pool): every shared-memory address a consumer lane forms
+// must lie inside the rows staged for its item [0]; every item a consumer reads must carry the sequence number it expects,
+// i.e. the stage was neither refilled early nor read before it was filled [1]; the producer poisons a stage with NaN before
+// refilling it, so a row that no copy or zero fill covered shows up as NaN in E, B and fails parity; the cell sort's scatter
+// index must be inside the list [2].  jefi_debug_check_errors() returns the counters (all zero = clean).
+__device__ unsigned long long g_jefi_check_errors[2];
+#ifdef JEFI_CHECKED
+#define JEFI_CHECK_FAIL(kind) atomicAdd(&g_jefi_check_errors[kind], 1ull)
+#endif
+cudaError_t jefi_field_check_errors(unsigned long long out[2]) { return cudaMemcpyFromSymbol(out, g_jefi_check_errors, 2 * sizeof(unsigned long long)); }
 
 // One observation cell against one source cell.  Az = item address + byte offset of the z layer.
 template <int MODE, bool LINEAR, int CELL>
@@ -267,6 +282,12 @@ __device__ __forceinline__ void one_pair(const item_addr& Az, float ax, float ay
   } else {
     addr = Az.K - (uint32_t)__float_as_int(t) * (uint32_t)JEFI_ROW_BYTES;  // row j = m_top - m
   }
+#ifdef JEFI_CHECKED
+  if (addr + SOFF < Az.lo || addr + DOFF + 16 > Az.hi) {  // outside the rows staged for this item
+    JEFI_CHECK_FAIL(0);
+    addr = Az.lo;
+  }
+#endif
   quad2 S = lds128_imm<SOFF>(addr);         // (Jx, Jz | rho, Jy)
   const quad2 D = lds128_imm<DOFF>(addr);   // (DJx, DJz | Drho, DJy)
   if (LINEAR) {  // JEFI_DELAY_LINEAR: S(t_r) = S - phi D with phi = s - m in [-1/2, 1/2) (3 scalar + 2 packed instructions)
@@ -292,12 +313,30 @@ __device__ __forceinline__ void one_pair(const item_addr& Az, float ax, float ay
   A.By12 = fma2(Azx, wxz, A.By12);                // (a_z wx, a_x wz)
 }
 
-// compile-time loop (the LDS offsets of one_pair are immediates)
-template <int I, int N, class F>
-__device__ __forceinline__ void static_for(F&& f) {
-  if constexpr (I < N) {
-    f(std::integral_constant<int, I>{});
-    static_for<I + 1, N>(f);
+// compile-time loops over the cells of the staged source tile (the LDS offsets of one_pair are immediates)
+template <class G, int MODE, bool LINEAR, int CELL0, int LX>
+__device__ __forceinline__ void row_pairs(const item_addr& Az, const float (&ax)[G::TSX], float ay, float az, float qyz, pair_acc& A) {
+  if constexpr (LX < G::TSX) {
+    one_pair<MODE, LINEAR, CELL0 + LX>(Az, ax[LX], ay, az, qyz, A);
+    row_pairs<G, MODE, LINEAR, CELL0, LX + 1>(Az, ax, ay, az, qyz, A);
+  }
+}
+template <class G, int MODE, bool LINEAR, int CELL0, int LY>
+__device__ __forceinline__ void layer_rows(const item_addr& Az, const float (&ax)[G::TSX], const float (&ay)[G::TSY], float az, float az2,
+                                           pair_acc& A) {
+  if constexpr (LY < G::TSY) {
+    const float qyz = fmaf(ay[LY], ay[LY], az2);
+    row_pairs<G, MODE, LINEAR, CELL0 + G::TSX * LY, 0>(Az, ax, ay[LY], az, qyz, A);
+    layer_rows<G, MODE, LINEAR, CELL0, LY + 1>(Az, ax, ay, az, az2, A);
+  }
+}
+template <class G, int MODE, bool LINEAR, int ZU, int ZO>
+__device__ __forceinline__ void z_layers(const item_addr& Az, float kz, const float (&ax)[G::TSX], const float (&ay)[G::TSY], float fz, pair_acc& A) {
+  if constexpr (ZO < ZU) {
+    const float az = kz * (fz - (float)ZO);
+    const float az2 = az * az;
+    layer_rows<G, MODE, LINEAR, ZO * G::TSX * G::TSY, 0>(Az, ax, ay, az, az2, A);
+    z_layers<G, MODE, LINEAR, ZU, ZO + 1>(Az, kz, ax, ay, fz, A);
   }
 }
 
@@ -311,24 +350,23 @@ __device__ __forceinline__ void tile_pairs(const item_addr& A0, float kz, const 
   for (int lz = 0; lz < G::TSZ; lz += ZU) {
     item_addr Az = A0;
     Az.K = A0.K + (uint32_t)(lz * LAYER * 16);
-    static_for<0, ZU>([&](auto zu) {
-      constexpr int ZO = decltype(zu)::value;
-      const float az = kz * (fz0 - (float)(lz + ZO));
-      const float az2 = az * az;
-      static_for<0, G::TSY>([&](auto ly) {
-        constexpr int LY = decltype(ly)::value;
-        const float qyz = fmaf(ay[LY], ay[LY], az2);
-        static_for<0, G::TSX>([&](auto lx) {
-          constexpr int LX = decltype(lx)::value;
-          one_pair<MODE, LINEAR, ZO * LAYER + G::TSX * LY + LX>(Az, ax[LX], ay[LY], az, qyz, A);
-        });
-      });
-    });
+#ifdef JEFI_CHECKED
+    Az.lo = A0.lo + (uint32_t)(lz * LAYER * 16);
+    Az.hi = A0.hi;
+#endif
+    z_layers<G, MODE, LINEAR, ZU, 0>(Az, kz, ax, ay, fz0 - (float)lz, A);
   }
 }
 
-template <class G, int WP, bool LINEAR>
-__global__ void __launch_bounds__(TILED_THREADS, 1) k_field_tiled(tiled_params P) {
+// MULTI: the grid has tile pairs whose window exceeds WP (compiled in only then: the common single-pass kernels carry neither
+// the third evaluation mode nor its registers)
+#ifdef JEFI_MAXNREG
+#define JEFI_TILED_BOUNDS __maxnreg__(JEFI_MAXNREG)
+#else
+#define JEFI_TILED_BOUNDS __launch_bounds__(TILED_THREADS, 1)
+#endif
+template <class G, int WP, bool LINEAR, bool MULTI>
+__global__ void JEFI_TILED_BOUNDS k_field_tiled(tiled_params P) {
   using L = stage_layout<WP>;
   extern __shared__ __align__(128) unsigned char smem[];
   const jefi_dims& d = P.d;
@@ -367,7 +405,7 @@ __global__ void __launch_bounds__(TILED_THREADS, 1) k_field_tiled(tiled_params P
       const int m_lo = self ? 0 : jefi_delay_fp32(jefi_q_fp32(P.g.kx, P.g.ky, P.g.kz, (float)mnx, (float)mny, (float)mnz));
       const int m_hi = jefi_delay_fp32(jefi_q_fp32(P.g.kx, P.g.ky, P.g.kz, (float)mxx, (float)mxy, (float)mxz));
       const int W = m_hi - m_lo + 1;
-      const int npass = (W + WP - 1) / WP;  // 1 unless the window exceeds the compiled pitch
+      const int npass = MULTI ? (W + WP - 1) / WP : 1;  // 1 unless the window exceeds the compiled pitch
       const size_t tile = (size_t)(t0 + it);
       const float4* rows = P.ring + tile * d.H * JEFI_ROW_QUADS;
       const int ix = (G::OBX / G::TSX) * obx - stx + (d.ntx - 1), iy = (G::OBY / G::TSY) * oby - sty + (d.nty - 1),
@@ -387,6 +425,13 @@ __global__ void __launch_bounds__(TILED_THREADS, 1) k_field_tiled(tiled_params P
         s0 += s0 < 0 ? d.H : 0;
         const int lenA = min(nvalid, d.H - s0), lenB = nvalid - lenA;  // ring wrap: at most two runs
         const uint32_t sb = sm0 + (uint32_t)s * L::BYTES;
+#ifdef JEFI_CHECKED
+        {  // poison the whole stage: a row that neither a copy nor the zero fill covers reads as NaN
+          uint32_t* zz = reinterpret_cast<uint32_t*>(smem + (size_t)s * L::BYTES);
+          for (int i = lane; i < (int)(L::ROWS / 4); i += 32) zz[i] = 0x7fc00000u;
+          __syncwarp();
+        }
+#endif
         if (jv > 0) {  // zero rows (only in the first steps of a run or with a shallow ring)
           float4* z = reinterpret_cast<float4*>(smem + (size_t)s * L::BYTES);
           for (int i = lane; i < jv * JEFI_ROW_QUADS; i += 32) z[i] = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -400,6 +445,9 @@ __global__ void __launch_bounds__(TILED_THREADS, 1) k_field_tiled(tiled_params P
           h.dx0 = ox0 - sx0; h.dy0 = oy0 - sy0; h.dz0 = oz0 - sz0;
           h.R = (uint32_t)R;
           h.last = (it == nt - 1 && p == npass - 1) ? 1 : 0;
+#ifdef JEFI_CHECKED
+          h.last |= item << 1;  // sequence number of the item, checked by every consumer thread
+#endif
           *reinterpret_cast<stage_hdr*>(smem + (size_t)s * L::BYTES + L::HDR) = h;
           fence_proxy_async();  // generic-proxy accesses of this stage (zero fill, earlier reads) before the async-proxy writes
           const uint32_t bar = barFull + 8 * s;
@@ -434,9 +482,15 @@ __global__ void __launch_bounds__(TILED_THREADS, 1) k_field_tiled(tiled_params P
     A.Ey = A.Fy = 0.f;
     item_addr I0;
     I0.K = h.K; I0.Mtop = h.Mtop; I0.R = h.R;
+#ifdef JEFI_CHECKED
+    if ((h.last >> 1) != item) JEFI_CHECK_FAIL(1);
+    I0.lo = sm0 + (uint32_t)s * L::BYTES;
+    I0.hi = I0.lo + h.R * (uint32_t)JEFI_ROW_BYTES;
+    if (h.R > (uint32_t)WP) JEFI_CHECK_FAIL(0);
+#endif
     if (h.mode == MODE_PLAIN)
       tile_pairs<G, MODE_PLAIN, LINEAR>(I0, P.g.kz, ax, ay, fz0, A);
-    else if (h.mode == MODE_SELF)
+    else if (!MULTI || h.mode == MODE_SELF)
       tile_pairs<G, MODE_SELF, LINEAR>(I0, P.g.kz, ax, ay, fz0, A);
     else
       tile_pairs<G, MODE_MULTI, LINEAR>(I0, P.g.kz, ax, ay, fz0, A);
@@ -451,7 +505,7 @@ __global__ void __launch_bounds__(TILED_THREADS, 1) k_field_tiled(tiled_params P
     accS[5 * OBCELLS + c] += hi32(A.Cxz) - hi32(A.Bxz);
     __syncwarp();
     if (lane == 0) mbar_arrive(barDone + 8 * s);  // stage s may be refilled; this warp's accumulator updates are done
-    if (h.last) break;
+    if (h.last & 1) break;
   }
 
   asm volatile("bar.sync 1, %0;" ::"n"(NCONS) : "memory");  // consumers only: all accumulator updates are visible
@@ -585,15 +639,18 @@ __global__ void __launch_bounds__(OBCELLS) k_build_perm(int ndx, int ndy, int nt
 static const int kPitches[] = {36, 48};
 typedef void (*tiled_fn)(tiled_params);
 template <class G>
-static tiled_fn tiled_kernel_of(int wp, bool linear) {
+static tiled_fn tiled_kernel_of(int wp, bool linear, bool multi) {
+  if (multi) return linear ? k_field_tiled<G, 48, true, true> : k_field_tiled<G, 48, false, true>;  // several passes: largest pitch
   switch (wp) {
-    case 36: return linear ? k_field_tiled<G, 36, true> : k_field_tiled<G, 36, false>;
-    case 48: return linear ? k_field_tiled<G, 48, true> : k_field_tiled<G, 48, false>;
+    case 36: return linear ? k_field_tiled<G, 36, true, false> : k_field_tiled<G, 36, false, false>;
+    case 48: return linear ? k_field_tiled<G, 48, true, false> : k_field_tiled<G, 48, false, false>;
   }
   return nullptr;
 }
-static tiled_fn tiled_kernel_for(int geom, int wp, bool linear) {
-  return geom == JEFI_GEOM_SLABX ? tiled_kernel_of<jefi_geom_slabx>(wp, linear) : tiled_kernel_of<jefi_geom_cube>(wp, linear);
+static tiled_fn tiled_kernel_for(const jefi_ctx* c) {
+  const bool linear = c->cfg.delay_rule == JEFI_DELAY_LINEAR, multi = c->wmax > c->wpitch;
+  return c->tile_geom == JEFI_GEOM_SLABX ? tiled_kernel_of<jefi_geom_slabx>(c->wpitch, linear, multi)
+                                         : tiled_kernel_of<jefi_geom_cube>(c->wpitch, linear, multi);
 }
 static size_t tiled_smem_for(int wp) {
   switch (wp) {
@@ -663,8 +720,7 @@ int jefi_tiled_prepare(jefi_ctx* c) {
     c->err = buf;
     return JEFI_ESTATE;
   }
-  const bool linear = c->cfg.delay_rule == JEFI_DELAY_LINEAR;
-  cudaError_t e = cudaFuncSetAttribute(tiled_kernel_for(c->tile_geom, wp, linear), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->tiled_smem);
+  cudaError_t e = cudaFuncSetAttribute(tiled_kernel_for(c), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->tiled_smem);
   if (e != cudaSuccess) { c->err = std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e); return JEFI_ECUDA; }
   int nsm = 148;
   cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
@@ -714,7 +770,7 @@ int jefi_launch_field_tiled(jefi_ctx* c, int k0, int k1, float* ex, float* ey, f
   P.obz0 = k0 / d.obz; P.k1 = k1;
   const int nlayers = (k1 - k0 + d.obz - 1) / d.obz;
   dim3 grid((unsigned)(P.nobx * P.noby * nlayers), (unsigned)c->nsplit);
-  tiled_kernel_for(c->tile_geom, c->wpitch, c->cfg.delay_rule == JEFI_DELAY_LINEAR)<<<grid, TILED_THREADS, c->tiled_smem, c->stream>>>(P);
+  tiled_kernel_for(c)<<<grid, TILED_THREADS, c->tiled_smem, c->stream>>>(P);
   JEFI_CUDA_TRY(c, cudaGetLastError());
   c->launches++;
   if (c->nsplit > 1) {

@@ -200,11 +200,18 @@ __global__ void __launch_bounds__(256) k_scan_add(unsigned* __restrict__ out, lo
   if (i < n) out[i] += sums[i / SCAN_TILE];
 }
 
+__device__ unsigned long long g_jefi_part_errors[2];  // -DJEFI_CHECKED: [0] scatter index outside the list
+cudaError_t jefi_particle_check_errors(unsigned long long out[2]) { return cudaMemcpyFromSymbol(out, g_jefi_part_errors, 2 * sizeof(unsigned long long)); }
+
 __global__ void __launch_bounds__(256) k_sort_scatter(long np, const int* __restrict__ key, const int* __restrict__ rank,
                                                       const unsigned* __restrict__ offset, int* __restrict__ order) {
   long p = (long)blockIdx.x * blockDim.x + threadIdx.x;
   if (p >= np) return;
-  order[offset[key[p]] + (unsigned)rank[p]] = (int)p;
+  const unsigned dst = offset[key[p]] + (unsigned)rank[p];
+#ifdef JEFI_CHECKED
+  if ((long)dst >= np) { atomicAdd(&g_jefi_part_errors[0], 1ull); return; }
+#endif
+  order[dst] = (int)p;
 }
 
 template <int ORDER>

@@ -12,7 +12,9 @@ from dataclasses import dataclass
 from typing import Optional, Sequence
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libjefi.so")
+# JEFI_LIBRARY selects another build of the same library, e.g. libjefi_checked.so (build.py --checked: the library's own
+# device-side memory checks; JefiContext.close() then raises if any check fired).
+LIB_PATH = os.environ.get("JEFI_LIBRARY") or os.path.join(_HERE, "libjefi.so")
 
 JEFI_OK, JEFI_EINVAL, JEFI_ENOMEM, JEFI_ECUDA, JEFI_ESTATE = 0, -1, -2, -3, -4
 JEFI_FIELD_AUTO, JEFI_FIELD_REFERENCE, JEFI_FIELD_TILED = 0, 1, 2
@@ -24,7 +26,7 @@ EXPORTS = [
     "jefi_field_step", "jefi_field_step_slab", "jefi_push_particles", "jefi_field_step_host", "jefi_launch_count",
     "jefi_last_field_kernel_ms", "jefi_debug_delay_table", "jefi_debug_cell_index", "jefi_debug_history_slot",
     "jefi_debug_cell_order", "jefi_sort_particles", "jefi_field_impl_reason", "jefi_get_tile_info", "jefi_field_step_packed",
-    "jefi_push_particles_packed", "jefi_field_kernel_ms",
+    "jefi_push_particles_packed", "jefi_field_kernel_ms", "jefi_debug_fp32_peak", "jefi_debug_check_errors",
 ]
 
 
@@ -84,6 +86,10 @@ def load_library() -> C.CDLL:
     lib.jefi_last_field_kernel_ms.restype = C.c_float
     lib.jefi_field_kernel_ms.argtypes = [vp, C.c_int]
     lib.jefi_field_kernel_ms.restype = C.c_float
+    lib.jefi_debug_check_errors.argtypes = [vp, C.POINTER(C.c_long * 4)]
+    lib.jefi_debug_check_errors.restype = C.c_int
+    lib.jefi_debug_fp32_peak.argtypes = [vp, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_int)]
+    lib.jefi_debug_fp32_peak.restype = C.c_int
     lib.jefi_debug_delay_table.argtypes = [vp, vp]
     lib.jefi_debug_delay_table.restype = C.c_int
     lib.jefi_debug_cell_index.argtypes = [vp, C.c_long, f32p, f32p, f32p, vp]
@@ -281,6 +287,22 @@ def jefi_field_kernel_ms(handle: int, calls_back: int) -> float:
     return float(load_library().jefi_field_kernel_ms(handle, int(calls_back)))
 
 
+def jefi_debug_check_errors(handle: int):
+    """(checked_build, [4 counters]) of the library's own device-side memory checks (include/jefi.h)."""
+    e = (C.c_long * 4)()
+    rc = load_library().jefi_debug_check_errors(handle, C.byref(e))
+    if rc < 0:
+        _check(handle, rc, "jefi_debug_check_errors")
+    return rc == 1, list(e)
+
+
+def jefi_debug_fp32_peak(handle: int, packed: bool = False) -> dict:
+    """Measured FP32 FMA throughput of the device (TFLOP/s) and its SM count."""
+    tf, nsm = C.c_double(), C.c_int()
+    _check(handle, load_library().jefi_debug_fp32_peak(handle, 1 if packed else 0, C.byref(tf), C.byref(nsm)), "jefi_debug_fp32_peak")
+    return dict(tflops=tf.value, sm_count=nsm.value, packed=bool(packed))
+
+
 def jefi_debug_delay_table(handle: int, nx: int, ny: int, nz: int):
     import numpy as np
 
@@ -379,8 +401,11 @@ class JefiContext:
 
     def close(self) -> None:
         if getattr(self, "handle", None):
+            checked, errs = jefi_debug_check_errors(self.handle) if _lib is not None else (False, [0])
             jefi_destroy(self.handle)
             self.handle = None
+            if checked and any(errs):
+                raise JefiError(f"libjefi (checked build): device-side memory checks fired: {errs}")
 
     __del__ = close
 

@@ -174,14 +174,20 @@ class SlabWorkload:
 SLABS: Dict[str, SlabWorkload] = {
     "point_emission": SlabWorkload("slab_1x101x101_point_emission", (1, 101, 101), 1e-5, 1e-13, (0.0, 0.0, 0.0), -5e-14, SEED0 + 11),
     "column_in_By": SlabWorkload("slab_1x251x111_column_in_By", (1, 251, 111), 1e-5, 1e-13, (0.0, 10.0, 0.0), -5e-14, SEED0 + 12),
+    # PAPER.md:356 (section 3.3.2, Fig. 14 caption at :368): electrons on the face y = 9 dy, z from 5 dz to 106 dz, speeds along
+    # +y uniform in [0, v0] (v0 = 10 eV), 10 T B_y; Table 1 prints JefiPIC's maximum
+    # displacement and velocity at 0.4 and 0.6 ns for this set-up.
+    "planar_emission": SlabWorkload("slab_1x251x111_planar_emission", (1, 251, 111), 1e-5, 1e-13, (0.0, 10.0, 0.0), -5e-14, SEED0 + 13),
 }
+V0_10EV = math.sqrt(2.0 * 10.0 * E_CHARGE / M_E)  # "the energy corresponding to the velocities v0 ... equals to 10 eV"
 
 
-def slab_particles(which: str, count: int) -> Dict[str, np.ndarray]:
+def slab_particles(which: str, count: int, variant: str = "") -> Dict[str, np.ndarray]:
     """`count` macro-electrons of total charge -5e-14 C.
     point_emission (Fig. 5): uniform in the cell j = k = 50, velocity in the yz plane, speed Gaussian about
     v0 (10 eV) with sigma 0.2 v0, direction uniform.  column_in_By (Fig. 8): uniform in the column
-    j = 124, k = 5..105, at rest."""
+    j = 124, k = 5..105, at rest.  planar_emission (Fig. 14): on the face y = 9 dy, z in [5, 106) dz, speed
+    along +y uniform in [0, v0]."""
     w = SLABS[which]
     rng = np.random.default_rng(w.seed)
     wt = w.total_charge / (-E_CHARGE) / count
@@ -194,6 +200,15 @@ def slab_particles(which: str, count: int) -> Dict[str, np.ndarray]:
         beta = speed / C_SI
         g = 1.0 / np.sqrt(1.0 - beta * beta)
         mom = [np.zeros(count), g * beta * np.cos(ang), g * beta * np.sin(ang)]
+    elif which == "planar_emission":
+        # variant: what Fig. 14 (an image) leaves open.  "" = on the plane y = 9 dy; "cell" = uniform in the cell layer
+        # 9 dy <= y < 10 dy; "xcentre" = all at x = dx/2 (no charge on the virtual x nodes of the one-cell-thick grid)
+        y = rng.uniform(9.0, 10.0, count) if variant == "cell" else np.full(count, 9.0)
+        z = rng.uniform(5.0, 106.0, count)
+        if variant == "xcentre":
+            x = np.full(count, 0.5)
+        beta = rng.uniform(0.0, V0_10EV, count) / C_SI
+        mom = [np.zeros(count), beta / np.sqrt(1.0 - beta * beta), np.zeros(count)]
     else:
         y, z = rng.uniform(124.0, 125.0, count), rng.uniform(5.0, 106.0, count)
         mom = [np.zeros(count) for _ in range(3)]
