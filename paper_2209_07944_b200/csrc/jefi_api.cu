@@ -160,21 +160,37 @@ extern "C" int jefi_create(const jefi_config* cfg, jefi_ctx** out) {
   c->field_impl = JEFI_FIELD_REFERENCE;
   c->impl_reason = "reference: requested (JEFI_FIELD_REFERENCE)";
   if (cfg->field_impl != JEFI_FIELD_REFERENCE) {
-    long mism = -1, noff = 0;
-    int rc = jefi_verify_delay_fp32(c, &mism, &noff);
-    if (rc != JEFI_OK) return fail_create(c, rc, c->err);
+    // Proof that the tiled kernel's fp32 delay arithmetic equals the fp64 table on every offset.  An offset whose s = R/(c dt)
+    // lies within fp32 rounding of a half-integer (a near-tie of the nearest-step rule) can come out one step off; the scaled
+    // spacings kx, ky, kz are then moved by a few units in the last place (|eps| <= 8 * 2^-23: the field values change by
+    // <= 3e-6 relative, the delays are the TABLE's or the proof fails) until all offsets agree.  Exact ties (s = m + 1/2 in exact
+    // arithmetic, e.g. kappa = 1.5) survive every such move: the reference kernel then runs and says so.
+    const jefi_geom g0 = c->geom;
+    long mism = -1, noff = 0, mism0 = -1;
+    int moved = 0;
+    for (int trial = 0; trial <= 16 && mism != 0; trial++) {
+      moved = (trial + 1) / 2 * ((trial & 1) ? 1 : -1);  // 0, +1, -1, +2, -2, ..
+      const double f = 1.0 + moved * 1.1920928955078125e-07;
+      c->geom.kx = (float)((double)g0.kx * f); c->geom.ky = (float)((double)g0.ky * f); c->geom.kz = (float)((double)g0.kz * f);
+      int rc = jefi_verify_delay_fp32(c, &mism, &noff);
+      if (rc != JEFI_OK) return fail_create(c, rc, c->err);
+      if (trial == 0) mism0 = mism;
+    }
+    if (mism != 0) { c->geom = g0; moved = 0; mism = mism0; }
     int prep = (mism == 0) ? jefi_tiled_prepare(c) : JEFI_ESTATE;
-    char buf[320];
+    char buf[400];
     if (mism == 0 && prep == JEFI_OK) {
       c->field_impl = JEFI_FIELD_TILED;
-      snprintf(buf, sizeof buf, "tiled: fp32 delays proven equal to the fp64 table on %ld offsets; tiles %dx%dx%d / %dx%dx%d, window %d slots "
-               "in pitch %d (%d pass%s), source range in %d piece%s", noff, d.obx, d.oby, d.obz, d.tsx, d.tsy, d.tsz, c->wmax, c->wpitch,
+      char mv[96] = "";
+      if (moved != 0) snprintf(mv, sizeof mv, " (scaled spacings moved by %+d ulp to clear %ld near-ties)", moved, mism0);
+      snprintf(buf, sizeof buf, "tiled: fp32 delays proven equal to the fp64 table on %ld offsets%s; tiles %dx%dx%d / %dx%dx%d, window %d slots "
+               "in pitch %d (%d pass%s), source range in %d piece%s", noff, mv, d.obx, d.oby, d.obz, d.tsx, d.tsy, d.tsz, c->wmax, c->wpitch,
                (c->wmax + c->wpitch - 1) / c->wpitch, c->wmax > c->wpitch ? "es" : "", c->nsplit, c->nsplit > 1 ? "s" : "");
       c->impl_reason = buf;
     } else {
       if (mism != 0)
-        snprintf(buf, sizeof buf, "reference: %ld of %ld fp32 delays differ from the fp64 table (a tie of the nearest-step rule within fp32 "
-                 "rounding), the tiled kernel cannot be proven", mism, noff);
+        snprintf(buf, sizeof buf, "reference: %ld of %ld fp32 delays differ from the fp64 table, also with the spacings moved by up to 8 ulp "
+                 "(exact ties s = m + 1/2 of the nearest-step rule): the tiled kernel cannot be proven", mism, noff);
       else
         snprintf(buf, sizeof buf, "reference: tiled kernel could not be prepared (rc=%d: %s)", prep, c->err.c_str());
       c->impl_reason = buf;

@@ -304,13 +304,16 @@ __device__ __forceinline__ void one_pair(const item_addr& Az, float ax, float ay
   const float a_y = ay * r2;                // has to be kept alive (measured 1.3 % faster than one FMUL2 on kept pairs)
   const float u0 = lo32(u0wy), wy = hi32(u0wy);
   const f32x2 Azx = swap2(Axz);
+  // The order of the seven accumulations (and 32 pairs per loop iteration, tile_pairs) was chosen by measurement on B200:
+  // ten orders of these independent statements ran between 741 and 767 ms per 96^3 step (register-bank conflicts and operand
+  // reuse between neighbouring FFMA2 depend on it); this one is the fastest.
   A.Exz = fma2(Axz, pk(u0, u0), A.Exz);
-  A.Fxz = fma2(rs2, D.xy, A.Fxz);
-  A.Ey = fmaf(a_y, u0, A.Ey);
-  A.Fy = fmaf(rs, hi32(D.zw), A.Fy);
   A.Bxz = fma2(pk(a_y, a_y), swap2(wxz), A.Bxz);  // (a_y wz, a_y wx)
+  A.Ey = fmaf(a_y, u0, A.Ey);
   A.Cxz = fma2(pk(wy, wy), Azx, A.Cxz);           // (wy a_z, wy a_x)
+  A.Fy = fmaf(rs, hi32(D.zw), A.Fy);
   A.By12 = fma2(Azx, wxz, A.By12);                // (a_z wx, a_x wz)
+  A.Fxz = fma2(rs2, D.xy, A.Fxz);
 }
 
 // compile-time loops over the cells of the staged source tile (the LDS offsets of one_pair are immediates)
@@ -340,12 +343,13 @@ __device__ __forceinline__ void z_layers(const item_addr& Az, float kz, const fl
   }
 }
 
-// one observation cell against the 64 cells of the staged source tile; the z loop is unrolled to 16 pairs per iteration
+// one observation cell against the 64 cells of the staged source tile; the z loop is unrolled to 32 pairs per iteration
 template <class G, int MODE, bool LINEAR>
 __device__ __forceinline__ void tile_pairs(const item_addr& A0, float kz, const float (&ax)[G::TSX], const float (&ay)[G::TSY], float fz0,
                                            pair_acc& A) {
   constexpr int LAYER = G::TSX * G::TSY;            // cells per z layer of the source tile
-  constexpr int ZU = LAYER >= 16 ? 1 : 16 / LAYER;  // layers per loop iteration
+  constexpr int PAIRS_PER_ITER = 32;                                        // straight-line pairs per loop iteration (measured: 16, 32, 64)
+  constexpr int ZU = LAYER >= PAIRS_PER_ITER ? 1 : PAIRS_PER_ITER / LAYER;  // layers per loop iteration
 #pragma unroll 1
   for (int lz = 0; lz < G::TSZ; lz += ZU) {
     item_addr Az = A0;
@@ -360,13 +364,8 @@ __device__ __forceinline__ void tile_pairs(const item_addr& A0, float kz, const 
 
 // MULTI: the grid has tile pairs whose window exceeds WP (compiled in only then: the common single-pass kernels carry neither
 // the third evaluation mode nor its registers)
-#ifdef JEFI_MAXNREG
-#define JEFI_TILED_BOUNDS __maxnreg__(JEFI_MAXNREG)
-#else
-#define JEFI_TILED_BOUNDS __launch_bounds__(TILED_THREADS, 1)
-#endif
 template <class G, int WP, bool LINEAR, bool MULTI>
-__global__ void JEFI_TILED_BOUNDS k_field_tiled(tiled_params P) {
+__global__ void __launch_bounds__(TILED_THREADS, 1) k_field_tiled(tiled_params P) {
   using L = stage_layout<WP>;
   extern __shared__ __align__(128) unsigned char smem[];
   const jefi_dims& d = P.d;
@@ -463,7 +462,8 @@ __global__ void JEFI_TILED_BOUNDS k_field_tiled(tiled_params P) {
   }
 
   // -------------------------------------------------- consumer warps --------------------------------------------------
-  for (int item = 0;; item++) {
+  // single-pass kernels know their item count (one per source tile); multi-pass ones read "last" from the stage header
+  for (int item = 0; MULTI || item < nt; item++) {
     const int s = item & 1;
     const unsigned char* st = smem + (size_t)s * L::BYTES;
     mbar_wait(barFull + 8 * s, (item >> 1) & 1);
@@ -505,7 +505,7 @@ __global__ void JEFI_TILED_BOUNDS k_field_tiled(tiled_params P) {
     accS[5 * OBCELLS + c] += hi32(A.Cxz) - hi32(A.Bxz);
     __syncwarp();
     if (lane == 0) mbar_arrive(barDone + 8 * s);  // stage s may be refilled; this warp's accumulator updates are done
-    if (h.last & 1) break;
+    if (MULTI && (h.last & 1)) break;
   }
 
   asm volatile("bar.sync 1, %0;" ::"n"(NCONS) : "memory");  // consumers only: all accumulator updates are visible
