@@ -170,6 +170,17 @@ int jefi_push_particles(jefi_ctx* ctx, long np, float* x, float* y, float* z, fl
 int jefi_push_particles_packed(jefi_ctx* ctx, long np, float* x, float* y, float* z, float* ux, float* uy, float* uz,
                                const float* q_over_m, unsigned char* alive, const float* eb_packed);
 
+/* One whole PIC step n (PAPER.md:85 section 2, :231 section 2.4) in one call: jefi_deposit(r^n, u^{n-1/2}) -> jefi_push_sources ->
+ * jefi_field_step_packed -> jefi_push_particles_packed, with the argument meanings of those calls (rho..jz: OUT, the deposited
+ * sources of step n; ex..bz and eb_packed: OUT, the fields of step n; particle arrays IN/OUT).  When the context's stream is
+ * not the legacy default stream, the sequence is captured into a CUDA graph on the first call (again whenever an argument
+ * changes) and replayed as ONE launch afterwards: on small grids, where the kernels of a step take tens of microseconds, the
+ * per-launch overhead is as large as the work.  The step counter lives on the device for the graph; it may be mixed freely with
+ * the individual calls.  On the legacy default stream (not capturable) the four calls are simply issued in turn. */
+int jefi_pic_step(jefi_ctx* ctx, long np, float* x, float* y, float* z, float* ux, float* uy, float* uz, const float* qw,
+                  const float* q_over_m, unsigned char* alive, float* rho, float* jx, float* jy, float* jz, float* ex, float* ey,
+                  float* ez, float* bx, float* by, float* bz, float* eb_packed);
+
 /* End-to-end variant of one field step with HOST buffers (pinned memory recommended): copies the newest source
  * slice (4 x N floats) host->device, does jefi_push_sources + jefi_field_step, copies E,B (6 x N floats)
  * device->host and synchronises the stream.  Host arrays: src_host = [rho|jx|jy|jz] (4N floats),

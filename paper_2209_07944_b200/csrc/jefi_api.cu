@@ -65,6 +65,11 @@ extern "C" int jefi_create(const jefi_config* cfg, jefi_ctx** out) {
   c->src_stage = c->eb_stage = nullptr;
   c->perm = nullptr;
   c->partial = nullptr;
+  c->step_dev = nullptr;
+  c->step_dev_value = -2;
+  c->capturing = false;
+  c->pic_exec = nullptr;
+  c->pic_launches = 0;
   c->wmax = c->wpitch = 0;
   c->chunk = 0;
   c->nsplit = 1;
@@ -147,6 +152,8 @@ extern "C" int jefi_create(const jefi_config* cfg, jefi_ctx** out) {
         double R = sqrt(ddx * ddx + ddy * ddy + ddz * ddz);
         c->mtab_host[ia + (size_t)ex * (jb + (size_t)ey * kc)] = (int)floor(R / L0 + 0.5);
       }
+  if ((e = cudaMalloc(&c->step_dev, 4 * sizeof(int))) != cudaSuccess)
+    return fail_create(c, JEFI_ENOMEM, std::string("step state allocation: ") + cudaGetErrorString(e));
   if ((e = cudaMalloc(&c->mtab_dev, tn * sizeof(int))) != cudaSuccess)
     return fail_create(c, JEFI_ENOMEM, std::string("delay table device allocation: ") + cudaGetErrorString(e));
   if ((e = cudaMemcpyAsync(c->mtab_dev, c->mtab_host, tn * sizeof(int), cudaMemcpyHostToDevice, c->stream)) != cudaSuccess)
@@ -212,6 +219,8 @@ extern "C" void jefi_destroy(jefi_ctx* c) {
   if (c->mtab_dev) cudaFree(c->mtab_dev);
   if (c->perm) cudaFree(c->perm);
   if (c->partial) cudaFree(c->partial);
+  if (c->step_dev) cudaFree(c->step_dev);
+  if (c->pic_exec) cudaGraphExecDestroy(c->pic_exec);
   if (c->src_stage) cudaFree(c->src_stage);
   if (c->eb_stage) cudaFree(c->eb_stage);
   if (c->sort_count) cudaFree(c->sort_count);
@@ -235,12 +244,14 @@ extern "C" void jefi_destroy(jefi_ctx* c) {
 // row are contiguous.  Reads the previous slot, writes value and backward difference.
 // Traffic: 16 B in (4 SoA floats) + 16 B read (previous) + 32 B written per cell.
 // ------------------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_push_sources(jefi_dims d, float inv_c, int slot, int prev_slot,
+// step_dev != NULL (jefi_pic_step's graph): slot and previous slot come from the device-side step state.
+__global__ void __launch_bounds__(256) k_push_sources(jefi_dims d, float inv_c, int slot, int prev_slot, const int* __restrict__ step_dev,
                                                       const float* __restrict__ rho, const float* __restrict__ jx,
                                                       const float* __restrict__ jy, const float* __restrict__ jz,
                                                       float4* __restrict__ ring) {
   long r = (long)blockIdx.x * blockDim.x + threadIdx.x;
   if (r >= d.ncell_pad) return;
+  if (step_dev) { slot = step_dev[1]; prev_slot = step_dev[2]; }
   const long tile = r / JEFI_TCELLS;
   const int cell = (int)(r - tile * JEFI_TCELLS);
   const int tx = (int)(tile % d.ntx), ty = (int)((tile / d.ntx) % d.nty), tz = (int)(tile / ((long)d.ntx * d.nty));
@@ -254,13 +265,27 @@ __global__ void __launch_bounds__(256) k_push_sources(jefi_dims d, float inv_c, 
   ring[q + JEFI_TCELLS] = make_float4(s.x - p.x, s.y - p.y, s.z - p.z, s.w - p.w);
 }
 
+__global__ void k_advance_step(int* __restrict__ st, int H) {  // n += 1 on the device (first kernel of the PIC-step graph)
+  const int n = st[0] + 1;
+  st[0] = n;
+  st[1] = n % H;
+  st[2] = n >= 1 ? (n - 1) % H : -1;
+}
+
 int jefi_launch_push_sources(jefi_ctx* c, const float* rho, const float* jx, const float* jy, const float* jz) {
   const jefi_dims& d = c->dims;
+  unsigned blocks = (unsigned)((d.ncell_pad + 255) / 256);
+  if (c->capturing) {  // recorded once, replayed every step: the step lives on the device, the host counter is advanced per replay
+    k_advance_step<<<1, 1, 0, c->stream>>>(c->step_dev, d.H);
+    k_push_sources<<<blocks, 256, 0, c->stream>>>(d, (float)(1.0 / c->c), 0, -1, c->step_dev, rho, jx, jy, jz, c->ring);
+    JEFI_CUDA_TRY(c, cudaGetLastError());
+    c->launches += 2;
+    return JEFI_OK;
+  }
   long n = c->step + 1;
   int slot = (int)(n % d.H);
   int prev = n >= 1 ? (int)((n - 1) % d.H) : -1;
-  unsigned blocks = (unsigned)((d.ncell_pad + 255) / 256);
-  k_push_sources<<<blocks, 256, 0, c->stream>>>(d, (float)(1.0 / c->c), slot, prev, rho, jx, jy, jz, c->ring);
+  k_push_sources<<<blocks, 256, 0, c->stream>>>(d, (float)(1.0 / c->c), slot, prev, nullptr, rho, jx, jy, jz, c->ring);
   JEFI_CUDA_TRY(c, cudaGetLastError());
   c->launches++;
   c->step = n;
@@ -274,12 +299,16 @@ extern "C" int jefi_push_sources(jefi_ctx* c, const float* rho, const float* jx,
   return jefi_launch_push_sources(c, rho, jx, jy, jz);
 }
 
-static int field_step_impl(jefi_ctx* c, int k0, int k1, float* ex, float* ey, float* ez, float* bx, float* by, float* bz,
-                           float* eb_packed) {
+int jefi_field_step_impl(jefi_ctx* c, int k0, int k1, float* ex, float* ey, float* ez, float* bx, float* by, float* bz,
+                         float* eb_packed) {
   if (!ex || !ey || !ez || !bx || !by || !bz) { c->err = "jefi_field_step: NULL array"; return JEFI_EINVAL; }
   if (k0 < 0 || k1 > c->dims.nz || k0 > k1 || (k0 % c->dims.obz) != 0) {
     c->err = "jefi_field_step_slab: need 0 <= k0 <= k1 <= nz with k0 a multiple of the observation tile's z edge (jefi_get_tile_info)";
     return JEFI_EINVAL;
+  }
+  if (c->capturing) {  // inside jefi_pic_step's graph: the push of this step precedes it; no event records in a graph
+    return c->field_impl == JEFI_FIELD_TILED ? jefi_launch_field_tiled(c, k0, k1, ex, ey, ez, bx, by, bz, eb_packed)
+                                             : jefi_launch_field_reference(c, k0, k1, ex, ey, ez, bx, by, bz, eb_packed);
   }
   if (c->step < 0) { c->err = "jefi_field_step before any jefi_push_sources"; return JEFI_ESTATE; }
   if (k0 == k1) return JEFI_OK;
@@ -296,20 +325,20 @@ static int field_step_impl(jefi_ctx* c, int k0, int k1, float* ex, float* ey, fl
 extern "C" int jefi_field_step_slab(jefi_ctx* c, int k0, int k1, float* ex, float* ey, float* ez, float* bx, float* by, float* bz) {
   if (!c) return JEFI_EINVAL;
   jefi_device_guard guard(c);
-  return field_step_impl(c, k0, k1, ex, ey, ez, bx, by, bz, nullptr);
+  return jefi_field_step_impl(c, k0, k1, ex, ey, ez, bx, by, bz, nullptr);
 }
 
 extern "C" int jefi_field_step(jefi_ctx* c, float* ex, float* ey, float* ez, float* bx, float* by, float* bz) {
   if (!c) return JEFI_EINVAL;
   jefi_device_guard guard(c);
-  return field_step_impl(c, 0, c->dims.nz, ex, ey, ez, bx, by, bz, nullptr);
+  return jefi_field_step_impl(c, 0, c->dims.nz, ex, ey, ez, bx, by, bz, nullptr);
 }
 
 extern "C" int jefi_field_step_packed(jefi_ctx* c, float* ex, float* ey, float* ez, float* bx, float* by, float* bz, float* eb_packed) {
   if (!c) return JEFI_EINVAL;
   jefi_device_guard guard(c);
   if (!eb_packed || ((uintptr_t)eb_packed & 15u)) { c->err = "jefi_field_step_packed: eb_packed must be a 16-byte aligned device array of 8 N floats"; return JEFI_EINVAL; }
-  return field_step_impl(c, 0, c->dims.nz, ex, ey, ez, bx, by, bz, eb_packed);
+  return jefi_field_step_impl(c, 0, c->dims.nz, ex, ey, ez, bx, by, bz, eb_packed);
 }
 
 extern "C" float jefi_field_kernel_ms(jefi_ctx* c, int calls_back) {
@@ -323,6 +352,68 @@ extern "C" float jefi_field_kernel_ms(jefi_ctx* c, int calls_back) {
 }
 
 extern "C" float jefi_last_field_kernel_ms(jefi_ctx* c) { return jefi_field_kernel_ms(c, 0); }
+
+// ------------------------------------------------------------------------------------------------------------
+// One whole PIC step: deposit -> push_sources -> field_step_packed -> push_particles_packed, as ONE CUDA
+// graph launch.  On 16^3 .. 32^3 grids the kernels of a step take tens of microseconds and the 6-8 launches + memset nodes
+// cost as much again; the graph is captured on the first call (and again whenever an argument changes) and replayed after.
+// ------------------------------------------------------------------------------------------------------------
+extern "C" int jefi_pic_step(jefi_ctx* c, long np, float* x, float* y, float* z, float* ux, float* uy, float* uz, const float* qw,
+                             const float* q_over_m, unsigned char* alive, float* rho, float* jx, float* jy, float* jz, float* ex,
+                             float* ey, float* ez, float* bx, float* by, float* bz, float* eb_packed) {
+  if (!c) return JEFI_EINVAL;
+  jefi_device_guard guard(c);
+  if (np < 0 || np > 0x7fffffffL || !rho || !jx || !jy || !jz || !ex || !ey || !ez || !bx || !by || !bz || !eb_packed || ((uintptr_t)eb_packed & 15u) ||
+      (np > 0 && (!x || !y || !z || !ux || !uy || !uz || !qw || !q_over_m || !alive))) {
+    c->err = "jefi_pic_step: NULL or misaligned array, or np out of range";
+    return JEFI_EINVAL;
+  }
+  auto direct = [&]() -> int {
+    int rc = jefi_deposit_impl(c, np, x, y, z, ux, uy, uz, qw, alive, rho, jx, jy, jz);
+    if (rc == JEFI_OK) rc = jefi_launch_push_sources(c, rho, jx, jy, jz);
+    if (rc == JEFI_OK) rc = jefi_field_step_impl(c, 0, c->dims.nz, ex, ey, ez, bx, by, bz, eb_packed);
+    if (rc == JEFI_OK) rc = jefi_push_packed_impl(c, np, x, y, z, ux, uy, uz, q_over_m, alive, eb_packed);
+    return rc;
+  };
+  if (c->stream == nullptr || c->stream == cudaStreamLegacy) return direct();  // the legacy default stream cannot be captured
+  const void* ptrs[] = {x, y, z, ux, uy, uz, qw, q_over_m, alive, rho, jx, jy, jz, ex, ey, ez, bx, by, bz, eb_packed};
+  unsigned long long key[24] = {0};
+  key[0] = (unsigned long long)np;
+  for (int i = 0; i < 20; i++) key[1 + i] = (unsigned long long)(uintptr_t)ptrs[i];
+  if (!c->pic_exec || memcmp(key, c->pic_key, sizeof key) != 0) {
+    if (c->pic_exec) { cudaGraphExecDestroy(c->pic_exec); c->pic_exec = nullptr; }
+    int rc = jefi_prepare_deposit_scratch(c, np);
+    if (rc != JEFI_OK) return rc;
+    JEFI_CUDA_TRY(c, cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
+    const long l0 = c->launches;
+    c->capturing = true;
+    rc = direct();
+    c->capturing = false;
+    c->pic_launches = c->launches - l0;
+    c->launches = l0;
+    cudaGraph_t graph = nullptr;
+    cudaError_t e = cudaStreamEndCapture(c->stream, &graph);
+    if (rc != JEFI_OK || e != cudaSuccess) {
+      if (graph) cudaGraphDestroy(graph);
+      if (rc == JEFI_OK) { c->err = std::string("jefi_pic_step: graph capture: ") + cudaGetErrorString(e); rc = JEFI_ECUDA; }
+      return rc;
+    }
+    e = cudaGraphInstantiate(&c->pic_exec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (e != cudaSuccess) { c->pic_exec = nullptr; c->err = std::string("jefi_pic_step: cudaGraphInstantiate: ") + cudaGetErrorString(e); return JEFI_ECUDA; }
+    memcpy(c->pic_key, key, sizeof key);
+  }
+  if (c->step_dev_value != c->step) {  // other calls advanced the step since the last replay: bring the device copy up to date
+    const jefi_dims& d = c->dims;
+    const int h[4] = {(int)c->step, c->step >= 0 ? (int)(c->step % d.H) : -1, c->step >= 1 ? (int)((c->step - 1) % d.H) : -1, 0};
+    JEFI_CUDA_TRY(c, cudaMemcpyAsync(c->step_dev, h, sizeof h, cudaMemcpyHostToDevice, c->stream));
+  }
+  JEFI_CUDA_TRY(c, cudaGraphLaunch(c->pic_exec, c->stream));
+  c->step += 1;
+  c->step_dev_value = c->step;
+  c->launches += c->pic_launches;
+  return JEFI_OK;
+}
 
 extern "C" int jefi_field_step_host(jefi_ctx* c, const float* src_host, float* eb_host) {
   if (!c) return JEFI_EINVAL;
@@ -345,7 +436,7 @@ extern "C" int jefi_field_step_host(jefi_ctx* c, const float* src_host, float* e
   int rc = jefi_launch_push_sources(c, s, s + N, s + 2 * N, s + 3 * N);
   if (rc != JEFI_OK) return rc;
   float* o = c->eb_stage;
-  rc = field_step_impl(c, 0, c->dims.nz, o, o + N, o + 2 * N, o + 3 * N, o + 4 * N, o + 5 * N, nullptr);
+  rc = jefi_field_step_impl(c, 0, c->dims.nz, o, o + N, o + 2 * N, o + 3 * N, o + 4 * N, o + 5 * N, nullptr);
   if (rc != JEFI_OK) return rc;
   JEFI_CUDA_TRY(c, cudaMemcpyAsync(eb_host, o, 6 * N * sizeof(float), cudaMemcpyDeviceToHost, c->stream));
   JEFI_CUDA_TRY(c, cudaStreamSynchronize(c->stream));

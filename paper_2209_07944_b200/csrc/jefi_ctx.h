@@ -99,6 +99,14 @@ struct jefi_ctx {
   long sort_cap;
   float4* eb_pack;                                 // jefi_push_particles: E, B packed two float4 per node
   void* sort_buf;                                  // jefi_sort_particles: permuted copies of the caller's arrays
+  // jefi_pic_step: one whole PIC step as a CUDA graph.  The step-dependent kernel arguments (n, ring slot, previous slot) are
+  // read from step_dev, which the graph's first kernel advances, so that the same executable graph replays every step.
+  int* step_dev;            // device int[4]: n, n mod H, (n-1) mod H or -1
+  long step_dev_value;      // the step step_dev currently holds (-2: nothing uploaded yet)
+  bool capturing;           // a graph capture is in progress: kernels take the step from step_dev, no event records
+  cudaGraphExec_t pic_exec;
+  unsigned long long pic_key[24];
+  long pic_launches;        // kernels per replay
   // host-variant staging
   float* src_stage;     // 4N floats, device staging of jefi_field_step_host
   float* eb_stage;      // 6N floats
@@ -152,6 +160,12 @@ __device__ __forceinline__ float jefi_q_fp32(float kx, float ky, float kz, float
 
 // implemented in the .cu files
 int jefi_launch_push_sources(jefi_ctx* c, const float* rho, const float* jx, const float* jy, const float* jz);
+int jefi_field_step_impl(jefi_ctx* c, int k0, int k1, float* ex, float* ey, float* ez, float* bx, float* by, float* bz, float* eb_packed);
+int jefi_deposit_impl(jefi_ctx* c, long np, const float* x, const float* y, const float* z, const float* ux, const float* uy,
+                      const float* uz, const float* qw, const unsigned char* alive, float* rho, float* jx, float* jy, float* jz);
+int jefi_push_packed_impl(jefi_ctx* c, long np, float* x, float* y, float* z, float* ux, float* uy, float* uz, const float* q_over_m,
+                          unsigned char* alive, const float* eb_packed);
+int jefi_prepare_deposit_scratch(jefi_ctx* c, long np);  // allocations a captured deposit must not make
 int jefi_launch_field_reference(jefi_ctx* c, int k0, int k1, float* ex, float* ey, float* ez, float* bx, float* by, float* bz,
                                 float* eb_packed);
 int jefi_launch_field_tiled(jefi_ctx* c, int k0, int k1, float* ex, float* ey, float* ez, float* bx, float* by, float* bz,

@@ -23,13 +23,15 @@
 // ------------------------------------------------------------------------------------------------------------
 // reference kernel
 // ------------------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(128) k_field_reference(jefi_dims d, jefi_geom g, int ex_, int ey_, long n, int linear, long oc0, long oc1,
+__global__ void __launch_bounds__(128) k_field_reference(jefi_dims d, jefi_geom g, int ex_, int ey_, long n, const int* __restrict__ step_dev,
+                                                         int linear, long oc0, long oc1,
                                                          const int* __restrict__ mtab, const float4* __restrict__ ring,
                                                          float* __restrict__ ex, float* __restrict__ ey,
                                                          float* __restrict__ ez, float* __restrict__ bx,
                                                          float* __restrict__ by, float* __restrict__ bz, float4* __restrict__ pack) {
   long oc = oc0 + (long)blockIdx.x * blockDim.x + threadIdx.x;
   if (oc >= oc1) return;
+  if (step_dev) n = step_dev[0];  // jefi_pic_step's graph
   const int I = (int)(oc % d.nx), J = (int)((oc / d.nx) % d.ny), K = (int)(oc / ((long)d.nx * d.ny));
   float aex = 0, aey = 0, aez = 0, abx = 0, aby = 0, abz = 0;
   for (int k = 0; k < d.nz; k++) {
@@ -78,7 +80,8 @@ int jefi_launch_field_reference(jefi_ctx* c, int k0, int k1, float* ex, float* e
   const jefi_dims& d = c->dims;
   const long oc0 = (long)k0 * d.nx * d.ny, oc1 = (long)k1 * d.nx * d.ny;  // observation cells of the z-planes [k0, k1)
   unsigned blocks = (unsigned)((oc1 - oc0 + 127) / 128);
-  k_field_reference<<<blocks, 128, 0, c->stream>>>(d, c->geom, c->tex, c->tey, c->step, c->cfg.delay_rule == JEFI_DELAY_LINEAR ? 1 : 0, oc0, oc1,
+  k_field_reference<<<blocks, 128, 0, c->stream>>>(d, c->geom, c->tex, c->tey, c->step, c->capturing ? c->step_dev : nullptr,
+                                                   c->cfg.delay_rule == JEFI_DELAY_LINEAR ? 1 : 0, oc0, oc1,
                                                    c->mtab_dev, c->ring, ex, ey, ez, bx, by, bz, reinterpret_cast<float4*>(eb_packed));
   JEFI_CUDA_TRY(c, cudaGetLastError());
   c->launches++;
@@ -139,6 +142,7 @@ struct tiled_params {
   int k1;          // observation planes k >= k1 are not written
   int chunk;       // source tiles per blockIdx.y
   int to_partial;  // 1: write this piece's sums to partial[blockIdx.y][6][N] (source range split over blockIdx.y)
+  const int* step_dev;  // non-NULL (jefi_pic_step's graph): n and nslot are read from the device-side step state
   const float4* ring;
   const unsigned short* perm;  // [ndz][ndy][ndx][512]
   float *ex, *ey, *ez, *bx, *by, *bz;
@@ -203,15 +207,13 @@ __device__ __forceinline__ f32x2 pk(float lo, float hi) {
   return r;
 }
 __device__ __forceinline__ float lo32(f32x2 v) {
-  float a, b;
-  asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v));
-  (void)b;
+  float a;
+  asm("{ .reg .b32 jf_unused; mov.b64 {%0, jf_unused}, %1; }" : "=f"(a) : "l"(v));
   return a;
 }
 __device__ __forceinline__ float hi32(f32x2 v) {
-  float a, b;
-  asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v));
-  (void)a;
+  float b;
+  asm("{ .reg .b32 jf_unused; mov.b64 {jf_unused, %0}, %1; }" : "=f"(b) : "l"(v));
   return b;
 }
 __device__ __forceinline__ f32x2 swap2(f32x2 v) { return pk(hi32(v), lo32(v)); }
@@ -392,6 +394,7 @@ __global__ void __launch_bounds__(TILED_THREADS, 1) k_field_tiled(tiled_params P
   if (warp == NCWARPS) {
     // ------------------------------------------------ producer warp ------------------------------------------------
     int stx = t0 % d.ntx, sty = (t0 / d.ntx) % d.nty, stz = t0 / (d.ntx * d.nty);
+    const int n_now = P.step_dev ? P.step_dev[0] : P.n, nslot_now = P.step_dev ? P.step_dev[1] : P.nslot;
     int item = 0;
     for (int it = 0; it < nt; it++) {
       const int sx0 = stx * G::TSX, sy0 = sty * G::TSY, sz0 = stz * G::TSZ;
@@ -417,10 +420,10 @@ __global__ void __launch_bounds__(TILED_THREADS, 1) k_field_tiled(tiled_params P
         const int R = min(WP, m_top - m_lo + 1);
         // row j <-> delay m = m_top - j <-> absolute step t = n - m_top + j.  Rows with t < 0 (before t0)
         // or m > H-2 (not stored, reading A15) are zero: j < jv.
-        int jv = max(m_top - P.n, m_top - (d.H - 2));
+        int jv = max(m_top - n_now, m_top - (d.H - 2));
         jv = jv < 0 ? 0 : (jv > R ? R : jv);
         const int nvalid = R - jv;          // <= H - 1
-        int s0 = P.nslot - (m_top - jv);    // ring slot of row jv; m_top - jv <= H - 2
+        int s0 = nslot_now - (m_top - jv);  // ring slot of row jv; m_top - jv <= H - 2
         s0 += s0 < 0 ? d.H : 0;
         const int lenA = min(nvalid, d.H - s0), lenB = nvalid - lenA;  // ring wrap: at most two runs
         const uint32_t sb = sm0 + (uint32_t)s * L::BYTES;
@@ -763,6 +766,7 @@ int jefi_launch_field_tiled(jefi_ctx* c, int k0, int k1, float* ex, float* ey, f
   P.ndx = c->ndx; P.ndy = c->ndy;
   P.chunk = c->chunk;
   P.to_partial = c->nsplit > 1 ? 1 : 0;
+  P.step_dev = c->capturing ? c->step_dev : nullptr;
   P.ring = c->ring; P.perm = c->perm;
   P.ex = ex; P.ey = ey; P.ez = ez; P.bx = bx; P.by = by; P.bz = bz;
   P.pack = reinterpret_cast<float4*>(eb_packed);

@@ -351,6 +351,16 @@ extern "C" int jefi_deposit(jefi_ctx* c, long np, const float* x, const float* y
     c->err = "jefi_deposit: NULL array or np out of range";
     return JEFI_EINVAL;
   }
+  return jefi_deposit_impl(c, np, x, y, z, ux, uy, uz, qw, alive, rho, jx, jy, jz);
+}
+
+int jefi_prepare_deposit_scratch(jefi_ctx* c, long np) {
+  int mode = c->cfg.deposit_mode;
+  return (mode == JEFI_DEPOSIT_SORTED && np > 0) ? ensure_sort_scratch(c, np) : JEFI_OK;
+}
+
+int jefi_deposit_impl(jefi_ctx* c, long np, const float* x, const float* y, const float* z, const float* ux, const float* uy,
+                      const float* uz, const float* qw, const unsigned char* alive, float* rho, float* jx, float* jy, float* jz) {
   const jefi_dims& d = c->dims;
   if (jx == rho + d.N && jy == jx + d.N && jz == jy + d.N) {  // one [4][N] block (the usual case): one memset node
     JEFI_CUDA_TRY(c, cudaMemsetAsync(rho, 0, 4 * d.N * sizeof(float), c->stream));
@@ -601,6 +611,11 @@ extern "C" int jefi_push_particles_packed(jefi_ctx* c, long np, float* x, float*
     c->err = "jefi_push_particles_packed: NULL or misaligned array, or negative np";
     return JEFI_EINVAL;
   }
+  return jefi_push_packed_impl(c, np, x, y, z, ux, uy, uz, q_over_m, alive, eb_packed);
+}
+
+int jefi_push_packed_impl(jefi_ctx* c, long np, float* x, float* y, float* z, float* ux, float* uy, float* uz, const float* q_over_m,
+                          unsigned char* alive, const float* eb_packed) {
   if (np == 0) return JEFI_OK;
   launch_push<true>(c, np, x, y, z, ux, uy, uz, q_over_m, alive, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr,
                     reinterpret_cast<const float4*>(eb_packed));

@@ -26,7 +26,7 @@ EXPORTS = [
     "jefi_field_step", "jefi_field_step_slab", "jefi_push_particles", "jefi_field_step_host", "jefi_launch_count",
     "jefi_last_field_kernel_ms", "jefi_debug_delay_table", "jefi_debug_cell_index", "jefi_debug_history_slot",
     "jefi_debug_cell_order", "jefi_sort_particles", "jefi_field_impl_reason", "jefi_get_tile_info", "jefi_field_step_packed",
-    "jefi_push_particles_packed", "jefi_field_kernel_ms", "jefi_debug_fp32_peak", "jefi_debug_check_errors",
+    "jefi_push_particles_packed", "jefi_field_kernel_ms", "jefi_debug_fp32_peak", "jefi_debug_check_errors", "jefi_pic_step",
 ]
 
 
@@ -86,6 +86,8 @@ def load_library() -> C.CDLL:
     lib.jefi_last_field_kernel_ms.restype = C.c_float
     lib.jefi_field_kernel_ms.argtypes = [vp, C.c_int]
     lib.jefi_field_kernel_ms.restype = C.c_float
+    lib.jefi_pic_step.argtypes = [vp, C.c_long] + [f32p] * 8 + [u8p] + [f32p] * 11
+    lib.jefi_pic_step.restype = C.c_int
     lib.jefi_debug_check_errors.argtypes = [vp, C.POINTER(C.c_long * 4)]
     lib.jefi_debug_check_errors.restype = C.c_int
     lib.jefi_debug_fp32_peak.argtypes = [vp, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_int)]
@@ -253,6 +255,18 @@ def jefi_push_particles_packed(handle: int, N: int, x, y, z, ux, uy, uz, q_over_
            "jefi_push_particles_packed")
 
 
+def jefi_pic_step(handle: int, N: int, x, y, z, ux, uy, uz, qw, q_over_m, alive, rho, jx, jy, jz, ex, ey, ez, bx, by, bz,
+                  eb_packed) -> None:
+    import torch
+
+    f = torch.float32
+    np_ = x.numel()
+    pp = [_dev(t, f, np_, n) for t, n in zip((x, y, z, ux, uy, uz, qw, q_over_m), ("x", "y", "z", "ux", "uy", "uz", "qw", "q_over_m"))]
+    pg = [_dev(t, f, N, n) for t, n in zip((rho, jx, jy, jz, ex, ey, ez, bx, by, bz), ("rho", "jx", "jy", "jz", "ex", "ey", "ez", "bx", "by", "bz"))]
+    rc = load_library().jefi_pic_step(handle, np_, *pp, _dev(alive, torch.uint8, np_, "alive"), *pg, _dev(eb_packed, f, 8 * N, "eb_packed"))
+    _check(handle, rc, "jefi_pic_step")
+
+
 def jefi_sort_particles(handle: int, x, y, z, ux, uy, uz, qw, q_over_m, alive, tag=None) -> None:
     import torch
 
@@ -367,7 +381,11 @@ class GridSpec:
 
 
 class JefiContext:
-    """Owns one jefi_ctx and the E/B/rho/J device tensors of a run; every method is one C-ABI call."""
+    """Owns one jefi_ctx and the E/B/rho/J device tensors of a run; every method is one C-ABI call.
+
+    The context enqueues on the torch stream that is current when it is created.  Created inside
+    ``with torch.cuda.stream(torch.cuda.Stream())`` (any stream but the legacy default one) ``pic_step`` is one CUDA-graph
+    launch per step (jefi_pic_step); the caller then keeps its own tensor work on that stream too."""
 
     def __init__(self, grid: GridSpec, device=None, field_impl: int = JEFI_FIELD_AUTO,
                  deposit_mode: int = JEFI_DEPOSIT_AUTO, sort_every: int = 8, delay_rule: int = JEFI_DELAY_NEAREST,
@@ -381,6 +399,7 @@ class JefiContext:
         self.N = grid.N
         torch.cuda.set_device(self.device)
         stream = torch.cuda.current_stream(self.device).cuda_stream
+        self.stream_handle = stream
         self.handle = jefi_create(grid.nx, grid.ny, grid.nz, grid.dx, grid.dy, grid.dz, grid.dt, grid.c, grid.eps0,
                                   grid.H, grid.hist_cap, grid.Eext, grid.Bext, self.device.index or 0, stream,
                                   field_impl, deposit_mode, delay_rule, shape_order, field_chunk)
@@ -458,12 +477,13 @@ class JefiContext:
         if self.sort_every > 0 and self._pic_steps % self.sort_every == 0:
             self.sort_particles(part)
         self._pic_steps += 1
-        self.deposit(part)
-        self.push_sources()
         if self.EBp is not None:
-            self.field_step_packed()
-            self.push_particles_packed(part)
+            s, o = self.src, self.EB
+            jefi_pic_step(self.handle, self.N, part["x"], part["y"], part["z"], part["ux"], part["uy"], part["uz"], part["qw"], part["qm"],
+                          part["alive"], s[0], s[1], s[2], s[3], o[0], o[1], o[2], o[3], o[4], o[5], self.EBp)
         else:
+            self.deposit(part)
+            self.push_sources()
             self.field_step()
             self.push_particles(part)
 

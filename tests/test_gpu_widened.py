@@ -333,3 +333,54 @@ def test_s2_closed_loop_config1_10_steps(J):
         _, E1, _ = o1.pic_step(p1)
     assert field_err(eb[:3], E1)[0] > 1e-3
     ctx.close()
+
+
+# ------------------------------------------------------------------------------------ jefi_pic_step: one CUDA graph per step
+@pytest.mark.parametrize("config,steps", [(1, 12), (2, 6)])
+def test_pic_step_graph_closed_loop(J, config, steps):
+    """On a non-default stream jefi_pic_step replays one captured CUDA graph per step (the step counter lives on the device).
+    Closed loop against the full fp64 oracle, with a cell sort every 3 steps (which changes no captured pointer) and, in the
+    middle, two steps issued through the four individual calls (the device-side step must be brought back in line)."""
+    import torch
+
+    w = wl.WORKLOADS[config]
+    part = wl.particles(config)
+    cfg = OracleConfig(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt)
+    orc = oracle.OracleJefi(cfg)
+    po = {k: v.astype(np.float64) for k, v in part.items() if k != "alive"}
+    po["alive"] = part["alive"].copy()
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        ctx = J.JefiContext(J.GridSpec(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt), sort_every=3)
+        assert ctx.stream_handle != 0
+        dp = to_dev(part, ctx.device)
+        dp["tag"] = torch.arange(part["x"].shape[0], dtype=torch.int32, device=ctx.device)
+        l_prev, per_step = ctx.launch_count(), []
+        for s in range(steps):
+            if s in (steps // 2, steps // 2 + 1):  # the individual calls, on the same context
+                ctx.deposit(dp)
+                ctx.push_sources()
+                ctx.field_step()
+                ctx.push_particles(dp)
+            else:
+                ctx.pic_step(dp)
+            per_step.append(ctx.launch_count() - l_prev)
+            l_prev = ctx.launch_count()
+        side.synchronize()
+        got = {k: v.cpu().numpy() for k, v in dp.items()}
+        eb = ctx.EB.cpu().numpy()
+        S = ctx.src.cpu().numpy()
+        assert J.jefi_get_info(ctx.handle)["step"] == steps - 1
+    for s in range(steps):
+        So, Eo, Bo = orc.pic_step(po)
+    inv = np.argsort(got.pop("tag"))
+    got = {k: v[inv] for k, v in got.items()}
+    both = (got["alive"] == 1) & (po["alive"] == 1)
+    assert (got["alive"] != po["alive"]).sum() <= 2
+    for k in "xyz":
+        assert np.abs(got[k][both] - po[k][both]).max() / w.n <= 1e-5, k
+    assert_field_parity(eb[:3], eb[3:], Eo, Bo, f"cfg{config} graph step {steps - 1}: ")
+    for a in range(4):
+        assert np.linalg.norm(S[a] - So[a]) <= 1e-5 * max(np.linalg.norm(So[a]), 1e-300)
+    assert min(per_step) >= 4  # every step, replayed or direct, accounts for its kernels in jefi_launch_count
+    ctx.close()
