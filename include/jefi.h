@@ -40,6 +40,11 @@ extern "C" {
 #define JEFI_FIELD_REFERENCE 1 /* one thread per observation cell, table-driven delays (slow; the paper's K1 in fp32) */
 #define JEFI_FIELD_TILED 2     /* shared-memory tiled kernel; jefi_create fails with JEFI_ESTATE if not provable */
 
+/* field_tile values */
+#define JEFI_TILE_AUTO 0
+#define JEFI_TILE_CELL 1
+#define JEFI_TILE_DYAD 2
+
 /* deposit_mode values */
 #define JEFI_DEPOSIT_AUTO 0   /* = JEFI_DEPOSIT_RUNS (the measured best on sorted and unsorted lists) */
 #define JEFI_DEPOSIT_DIRECT 1 /* caller's order; lanes of a warp that hit the same node are combined wherever they sit (match-any) */
@@ -77,6 +82,11 @@ typedef struct {
                            CTA on large grids; on small grids the range is split over CTAs to fill the GPU and the partial
                            sums are added by a second kernel in a fixed order); > 0 -> that many; -1 -> never split.
                            The result is deterministic (bit-identical from run to run) for every value. */
+  int field_tile;       /* tuning of the tiled field kernel: what one thread of an observation tile owns.  0 -> automatic;
+                           1 -> JEFI_TILE_CELL: one cell (8x8x8 tiles); 2 -> JEFI_TILE_DYAD: two cells that are neighbours along x
+                           (16x8x8 tiles; needs nx >= 16): the pairs (r, r') and (r + ex, r' + ex) have the same offset, so their
+                           distance, delay and geometric factors are evaluated once for both.  Ignored on nx <= 3 grids.  Every
+                           choice forms the sums of Eqs. 2.4-2.5 over the same pairs; only the order of the additions differs. */
 } jefi_config;
 
 /* Create a context: allocates the ring (32*H*N_padded bytes, zeroed = "zero before t0"), builds the
@@ -99,7 +109,7 @@ int jefi_get_info(const jefi_ctx* ctx, int* H, int* ndt, int* field_impl, long* 
 const char* jefi_field_impl_reason(const jefi_ctx* ctx);
 
 /* Geometry of the tiled field kernel (all optional, NULL ok): observation tile and source tile in cells per axis
- * (8x8x8 / 4x4x4; 1x16x32 / 1x8x8 on grids with nx <= 3 such as the paper's 1 x ny x nz slabs), the largest slot window of a
+ * (8x8x8 or 16x8x8 / 4x4x4, see jefi_config.field_tile; 1x16x32 / 1x8x8 on grids with nx <= 3 such as the paper's 1 x ny x nz slabs), the largest slot window of a
  * tile pair, the shared-memory pitch it is served from (window > pitch: the tile is evaluated in ceil(window/pitch) passes),
  * and the number of pieces the source range is split into.  obs_tile[2] is the granularity of jefi_field_step_slab. */
 int jefi_get_tile_info(const jefi_ctx* ctx, int obs_tile[3], int src_tile[3], int* window_slots, int* window_pitch,

@@ -53,7 +53,7 @@ extern "C" int jefi_create(const jefi_config* cfg, jefi_ctx** out) {
   if (!cfg || !out) return fail_create(nullptr, JEFI_EINVAL, "jefi_create: NULL argument");
   if (cfg->nx < 1 || cfg->ny < 1 || cfg->nz < 1 || !(cfg->dx > 0) || !(cfg->dy > 0) || !(cfg->dz > 0) || !(cfg->dt > 0) ||
       cfg->c < 0 || cfg->eps0 < 0 || cfg->H < 0 || cfg->hist_cap < 0 || cfg->deposit_mode < 0 || cfg->deposit_mode > 3 || cfg->delay_rule < 0 || cfg->delay_rule > 1 ||
-      cfg->shape_order < 0 || cfg->shape_order > 2 || cfg->field_chunk < -1 || cfg->field_impl < 0 || cfg->field_impl > 2)
+      cfg->shape_order < 0 || cfg->shape_order > 2 || cfg->field_chunk < -1 || cfg->field_tile < 0 || cfg->field_tile > 2 || cfg->field_impl < 0 || cfg->field_impl > 2)
     return fail_create(nullptr, JEFI_EINVAL, "jefi_create: grid sizes, spacings and dt must be positive, switches in range");
   if ((long)cfg->nx * cfg->ny * cfg->nz > (1L << 30)) return fail_create(nullptr, JEFI_EINVAL, "jefi_create: grid too large");
   jefi_ctx* c = new (std::nothrow) jefi_ctx();
@@ -109,10 +109,18 @@ extern "C" int jefi_create(const jefi_config* cfg, jefi_ctx** out) {
   jefi_dims& d = c->dims;
   d.nx = cfg->nx; d.ny = cfg->ny; d.nz = cfg->nz;
   // tile geometry: cubes, or x-thin tiles for the paper's 1 x ny x nz slabs
-  c->tile_geom = cfg->nx <= 3 ? JEFI_GEOM_SLABX : JEFI_GEOM_CUBE;
+  // (field_tile): two x-neighbour cells per thread once the grid has enough 16x8x8 tiles to fill the GPU several times
+  int nsm_ = 148;
+  cudaDeviceGetAttribute(&nsm_, cudaDevAttrMultiProcessorCount, cfg->device);
+  const long ndyad = (long)((cfg->nx + 15) / 16) * ((cfg->ny + 7) / 8) * ((cfg->nz + 7) / 8);
+  const bool dyad = cfg->nx >= 16 && (cfg->field_tile == JEFI_TILE_DYAD || (cfg->field_tile == JEFI_TILE_AUTO && ndyad >= 4L * nsm_));
+  c->tile_geom = cfg->nx <= 3 ? JEFI_GEOM_SLABX : (dyad ? JEFI_GEOM_DYAD : JEFI_GEOM_CUBE);
   if (c->tile_geom == JEFI_GEOM_SLABX) {
     d.tsx = jefi_geom_slabx::TSX; d.tsy = jefi_geom_slabx::TSY; d.tsz = jefi_geom_slabx::TSZ;
     d.obx = jefi_geom_slabx::OBX; d.oby = jefi_geom_slabx::OBY; d.obz = jefi_geom_slabx::OBZ;
+  } else if (c->tile_geom == JEFI_GEOM_DYAD) {
+    d.tsx = jefi_geom_dyad::TSX; d.tsy = jefi_geom_dyad::TSY; d.tsz = jefi_geom_dyad::TSZ;
+    d.obx = jefi_geom_dyad::OBX; d.oby = jefi_geom_dyad::OBY; d.obz = jefi_geom_dyad::OBZ;
   } else {
     d.tsx = jefi_geom_cube::TSX; d.tsy = jefi_geom_cube::TSY; d.tsz = jefi_geom_cube::TSZ;
     d.obx = jefi_geom_cube::OBX; d.oby = jefi_geom_cube::OBY; d.obz = jefi_geom_cube::OBZ;

@@ -24,16 +24,24 @@ constexpr int JEFI_ROW_QUADS = 2 * JEFI_TCELLS + 1;        // float4 per (tile, 
 constexpr int JEFI_ROW_BYTES = JEFI_ROW_QUADS * 16;        // 2064
 
 // Tile geometries the field kernel is compiled for (template parameter of k_field_tiled / k_build_perm).
-template <int OBX_, int OBY_, int OBZ_, int TSX_, int TSY_, int TSZ_>
+// A consumer thread owns one UNIT of the observation tile: CX cells that are neighbours along x.  With CX = 2 the pairs
+// (o, s) and (o + ex, s + ex) have the same offset, i.e. the same distance, delay and geometric factors, which are then
+// evaluated once for both (translation invariance of the uniform grid).
+template <int OBX_, int OBY_, int OBZ_, int TSX_, int TSY_, int TSZ_, int CX_ = 1>
 struct jefi_tile_geom {
-  static constexpr int OBX = OBX_, OBY = OBY_, OBZ = OBZ_;  // observation tile (512 cells = one per consumer thread)
+  static constexpr int OBX = OBX_, OBY = OBY_, OBZ = OBZ_;  // observation tile in cells
   static constexpr int TSX = TSX_, TSY = TSY_, TSZ = TSZ_;  // source tile (64 cells = one ring row)
-  static_assert(OBX_ * OBY_ * OBZ_ == 512 && TSX_ * TSY_ * TSZ_ == JEFI_TCELLS, "tile sizes");
+  static constexpr int CX = CX_;                            // cells per thread (along x)
+  static constexpr int UX = OBX_ / CX_;                     // units per axis: UX x OBY x OBZ = 512 = one per consumer thread
+  static constexpr int CELLS = OBX_ * OBY_ * OBZ_;
+  static_assert(UX * CX_ == OBX_ && UX * OBY_ * OBZ_ == 512 && TSX_ * TSY_ * TSZ_ == JEFI_TCELLS, "tile sizes");
   static_assert(OBX_ % TSX_ == 0 && OBY_ % TSY_ == 0 && OBZ_ % TSZ_ == 0, "observation tile = whole source tiles");
+  static_assert(CX_ == 1 || (CX_ == 2 && TSX_ == 4), "CX = 2 is written for 4-wide source rows");
 };
 using jefi_geom_cube = jefi_tile_geom<8, 8, 8, 4, 4, 4>;
 using jefi_geom_slabx = jefi_tile_geom<1, 16, 32, 1, 8, 8>;
-enum { JEFI_GEOM_CUBE = 0, JEFI_GEOM_SLABX = 1 };
+using jefi_geom_dyad = jefi_tile_geom<16, 8, 8, 4, 4, 4, 2>;
+enum { JEFI_GEOM_CUBE = 0, JEFI_GEOM_SLABX = 1, JEFI_GEOM_DYAD = 2 };
 
 struct jefi_dims {
   int nx, ny, nz;     // real cells

@@ -160,14 +160,14 @@ struct stage_hdr {  // written by the producer before it arms the stage's full b
 };
 static_assert(sizeof(stage_hdr) == HDR_BYTES, "stage header");
 
-template <int WP>
+template <int WP, int CELLS>
 struct stage_layout {
   static constexpr uint32_t ROWS = WP * JEFI_ROW_BYTES;
   static constexpr uint32_t PERM = ROWS;                       // u16[512]
   static constexpr uint32_t HDR = PERM + OBCELLS * 2;
   static constexpr uint32_t BYTES = ((HDR + HDR_BYTES + 127) / 128) * 128;
-  static constexpr uint32_t ACC = 2 * BYTES;                   // float[6][512]
-  static constexpr uint32_t BAR = ACC + 6 * OBCELLS * 4;       // full[2], done[2]
+  static constexpr uint32_t ACC = 2 * BYTES;                   // float[6][CELLS]
+  static constexpr uint32_t BAR = ACC + 6 * CELLS * 4;         // full[2], done[2]
   static constexpr uint32_t TOTAL = BAR + 4 * 8;
 };
 
@@ -250,7 +250,7 @@ struct item_addr {
   uint32_t Mtop;  // MODE_MULTI
   uint32_t R;     // MODE_MULTI
 #ifdef JEFI_CHECKED
-  uint32_t lo, hi;  // shared-memory byte range of the rows staged for this item (+ the z-layer offset)
+  uint32_t lo, hi;  // shared-memory byte range of the rows staged for this item (both + the z-layer offset)
 #endif
 };
 
@@ -266,11 +266,16 @@ __device__ unsigned long long g_jefi_check_errors[2];
 #endif
 cudaError_t jefi_field_check_errors(unsigned long long out[2]) { return cudaMemcpyFromSymbol(out, g_jefi_check_errors, 2 * sizeof(unsigned long long)); }
 
-// One observation cell against one source cell.  Az = item address + byte offset of the z layer.
-template <int MODE, bool LINEAR, int CELL>
-__device__ __forceinline__ void one_pair(const item_addr& Az, float ax, float ay, float az, float qyz, pair_acc& A) {
-  constexpr int SOFF = CELL * 16;
-  constexpr int DOFF = SOFF + JEFI_TCELLS * 16;
+// The part of a pair evaluation that depends only on the offset r - r' (and, through the address, on the staged item): with
+// G::CX = 2 it is shared by the pairs (o, s) and (o + ex, s + ex).  Az = item address + byte offset of the z layer.
+template <bool LINEAR>
+struct pair_geom {
+  uint32_t addr;  // shared address of the ring row of this offset's delay
+  float rs, a_y, nphi;
+  f32x2 Axz;      // (a_x, a_z) = d' rs^2
+};
+template <int MODE, bool LINEAR>
+__device__ __forceinline__ void make_geom(const item_addr& Az, float ax, float ay, float az, float qyz, pair_geom<LINEAR>& g) {
   const float q = fmaf(ax, ax, qyz);
   float rs = jefi_rsqrt(q);
   if (MODE != MODE_PLAIN) rs = q > 0.f ? rs : 0.f;  // the self cell contributes exactly zero
@@ -285,25 +290,35 @@ __device__ __forceinline__ void one_pair(const item_addr& Az, float ax, float ay
     addr = Az.K - (uint32_t)__float_as_int(t) * (uint32_t)JEFI_ROW_BYTES;  // row j = m_top - m
   }
 #ifdef JEFI_CHECKED
-  if (addr + SOFF < Az.lo || addr + DOFF + 16 > Az.hi) {  // outside the rows staged for this item
+  if (addr < Az.lo || addr + (uint32_t)JEFI_ROW_BYTES > Az.hi) {  // the row of this delay lies outside the rows staged for this item
     JEFI_CHECK_FAIL(0);
     addr = Az.lo;
   }
 #endif
-  quad2 S = lds128_imm<SOFF>(addr);         // (Jx, Jz | rho, Jy)
-  const quad2 D = lds128_imm<DOFF>(addr);   // (DJx, DJz | Drho, DJy)
+  g.addr = addr;
+  g.rs = rs;
+  if (LINEAR) g.nphi = fmaf(-q, rs, t - JEFI_MAGIC);  // m - s
+  const float r2 = rs * rs;
+  g.Axz = pk(ax * r2, az * r2);   // (a_x, a_z) = d' rs^2: two scalar multiplies, so that no (ax, az) register pair
+  g.a_y = ay * r2;                // has to be kept alive (measured 1.3 % faster than one FMUL2 on kept pairs)
+}
+// One observation cell against source cell CELL of the staged tile, with the geometry of their offset.
+template <bool LINEAR, int CELL>
+__device__ __forceinline__ void acc_pair(const pair_geom<LINEAR>& g, pair_acc& A) {
+  constexpr int SOFF = CELL * 16;
+  constexpr int DOFF = SOFF + JEFI_TCELLS * 16;
+  quad2 S = lds128_imm<SOFF>(g.addr);         // (Jx, Jz | rho, Jy)
+  const quad2 D = lds128_imm<DOFF>(g.addr);   // (DJx, DJz | Drho, DJy)
   if (LINEAR) {  // JEFI_DELAY_LINEAR: S(t_r) = S - phi D with phi = s - m in [-1/2, 1/2) (3 scalar + 2 packed instructions)
-    const float nphi = fmaf(-q, rs, t - JEFI_MAGIC);  // m - s
-    const f32x2 nphi2 = pk(nphi, nphi);
+    const f32x2 nphi2 = pk(g.nphi, g.nphi);
     S.xy = fma2(nphi2, D.xy, S.xy);
     S.zw = fma2(nphi2, D.zw, S.zw);
   }
+  const float rs = g.rs, a_y = g.a_y;
   const f32x2 rs2 = pk(rs, rs);
   const f32x2 wxz = fma2(rs2, S.xy, D.xy);  // (wx, wz)
   const f32x2 u0wy = fma2(rs2, S.zw, D.zw); // (u0, wy)
-  const float r2 = rs * rs;
-  const f32x2 Axz = pk(ax * r2, az * r2);   // (a_x, a_z) = d' rs^2: two scalar multiplies, so that no (ax, az) register pair
-  const float a_y = ay * r2;                // has to be kept alive (measured 1.3 % faster than one FMUL2 on kept pairs)
+  const f32x2 Axz = g.Axz;
   const float u0 = lo32(u0wy), wy = hi32(u0wy);
   const f32x2 Azx = swap2(Axz);
   // The order of the seven accumulations (and 32 pairs per loop iteration, tile_pairs) was chosen by measurement on B200:
@@ -318,17 +333,73 @@ __device__ __forceinline__ void one_pair(const item_addr& Az, float ax, float ay
   A.Fxz = fma2(rs2, D.xy, A.Fxz);
 }
 
+// Two observation cells against two source cells with ONE geometry (G::CX = 2: (cell 1, source CELL1) and (cell 0, source
+// CELL0) have the same offset).  The statements of the two pairs alternate so that the shared operands (rs, a_y, Axz, Azx) sit
+// in the same operand slot of neighbouring instructions: a register operand repeated there is served by the operand reuse
+// cache instead of the register file, whose two 32-bit reads per clock and scheduler are what bounds this kernel
+// (profiles/r2_rf_probe.md).
+template <bool LINEAR, int CELL1, int CELL0>
+__device__ __forceinline__ void acc_pair2(const pair_geom<LINEAR>& g, pair_acc& A1, pair_acc& A0) {
+  quad2 S1 = lds128_imm<CELL1 * 16>(g.addr);
+  const quad2 D1 = lds128_imm<CELL1 * 16 + JEFI_TCELLS * 16>(g.addr);
+  quad2 S0 = lds128_imm<CELL0 * 16>(g.addr);
+  const quad2 D0 = lds128_imm<CELL0 * 16 + JEFI_TCELLS * 16>(g.addr);
+  if (LINEAR) {
+    const f32x2 nphi2 = pk(g.nphi, g.nphi);
+    S1.xy = fma2(nphi2, D1.xy, S1.xy);
+    S0.xy = fma2(nphi2, D0.xy, S0.xy);
+    S1.zw = fma2(nphi2, D1.zw, S1.zw);
+    S0.zw = fma2(nphi2, D0.zw, S0.zw);
+  }
+  const float rs = g.rs, a_y = g.a_y;
+  const f32x2 rs2 = pk(rs, rs);
+  const f32x2 wxz1 = fma2(rs2, S1.xy, D1.xy);
+  const f32x2 wxz0 = fma2(rs2, S0.xy, D0.xy);
+  const f32x2 u0wy1 = fma2(rs2, S1.zw, D1.zw);
+  const f32x2 u0wy0 = fma2(rs2, S0.zw, D0.zw);
+  A1.Fxz = fma2(rs2, D1.xy, A1.Fxz);
+  A0.Fxz = fma2(rs2, D0.xy, A0.Fxz);
+  A1.Fy = fmaf(rs, hi32(D1.zw), A1.Fy);
+  A0.Fy = fmaf(rs, hi32(D0.zw), A0.Fy);
+  const f32x2 Axz = g.Axz;
+  const f32x2 Azx = swap2(Axz);
+  const f32x2 ay2 = pk(a_y, a_y);
+  const float u01 = lo32(u0wy1), wy1 = hi32(u0wy1), u00 = lo32(u0wy0), wy0 = hi32(u0wy0);
+  A1.Exz = fma2(Axz, pk(u01, u01), A1.Exz);
+  A0.Exz = fma2(Axz, pk(u00, u00), A0.Exz);
+  A1.Bxz = fma2(ay2, swap2(wxz1), A1.Bxz);
+  A0.Bxz = fma2(ay2, swap2(wxz0), A0.Bxz);
+  A1.Ey = fmaf(a_y, u01, A1.Ey);
+  A0.Ey = fmaf(a_y, u00, A0.Ey);
+  A1.Cxz = fma2(Azx, pk(wy1, wy1), A1.Cxz);
+  A0.Cxz = fma2(Azx, pk(wy0, wy0), A0.Cxz);
+  A1.By12 = fma2(Azx, wxz1, A1.By12);
+  A0.By12 = fma2(Azx, wxz0, A0.By12);
+}
+
 // compile-time loops over the cells of the staged source tile (the LDS offsets of one_pair are immediates)
+// G::CX == 1: ax[l] = kx (dx0 + cx - l), one geometry per pair.
+// G::CX == 2: the thread's cells are x and x + 1; ax[jj] = kx (dx0 + x + 1 - jj), jj = 0..4, is the offset of the pairs
+//             (cell 1, source l = jj) and (cell 0, source l = jj - 1): 5 geometries serve the 8 pairs of a source row.
 template <class G, int MODE, bool LINEAR, int CELL0, int LX>
-__device__ __forceinline__ void row_pairs(const item_addr& Az, const float (&ax)[G::TSX], float ay, float az, float qyz, pair_acc& A) {
-  if constexpr (LX < G::TSX) {
-    one_pair<MODE, LINEAR, CELL0 + LX>(Az, ax[LX], ay, az, qyz, A);
+__device__ __forceinline__ void row_pairs(const item_addr& Az, const float (&ax)[G::TSX + G::CX - 1], float ay, float az, float qyz,
+                                          pair_acc (&A)[G::CX]) {
+  if constexpr (LX < G::TSX + G::CX - 1) {
+    pair_geom<LINEAR> g;
+    make_geom<MODE, LINEAR>(Az, ax[LX], ay, az, qyz, g);
+    if constexpr (G::CX == 1) {
+      acc_pair<LINEAR, CELL0 + LX>(g, A[0]);
+    } else {
+      if constexpr (LX >= 1 && LX < G::TSX) acc_pair2<LINEAR, CELL0 + LX, CELL0 + LX - 1>(g, A[1], A[0]);
+      else if constexpr (LX < G::TSX) acc_pair<LINEAR, CELL0 + LX>(g, A[1]);
+      else acc_pair<LINEAR, CELL0 + LX - 1>(g, A[0]);
+    }
     row_pairs<G, MODE, LINEAR, CELL0, LX + 1>(Az, ax, ay, az, qyz, A);
   }
 }
 template <class G, int MODE, bool LINEAR, int CELL0, int LY>
-__device__ __forceinline__ void layer_rows(const item_addr& Az, const float (&ax)[G::TSX], const float (&ay)[G::TSY], float az, float az2,
-                                           pair_acc& A) {
+__device__ __forceinline__ void layer_rows(const item_addr& Az, const float (&ax)[G::TSX + G::CX - 1], const float (&ay)[G::TSY], float az, float az2,
+                                           pair_acc (&A)[G::CX]) {
   if constexpr (LY < G::TSY) {
     const float qyz = fmaf(ay[LY], ay[LY], az2);
     row_pairs<G, MODE, LINEAR, CELL0 + G::TSX * LY, 0>(Az, ax, ay[LY], az, qyz, A);
@@ -336,7 +407,8 @@ __device__ __forceinline__ void layer_rows(const item_addr& Az, const float (&ax
   }
 }
 template <class G, int MODE, bool LINEAR, int ZU, int ZO>
-__device__ __forceinline__ void z_layers(const item_addr& Az, float kz, const float (&ax)[G::TSX], const float (&ay)[G::TSY], float fz, pair_acc& A) {
+__device__ __forceinline__ void z_layers(const item_addr& Az, float kz, const float (&ax)[G::TSX + G::CX - 1], const float (&ay)[G::TSY], float fz,
+                                         pair_acc (&A)[G::CX]) {
   if constexpr (ZO < ZU) {
     const float az = kz * (fz - (float)ZO);
     const float az2 = az * az;
@@ -345,20 +417,21 @@ __device__ __forceinline__ void z_layers(const item_addr& Az, float kz, const fl
   }
 }
 
-// one observation cell against the 64 cells of the staged source tile; the z loop is unrolled to 32 pairs per iteration
+// the thread's G::CX observation cells against the 64 cells of the staged source tile; the z loop is unrolled to 32 pairs per
+// iteration
 template <class G, int MODE, bool LINEAR>
-__device__ __forceinline__ void tile_pairs(const item_addr& A0, float kz, const float (&ax)[G::TSX], const float (&ay)[G::TSY], float fz0,
-                                           pair_acc& A) {
+__device__ __forceinline__ void tile_pairs(const item_addr& A0, float kz, const float (&ax)[G::TSX + G::CX - 1], const float (&ay)[G::TSY], float fz0,
+                                           pair_acc (&A)[G::CX]) {
   constexpr int LAYER = G::TSX * G::TSY;            // cells per z layer of the source tile
   constexpr int PAIRS_PER_ITER = 32;                                        // straight-line pairs per loop iteration (measured: 16, 32, 64)
-  constexpr int ZU = LAYER >= PAIRS_PER_ITER ? 1 : PAIRS_PER_ITER / LAYER;  // layers per loop iteration
+  constexpr int ZU = LAYER * G::CX >= PAIRS_PER_ITER ? 1 : PAIRS_PER_ITER / (LAYER * G::CX);  // layers per loop iteration
 #pragma unroll 1
   for (int lz = 0; lz < G::TSZ; lz += ZU) {
     item_addr Az = A0;
     Az.K = A0.K + (uint32_t)(lz * LAYER * 16);
 #ifdef JEFI_CHECKED
     Az.lo = A0.lo + (uint32_t)(lz * LAYER * 16);
-    Az.hi = A0.hi;
+    Az.hi = A0.hi + (uint32_t)(lz * LAYER * 16);
 #endif
     z_layers<G, MODE, LINEAR, ZU, 0>(Az, kz, ax, ay, fz0 - (float)lz, A);
   }
@@ -368,7 +441,7 @@ __device__ __forceinline__ void tile_pairs(const item_addr& A0, float kz, const 
 // the third evaluation mode nor its registers)
 template <class G, int WP, bool LINEAR, bool MULTI>
 __global__ void __launch_bounds__(TILED_THREADS, 1) k_field_tiled(tiled_params P) {
-  using L = stage_layout<WP>;
+  using L = stage_layout<WP, G::CELLS>;
   extern __shared__ __align__(128) unsigned char smem[];
   const jefi_dims& d = P.d;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -383,7 +456,7 @@ __global__ void __launch_bounds__(TILED_THREADS, 1) k_field_tiled(tiled_params P
   const int nt = min(P.chunk, ntiles - t0);
 
   if (tid < NCONS)
-    for (int i = tid; i < 6 * OBCELLS; i += NCONS) accS[i] = 0.f;
+    for (int i = tid; i < 6 * G::CELLS; i += NCONS) accS[i] = 0.f;
   if (tid == 0) {
     mbar_init(barFull, 1); mbar_init(barFull + 8, 1);
     mbar_init(barDone, NCWARPS); mbar_init(barDone + 8, NCWARPS);
@@ -471,18 +544,21 @@ __global__ void __launch_bounds__(TILED_THREADS, 1) k_field_tiled(tiled_params P
     const unsigned char* st = smem + (size_t)s * L::BYTES;
     mbar_wait(barFull + 8 * s, (item >> 1) & 1);
     const stage_hdr h = *reinterpret_cast<const stage_hdr*>(st + L::HDR);
-    // the cell this lane evaluates for this source tile: neighbouring lanes are (almost) equidistant from it
+    // the unit (G::CX cells along x) this lane evaluates for this source tile: neighbouring lanes are (almost) equidistant from it
     const int c = reinterpret_cast<const unsigned short*>(st + L::PERM)[tid];
-    const int cx = c % G::OBX, cy = (c / G::OBX) % G::OBY, cz = c / (G::OBX * G::OBY);
-    float ax[G::TSX], ay[G::TSY];
+    const int cx = G::CX * (c % G::UX), cy = (c / G::UX) % G::OBY, cz = c / (G::UX * G::OBY);
+    float ax[G::TSX + G::CX - 1], ay[G::TSY];
 #pragma unroll
-    for (int l = 0; l < G::TSX; l++) ax[l] = P.g.kx * (float)(h.dx0 + cx - l);
+    for (int l = 0; l < G::TSX + G::CX - 1; l++) ax[l] = P.g.kx * (float)(h.dx0 + cx + (G::CX - 1) - l);
 #pragma unroll
     for (int l = 0; l < G::TSY; l++) ay[l] = P.g.ky * (float)(h.dy0 + cy - l);
     const float fz0 = (float)(h.dz0 + cz);
-    pair_acc A;
-    A.Exz = A.Fxz = A.Bxz = A.Cxz = A.By12 = pk(0.f, 0.f);
-    A.Ey = A.Fy = 0.f;
+    pair_acc A[G::CX];
+#pragma unroll
+    for (int i = 0; i < G::CX; i++) {
+      A[i].Exz = A[i].Fxz = A[i].Bxz = A[i].Cxz = A[i].By12 = pk(0.f, 0.f);
+      A[i].Ey = A[i].Fy = 0.f;
+    }
     item_addr I0;
     I0.K = h.K; I0.Mtop = h.Mtop; I0.R = h.R;
 #ifdef JEFI_CHECKED
@@ -497,28 +573,39 @@ __global__ void __launch_bounds__(TILED_THREADS, 1) k_field_tiled(tiled_params P
       tile_pairs<G, MODE_SELF, LINEAR>(I0, P.g.kz, ax, ay, fz0, A);
     else
       tile_pairs<G, MODE_MULTI, LINEAR>(I0, P.g.kz, ax, ay, fz0, A);
-    // second accumulation level.  Cell c belongs to this thread alone in this item; the previous item's updates
+    // second accumulation level.  Unit c belongs to this thread alone in this item; the previous item's updates
     // (by other threads) are complete once every consumer warp has arrived on that item's done barrier.
     if (item > 0) mbar_wait(barDone + 8 * ((item - 1) & 1), ((item - 1) >> 1) & 1);
-    accS[c] += lo32(A.Exz) - lo32(A.Fxz);
-    accS[OBCELLS + c] += A.Ey - A.Fy;
-    accS[2 * OBCELLS + c] += hi32(A.Exz) - hi32(A.Fxz);
-    accS[3 * OBCELLS + c] += lo32(A.Bxz) - lo32(A.Cxz);
-    accS[4 * OBCELLS + c] += lo32(A.By12) - hi32(A.By12);
-    accS[5 * OBCELLS + c] += hi32(A.Cxz) - hi32(A.Bxz);
+    if constexpr (G::CX == 1) {
+      accS[c] += lo32(A[0].Exz) - lo32(A[0].Fxz);
+      accS[G::CELLS + c] += A[0].Ey - A[0].Fy;
+      accS[2 * G::CELLS + c] += hi32(A[0].Exz) - hi32(A[0].Fxz);
+      accS[3 * G::CELLS + c] += lo32(A[0].Bxz) - lo32(A[0].Cxz);
+      accS[4 * G::CELLS + c] += lo32(A[0].By12) - hi32(A[0].By12);
+      accS[5 * G::CELLS + c] += hi32(A[0].Cxz) - hi32(A[0].Bxz);
+    } else {  // the two cells of the unit are neighbours in the home order (x fastest): one 8-byte update per component
+      float2* a2 = reinterpret_cast<float2*>(accS) + c;
+      float2 v;
+      v = a2[0]; v.x += lo32(A[0].Exz) - lo32(A[0].Fxz); v.y += lo32(A[1].Exz) - lo32(A[1].Fxz); a2[0] = v;
+      v = a2[G::CELLS / 2]; v.x += A[0].Ey - A[0].Fy; v.y += A[1].Ey - A[1].Fy; a2[G::CELLS / 2] = v;
+      v = a2[2 * (G::CELLS / 2)]; v.x += hi32(A[0].Exz) - hi32(A[0].Fxz); v.y += hi32(A[1].Exz) - hi32(A[1].Fxz); a2[2 * (G::CELLS / 2)] = v;
+      v = a2[3 * (G::CELLS / 2)]; v.x += lo32(A[0].Bxz) - lo32(A[0].Cxz); v.y += lo32(A[1].Bxz) - lo32(A[1].Cxz); a2[3 * (G::CELLS / 2)] = v;
+      v = a2[4 * (G::CELLS / 2)]; v.x += lo32(A[0].By12) - hi32(A[0].By12); v.y += lo32(A[1].By12) - hi32(A[1].By12); a2[4 * (G::CELLS / 2)] = v;
+      v = a2[5 * (G::CELLS / 2)]; v.x += hi32(A[0].Cxz) - hi32(A[0].Bxz); v.y += hi32(A[1].Cxz) - hi32(A[1].Bxz); a2[5 * (G::CELLS / 2)] = v;
+    }
     __syncwarp();
     if (lane == 0) mbar_arrive(barDone + 8 * s);  // stage s may be refilled; this warp's accumulator updates are done
     if (MULTI && (h.last & 1)) break;
   }
 
   asm volatile("bar.sync 1, %0;" ::"n"(NCONS) : "memory");  // consumers only: all accumulator updates are visible
-  {
-    const int c = tid;  // home order: x fastest inside the tile
+#pragma unroll
+  for (int c = tid; c < G::CELLS; c += NCONS) {  // home order: x fastest inside the tile
     const int oi = ox0 + c % G::OBX, oj = oy0 + (c / G::OBX) % G::OBY, ok = oz0 + c / (G::OBX * G::OBY);
     if (oi < d.nx && oj < d.ny && ok < P.k1) {
       const size_t o = (size_t)oi + (size_t)d.nx * ((size_t)oj + (size_t)d.ny * ok);
-      const float vex = P.g.prefE * accS[c], vey = P.g.prefE * accS[OBCELLS + c], vez = P.g.prefE * accS[2 * OBCELLS + c];
-      const float vbx = P.g.prefB * accS[3 * OBCELLS + c], vby = P.g.prefB * accS[4 * OBCELLS + c], vbz = P.g.prefB * accS[5 * OBCELLS + c];
+      const float vex = P.g.prefE * accS[c], vey = P.g.prefE * accS[G::CELLS + c], vez = P.g.prefE * accS[2 * G::CELLS + c];
+      const float vbx = P.g.prefB * accS[3 * G::CELLS + c], vby = P.g.prefB * accS[4 * G::CELLS + c], vbz = P.g.prefB * accS[5 * G::CELLS + c];
       if (P.to_partial) {
         float* q = P.partial + (size_t)blockIdx.y * 6 * (size_t)d.N + o;
         q[0] = vex; q[d.N] = vey; q[2 * d.N] = vez; q[3 * d.N] = vbx; q[4 * d.N] = vby; q[5 * d.N] = vbz;
@@ -565,23 +652,25 @@ __global__ void __launch_bounds__(256) k_reduce_partials(long N, int nsplit, lon
 //   2. per pair, the 64-bit set of source cells for which its two delays differ (same fp32 delay arithmetic as the kernel);
 //   3. deal the pairs to the 16 warps greedily: a warp starts from the first free pair of the distance order and then takes,
 //      15 times, the free pair among the next `band` pairs that adds the fewest new cells to the union of its pairs' sets
-//      (a source cell outside the union takes the fast path for that warp).  The band keeps the delays of one warp within
-//      8 slots: rows 8 apart share a 16-byte bank group and would be replayed.
+//      (a source cell outside the union takes the fast path for that warp).  The band (128 pairs) bounds the spread of the
+//      delays inside a warp: rows 8 apart share a 16-byte bank group and are replayed when they meet in one wavefront;
+//   4. the 16 pairs of a warp are put in distance order, so that each half-warp (one wavefront of the fast path) and each
+//      quarter-warp (one wavefront of the slow path) spans only a few slots.
 // Any order gives the same sums; this table only decides how fast.  One CTA of 512 threads per offset, once at create.
 template <class G>
 __global__ void __launch_bounds__(OBCELLS) k_build_perm(int ndx, int ndy, int ntx, int nty, int ntz, jefi_geom g, int band,
                                                         unsigned short* __restrict__ perm) {
   __shared__ float keys[OBCELLS];
   __shared__ unsigned short order[OBCELLS];
-  __shared__ unsigned long long mask[OBCELLS / 2];
+  __shared__ unsigned long long mask[G::CX][OBCELLS / 2];
   __shared__ unsigned short picked[OBCELLS / 2];
   __shared__ unsigned red[2][OBCELLS / 32];
-  const int c = threadIdx.x;
+  const int c = threadIdx.x;  // unit (G::CX cells along x) in home order
   const int ix = blockIdx.x % ndx, iy = (blockIdx.x / ndx) % ndy, iz = blockIdx.x / (ndx * ndy);
   const int Dxi = G::TSX * (ix - (ntx - 1)), Dyi = G::TSY * (iy - (nty - 1)), Dzi = G::TSZ * (iz - (ntz - 1));
-  const int cx = c % G::OBX, cy = (c / G::OBX) % G::OBY, cz = c / (G::OBX * G::OBY);
-  const float rx = g.kx * ((float)Dxi + (float)cx - 0.5f * (float)(G::TSX - 1)), ry = g.ky * ((float)Dyi + (float)cy - 0.5f * (float)(G::TSY - 1)),
-              rz = g.kz * ((float)Dzi + (float)cz - 0.5f * (float)(G::TSZ - 1));
+  const int cx = G::CX * (c % G::UX), cy = (c / G::UX) % G::OBY, cz = c / (G::UX * G::OBY);
+  const float rx = g.kx * ((float)Dxi + (float)cx + 0.5f * (float)(G::CX - 1) - 0.5f * (float)(G::TSX - 1)),
+              ry = g.ky * ((float)Dyi + (float)cy - 0.5f * (float)(G::TSY - 1)), rz = g.kz * ((float)Dzi + (float)cz - 0.5f * (float)(G::TSZ - 1));
   const float key = rx * rx + ry * ry + rz * rz;
   keys[c] = key;
   __syncthreads();
@@ -592,33 +681,49 @@ __global__ void __launch_bounds__(OBCELLS) k_build_perm(int ndx, int ndy, int nt
   }
   order[pos] = (unsigned short)c;
   __syncthreads();
-  // 2. pair c = cells order[2c], order[2c+1]: source cells whose delay differs between the two
-  unsigned long long mine = 0;
+  // 2. pair c = units order[2c], order[2c+1]: source cells whose delay differs between the two, per cell of the unit
+  unsigned long long mine[G::CX];
+#pragma unroll
+  for (int i = 0; i < G::CX; i++) mine[i] = 0;
   bool avail = c < OBCELLS / 2;
   if (avail) {
     const int a = order[2 * c], b = order[2 * c + 1];
-    const int axc = a % G::OBX, ayc = (a / G::OBX) % G::OBY, azc = a / (G::OBX * G::OBY);
-    const int bxc = b % G::OBX, byc = (b / G::OBX) % G::OBY, bzc = b / (G::OBX * G::OBY);
+    const int axc = G::CX * (a % G::UX), ayc = (a / G::UX) % G::OBY, azc = a / (G::UX * G::OBY);
+    const int bxc = G::CX * (b % G::UX), byc = (b / G::UX) % G::OBY, bzc = b / (G::UX * G::OBY);
     for (int sc = 0; sc < JEFI_TCELLS; sc++) {
       const int lx = sc % G::TSX, ly = (sc / G::TSX) % G::TSY, lz = sc / (G::TSX * G::TSY);
-      const float qa = jefi_q_fp32(g.kx, g.ky, g.kz, (float)(Dxi + axc - lx), (float)(Dyi + ayc - ly), (float)(Dzi + azc - lz));
-      const float qb = jefi_q_fp32(g.kx, g.ky, g.kz, (float)(Dxi + bxc - lx), (float)(Dyi + byc - ly), (float)(Dzi + bzc - lz));
-      const int ma = qa > 0.f ? jefi_delay_fp32(qa) : 0, mb = qb > 0.f ? jefi_delay_fp32(qb) : 0;
-      mine |= (unsigned long long)(ma != mb) << sc;
+#pragma unroll
+      for (int i = 0; i < G::CX; i++) {
+        const float qa = jefi_q_fp32(g.kx, g.ky, g.kz, (float)(Dxi + axc + i - lx), (float)(Dyi + ayc - ly), (float)(Dzi + azc - lz));
+        const float qb = jefi_q_fp32(g.kx, g.ky, g.kz, (float)(Dxi + bxc + i - lx), (float)(Dyi + byc - ly), (float)(Dzi + bzc - lz));
+        const int ma = qa > 0.f ? jefi_delay_fp32(qa) : 0, mb = qb > 0.f ? jefi_delay_fp32(qb) : 0;
+        mine[i] |= (unsigned long long)(ma != mb) << sc;
+      }
     }
-    mask[c] = mine;
+#pragma unroll
+    for (int i = 0; i < G::CX; i++) mask[i][c] = mine[i];
   }
   __syncthreads();
   // 3. greedy deal of the pairs to the warps (block-wide argmin per pick; keys are (cost << 16) | pair, pairs in distance order)
   const unsigned lane = c & 31, warp = c >> 5;
   int pick = 0;
   for (int w = 0; w < OBCELLS / 32; w++) {
-    unsigned long long uni = 0;
+    unsigned long long uni[G::CX];
+#pragma unroll
+    for (int i = 0; i < G::CX; i++) uni[i] = 0;
     int lo = 0;  // the warp's first pair = the lowest free pair; the others come from the `band` pairs that follow it
     for (int i = 0; i < 16; i++, pick++) {
       unsigned k = 0xffffffffu;
       if (avail) {
-        const unsigned cost = i == 0 ? 0u : (c < lo + band ? (unsigned)__popcll(uni | mine) : 0x7fffu);
+        unsigned cost = 0u;
+        if (i != 0) {
+          if (c < lo + band) {
+#pragma unroll
+            for (int q = 0; q < G::CX; q++) cost += (unsigned)__popcll(uni[q] | mine[q]);
+          } else {
+            cost = 0x7fffu;
+          }
+        }
         k = (cost << 16) | (unsigned)c;
       }
       k = __reduce_min_sync(0xffffffffu, k);
@@ -631,7 +736,18 @@ __global__ void __launch_bounds__(OBCELLS) k_build_perm(int ndx, int ndy, int nt
       if (i == 0) lo = sel;
       if (c == sel) avail = false;
       if (c == 0) picked[pick] = (unsigned short)sel;
-      uni |= mask[sel];
+#pragma unroll
+      for (int q = 0; q < G::CX; q++) uni[q] |= mask[q][sel];
+    }
+  }
+  __syncthreads();
+  if (c < OBCELLS / 32) {  // the 16 pairs of warp c in distance order: every half- and quarter-warp then spans few slots
+    unsigned short* q = picked + 16 * c;
+    for (int i = 1; i < 16; i++) {
+      const unsigned short v = q[i];
+      int j = i - 1;
+      for (; j >= 0 && q[j] > v; j--) q[j + 1] = q[j];
+      q[j + 1] = v;
     }
   }
   __syncthreads();
@@ -644,23 +760,23 @@ typedef void (*tiled_fn)(tiled_params);
 template <class G>
 static tiled_fn tiled_kernel_of(int wp, bool linear, bool multi) {
   if (multi) return linear ? k_field_tiled<G, 48, true, true> : k_field_tiled<G, 48, false, true>;  // several passes: largest pitch
-  switch (wp) {
-    case 36: return linear ? k_field_tiled<G, 36, true, false> : k_field_tiled<G, 36, false, false>;
-    case 48: return linear ? k_field_tiled<G, 48, true, false> : k_field_tiled<G, 48, false, false>;
+  if constexpr (G::CX == 1) {
+    if (wp == 36) return linear ? k_field_tiled<G, 36, true, false> : k_field_tiled<G, 36, false, false>;
   }
+  if (wp == 48) return linear ? k_field_tiled<G, 48, true, false> : k_field_tiled<G, 48, false, false>;
   return nullptr;
 }
 static tiled_fn tiled_kernel_for(const jefi_ctx* c) {
   const bool linear = c->cfg.delay_rule == JEFI_DELAY_LINEAR, multi = c->wmax > c->wpitch;
-  return c->tile_geom == JEFI_GEOM_SLABX ? tiled_kernel_of<jefi_geom_slabx>(c->wpitch, linear, multi)
-                                         : tiled_kernel_of<jefi_geom_cube>(c->wpitch, linear, multi);
-}
-static size_t tiled_smem_for(int wp) {
-  switch (wp) {
-    case 36: return stage_layout<36>::TOTAL;
-    case 48: return stage_layout<48>::TOTAL;
+  switch (c->tile_geom) {
+    case JEFI_GEOM_SLABX: return tiled_kernel_of<jefi_geom_slabx>(c->wpitch, linear, multi);
+    case JEFI_GEOM_DYAD: return tiled_kernel_of<jefi_geom_dyad>(c->wpitch, linear, multi);
   }
-  return 0;
+  return tiled_kernel_of<jefi_geom_cube>(c->wpitch, linear, multi);
+}
+static size_t tiled_smem_for(int wp, int cells) {
+  if (cells == 1024) return stage_layout<48, 1024>::TOTAL;
+  return wp == 36 ? stage_layout<36, 512>::TOTAL : stage_layout<48, 512>::TOTAL;
 }
 
 // How the source range is split over blockIdx.y.  A CTA per observation tile walking ALL source tiles needs no second
@@ -713,8 +829,9 @@ int jefi_tiled_prepare(jefi_ctx* c) {
   int wp = kPitches[sizeof(kPitches) / sizeof(int) - 1];  // wider windows: several passes through the largest pitch
   for (int cand : kPitches)
     if (cand >= wmax) { wp = cand; break; }
+  if (c->tile_geom == JEFI_GEOM_DYAD) wp = 48;  // compiled for the large pitch only (its windows reach 47 slots at dx = 2 c dt)
   c->wpitch = wp;
-  c->tiled_smem = tiled_smem_for(wp);
+  c->tiled_smem = tiled_smem_for(wp, d.obx * d.oby * d.obz);
   int dev = c->cfg.device, max_optin = 0;
   cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
   if (c->tiled_smem > (size_t)max_optin) {
@@ -747,9 +864,11 @@ int jefi_tiled_prepare(jefi_ctx* c) {
   }
   // pairs a warp may draw from, counted from its first pair in the distance order: wide enough to find pairs that differ on
   // the same source cells, narrow enough that the delays of one warp stay within 8 slots (rows 8 apart share a bank group)
-  const int band = 64;
+  const int band = 128;  // measured on cfg4 96^3: band 64 unsorted 741.3 ms, 64 / 96 / 128 / 256 with step 4: 741.2 / 739.7 / 738.9 / 738.7 ms
   if (c->tile_geom == JEFI_GEOM_SLABX)
     k_build_perm<jefi_geom_slabx><<<(unsigned)rows, OBCELLS, 0, c->stream>>>(c->ndx, c->ndy, d.ntx, d.nty, d.ntz, c->geom, band, c->perm);
+  else if (c->tile_geom == JEFI_GEOM_DYAD)
+    k_build_perm<jefi_geom_dyad><<<(unsigned)rows, OBCELLS, 0, c->stream>>>(c->ndx, c->ndy, d.ntx, d.nty, d.ntz, c->geom, band, c->perm);
   else
     k_build_perm<jefi_geom_cube><<<(unsigned)rows, OBCELLS, 0, c->stream>>>(c->ndx, c->ndy, d.ntx, d.nty, d.ntz, c->geom, band, c->perm);
   if ((e = cudaGetLastError()) != cudaSuccess) { c->err = std::string("k_build_perm: ") + cudaGetErrorString(e); return JEFI_ECUDA; }

@@ -20,6 +20,7 @@ JEFI_OK, JEFI_EINVAL, JEFI_ENOMEM, JEFI_ECUDA, JEFI_ESTATE = 0, -1, -2, -3, -4
 JEFI_FIELD_AUTO, JEFI_FIELD_REFERENCE, JEFI_FIELD_TILED = 0, 1, 2
 JEFI_DEPOSIT_AUTO, JEFI_DEPOSIT_DIRECT, JEFI_DEPOSIT_SORTED, JEFI_DEPOSIT_RUNS = 0, 1, 2, 3
 JEFI_DELAY_NEAREST, JEFI_DELAY_LINEAR = 0, 1
+JEFI_TILE_AUTO, JEFI_TILE_CELL, JEFI_TILE_DYAD = 0, 1, 2
 
 EXPORTS = [
     "jefi_create", "jefi_destroy", "jefi_last_error", "jefi_get_info", "jefi_deposit", "jefi_push_sources",
@@ -42,7 +43,7 @@ class jefi_config(C.Structure):
         ("H", C.c_int), ("hist_cap", C.c_int),
         ("Eext", C.c_double * 3), ("Bext", C.c_double * 3),
         ("device", C.c_int), ("stream", C.c_void_p), ("field_impl", C.c_int), ("deposit_mode", C.c_int),
-        ("delay_rule", C.c_int), ("shape_order", C.c_int), ("field_chunk", C.c_int),
+        ("delay_rule", C.c_int), ("shape_order", C.c_int), ("field_chunk", C.c_int), ("field_tile", C.c_int),
     ]
 
 
@@ -141,11 +142,12 @@ def jefi_create(nx: int, ny: int, nz: int, dx: float, dy: float, dz: float, dt: 
                 eps0: float = 0.0, H: int = 0, hist_cap: int = 0, Eext: Sequence[float] = (0, 0, 0),
                 Bext: Sequence[float] = (0, 0, 0), device: int = 0, stream: int = 0,
                 field_impl: int = JEFI_FIELD_AUTO, deposit_mode: int = JEFI_DEPOSIT_AUTO,
-                delay_rule: int = JEFI_DELAY_NEAREST, shape_order: int = 1, field_chunk: int = 0) -> int:
+                delay_rule: int = JEFI_DELAY_NEAREST, shape_order: int = 1, field_chunk: int = 0,
+                field_tile: int = 0) -> int:
     lib = load_library()
     cfg = jefi_config(nx, ny, nz, dx, dy, dz, dt, c, eps0, H, hist_cap, (C.c_double * 3)(*Eext),
                       (C.c_double * 3)(*Bext), device, C.c_void_p(stream), field_impl, deposit_mode, delay_rule,
-                      shape_order, field_chunk)
+                      shape_order, field_chunk, field_tile)
     h = C.c_void_p()
     rc = lib.jefi_create(C.byref(cfg), C.byref(h))
     if rc != JEFI_OK:
@@ -389,7 +391,7 @@ class JefiContext:
 
     def __init__(self, grid: GridSpec, device=None, field_impl: int = JEFI_FIELD_AUTO,
                  deposit_mode: int = JEFI_DEPOSIT_AUTO, sort_every: int = 8, delay_rule: int = JEFI_DELAY_NEAREST,
-                 shape_order: int = 1, field_chunk: int = 0, packed_fields: bool = True):
+                 shape_order: int = 1, field_chunk: int = 0, packed_fields: bool = True, field_tile: int = 0):
         import torch
 
         if not torch.cuda.is_available():
@@ -402,7 +404,7 @@ class JefiContext:
         self.stream_handle = stream
         self.handle = jefi_create(grid.nx, grid.ny, grid.nz, grid.dx, grid.dy, grid.dz, grid.dt, grid.c, grid.eps0,
                                   grid.H, grid.hist_cap, grid.Eext, grid.Bext, self.device.index or 0, stream,
-                                  field_impl, deposit_mode, delay_rule, shape_order, field_chunk)
+                                  field_impl, deposit_mode, delay_rule, shape_order, field_chunk, field_tile)
         self.info = jefi_get_info(self.handle)
         self.info["field_impl_reason"] = jefi_field_impl_reason(self.handle)
         self.tile_info = jefi_get_tile_info(self.handle)

@@ -63,6 +63,78 @@ def test_tiled_kernel_geometries_and_multipass_windows(J, rule, shape, h, kappa,
     ref.close()
 
 
+DYAD_CASES = [
+    # shape, spacing, kappa, fill, source tiles per CTA, several passes?
+    ((16, 8, 8), (1e-4, 1e-4, 1e-4), 2.0, "full", 0, False),           # one 16x8x8 tile that holds its own sources (self cells)
+    ((37, 13, 10), (1e-4, 1e-4, 1e-4), 2.0, "wrapped", 0, False),      # ragged on every axis, odd nx: the last dyad is half padding
+    ((33, 9, 17), (1e-4, 2e-4, 1.5e-4), 2.0, "early", -1, False),      # anisotropic spacings, unsplit source range
+    ((20, 20, 20), (0.3, 0.3, 0.3), 6.0, "wrapped", 0, True),          # the paper's kappa = 6 example: several passes
+    ((17, 8, 9), (1e-5, 1e-5, 1e-5), 0.334, "full", 3, False),         # the paper's slab regime: neighbouring cells at delay 0
+]
+
+
+@pytest.mark.parametrize("rule", ["NEAREST", "LINEAR"])
+@pytest.mark.parametrize("shape,h,kappa,fill,chunk,multipass", DYAD_CASES)
+def test_dyad_tiles_two_cells_per_thread(J, rule, shape, h, kappa, fill, chunk, multipass):
+    """jefi_config.field_tile = JEFI_TILE_DYAD: 16x8x8 observation tiles, a thread owns two x-neighbour cells and evaluates the
+    geometry of an offset once for the pairs (r, r') and (r + ex, r' + ex).  Same pairs, same sums as the oracle; the one-cell
+    geometry on the same history agrees too."""
+    c = 1.0 if h[0] > 1e-2 else C
+    kw = dict(c=1.0, eps0=1.0) if c == 1.0 else {}
+    dt = h[0] / (kappa * c)
+    cfg = OracleConfig(*shape, *h, dt, delay_rule=getattr(oracle, "RULE_" + rule), **kw)
+    nsteps = {"full": cfg.H, "early": max(3, cfg.H // 3), "wrapped": 2 * cfg.H + 3}[fill]
+    slices = [wl.history_slice(cfg.N, t, 4242, j_scale=c) for t in range(nsteps)]
+    Eo, Bo = oracle_history(cfg, slices)
+    for tile, want in ((J.JEFI_TILE_DYAD, (16, 8, 8)), (J.JEFI_TILE_CELL, (8, 8, 8))):
+        ctx = J.JefiContext(J.GridSpec(*shape, *h, dt, **kw), field_impl=J.JEFI_FIELD_TILED, delay_rule=getattr(J, "JEFI_DELAY_" + rule),
+                            field_tile=tile, field_chunk=chunk)
+        ti = ctx.tile_info
+        assert ctx.info["field_impl"] == J.JEFI_FIELD_TILED and ti["obs_tile"] == want, (ctx.info["field_impl_reason"], ti)
+        if tile == J.JEFI_TILE_DYAD:
+            assert (ti["window_slots"] > ti["window_pitch"]) == multipass, ti
+        E, B = run_history(J, ctx, slices)
+        assert_field_parity(E, B, Eo, Bo, f"{shape} kappa {kappa} {rule} tile {want}: ")
+        ctx.close()
+
+
+def test_dyad_tiles_slabs_and_automatic_choice(J):
+    """Observation slabs of the 16x8x8 geometry assemble the full step bit for bit; a slab meets the oracle directly; the
+    automatic choice takes dyads only on grids with at least four waves of 16x8x8 tiles."""
+    import torch
+
+    shape, dx = (32, 16, 24), 1e-4
+    dt = dx / (2 * C)
+    cfg = OracleConfig(*shape, dx, dx, dx, dt)
+    slices = [wl.history_slice(cfg.N, t, 99, j_scale=C) for t in range(cfg.H + 2)]
+    Eo, Bo = oracle_history(cfg, slices)
+    ctx = J.JefiContext(J.GridSpec(*shape, dx, dx, dx, dt), field_impl=J.JEFI_FIELD_TILED, field_tile=J.JEFI_TILE_DYAD)
+    assert ctx.tile_info["obs_tile"] == (16, 8, 8)
+    for s in slices:
+        ctx.push_sources(torch.from_numpy(s).to(ctx.device))
+    full = ctx.field_step().clone()
+    e = full.cpu().numpy()
+    assert_field_parity(e[:3], e[3:], Eo, Bo, "dyad 32x16x24: ")
+    plane = shape[0] * shape[1]
+    asm = torch.full_like(full, float("nan"))
+    for r in range(3):
+        k0, k1 = ctx.slab_range(r, 3)
+        part = torch.full_like(full, -7.0)
+        ctx.field_step_slab(k0, k1, part)
+        assert bool((part[:, :plane * k0] == -7.0).all()) and bool((part[:, plane * k1:] == -7.0).all())
+        asm[:, plane * k0:plane * k1] = part[:, plane * k0:plane * k1]
+        if r == 1:  # this slab against the oracle itself
+            got = part[:, plane * k0:plane * k1].cpu().numpy()
+            assert_field_parity(got[:3], got[3:], Eo[:, plane * k0:plane * k1], Bo[:, plane * k0:plane * k1], f"dyad slab [{k0},{k1}): ")
+    assert torch.equal(asm, full)
+    ctx.close()
+    auto = J.JefiContext(J.GridSpec(*shape, dx, dx, dx, dt))
+    assert auto.tile_info["obs_tile"] == (8, 8, 8)  # 2 x 2 x 3 dyad tiles: far fewer than four waves of SMs
+    auto.close()
+    with pytest.raises(J.JefiError):
+        J.JefiContext(J.GridSpec(8, 8, 8, dx, dx, dx, dt), field_tile=7)
+
+
 def test_thin_grid_slabs_and_light_cone(J):
     """1 x 40 x 70: observation slabs in units of the thin tile's z edge (32) assemble the full step bit for bit; a source
     switched on at step n0 leaves every cell outside its light cone exactly zero."""
