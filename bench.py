@@ -43,7 +43,9 @@ FLOP_PER_PAIR = 48.0  # 24 FMA per source-observation pair
 # and the sha1 (first 12 hex digits) of csrc/jefi_field.cu + csrc/jefi_ctx.h of that build.  With a different kernel source
 # `traffic` is null and `traffic_source` says the capture is stale.
 FIELD_DRAM_BYTES = {
-    # (workload name, rule): (bytes, profile, kernel source sha)  -- filled from profiles/r2_*_ncu_full.md
+    # (workload name, rule): (bytes, profile, kernel source sha)
+    ("cfg4_96c_field_only", "nearest"): (264.339052e9 + 51.057920e6, "profiles/r2c_field_tiled_ncu_full.md", "d6a44ef75e6a"),
+    ("cfg4_96c_field_only", "linear"): (111.224354e9 + 52.626432e6, "profiles/r2c_field_tiled_ncu_full.md", "d6a44ef75e6a"),
 }
 
 
@@ -489,7 +491,10 @@ def run_product(args, w: wl.FieldWorkload) -> dict:
     checksum = float(eb_pin[:N].double().abs().sum())
 
     # measured FP32 pipe throughput of this GPU, in this run (scalar FFMA chains and packed FFMA2 chains)
-    probe = {"ffma": J.jefi_debug_fp32_peak(ctx.handle, False), "ffma2": J.jefi_debug_fp32_peak(ctx.handle, True)} if rank == 0 else None
+    probe = ({"ffma": J.jefi_debug_fp32_peak(ctx.handle, 0), "ffma2": J.jefi_debug_fp32_peak(ctx.handle, 1),
+              "ffma_3reg": J.jefi_debug_fp32_peak(ctx.handle, 2), "ffma2_3reg": J.jefi_debug_fp32_peak(ctx.handle, 3)} if rank == 0 else None)
+    lds = ({k: J.jefi_debug_lds128_cycles(ctx.handle, i) for i, k in enumerate(("broadcast", "lane_pairs_share", "32_rows", "one_pair_differs",
+                                                                                "pairs_share_rows_8_apart"))} if rank == 0 else None)
     impl, reason, tiles = ctx.info["field_impl"], ctx.info["field_impl_reason"], ctx.tile_info
     ctx.close()
     del flush
@@ -515,9 +520,13 @@ def run_product(args, w: wl.FieldWorkload) -> dict:
                             "kernel_ms": kernel_ms, "kernel_ms_source": f"CUDA events around the field kernel of the {len(kms)} timed steps",
                             "flop_per_pair": FLOP_PER_PAIR, "peak_source": PEAK_SOURCE, "kernel_source_sha": kernel_source_sha(),
                             "peak_measured": {"ffma_tflops": probe["ffma"]["tflops"], "ffma2_tflops": probe["ffma2"]["tflops"],
+                                              "ffma_3reg_tflops": probe["ffma_3reg"]["tflops"], "ffma2_3reg_tflops": probe["ffma2_3reg"]["tflops"],
                                               "sm_count": probe["ffma"]["sm_count"],
-                                              "how": "jefi_debug_fp32_peak: 2048 threads/SM x 16 independent FMA chains, CUDA events, best of 3",
+                                              "how": "jefi_debug_fp32_peak: 2048 threads/SM x 16 independent FMA chains, CUDA events, best of 3; ffma/ffma2: multiplier "
+                                                     "and addend shared by the chains, *_3reg: three registers of its own per FMA (register-file bound)",
                                               "frac_of_measured": achieved / max(probe["ffma"]["tflops"], probe["ffma2"]["tflops"])}},
+               "smem_probe": {"lds128_sm_cycles": lds, "how": "jefi_debug_lds128_cycles: 16 warps/SM issuing LDS.128 only, rows per lane as named; "
+                                     "the field kernel issues 2 LDS.128 per source-observation pair"},
                "e2e": {"value": e2e_val, "unit": "Gpairs/s", "h2d_bytes_per_step": 16 * N, "d2h_bytes_per_step": 24 * N,
                        "ms_per_step": e2e_ms_max, "checksum_abs_ex": checksum},
                "gpu_launches": int(launches), "clocks": clocks}

@@ -49,8 +49,12 @@ extern "C" {
 #define JEFI_DEPOSIT_AUTO 0   /* = JEFI_DEPOSIT_RUNS (the measured best on sorted and unsorted lists) */
 #define JEFI_DEPOSIT_DIRECT 1 /* caller's order; lanes of a warp that hit the same node are combined wherever they sit (match-any) */
 #define JEFI_DEPOSIT_SORTED 2 /* internal counting sort by cell (context scratch, every call), then JEFI_DEPOSIT_RUNS over that order */
-#define JEFI_DEPOSIT_RUNS 3   /* caller's order; runs of neighbouring lanes in the same cell are combined by a segmented shuffle
-                                 reduction: one reduction per (warp, cell, node) when the list is cell-sorted (jefi_sort_particles) */
+#define JEFI_DEPOSIT_RUNS 3   /* caller's order; runs of neighbouring lanes in the same cell are combined before the fp32 reductions
+                                 leave the SM: one reduction per (warp, cell, node, quantity) when the list is cell-sorted
+                                 (jefi_sort_particles).  Two kernels do this (segmented shuffle reduction; transposition through
+                                 shared memory, one 32-lane reduction per run); the context takes the first while the caller's
+                                 list was sorted by jefi_sort_particles within the last 64 deposits, else the second
+                                 (DESIGN.md section 6.3).  Same sums up to the order of the additions. */
 
 /* delay_rule values: how the retarded time t_r = t^n - R/c of Eq. (2.6), which is not a stored step, is served */
 #define JEFI_DELAY_NEAREST 0 /* sources and differences at the nearest stored step, m = floor(R/(c dt) + 1/2) (A1) */
@@ -82,7 +86,8 @@ typedef struct {
                            CTA on large grids; on small grids the range is split over CTAs to fill the GPU and the partial
                            sums are added by a second kernel in a fixed order); > 0 -> that many; -1 -> never split.
                            The result is deterministic (bit-identical from run to run) for every value. */
-  int field_tile;       /* tuning of the tiled field kernel: what one thread of an observation tile owns.  0 -> automatic;
+  int field_tile;       /* tuning of the tiled field kernel: what one thread of an observation tile owns.  0 -> automatic (dyads
+                           once the grid has at least one 16x8x8 tile per SM);
                            1 -> JEFI_TILE_CELL: one cell (8x8x8 tiles); 2 -> JEFI_TILE_DYAD: two cells that are neighbours along x
                            (16x8x8 tiles; needs nx >= 16): the pairs (r, r') and (r + ex, r' + ex) have the same offset, so their
                            distance, delay and geometric factors are evaluated once for both.  Ignored on nx <= 3 grids.  Every
@@ -215,10 +220,19 @@ float jefi_field_kernel_ms(jefi_ctx* ctx, int calls_back);
  * stages with NaN before refilling them.  errors_host = HOST long[4] of violation counts since the library was loaded;
  * returns 1 in a checked build, 0 (JEFI_OK, counters always zero) in the normal one, < 0 on error.  Synchronises. */
 int jefi_debug_check_errors(jefi_ctx* ctx, long errors_host[4]);
-/* FP32 roofline probe: all SMs run independent register-resident FMA chains (packed = 0: scalar fma.rn.f32, 1: fma.rn.f32x2),
- * timed with CUDA events on the context's stream; *tflops_out = 2 * FMAs / time (HOST double), *sm_count_out the SM count
- * (optional).  This is the measured denominator next to the derived 148 x 128 x 2 x clock figure. */
-int jefi_debug_fp32_peak(jefi_ctx* ctx, int packed, double* tflops_out, int* sm_count_out);
+/* FP32 roofline probe: all SMs run independent register-resident FMA chains, timed with CUDA events on the context's stream;
+ * *tflops_out = 2 * FMAs / time (HOST double), *sm_count_out the SM count (optional).  mode 0: scalar fma.rn.f32 whose
+ * multiplier and addend are shared by all chains (the pipe itself); 1: the same with fma.rn.f32x2 (SASS FFMA2); 2 and 3: scalar /
+ * packed chains in which every FMA reads three registers of its own (the register-file side of the pipe, which is what
+ * bounds the field kernel).  Mode 0 is the measured denominator next to the derived
+ * 148 x 128 x 2 x clock figure.  JEFI_EINVAL for any other mode. */
+int jefi_debug_fp32_peak(jefi_ctx* ctx, int mode, double* tflops_out, int* sm_count_out);
+/* Shared-memory delivery probe: SM cycles (at the maximum SM clock) one warp-wide LDS.128 costs the data pipe when the 32 lanes
+ * read ring rows in a given pattern; 16 warps per SM issue nothing else.  pattern 0: all lanes one quad; 1: lane pairs
+ * (2k, 2k+1) share a quad, 16 rows; 2: 32 rows; 3: as 1 but one pair differs; 4: as 1 with rows 8 slots apart inside a
+ * half-warp (same 16-byte bank group).  *cycles_out is a HOST double.  This is the second roofline of the field kernel
+ * (two LDS.128 per source-observation pair).  JEFI_EINVAL for any other pattern. */
+int jefi_debug_lds128_cycles(jefi_ctx* ctx, int pattern, double* cycles_out);
 /* m for every non-negative offset (a,b,c): m_out[a + nx*(b + ny*c)], HOST int array of N entries (SURVEY.md §8(b) sketched
  * short*; delays reach the history cap of 10000 and the device table is int, so int it is). */
 int jefi_debug_delay_table(jefi_ctx* ctx, int* m_out_host);

@@ -78,6 +78,8 @@ extern "C" int jefi_create(const jefi_config* cfg, jefi_ctx** out) {
   c->sort_count = c->sort_offset = c->sort_sums = nullptr;
   c->sort_key = c->sort_rank = c->sort_order = nullptr;
   c->sort_cap = 0;
+  c->sorted_np = -1;
+  c->deposits_since_sort = 0;
   c->sort_buf = nullptr;
   c->eb_pack = nullptr;
   for (int i = 0; i < JEFI_NEVENTS; i++) c->ev0[i] = c->ev1[i] = nullptr;
@@ -109,11 +111,12 @@ extern "C" int jefi_create(const jefi_config* cfg, jefi_ctx** out) {
   jefi_dims& d = c->dims;
   d.nx = cfg->nx; d.ny = cfg->ny; d.nz = cfg->nz;
   // tile geometry: cubes, or x-thin tiles for the paper's 1 x ny x nz slabs
-  // (field_tile): two x-neighbour cells per thread once the grid has enough 16x8x8 tiles to fill the GPU several times
+  // (field_tile): two x-neighbour cells per thread once the grid has at least one 16x8x8 tile per SM (measured on B200, kernel ms
+  // of one step, 8x8x8 / 16x8x8 tiles: 32^3 1.068 / 1.072, 48^3 11.38 / 11.31, 64^3 63.2 / 61.4, 80^3 248.3 / 229.5, 96^3 741 / 692)
   int nsm_ = 148;
   cudaDeviceGetAttribute(&nsm_, cudaDevAttrMultiProcessorCount, cfg->device);
   const long ndyad = (long)((cfg->nx + 15) / 16) * ((cfg->ny + 7) / 8) * ((cfg->nz + 7) / 8);
-  const bool dyad = cfg->nx >= 16 && (cfg->field_tile == JEFI_TILE_DYAD || (cfg->field_tile == JEFI_TILE_AUTO && ndyad >= 4L * nsm_));
+  const bool dyad = cfg->nx >= 16 && (cfg->field_tile == JEFI_TILE_DYAD || (cfg->field_tile == JEFI_TILE_AUTO && ndyad >= (long)nsm_));
   c->tile_geom = cfg->nx <= 3 ? JEFI_GEOM_SLABX : (dyad ? JEFI_GEOM_DYAD : JEFI_GEOM_CUBE);
   if (c->tile_geom == JEFI_GEOM_SLABX) {
     d.tsx = jefi_geom_slabx::TSX; d.tsy = jefi_geom_slabx::TSY; d.tsz = jefi_geom_slabx::TSZ;

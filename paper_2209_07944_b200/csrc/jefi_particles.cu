@@ -291,6 +291,95 @@ __global__ void __launch_bounds__(256) k_deposit_sorted(int nx, int ny, int nz, 
       }
 }
 
+// ------------------------------------------------------------------------------------------------------------
+// Run deposit for S^(1), transposed through shared memory (JEFI_DEPOSIT_RUNS on lists the context does not know to be sorted).
+//
+// Phase 1, lane = particle: the 8 node weights x (rho, Jx, Jy, Jz) = 32 contributions of the particle go to the warp's
+// shared-memory tile V[value][particle] (pitch 33 floats: conflict-free both ways), with the particle's base node as a linear
+// index and the 8-bit mask of its nodes that lie inside the grid.
+// Phase 2, lane = value (node = lane / 4, quantity = lane % 4): the lane adds its value over the particles of the warp in
+// order and, at the end of every run of equal base nodes (warp-uniform: the ballot of run heads), issues ONE reduction for
+// (run, node, quantity).  So a run costs one 32-lane RED instruction whose lanes hit the 8 nodes of one cell in the four
+// grids (x-neighbour nodes share a sector), instead of 32 RED instructions with one active lane per run, and the
+// 32 x 5 segmented shuffle steps of k_deposit_sorted become 32 conflict-free LDS + FADD.  Correct for any particle order
+// (an unsorted list simply has 32 runs per warp).  Sums inside a run are taken in lane order.
+// ------------------------------------------------------------------------------------------------------------
+constexpr int DEP_WARPS = 8, DEP_PITCH = 33, DEP_TILE = 32 * DEP_PITCH + 64;  // floats per warp: V[32][33], base[32], mask[32]
+__global__ void __launch_bounds__(32 * DEP_WARPS) k_deposit_runs(int nx, int ny, int nz, float inv_dV, float cc, long np,
+                                                                 const unsigned* __restrict__ n_alive, const int* __restrict__ order,
+                                                                 const unsigned char* __restrict__ alive, const float* __restrict__ x,
+                                                                 const float* __restrict__ y, const float* __restrict__ z,
+                                                                 const float* __restrict__ ux, const float* __restrict__ uy,
+                                                                 const float* __restrict__ uz, const float* __restrict__ qw,
+                                                                 float* __restrict__ rho, float* __restrict__ jx,
+                                                                 float* __restrict__ jy, float* __restrict__ jz) {
+  __shared__ float tile[DEP_WARPS][DEP_TILE];
+  const long t = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  const long na = order ? (long)*n_alive : np;
+  if (((long)blockIdx.x * blockDim.x + (threadIdx.x & ~31)) >= na) return;  // whole warp beyond the last particle
+  const unsigned FULL = 0xffffffffu, lane = threadIdx.x & 31;
+  float* V = tile[threadIdx.x >> 5];
+  int* Bs = reinterpret_cast<int*>(V + 32 * DEP_PITCH);
+  unsigned* Ms = reinterpret_cast<unsigned*>(Bs + 32);
+  bool live = t < na;
+  int kk = -2 - (int)lane;  // padding lanes and non-depositing particles: unique keys, never merged
+  axis_stencil<1> sx, sy, sz;
+  sx.set(0.f); sy.set(0.f); sz.set(0.f);
+  float r0 = 0, vx = 0, vy = 0, vz = 0;
+  long p = t;
+  if (live) {
+    if (order) p = order[t];
+    else live = alive == nullptr || alive[p] != 0;
+  }
+  if (live) {
+    sx.set(x[p]); sy.set(y[p]); sz.set(z[p]);
+    int k2;  // a particle with no node inside the grid keeps its unique negative key (see k_deposit_sorted)
+    if (base_key<1>(nx, ny, nz, sx.i0, sy.i0, sz.i0, k2)) kk = k2;
+    else live = false;
+  }
+  if (live) {
+    float u0 = ux[p], u1 = uy[p], u2 = uz[p];
+    float ig = rsqrtf(1.f + u0 * u0 + u1 * u1 + u2 * u2);
+    vx = cc * u0 * ig; vy = cc * u1 * ig; vz = cc * u2 * ig;
+    r0 = qw[p] * inv_dV;
+  }
+  const int kprev = __shfl_up_sync(FULL, kk, 1);
+  const unsigned heads = __ballot_sync(FULL, lane == 0 || kprev != kk);  // bit l: lane l starts a run
+  unsigned inside = 0;
+#pragma unroll
+  for (int c = 0; c < 2; c++)
+#pragma unroll
+    for (int b = 0; b < 2; b++)
+#pragma unroll
+      for (int a = 0; a < 2; a++) {
+        const int node = a + 2 * b + 4 * c;
+        const float a0 = r0 * (sx.w[a] * sy.w[b] * sz.w[c]);  // Eq. (2.16), (2.18)
+        V[(4 * node + 0) * DEP_PITCH + lane] = a0;
+        V[(4 * node + 1) * DEP_PITCH + lane] = a0 * vx;         // Eq. (2.19)
+        V[(4 * node + 2) * DEP_PITCH + lane] = a0 * vy;
+        V[(4 * node + 3) * DEP_PITCH + lane] = a0 * vz;
+        const int ii = sx.i0 + a, jj = sy.i0 + b, kz = sz.i0 + c;
+        inside |= (live && ii >= 0 && ii < nx && jj >= 0 && jj < ny && kz >= 0 && kz < nz ? 1u : 0u) << node;  // virtual nodes dropped
+      }
+  Bs[lane] = sx.i0 + nx * (sy.i0 + ny * sz.i0);  // linear index of the base node; exact for every node that is inside
+  Ms[lane] = inside;
+  __syncwarp();
+  // phase 2: this lane owns value (node, quantity) of every run
+  const int node = (int)lane >> 2;
+  const int off = (node & 1) + nx * (((node >> 1) & 1) + ny * (node >> 2));
+  float* const arr = (lane & 3) == 0 ? rho : (lane & 3) == 1 ? jx : (lane & 3) == 2 ? jy : jz;
+  const float* Vl = V + lane * DEP_PITCH;
+  float acc = 0.f;
+#pragma unroll
+  for (int q = 0; q < 32; q++) {
+    acc += Vl[q];
+    if (q == 31 || ((heads >> (q + 1)) & 1u)) {  // warp-uniform: particle q ends a run
+      if ((Ms[q] >> node) & 1u) atomicAdd(arr + (Bs[q] + off), acc);
+      acc = 0.f;
+    }
+  }
+}
+
 static inline long sort_bins(const jefi_ctx* c) {
   const jefi_dims& d = c->dims;
   const int s = c->shape_order;  // nodes per axis - 1
@@ -372,11 +461,19 @@ int jefi_deposit_impl(jefi_ctx* c, long np, const float* x, const float* y, cons
   }
   if (np == 0) return JEFI_OK;
   float inv_dV = (float)(1.0 / (c->cfg.dx * c->cfg.dy * c->cfg.dz));
+  static_assert(32 * DEP_WARPS == 256, "one block size for every deposit kernel");
   unsigned blocks = (unsigned)((np + 255) / 256);
   int mode = c->cfg.deposit_mode;
   if (mode == JEFI_DEPOSIT_AUTO) mode = JEFI_DEPOSIT_RUNS;  // cheapest on sorted and unsorted lists alike
   const float cc = (float)c->c;
   const bool s2 = c->shape_order == 2;
+  // Two kernels combine runs of equal cells (both correct for any order).  On a cell-sorted list (a few particles per cell,
+  // most runs short) the segmented shuffle reduction of k_deposit_sorted is the cheaper one (config-5 set: 0.214 ms against
+  // 0.253 ms); on a list in arbitrary order, where every lane is its own run and the L2 reductions bind, k_deposit_runs issues one
+  // 32-lane reduction per particle covering its 8 nodes x 4 grids (half the L2 sectors: 0.82 ms against 1.44 ms).  The context
+  // takes the first when the caller's list was put in cell order by jefi_sort_particles within the last 64 deposits.
+  const bool sorted_hint = c->sorted_np == np && c->deposits_since_sort < 64;
+  if (c->deposits_since_sort < (1 << 30)) c->deposits_since_sort++;
   if (mode == JEFI_DEPOSIT_SORTED) {
     int rc = build_cell_order(c, np, x, y, z, alive);
     if (rc != JEFI_OK) return rc;
@@ -385,7 +482,8 @@ int jefi_deposit_impl(jefi_ctx* c, long np, const float* x, const float* y, cons
     else k_deposit_sorted<1><<<blocks, 256, 0, c->stream>>>(d.nx, d.ny, d.nz, inv_dV, cc, np, na, c->sort_order, alive, x, y, z, ux, uy, uz, qw, rho, jx, jy, jz);
   } else if (mode == JEFI_DEPOSIT_RUNS) {
     if (s2) k_deposit_sorted<2><<<blocks, 256, 0, c->stream>>>(d.nx, d.ny, d.nz, inv_dV, cc, np, nullptr, nullptr, alive, x, y, z, ux, uy, uz, qw, rho, jx, jy, jz);
-    else k_deposit_sorted<1><<<blocks, 256, 0, c->stream>>>(d.nx, d.ny, d.nz, inv_dV, cc, np, nullptr, nullptr, alive, x, y, z, ux, uy, uz, qw, rho, jx, jy, jz);
+    else if (sorted_hint) k_deposit_sorted<1><<<blocks, 256, 0, c->stream>>>(d.nx, d.ny, d.nz, inv_dV, cc, np, nullptr, nullptr, alive, x, y, z, ux, uy, uz, qw, rho, jx, jy, jz);
+    else k_deposit_runs<<<blocks, 32 * DEP_WARPS, 0, c->stream>>>(d.nx, d.ny, d.nz, inv_dV, cc, np, nullptr, nullptr, alive, x, y, z, ux, uy, uz, qw, rho, jx, jy, jz);
   } else {
     if (s2) k_deposit<2><<<blocks, 256, 0, c->stream>>>(d.nx, d.ny, d.nz, inv_dV, cc, np, x, y, z, ux, uy, uz, qw, alive, rho, jx, jy, jz);
     else k_deposit<1><<<blocks, 256, 0, c->stream>>>(d.nx, d.ny, d.nz, inv_dV, cc, np, x, y, z, ux, uy, uz, qw, alive, rho, jx, jy, jz);
@@ -464,6 +562,8 @@ extern "C" int jefi_sort_particles(jefi_ctx* c, long np, float* x, float* y, flo
   k_permute_copyback<<<pb, 256, 0, c->stream>>>(np, A, buf, abuf, tbuf);
   JEFI_CUDA_TRY(c, cudaGetLastError());
   c->launches += 2;
+  c->sorted_np = np;
+  c->deposits_since_sort = 0;
   return JEFI_OK;
 }
 

@@ -28,6 +28,7 @@ EXPORTS = [
     "jefi_last_field_kernel_ms", "jefi_debug_delay_table", "jefi_debug_cell_index", "jefi_debug_history_slot",
     "jefi_debug_cell_order", "jefi_sort_particles", "jefi_field_impl_reason", "jefi_get_tile_info", "jefi_field_step_packed",
     "jefi_push_particles_packed", "jefi_field_kernel_ms", "jefi_debug_fp32_peak", "jefi_debug_check_errors", "jefi_pic_step",
+    "jefi_debug_lds128_cycles",
 ]
 
 
@@ -93,6 +94,8 @@ def load_library() -> C.CDLL:
     lib.jefi_debug_check_errors.restype = C.c_int
     lib.jefi_debug_fp32_peak.argtypes = [vp, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_int)]
     lib.jefi_debug_fp32_peak.restype = C.c_int
+    lib.jefi_debug_lds128_cycles.argtypes = [vp, C.c_int, C.POINTER(C.c_double)]
+    lib.jefi_debug_lds128_cycles.restype = C.c_int
     lib.jefi_debug_delay_table.argtypes = [vp, vp]
     lib.jefi_debug_delay_table.restype = C.c_int
     lib.jefi_debug_cell_index.argtypes = [vp, C.c_long, f32p, f32p, f32p, vp]
@@ -312,11 +315,19 @@ def jefi_debug_check_errors(handle: int):
     return rc == 1, list(e)
 
 
-def jefi_debug_fp32_peak(handle: int, packed: bool = False) -> dict:
-    """Measured FP32 FMA throughput of the device (TFLOP/s) and its SM count."""
+def jefi_debug_fp32_peak(handle: int, mode: int = 0) -> dict:
+    """Measured FP32 FMA throughput of the device (TFLOP/s) and its SM count.  mode 0 / 1: scalar / packed FMA chains with
+    shared multiplier and addend; 2 / 3: scalar / packed chains reading three registers of their own per FMA (include/jefi.h)."""
     tf, nsm = C.c_double(), C.c_int()
-    _check(handle, load_library().jefi_debug_fp32_peak(handle, 1 if packed else 0, C.byref(tf), C.byref(nsm)), "jefi_debug_fp32_peak")
-    return dict(tflops=tf.value, sm_count=nsm.value, packed=bool(packed))
+    _check(handle, load_library().jefi_debug_fp32_peak(handle, int(mode), C.byref(tf), C.byref(nsm)), "jefi_debug_fp32_peak")
+    return dict(tflops=tf.value, sm_count=nsm.value, mode=int(mode))
+
+
+def jefi_debug_lds128_cycles(handle: int, pattern: int) -> float:
+    """SM cycles per warp-wide LDS.128 for an address pattern (include/jefi.h)."""
+    cyc = C.c_double()
+    _check(handle, load_library().jefi_debug_lds128_cycles(handle, int(pattern), C.byref(cyc)), "jefi_debug_lds128_cycles")
+    return cyc.value
 
 
 def jefi_debug_delay_table(handle: int, nx: int, ny: int, nz: int):

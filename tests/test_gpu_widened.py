@@ -67,7 +67,8 @@ DYAD_CASES = [
     # shape, spacing, kappa, fill, source tiles per CTA, several passes?
     ((16, 8, 8), (1e-4, 1e-4, 1e-4), 2.0, "full", 0, False),           # one 16x8x8 tile that holds its own sources (self cells)
     ((37, 13, 10), (1e-4, 1e-4, 1e-4), 2.0, "wrapped", 0, False),      # ragged on every axis, odd nx: the last dyad is half padding
-    ((33, 9, 17), (1e-4, 2e-4, 1.5e-4), 2.0, "early", -1, False),      # anisotropic spacings, unsplit source range
+    ((33, 9, 17), (1e-4, 2e-4, 1.5e-4), 2.0, "early", -1, True),       # anisotropic spacings (dy = 2 dx, dz = 1.5 dx: the 16x8x8 tile spans
+                                                                       # 63 slots, two passes), unsplit source range
     ((20, 20, 20), (0.3, 0.3, 0.3), 6.0, "wrapped", 0, True),          # the paper's kappa = 6 example: several passes
     ((17, 8, 9), (1e-5, 1e-5, 1e-5), 0.334, "full", 3, False),         # the paper's slab regime: neighbouring cells at delay 0
 ]
@@ -100,7 +101,7 @@ def test_dyad_tiles_two_cells_per_thread(J, rule, shape, h, kappa, fill, chunk, 
 
 def test_dyad_tiles_slabs_and_automatic_choice(J):
     """Observation slabs of the 16x8x8 geometry assemble the full step bit for bit; a slab meets the oracle directly; the
-    automatic choice takes dyads only on grids with at least four waves of 16x8x8 tiles."""
+    automatic choice takes dyads only on grids with at least one 16x8x8 tile per SM."""
     import torch
 
     shape, dx = (32, 16, 24), 1e-4
@@ -129,7 +130,7 @@ def test_dyad_tiles_slabs_and_automatic_choice(J):
     assert torch.equal(asm, full)
     ctx.close()
     auto = J.JefiContext(J.GridSpec(*shape, dx, dx, dx, dt))
-    assert auto.tile_info["obs_tile"] == (8, 8, 8)  # 2 x 2 x 3 dyad tiles: far fewer than four waves of SMs
+    assert auto.tile_info["obs_tile"] == (8, 8, 8)  # 2 x 2 x 3 dyad tiles: fewer than one per SM
     auto.close()
     with pytest.raises(J.JefiError):
         J.JefiContext(J.GridSpec(8, 8, 8, dx, dx, dx, dt), field_tile=7)
