@@ -87,7 +87,7 @@ typedef struct {
                            sums are added by a second kernel in a fixed order); > 0 -> that many; -1 -> never split.
                            The result is deterministic (bit-identical from run to run) for every value. */
   int field_tile;       /* tuning of the tiled field kernel: what one thread of an observation tile owns.  0 -> automatic (dyads
-                           once the grid has at least one 16x8x8 tile per SM);
+                           once the grid has 32 tiles of 16x8x8 cells and nx pads no worse than with 8-wide tiles);
                            1 -> JEFI_TILE_CELL: one cell (8x8x8 tiles); 2 -> JEFI_TILE_DYAD: two cells that are neighbours along x
                            (16x8x8 tiles; needs nx >= 16): the pairs (r, r') and (r + ex, r' + ex) have the same offset, so their
                            distance, delay and geometric factors are evaluated once for both.  Ignored on nx <= 3 grids.  Every

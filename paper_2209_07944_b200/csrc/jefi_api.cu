@@ -111,12 +111,12 @@ extern "C" int jefi_create(const jefi_config* cfg, jefi_ctx** out) {
   jefi_dims& d = c->dims;
   d.nx = cfg->nx; d.ny = cfg->ny; d.nz = cfg->nz;
   // tile geometry: cubes, or x-thin tiles for the paper's 1 x ny x nz slabs
-  // (field_tile): two x-neighbour cells per thread once the grid has at least one 16x8x8 tile per SM (measured on B200, kernel ms
-  // of one step, 8x8x8 / 16x8x8 tiles: 32^3 1.068 / 1.072, 48^3 11.38 / 11.31, 64^3 63.2 / 61.4, 80^3 248.3 / 229.5, 96^3 741 / 692)
-  int nsm_ = 148;
-  cudaDeviceGetAttribute(&nsm_, cudaDevAttrMultiProcessorCount, cfg->device);
+  // (field_tile): two x-neighbour cells per thread once the grid has 32 tiles of 16x8x8 and x does not pad much worse than with
+  // 8-wide tiles (measured on B200, kernel ms of one step, 8x8x8 / 16x8x8 tiles: 32^3 1.056 / 1.035, 48^3 11.33 / 10.99,
+  // 64^3 63.1 / 59.8, 80^3 248.1 / 223.4, 96^3 741 / 675)
   const long ndyad = (long)((cfg->nx + 15) / 16) * ((cfg->ny + 7) / 8) * ((cfg->nz + 7) / 8);
-  const bool dyad = cfg->nx >= 16 && (cfg->field_tile == JEFI_TILE_DYAD || (cfg->field_tile == JEFI_TILE_AUTO && ndyad >= (long)nsm_));
+  const bool xpad_ok = ((cfg->nx + 15) / 16) * 16 == ((cfg->nx + 7) / 8) * 8 || cfg->nx >= 64;
+  const bool dyad = cfg->nx >= 16 && (cfg->field_tile == JEFI_TILE_DYAD || (cfg->field_tile == JEFI_TILE_AUTO && ndyad >= 32 && xpad_ok));
   c->tile_geom = cfg->nx <= 3 ? JEFI_GEOM_SLABX : (dyad ? JEFI_GEOM_DYAD : JEFI_GEOM_CUBE);
   if (c->tile_geom == JEFI_GEOM_SLABX) {
     d.tsx = jefi_geom_slabx::TSX; d.tsy = jefi_geom_slabx::TSY; d.tsz = jefi_geom_slabx::TSZ;

@@ -335,9 +335,8 @@ __device__ __forceinline__ void acc_pair(const pair_geom<LINEAR>& g, pair_acc& A
 
 // Two observation cells against two source cells with ONE geometry (G::CX = 2: (cell 1, source CELL1) and (cell 0, source
 // CELL0) have the same offset).  The statements of the two pairs alternate so that the shared operands (rs, a_y, Axz, Azx) sit
-// in the same operand slot of neighbouring instructions: a register operand repeated there is served by the operand reuse
-// cache instead of the register file, whose two 32-bit reads per clock and scheduler are what bounds this kernel
-// (profiles/r2_rf_probe.md).
+// in the same operand slot of neighbouring instructions (a register operand repeated there can be served by the operand
+// reuse cache); the order was chosen by A/B on B200 like the one of acc_pair.
 template <bool LINEAR, int CELL1, int CELL0>
 __device__ __forceinline__ void acc_pair2(const pair_geom<LINEAR>& g, pair_acc& A1, pair_acc& A0) {
   quad2 S1 = lds128_imm<CELL1 * 16>(g.addr);
@@ -576,15 +575,16 @@ __global__ void __launch_bounds__(TILED_THREADS, 1) k_field_tiled(tiled_params P
     // second accumulation level.  Unit c belongs to this thread alone in this item; the previous item's updates
     // (by other threads) are complete once every consumer warp has arrived on that item's done barrier.
     if (item > 0) mbar_wait(barDone + 8 * ((item - 1) & 1), ((item - 1) >> 1) & 1);
+    const int sc = G::acc_slot(c);  // bank-spreading home of unit c's accumulators (jefi_ctx.h)
     if constexpr (G::CX == 1) {
-      accS[c] += lo32(A[0].Exz) - lo32(A[0].Fxz);
-      accS[G::CELLS + c] += A[0].Ey - A[0].Fy;
-      accS[2 * G::CELLS + c] += hi32(A[0].Exz) - hi32(A[0].Fxz);
-      accS[3 * G::CELLS + c] += lo32(A[0].Bxz) - lo32(A[0].Cxz);
-      accS[4 * G::CELLS + c] += lo32(A[0].By12) - hi32(A[0].By12);
-      accS[5 * G::CELLS + c] += hi32(A[0].Cxz) - hi32(A[0].Bxz);
+      accS[sc] += lo32(A[0].Exz) - lo32(A[0].Fxz);
+      accS[G::CELLS + sc] += A[0].Ey - A[0].Fy;
+      accS[2 * G::CELLS + sc] += hi32(A[0].Exz) - hi32(A[0].Fxz);
+      accS[3 * G::CELLS + sc] += lo32(A[0].Bxz) - lo32(A[0].Cxz);
+      accS[4 * G::CELLS + sc] += lo32(A[0].By12) - hi32(A[0].By12);
+      accS[5 * G::CELLS + sc] += hi32(A[0].Cxz) - hi32(A[0].Bxz);
     } else {  // the two cells of the unit are neighbours in the home order (x fastest): one 8-byte update per component
-      float2* a2 = reinterpret_cast<float2*>(accS) + c;
+      float2* a2 = reinterpret_cast<float2*>(accS) + sc;
       float2 v;
       v = a2[0]; v.x += lo32(A[0].Exz) - lo32(A[0].Fxz); v.y += lo32(A[1].Exz) - lo32(A[1].Fxz); a2[0] = v;
       v = a2[G::CELLS / 2]; v.x += A[0].Ey - A[0].Fy; v.y += A[1].Ey - A[1].Fy; a2[G::CELLS / 2] = v;
@@ -604,8 +604,9 @@ __global__ void __launch_bounds__(TILED_THREADS, 1) k_field_tiled(tiled_params P
     const int oi = ox0 + c % G::OBX, oj = oy0 + (c / G::OBX) % G::OBY, ok = oz0 + c / (G::OBX * G::OBY);
     if (oi < d.nx && oj < d.ny && ok < P.k1) {
       const size_t o = (size_t)oi + (size_t)d.nx * ((size_t)oj + (size_t)d.ny * ok);
-      const float vex = P.g.prefE * accS[c], vey = P.g.prefE * accS[G::CELLS + c], vez = P.g.prefE * accS[2 * G::CELLS + c];
-      const float vbx = P.g.prefB * accS[3 * G::CELLS + c], vby = P.g.prefB * accS[4 * G::CELLS + c], vbz = P.g.prefB * accS[5 * G::CELLS + c];
+      const int a = G::CX * G::acc_slot(c / G::CX) + c % G::CX;  // cell c belongs to unit c / CX (x fastest)
+      const float vex = P.g.prefE * accS[a], vey = P.g.prefE * accS[G::CELLS + a], vez = P.g.prefE * accS[2 * G::CELLS + a];
+      const float vbx = P.g.prefB * accS[3 * G::CELLS + a], vby = P.g.prefB * accS[4 * G::CELLS + a], vbz = P.g.prefB * accS[5 * G::CELLS + a];
       if (P.to_partial) {
         float* q = P.partial + (size_t)blockIdx.y * 6 * (size_t)d.N + o;
         q[0] = vex; q[d.N] = vey; q[2 * d.N] = vez; q[3 * d.N] = vbx; q[4 * d.N] = vby; q[5 * d.N] = vbz;
@@ -647,8 +648,9 @@ __global__ void __launch_bounds__(256) k_reduce_partials(long N, int nsplit, lon
 // Evaluation order of the 512 cells of an observation tile for one relative tile offset D = (ox0 - sx0, ..).
 // What it is for: an LDS.128 costs 2 data-pipe cycles instead of 4 when EVERY lane pair (2k, 2k+1) of the warp reads one
 // quad, i.e. when the two observation cells of every pair have the same delay to the source cell being evaluated.
-//   1. rank the cells by their distance to the centre of the source tile (ties in home order, x fastest): neighbours in
-//      this order are almost equidistant from every cell of the tile; consecutive cells form the 256 lane pairs;
+//   1. rank the cells by their distance to the centre of the source tile (ties in home order, x fastest); going down this order,
+//      the first free cell takes as partner the one of the next 8 free cells that agrees with it on the delay to the most source
+//      cells (equidistant AND close together): these are the 256 lane pairs;
 //   2. per pair, the 64-bit set of source cells for which its two delays differ (same fp32 delay arithmetic as the kernel);
 //   3. deal the pairs to the 16 warps greedily: a warp starts from the first free pair of the distance order and then takes,
 //      15 times, the free pair among the next `band` pairs that adds the fewest new cells to the union of its pairs' sets
@@ -665,6 +667,9 @@ __global__ void __launch_bounds__(OBCELLS) k_build_perm(int ndx, int ndy, int nt
   __shared__ unsigned long long mask[G::CX][OBCELLS / 2];
   __shared__ unsigned short picked[OBCELLS / 2];
   __shared__ unsigned red[2][OBCELLS / 32];
+  __shared__ unsigned short pairU[OBCELLS];  // units of lane pair p: pairU[2p], pairU[2p+1]
+  __shared__ unsigned char usedr[OBCELLS];   // by position in the distance order
+  __shared__ int cand[8];
   const int c = threadIdx.x;  // unit (G::CX cells along x) in home order
   const int ix = blockIdx.x % ndx, iy = (blockIdx.x / ndx) % ndy, iz = blockIdx.x / (ndx * ndy);
   const int Dxi = G::TSX * (ix - (ntx - 1)), Dyi = G::TSY * (iy - (nty - 1)), Dzi = G::TSZ * (iz - (ntz - 1));
@@ -681,13 +686,60 @@ __global__ void __launch_bounds__(OBCELLS) k_build_perm(int ndx, int ndy, int nt
   }
   order[pos] = (unsigned short)c;
   __syncthreads();
-  // 2. pair c = units order[2c], order[2c+1]: source cells whose delay differs between the two, per cell of the unit
+  // 1b. lane pairs.  Unit `a` = the first free unit of the distance order; its partner = the one of the next 8 free units whose
+  // delays agree with a's on the most source cells (ties: the nearer in the order).  Equal distance to the tile's centre makes
+  // the delays to the centre agree; how they vary over the 64 source cells depends on how far apart the two units are, which the
+  // distance order alone does not see.  8 groups of 64 threads: group = candidate, thread = source cell.
+  {
+    const int grp = c >> 6, sc = c & 63;
+    const int lx = sc % G::TSX, ly = (sc / G::TSX) % G::TSY, lz = sc / (G::TSX * G::TSY);
+    usedr[c] = 0;
+    __syncthreads();
+    int head = 0;
+    for (int p = 0; p < OBCELLS / 2; p++) {
+      while (usedr[head]) head++;  // the same in every thread (shared flags, read after the barrier below)
+      int found = -1;
+      for (int j = head + 1, cnt = -1; j < OBCELLS; j++)
+        if (!usedr[j] && ++cnt == grp) { found = j; break; }
+      unsigned bits = 0;
+      if (found >= 0) {
+        const int a = order[head], b = order[found];
+        const int axc = G::CX * (a % G::UX), ayc = (a / G::UX) % G::OBY, azc = a / (G::UX * G::OBY);
+        const int bxc = G::CX * (b % G::UX), byc = (b / G::UX) % G::OBY, bzc = b / (G::UX * G::OBY);
+#pragma unroll
+        for (int i = 0; i < G::CX; i++) {
+          const float qa = jefi_q_fp32(g.kx, g.ky, g.kz, (float)(Dxi + axc + i - lx), (float)(Dyi + ayc - ly), (float)(Dzi + azc - lz));
+          const float qb = jefi_q_fp32(g.kx, g.ky, g.kz, (float)(Dxi + bxc + i - lx), (float)(Dyi + byc - ly), (float)(Dzi + bzc - lz));
+          const int ma = qa > 0.f ? jefi_delay_fp32(qa) : 0, mb = qb > 0.f ? jefi_delay_fp32(qb) : 0;
+          bits += (ma != mb) ? 1u : 0u;
+        }
+      }
+      const unsigned tot = __reduce_add_sync(0xffffffffu, bits);
+      if ((c & 31) == 0) red[0][c >> 5] = tot;
+      if (sc == 0) cand[grp] = found;
+      __syncthreads();
+      unsigned best = 0xffffffffu;
+#pragma unroll
+      for (int q = 0; q < 8; q++)
+        if (cand[q] >= 0) best = min(best, ((red[0][2 * q] + red[0][2 * q + 1]) << 16) | (unsigned)cand[q]);
+      const int partner = (int)(best & 0xffffu);
+      __syncthreads();  // everyone has read red / cand / usedr of this step
+      if (c == 0) {
+        pairU[2 * p] = order[head];
+        pairU[2 * p + 1] = order[partner];
+        usedr[head] = 1;
+        usedr[partner] = 1;
+      }
+      __syncthreads();
+    }
+  }
+  // 2. pair c = units pairU[2c], pairU[2c+1]: source cells whose delay differs between the two, per cell of the unit
   unsigned long long mine[G::CX];
 #pragma unroll
   for (int i = 0; i < G::CX; i++) mine[i] = 0;
   bool avail = c < OBCELLS / 2;
   if (avail) {
-    const int a = order[2 * c], b = order[2 * c + 1];
+    const int a = pairU[2 * c], b = pairU[2 * c + 1];
     const int axc = G::CX * (a % G::UX), ayc = (a / G::UX) % G::OBY, azc = a / (G::UX * G::OBY);
     const int bxc = G::CX * (b % G::UX), byc = (b / G::UX) % G::OBY, bzc = b / (G::UX * G::OBY);
     for (int sc = 0; sc < JEFI_TCELLS; sc++) {
@@ -751,7 +803,7 @@ __global__ void __launch_bounds__(OBCELLS) k_build_perm(int ndx, int ndy, int nt
     }
   }
   __syncthreads();
-  perm[(size_t)blockIdx.x * OBCELLS + c] = order[2 * picked[c >> 1] + (c & 1)];
+  perm[(size_t)blockIdx.x * OBCELLS + c] = pairU[2 * picked[c >> 1] + (c & 1)];
 }
 
 // window pitches the kernel is compiled for (ring rows per stage); a wider window is served in several passes

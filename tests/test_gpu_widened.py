@@ -101,7 +101,7 @@ def test_dyad_tiles_two_cells_per_thread(J, rule, shape, h, kappa, fill, chunk, 
 
 def test_dyad_tiles_slabs_and_automatic_choice(J):
     """Observation slabs of the 16x8x8 geometry assemble the full step bit for bit; a slab meets the oracle directly; the
-    automatic choice takes dyads only on grids with at least one 16x8x8 tile per SM."""
+    automatic choice takes dyads only on grids with at least 32 tiles of 16x8x8 cells."""
     import torch
 
     shape, dx = (32, 16, 24), 1e-4
@@ -130,7 +130,7 @@ def test_dyad_tiles_slabs_and_automatic_choice(J):
     assert torch.equal(asm, full)
     ctx.close()
     auto = J.JefiContext(J.GridSpec(*shape, dx, dx, dx, dt))
-    assert auto.tile_info["obs_tile"] == (8, 8, 8)  # 2 x 2 x 3 dyad tiles: fewer than one per SM
+    assert auto.tile_info["obs_tile"] == (8, 8, 8)  # 2 x 2 x 3 dyad tiles: fewer than 32
     auto.close()
     with pytest.raises(J.JefiError):
         J.JefiContext(J.GridSpec(8, 8, 8, dx, dx, dx, dt), field_tile=7)
