@@ -82,9 +82,10 @@ typedef struct {
   int shape_order;      /* particle shape function of jefi_deposit / jefi_push_particles: 0 or 1 -> S^(1), the linear (CIC,
                            volume-weighted) weights the paper uses, Eqs. (2.13), (2.16), (2.20); 2 -> S^(2), the quadratic
                            spline of Eq. (2.14) on 27 nodes (DESIGN.md section 3 A11) */
-  int field_chunk;      /* tuning of the tiled field kernel: source tiles per CTA.  0 -> automatic (whole source range per
-                           CTA on large grids; on small grids the range is split over CTAs to fill the GPU and the partial
-                           sums are added by a second kernel in a fixed order); > 0 -> that many; -1 -> never split.
+  int field_chunk;      /* tuning of the tiled field kernel: source tiles per CTA.  0 -> automatic (the range is
+                           split over CTAs, into 32 pieces on large grids for L2 locality and to fill the GPU on small ones;
+                           the partial sums, 24 N bytes per piece in context scratch, are added by a second kernel in a
+                           fixed order); > 0 -> that many; -1 -> never split.
                            The result is deterministic (bit-identical from run to run) for every value. */
   int field_tile;       /* tuning of the tiled field kernel: what one thread of an observation tile owns.  0 -> automatic (dyads
                            once the grid has 32 tiles of 16x8x8 cells and nx pads no worse than with 8-wide tiles);

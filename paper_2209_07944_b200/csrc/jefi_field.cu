@@ -831,13 +831,17 @@ static size_t tiled_smem_for(int wp, int cells) {
   return wp == 36 ? stage_layout<36, 512>::TOTAL : stage_layout<48, 512>::TOTAL;
 }
 
-// How the source range is split over blockIdx.y.  A CTA per observation tile walking ALL source tiles needs no second
-// kernel; that is used once there are at least four waves of observation tiles.  Smaller grids split the source tiles so
-// that the CTAs fill whole waves of the GPU: cost model = waves x (tiles per CTA + c0), c0 = 1.5 tiles of fixed cost per CTA
+// How the source range is split over blockIdx.y.  Grids with at least four waves of observation tiles use 32 pieces (L2
+// locality, below).  Smaller grids split the source tiles so that the CTAs fill whole waves of the GPU: cost model = waves x (tiles per CTA + c0), c0 = 1.5 tiles of fixed cost per CTA
 // (accumulator zeroing, barrier set-up, first copy latency, epilogue).
 static void choose_split(int nobs, int ntiles, int nsm, int request, int& chunk, int& nsplit) {
-  if (request == -1 || (request == 0 && nobs >= 4 * nsm)) {
+  if (request == -1) {
     chunk = ntiles;
+  } else if (request == 0 && nobs >= 4 * nsm) {
+    // Large grids: 32 pieces.  CTAs are scheduled blockIdx.y-major, so all observation tiles work through the same 1/32 of the
+    // ring before any moves on, and the windows they fetch overlap in L2 (96^3: 1 / 8 / 32 / 128 pieces = 670.8 / 656.8 / 653.2 /
+    // 652.6 ms including k_reduce_partials; the partial sums take 24 N bytes per piece).
+    chunk = (ntiles + 31) / 32;
   } else if (request > 0) {
     chunk = request < ntiles ? request : ntiles;
   } else {

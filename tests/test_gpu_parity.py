@@ -605,3 +605,24 @@ def test_error_paths(J):
     assert lib.jefi_field_step(None, None, None, None, None, None, None) == J.JEFI_EINVAL
     lib.jefi_destroy(None)  # NULL is a no-op
     ctx.close()
+
+
+def test_roofline_probes_report_plausible_numbers(J):
+    """jefi_debug_fp32_peak / jefi_debug_lds128_cycles (the denominators bench.py prints next to the derived FP32 peak): the FMA
+    pipe delivers most of 148 x 128 x 2 x clock, an LDS.128 costs the data pipe about 2 cycles when every lane pair shares a quad
+    and about 4 when one pair differs, and out-of-range modes are refused."""
+    n, dx = 4, 1e-4
+    ctx = make_ctx(J, (n, n, n), (dx, dx, dx), dx / (2 * C), J.JEFI_FIELD_AUTO)
+    derived = 148 * 128 * 2 * 1.965e9 / 1e12
+    for mode in range(4):
+        r = J.jefi_debug_fp32_peak(ctx.handle, mode)
+        assert r["sm_count"] >= 100 and 0.5 * derived < r["tflops"] < 1.1 * derived, (mode, r)
+    cyc = [J.jefi_debug_lds128_cycles(ctx.handle, p) for p in range(5)]
+    assert 1.5 < cyc[0] < 2.8 and 1.5 < cyc[1] < 2.8 and 3.2 < cyc[2] < 5.5 and 3.2 < cyc[3] < 5.5 and cyc[4] > cyc[1], cyc
+    lib = J.load_library()
+    import ctypes
+
+    out = ctypes.c_double()
+    assert lib.jefi_debug_fp32_peak(ctx.handle, 4, ctypes.byref(out), None) == J.JEFI_EINVAL
+    assert lib.jefi_debug_lds128_cycles(ctx.handle, 5, ctypes.byref(out)) == J.JEFI_EINVAL
+    ctx.close()
