@@ -39,11 +39,12 @@ struct jefi_tile_geom {
   static_assert(CX_ == 1 || (CX_ == 2 && TSX_ == 4), "CX = 2 is written for 4-wide source rows");
   // Where unit u (home order, x fastest) keeps its second-level accumulators in shared memory: a rotation of the low index bits
   // by the high ones.  The 32 units a warp evaluates for one source tile are (nearly) equidistant from it, i.e. they lie on a
-  // plane through the observation tile; in home order a plane x = const puts them in 2 (CX = 2) or 4 (CX = 1) of the banks an
-  // 8-byte (4-byte) access spreads over, so the read-modify-write of every item was replayed ~4 times.  With the rotation the
-  // units of a plane of any axis orientation fall evenly on all banks.
+  // plane through the observation tile, and neighbours in the evaluation order are neighbours on that plane; in home order a
+  // plane x = const puts them all in one or two of the 8 bank groups a quarter-warp's 16-byte accesses spread over (CX = 2,
+  // 48 bytes per unit) or in 4 of the 32 banks (CX = 1, 4-byte accesses), so the read-modify-write of every item was replayed
+  // ~4 times.  With the rotation the units of a plane of any axis orientation fall evenly on all banks.
   __host__ __device__ static constexpr int acc_slot(int u) {
-    if (CX_ == 2) return (u & ~15) | ((u + (u >> 4)) & 15);                              // u = ux + 8 cy + 64 cz: + (cy >> 1) + 4 cz
+    if (CX_ == 2) return (u & ~7) | ((u + (u >> 3) + 2 * (u >> 6)) & 7);                // u = ux + 8 cy + 64 cz: low bits (ux + cy + 2 cz) mod 8
     if (OBX_ == 8) return (u & ~31) | ((u + 9 * (u >> 6) + 4 * ((u >> 5) & 1)) & 31);   // u = cx + 8 cy + 64 cz: + 9 cz + 4 (cy >> 2)
     return u;
   }

@@ -121,8 +121,8 @@ int jefi_launch_field_reference(jefi_ctx* c, int k0, int k1, float* ex, float* e
 // every lane l reads the same address as lane l^1.  Which lane evaluates which observation cell is free (any assignment
 // gives the same sums), so for every source tile the 512 cells are taken in an order tabulated per relative tile offset
 // (k_build_perm): neighbouring lanes then mostly share a slot.  Per-tile partial sums are added to a shared-memory
-// accumulator [6][512] (second level of the two-level accumulation), because a cell is evaluated by a different thread
-// in every tile; the `done` barrier of item-1 orders these updates between items.
+// accumulator (6 sums per cell: [6][512] for one-cell units, [512][12] for dyads; second level of the two-level accumulation),
+// because a cell is evaluated by a different thread in every tile; the `done` barrier of item-1 orders these updates between items.
 // ------------------------------------------------------------------------------------------------------------
 constexpr int OBCELLS = 512;
 constexpr int NCONS = 512;  // consumer threads = observation cells of a tile
@@ -583,15 +583,24 @@ __global__ void __launch_bounds__(TILED_THREADS, 1) k_field_tiled(tiled_params P
       accS[3 * G::CELLS + sc] += lo32(A[0].Bxz) - lo32(A[0].Cxz);
       accS[4 * G::CELLS + sc] += lo32(A[0].By12) - hi32(A[0].By12);
       accS[5 * G::CELLS + sc] += hi32(A[0].Cxz) - hi32(A[0].Bxz);
-    } else {  // the two cells of the unit are neighbours in the home order (x fastest): one 8-byte update per component
-      float2* a2 = reinterpret_cast<float2*>(accS) + sc;
-      float2 v;
-      v = a2[0]; v.x += lo32(A[0].Exz) - lo32(A[0].Fxz); v.y += lo32(A[1].Exz) - lo32(A[1].Fxz); a2[0] = v;
-      v = a2[G::CELLS / 2]; v.x += A[0].Ey - A[0].Fy; v.y += A[1].Ey - A[1].Fy; a2[G::CELLS / 2] = v;
-      v = a2[2 * (G::CELLS / 2)]; v.x += hi32(A[0].Exz) - hi32(A[0].Fxz); v.y += hi32(A[1].Exz) - hi32(A[1].Fxz); a2[2 * (G::CELLS / 2)] = v;
-      v = a2[3 * (G::CELLS / 2)]; v.x += lo32(A[0].Bxz) - lo32(A[0].Cxz); v.y += lo32(A[1].Bxz) - lo32(A[1].Cxz); a2[3 * (G::CELLS / 2)] = v;
-      v = a2[4 * (G::CELLS / 2)]; v.x += lo32(A[0].By12) - hi32(A[0].By12); v.y += lo32(A[1].By12) - hi32(A[1].By12); a2[4 * (G::CELLS / 2)] = v;
-      v = a2[5 * (G::CELLS / 2)]; v.x += hi32(A[0].Cxz) - hi32(A[0].Bxz); v.y += hi32(A[1].Cxz) - hi32(A[1].Bxz); a2[5 * (G::CELLS / 2)] = v;
+    } else {
+      // dyads keep their 12 sums together (48 bytes per unit: Ex0 Ex1 Ey0 Ey1 | Ez0 Ez1 Bx0 Bx1 | By0 By1 Bz0 Bz1): three
+      // 16-byte read-modify-writes.  A 16-byte access is served per quarter-warp, and 8 permuted units collide on fewer of the 8
+      // bank groups ((3 sc + k) mod 8) than 16 units do on the 16 bank pairs of an 8-byte access.
+      float4* a4 = reinterpret_cast<float4*>(accS) + 3 * sc;
+      float4 v;
+      v = a4[0];
+      v.x += lo32(A[0].Exz) - lo32(A[0].Fxz); v.y += lo32(A[1].Exz) - lo32(A[1].Fxz);
+      v.z += A[0].Ey - A[0].Fy; v.w += A[1].Ey - A[1].Fy;
+      a4[0] = v;
+      v = a4[1];
+      v.x += hi32(A[0].Exz) - hi32(A[0].Fxz); v.y += hi32(A[1].Exz) - hi32(A[1].Fxz);
+      v.z += lo32(A[0].Bxz) - lo32(A[0].Cxz); v.w += lo32(A[1].Bxz) - lo32(A[1].Cxz);
+      a4[1] = v;
+      v = a4[2];
+      v.x += lo32(A[0].By12) - hi32(A[0].By12); v.y += lo32(A[1].By12) - hi32(A[1].By12);
+      v.z += hi32(A[0].Cxz) - hi32(A[0].Bxz); v.w += hi32(A[1].Cxz) - hi32(A[1].Bxz);
+      a4[2] = v;
     }
     __syncwarp();
     if (lane == 0) mbar_arrive(barDone + 8 * s);  // stage s may be refilled; this warp's accumulator updates are done
@@ -604,9 +613,11 @@ __global__ void __launch_bounds__(TILED_THREADS, 1) k_field_tiled(tiled_params P
     const int oi = ox0 + c % G::OBX, oj = oy0 + (c / G::OBX) % G::OBY, ok = oz0 + c / (G::OBX * G::OBY);
     if (oi < d.nx && oj < d.ny && ok < P.k1) {
       const size_t o = (size_t)oi + (size_t)d.nx * ((size_t)oj + (size_t)d.ny * ok);
-      const int a = G::CX * G::acc_slot(c / G::CX) + c % G::CX;  // cell c belongs to unit c / CX (x fastest)
-      const float vex = P.g.prefE * accS[a], vey = P.g.prefE * accS[G::CELLS + a], vez = P.g.prefE * accS[2 * G::CELLS + a];
-      const float vbx = P.g.prefB * accS[3 * G::CELLS + a], vby = P.g.prefB * accS[4 * G::CELLS + a], vbz = P.g.prefB * accS[5 * G::CELLS + a];
+      // cell c belongs to unit c / CX (x fastest).  CX = 1: component-major [6][cells]; CX = 2: 12 sums per unit (see above)
+      const int a = G::CX == 1 ? G::acc_slot(c) : 12 * G::acc_slot(c / G::CX) + c % G::CX;
+      constexpr int CS = G::CX == 1 ? G::CELLS : 2;  // stride between the components of a cell
+      const float vex = P.g.prefE * accS[a], vey = P.g.prefE * accS[CS + a], vez = P.g.prefE * accS[2 * CS + a];
+      const float vbx = P.g.prefB * accS[3 * CS + a], vby = P.g.prefB * accS[4 * CS + a], vbz = P.g.prefB * accS[5 * CS + a];
       if (P.to_partial) {
         float* q = P.partial + (size_t)blockIdx.y * 6 * (size_t)d.N + o;
         q[0] = vex; q[d.N] = vey; q[2 * d.N] = vez; q[3 * d.N] = vbx; q[4 * d.N] = vby; q[5 * d.N] = vbz;
