@@ -8,7 +8,8 @@ configs[3], the one the metric "G source-obs pairs/s and % FP32 peak" is quoted 
 seeded source slice already resident in HBM + jefi_field_step.  The ring (9.5 GB) is far larger than L2, so no
 L2 flush is needed between iterations (workloads whose ring would fit in L2 are timed step by step with a 512 MB fill
 in between).  `e2e` repeats it through jefi_field_step_host with pinned HOST buffers.
-`pic` adds PIC steps/s (deposit -> push_sources -> field_step -> push_particles) on configs 1, 2, 3, 5;
+`pic` adds PIC steps/s (deposit -> push_sources -> field_step -> push_particles) over BASELINE.json's whole runs of configs
+1, 2, 3, 5 from t0, and the field-kernel time with the history at full depth;
 `paper_workloads` the pairs/s of the paper's own shapes (20^3 at kappa = 6, the 1x251x111 slab).
 Reference arm (--impl reference): the fp64 CPU oracle, as it stands, on a bounded sample of the same workload.
 N > 1: one process per GPU.  Under torchrun (WORLD_SIZE set) this process is one rank; without it `--gpus N` re-executes
@@ -217,33 +218,52 @@ def aggregate_rate(world: int, pairs_per_rank: float, ms_max: float) -> float:
 def time_pic(J, torch, device, config: int, steps: int, warmup: int) -> dict:
     """PIC steps/s of one config through JefiContext.pic_step = jefi_pic_step: on its own (non-default) stream, so that a step
     is ONE CUDA-graph launch (deposit, history push, field solve with packed E/B output, particle push), particles re-sorted
-    by cell every 8 steps.  CUDA events on that stream."""
+    by cell every 8 steps.  CUDA events on that stream.
+    `steps` = BASELINE.json's run length for the config, FROM t0 (a fresh context: empty history).  The field kernel skips
+    tile pairs whose whole slot window lies before t0 (their sources are exactly zero), so a step costs what its
+    light cone holds: the whole run is timed (`steps_per_s`, the figure SURVEY.md section 8(d)(4) asks for), the last step alone
+    (`last_step_ms`), and one field step with the history filled to its full depth (`field_kernel_ms_full_history`: the rate a
+    run longer than H steps settles at).  `warmup` steps run first on a throw-away context (graph capture, module load)."""
     w = wl.WORKLOADS[config]
     side = torch.cuda.Stream(device)
     with torch.cuda.stream(side):
+        if warmup > 0:
+            wctx = J.JefiContext(J.GridSpec(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt), device=device)
+            wpart = {k: torch.from_numpy(v).to(device) for k, v in wl.particles(config).items()}
+            for _ in range(warmup):
+                wctx.pic_step(wpart)
+            side.synchronize()
+            wctx.close()
+            del wpart
         ctx = J.JefiContext(J.GridSpec(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt), device=device)
         part = {k: torch.from_numpy(v).to(device) for k, v in wl.particles(config).items()}
-        for _ in range(warmup):
-            ctx.pic_step(part)
         side.synchronize()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        evs = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
         l0 = ctx.launch_count()
-        e0.record(side)
-        for _ in range(steps):
+        evs[0].record(side)
+        for i in range(steps):
             ctx.pic_step(part)
-        e1.record(side)
+            evs[i + 1].record(side)
         side.synchronize()
-        ms = e0.elapsed_time(e1) / steps
+        total_ms = evs[0].elapsed_time(evs[steps])
+        per_step = [evs[i].elapsed_time(evs[i + 1]) for i in range(steps)]
         launches = ctx.launch_count() - l0
+        alive = int(part["alive"].sum().item())
+        # the field kernel alone with the history at full depth: H more pushes of the last deposited sources, then timed steps
+        for _ in range(ctx.H):
+            ctx.push_sources()
         kms = []
-        for _ in range(3):  # the field kernel alone, timed by the library's events (not recorded inside a graph)
+        for _ in range(2):
             ctx.push_sources()
             ctx.field_step()
             kms.append(ctx.last_field_kernel_ms())
         side.synchronize()
-    out = {"workload": w.name, "steps": steps, "warmup": warmup, "ms_per_step": ms, "steps_per_s": 1e3 / ms,
-           "particles": int(part["x"].numel()), "field_kernel_ms": float(np.mean(kms)), "launches": launches,
-           "graph": "one CUDA-graph launch per step (jefi_pic_step)", "field_impl": ctx.info["field_impl"], "tiles": ctx.tile_info}
+    full_ms = float(np.mean(kms))
+    out = {"workload": w.name, "steps": steps, "from": "t0 (empty history)", "warmup": warmup, "total_ms": total_ms,
+           "ms_per_step": total_ms / steps, "steps_per_s": 1e3 * steps / total_ms, "first_step_ms": per_step[0], "last_step_ms": per_step[-1],
+           "particles": int(part["x"].numel()), "alive_at_end": alive, "H": ctx.H,
+           "field_kernel_ms_full_history": full_ms,
+           "launches": launches, "graph": "one CUDA-graph launch per step (jefi_pic_step)", "field_impl": ctx.info["field_impl"], "tiles": ctx.tile_info}
     ctx.close()
     return out
 
@@ -532,7 +552,7 @@ def run_product(args, w: wl.FieldWorkload) -> dict:
                "gpu_launches": int(launches), "clocks": clocks}
         if not args.no_pic and world == 1:
             out["pic"] = []
-            for cfgno, st, wu in ((1, 64, 5), (2, 20, 3), (3, 10, 3), (5, 3, 1)):
+            for cfgno, st, wu in ((1, 64, 3), (2, 100, 3), (3, 200, 3), (5, 50, 2)):  # BASELINE.json's run lengths
                 try:
                     out["pic"].append(time_pic(J, torch, device, cfgno, st, wu))
                 except Exception as e:  # noqa: BLE001

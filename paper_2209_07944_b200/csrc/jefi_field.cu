@@ -104,7 +104,10 @@ int jefi_launch_field_reference(jefi_ctx* c, int k0, int k1, float* ex, float* e
 // holds delay m = m_top - j.  A window wider than the compiled pitch WP (large dx/(c dt), e.g. the paper's kappa = 6
 // example) is served in ceil(W/WP) passes over the same source tile: pass p stages the delays
 // [m_hi - p WP - (R-1), m_hi - p WP] and every lane whose delay falls outside contributes exactly zero (MODE_MULTI).
-// The pipeline runs over (tile, pass) items; the stage header tells the consumers what an item is and which is the last.
+// The pipeline runs over (tile, pass) items; the stage header tells the consumers what an item is, and a terminal item
+// (MODE_END) that nothing follows.  An item whose rows would ALL be zero - every delay of the tile pair reaches back before t0
+// or beyond the stored depth (reading A15) - is not staged: its pairs add exactly nothing.  In the first steps of
+// a run the kernel therefore evaluates only the sources inside the light cone of t0 of each observation tile.
 //
 // Pair evaluation: the source cell is warp-uniform, the delay per lane:
 //   q = |d'|^2 (FFMA), rs = rsqrt(q) (MUFU), t = q*rs + 1.5*2^23 (FFMA; the integer m sits in the mantissa),
@@ -129,7 +132,7 @@ constexpr int NCONS = 512;  // consumer threads = observation cells of a tile
 constexpr int NCWARPS = NCONS / 32;
 constexpr int TILED_THREADS = NCONS + 32;  // + producer warp
 constexpr int HDR_BYTES = 32;
-enum { MODE_PLAIN = 0, MODE_SELF = 1, MODE_MULTI = 2 };
+enum { MODE_PLAIN = 0, MODE_SELF = 1, MODE_MULTI = 2, MODE_END = 3 };
 
 struct tiled_params {
   jefi_dims d;
@@ -152,11 +155,11 @@ struct tiled_params {
 
 struct stage_hdr {  // written by the producer before it arms the stage's full barrier
   uint32_t K;       // shared address of the stage's row 0 + 2064*(m_top + 0x4B400000)  (mod 2^32)
-  int mode;         // MODE_PLAIN / MODE_SELF (the source tile contains r' = r) / MODE_MULTI (one of several passes)
+  int mode;         // MODE_PLAIN / MODE_SELF (the source tile contains r' = r) / MODE_MULTI (one of several passes) / MODE_END
   int dx0, dy0, dz0;  // ox0 - sx0, oy0 - sy0, oz0 - sz0
   uint32_t Mtop;    // m_top + 0x4B400000 (MODE_MULTI)
   uint32_t R;       // rows staged in this item (MODE_MULTI)
-  int last;         // this is the CTA's last item
+  int last;         // bit 0: terminal item (MODE_END), nothing follows; JEFI_CHECKED: bits 1.. = sequence number of the item
 };
 static_assert(sizeof(stage_hdr) == HDR_BYTES, "stage header");
 
@@ -485,9 +488,7 @@ __global__ void __launch_bounds__(TILED_THREADS, 1) k_field_tiled(tiled_params P
       const int ix = (G::OBX / G::TSX) * obx - stx + (d.ntx - 1), iy = (G::OBY / G::TSY) * oby - sty + (d.nty - 1),
                 iz = (G::OBZ / G::TSZ) * obz - stz + (d.ntz - 1);
       const size_t prow = (size_t)ix + (size_t)P.ndx * ((size_t)iy + (size_t)P.ndy * iz);
-      for (int p = 0; p < npass; p++, item++) {
-        const int s = item & 1;
-        if (item >= 2) mbar_wait(barDone + 8 * s, ((item - 2) >> 1) & 1);  // consumers are done with item-2 (same stage)
+      for (int p = 0; p < npass; p++) {
         const int m_top = m_hi - p * WP;
         const int R = min(WP, m_top - m_lo + 1);
         // row j <-> delay m = m_top - j <-> absolute step t = n - m_top + j.  Rows with t < 0 (before t0)
@@ -495,6 +496,12 @@ __global__ void __launch_bounds__(TILED_THREADS, 1) k_field_tiled(tiled_params P
         int jv = max(m_top - n_now, m_top - (d.H - 2));
         jv = jv < 0 ? 0 : (jv > R ? R : jv);
         const int nvalid = R - jv;          // <= H - 1
+        // Nothing of this window has been emitted yet (every delay of the tile pair reaches back before t0) or is stored: all
+        // its sources are exactly zero, so the pairs add exactly nothing and the item is not staged at all.  In the first
+        // n steps of a run only sources within n c dt of an observation tile are evaluated (the light cone of t0).
+        if (nvalid == 0) continue;
+        const int s = item & 1;
+        if (item >= 2) mbar_wait(barDone + 8 * s, ((item - 2) >> 1) & 1);  // consumers are done with item-2 (same stage)
         int s0 = nslot_now - (m_top - jv);  // ring slot of row jv; m_top - jv <= H - 2
         s0 += s0 < 0 ? d.H : 0;
         const int lenA = min(nvalid, d.H - s0), lenB = nvalid - lenA;  // ring wrap: at most two runs
@@ -518,7 +525,7 @@ __global__ void __launch_bounds__(TILED_THREADS, 1) k_field_tiled(tiled_params P
           h.mode = npass > 1 ? MODE_MULTI : (self ? MODE_SELF : MODE_PLAIN);
           h.dx0 = ox0 - sx0; h.dy0 = oy0 - sy0; h.dz0 = oz0 - sz0;
           h.R = (uint32_t)R;
-          h.last = (it == nt - 1 && p == npass - 1) ? 1 : 0;
+          h.last = 0;
 #ifdef JEFI_CHECKED
           h.last |= item << 1;  // sequence number of the item, checked by every consumer thread
 #endif
@@ -530,19 +537,38 @@ __global__ void __launch_bounds__(TILED_THREADS, 1) k_field_tiled(tiled_params P
           if (lenB > 0) bulk_g2s(sb + (uint32_t)((jv + lenA) * JEFI_ROW_BYTES), rows, (uint32_t)(lenB * JEFI_ROW_BYTES), bar);
           bulk_g2s(sb + L::PERM, P.perm + prow * OBCELLS, OBCELLS * 2, bar);
         }
+        item++;
       }
       if (++stx == d.ntx) { stx = 0; if (++sty == d.nty) { sty = 0; ++stz; } }
+    }
+    {  // terminal item: tells the consumers that nothing follows (how many items were staged depends on the light cone)
+      const int s = item & 1;
+      if (item >= 2) mbar_wait(barDone + 8 * s, ((item - 2) >> 1) & 1);
+      if (lane == 0) {
+        stage_hdr h;
+        h.K = 0; h.mode = MODE_END; h.dx0 = h.dy0 = h.dz0 = 0; h.Mtop = 0; h.R = 0;
+        h.last = 1;
+#ifdef JEFI_CHECKED
+        h.last |= item << 1;
+#endif
+        *reinterpret_cast<stage_hdr*>(smem + (size_t)s * L::BYTES + L::HDR) = h;
+        mbar_expect_tx(barFull + 8 * s, 0u);  // no bytes follow: the phase completes with this arrival
+      }
     }
     return;
   }
 
   // -------------------------------------------------- consumer warps --------------------------------------------------
-  // single-pass kernels know their item count (one per source tile); multi-pass ones read "last" from the stage header
-  for (int item = 0; MULTI || item < nt; item++) {
+  // the consumers take items until the terminal one (MODE_END): how many were staged depends on the step (light cone of t0)
+  for (int item = 0;; item++) {
     const int s = item & 1;
     const unsigned char* st = smem + (size_t)s * L::BYTES;
     mbar_wait(barFull + 8 * s, (item >> 1) & 1);
     const stage_hdr h = *reinterpret_cast<const stage_hdr*>(st + L::HDR);
+#ifdef JEFI_CHECKED
+    if ((h.last >> 1) != item) JEFI_CHECK_FAIL(1);
+#endif
+    if (h.mode == MODE_END) break;
     // the unit (G::CX cells along x) this lane evaluates for this source tile: neighbouring lanes are (almost) equidistant from it
     const int c = reinterpret_cast<const unsigned short*>(st + L::PERM)[tid];
     const int cx = G::CX * (c % G::UX), cy = (c / G::UX) % G::OBY, cz = c / (G::UX * G::OBY);
@@ -561,7 +587,6 @@ __global__ void __launch_bounds__(TILED_THREADS, 1) k_field_tiled(tiled_params P
     item_addr I0;
     I0.K = h.K; I0.Mtop = h.Mtop; I0.R = h.R;
 #ifdef JEFI_CHECKED
-    if ((h.last >> 1) != item) JEFI_CHECK_FAIL(1);
     I0.lo = sm0 + (uint32_t)s * L::BYTES;
     I0.hi = I0.lo + h.R * (uint32_t)JEFI_ROW_BYTES;
     if (h.R > (uint32_t)WP) JEFI_CHECK_FAIL(0);
@@ -604,7 +629,6 @@ __global__ void __launch_bounds__(TILED_THREADS, 1) k_field_tiled(tiled_params P
     }
     __syncwarp();
     if (lane == 0) mbar_arrive(barDone + 8 * s);  // stage s may be refilled; this warp's accumulator updates are done
-    if (MULTI && (h.last & 1)) break;
   }
 
   asm volatile("bar.sync 1, %0;" ::"n"(NCONS) : "memory");  // consumers only: all accumulator updates are visible
