@@ -156,8 +156,10 @@ int jefi_push_sources(jefi_ctx* ctx, const float* rho, const float* jx, const fl
  *   B(r) = -mu0 dV/(4 pi)  sum_{r'!=r} [ d x J/R^3 + d x J_dot/(c R^2) ]
  * with d = r - r', sources at step n - m(d), time derivatives from steps n-m and n-m-1, the self cell skipped
  * (PAPER.md:221).  ex..bz: OUT, N floats each (V/m, tesla), overwritten.
- * Sources before step 0 are zero: tile pairs all of whose delays reach back before step 0 are skipped, so the
- * first steps of a run cost only what the light cone of t0 holds (results are identical: those pairs add exactly zero).
+ * Sources before step 0 are zero: tile pairs all of whose delays reach back before step 0 are skipped, and so
+ * are source tiles that held no charge or current during the steps a window reads (jefi_push_sources tracks that per tile).
+ * The first steps of a run and mostly empty grids cost only what can contribute; results are identical, the skipped pairs
+ * add exactly zero.
  * JEFI_ESTATE before the first jefi_push_sources. */
 int jefi_field_step(jefi_ctx* ctx, float* ex, float* ey, float* ez, float* bx, float* by, float* bz);
 

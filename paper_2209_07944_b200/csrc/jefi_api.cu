@@ -64,6 +64,7 @@ extern "C" int jefi_create(const jefi_config* cfg, jefi_ctx** out) {
   c->mtab_host = nullptr;
   c->src_stage = c->eb_stage = nullptr;
   c->perm = nullptr;
+  c->tile_first = c->tile_last = nullptr;
   c->partial = nullptr;
   c->step_dev = nullptr;
   c->step_dev_value = -2;
@@ -149,6 +150,14 @@ extern "C" int jefi_create(const jefi_config* cfg, jefi_ctx** out) {
     return fail_create(c, JEFI_ENOMEM, std::string("ring allocation (") + std::to_string(c->ring_bytes) + " B): " + cudaGetErrorString(e));
   if ((e = cudaMemsetAsync(c->ring, 0, ring_quads * sizeof(float4), c->stream)) != cudaSuccess)
     return fail_create(c, JEFI_ECUDA, std::string("ring zero fill: ") + cudaGetErrorString(e));
+  // per source tile, the span of steps whose ring row holds anything but zeros (k_push_sources keeps it; the tiled kernel skips
+  // tile pairs whose window lies outside it): first = 0x7f7f7f7f, last = -1 mean "never"
+  const size_t ntile_all = (size_t)d.ntx * d.nty * d.ntz;
+  if ((e = cudaMalloc(&c->tile_first, ntile_all * sizeof(int))) != cudaSuccess || (e = cudaMalloc(&c->tile_last, ntile_all * sizeof(int))) != cudaSuccess)
+    return fail_create(c, JEFI_ENOMEM, std::string("tile occupancy allocation: ") + cudaGetErrorString(e));
+  if ((e = cudaMemsetAsync(c->tile_first, 0x7f, ntile_all * sizeof(int), c->stream)) != cudaSuccess ||
+      (e = cudaMemsetAsync(c->tile_last, 0xff, ntile_all * sizeof(int), c->stream)) != cudaSuccess)
+    return fail_create(c, JEFI_ECUDA, std::string("tile occupancy fill: ") + cudaGetErrorString(e));
 
   // ---- delay table, fp64 on the host: m = floor(R/(c dt) + 1/2) (Eq. 2.6, reading A1) ----
   const int ex = jefi_table_extent(d.nx, d.obx), ey = jefi_table_extent(d.ny, d.oby), ez = jefi_table_extent(d.nz, d.obz);
@@ -229,6 +238,8 @@ extern "C" void jefi_destroy(jefi_ctx* c) {
   if (c->ring) cudaFree(c->ring);
   if (c->mtab_dev) cudaFree(c->mtab_dev);
   if (c->perm) cudaFree(c->perm);
+  if (c->tile_first) cudaFree(c->tile_first);
+  if (c->tile_last) cudaFree(c->tile_last);
   if (c->partial) cudaFree(c->partial);
   if (c->step_dev) cudaFree(c->step_dev);
   if (c->pic_exec) cudaGraphExecDestroy(c->pic_exec);
@@ -256,24 +267,32 @@ extern "C" void jefi_destroy(jefi_ctx* c) {
 // Traffic: 16 B in (4 SoA floats) + 16 B read (previous) + 32 B written per cell.
 // ------------------------------------------------------------------------------------------------------------
 // step_dev != NULL (jefi_pic_step's graph): slot and previous slot come from the device-side step state.
-__global__ void __launch_bounds__(256) k_push_sources(jefi_dims d, float inv_c, int slot, int prev_slot, const int* __restrict__ step_dev,
+__global__ void __launch_bounds__(256) k_push_sources(jefi_dims d, float inv_c, int n, int slot, int prev_slot, const int* __restrict__ step_dev,
                                                       const float* __restrict__ rho, const float* __restrict__ jx,
                                                       const float* __restrict__ jy, const float* __restrict__ jz,
-                                                      float4* __restrict__ ring) {
-  long r = (long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (r >= d.ncell_pad) return;
-  if (step_dev) { slot = step_dev[1]; prev_slot = step_dev[2]; }
+                                                      float4* __restrict__ ring, int* __restrict__ tile_first, int* __restrict__ tile_last) {
+  const long r = (long)blockIdx.x * blockDim.x + threadIdx.x;  // a warp's 32 cells belong to one tile (64 cells per tile)
+  if (step_dev) { n = step_dev[0]; slot = step_dev[1]; prev_slot = step_dev[2]; }
   const long tile = r / JEFI_TCELLS;
   const int cell = (int)(r - tile * JEFI_TCELLS);
   const int tx = (int)(tile % d.ntx), ty = (int)((tile / d.ntx) % d.nty), tz = (int)(tile / ((long)d.ntx * d.nty));
   const int i = tx * d.tsx + cell % d.tsx, j = ty * d.tsy + (cell / d.tsx) % d.tsy, k = tz * d.tsz + cell / (d.tsx * d.tsy);
-  if (i >= d.nx || j >= d.ny || k >= d.nz) return;  // padded cells stay zero
-  const size_t cidx = (size_t)i + (size_t)d.nx * ((size_t)j + (size_t)d.ny * k);
-  const size_t q = jefi_ring_quad(d, tile, slot, cell);
-  const float4 s = make_float4(jx[cidx] * inv_c, jz[cidx] * inv_c, rho[cidx], jy[cidx] * inv_c);
-  const float4 p = prev_slot >= 0 ? ring[jefi_ring_quad(d, tile, prev_slot, cell)] : make_float4(0.f, 0.f, 0.f, 0.f);
-  ring[q] = s;
-  ring[q + JEFI_TCELLS] = make_float4(s.x - p.x, s.y - p.y, s.z - p.z, s.w - p.w);
+  bool nz = false;
+  if (r < d.ncell_pad && i < d.nx && j < d.ny && k < d.nz) {  // padded cells stay zero
+    const size_t cidx = (size_t)i + (size_t)d.nx * ((size_t)j + (size_t)d.ny * k);
+    const size_t q = jefi_ring_quad(d, tile, slot, cell);
+    const float4 s = make_float4(jx[cidx] * inv_c, jz[cidx] * inv_c, rho[cidx], jy[cidx] * inv_c);
+    const float4 p = prev_slot >= 0 ? ring[jefi_ring_quad(d, tile, prev_slot, cell)] : make_float4(0.f, 0.f, 0.f, 0.f);
+    const float4 dd = make_float4(s.x - p.x, s.y - p.y, s.z - p.z, s.w - p.w);
+    ring[q] = s;
+    ring[q + JEFI_TCELLS] = dd;
+    nz = !(s.x == 0.f && s.y == 0.f && s.z == 0.f && s.w == 0.f && dd.x == 0.f && dd.y == 0.f && dd.z == 0.f && dd.w == 0.f);  // NaN counts
+  }
+  // the span of steps in which this tile's row is not all zero (read by the tiled field kernel to skip empty source tiles)
+  if (__any_sync(0xffffffffu, nz) && (threadIdx.x & 31) == 0) {
+    atomicMin(tile_first + tile, n);
+    atomicMax(tile_last + tile, n);
+  }
 }
 
 __global__ void k_advance_step(int* __restrict__ st, int H) {  // n += 1 on the device (first kernel of the PIC-step graph)
@@ -288,7 +307,7 @@ int jefi_launch_push_sources(jefi_ctx* c, const float* rho, const float* jx, con
   unsigned blocks = (unsigned)((d.ncell_pad + 255) / 256);
   if (c->capturing) {  // recorded once, replayed every step: the step lives on the device, the host counter is advanced per replay
     k_advance_step<<<1, 1, 0, c->stream>>>(c->step_dev, d.H);
-    k_push_sources<<<blocks, 256, 0, c->stream>>>(d, (float)(1.0 / c->c), 0, -1, c->step_dev, rho, jx, jy, jz, c->ring);
+    k_push_sources<<<blocks, 256, 0, c->stream>>>(d, (float)(1.0 / c->c), 0, 0, -1, c->step_dev, rho, jx, jy, jz, c->ring, c->tile_first, c->tile_last);
     JEFI_CUDA_TRY(c, cudaGetLastError());
     c->launches += 2;
     return JEFI_OK;
@@ -296,7 +315,7 @@ int jefi_launch_push_sources(jefi_ctx* c, const float* rho, const float* jx, con
   long n = c->step + 1;
   int slot = (int)(n % d.H);
   int prev = n >= 1 ? (int)((n - 1) % d.H) : -1;
-  k_push_sources<<<blocks, 256, 0, c->stream>>>(d, (float)(1.0 / c->c), slot, prev, nullptr, rho, jx, jy, jz, c->ring);
+  k_push_sources<<<blocks, 256, 0, c->stream>>>(d, (float)(1.0 / c->c), (int)n, slot, prev, nullptr, rho, jx, jy, jz, c->ring, c->tile_first, c->tile_last);
   JEFI_CUDA_TRY(c, cudaGetLastError());
   c->launches++;
   c->step = n;

@@ -111,6 +111,7 @@ struct jefi_ctx {
   int nsplit;           // pieces of the source range; > 1: partial sums go to `partial` and k_reduce_partials adds them
   float* partial;       // [nsplit][6][N]
   unsigned short* perm; // evaluation order of the 512 cells of an observation tile per relative tile offset
+  int *tile_first, *tile_last;  // per source tile: first and last step whose ring row (S or D) was not all zero (INT-ish max / -1: never)
   int ndx, ndy, ndz;
   // cell-sorted deposit scratch (jefi_particles.cu)
   unsigned *sort_count, *sort_offset, *sort_sums;  // per-bin counts, exclusive offsets, scan tile sums (+ grand total)

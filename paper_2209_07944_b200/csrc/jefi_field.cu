@@ -148,6 +148,7 @@ struct tiled_params {
   const int* step_dev;  // non-NULL (jefi_pic_step's graph): n and nslot are read from the device-side step state
   const float4* ring;
   const unsigned short* perm;  // [ndz][ndy][ndx][512]
+  const int *tile_first, *tile_last;  // per source tile: span of steps whose ring row is not all zero (k_push_sources)
   float *ex, *ey, *ez, *bx, *by, *bz;
   float4* pack;    // optional interleaved output (jefi_field_step_packed)
   float* partial;
@@ -468,19 +469,46 @@ __global__ void __launch_bounds__(TILED_THREADS, 1) k_field_tiled(tiled_params P
 
   if (warp == NCWARPS) {
     // ------------------------------------------------ producer warp ------------------------------------------------
-    int stx = t0 % d.ntx, sty = (t0 / d.ntx) % d.nty, stz = t0 / (d.ntx * d.nty);
     const int n_now = P.step_dev ? P.step_dev[0] : P.n, nslot_now = P.step_dev ? P.step_dev[1] : P.nslot;
-    int item = 0;
-    for (int it = 0; it < nt; it++) {
+    // delays of the tile pair (observation tile, source tile tt) from the extreme offsets
+    auto tile_window = [&](int tt, int& stx, int& sty, int& stz, int& m_lo, int& m_hi, bool& self) {
+      stx = tt % d.ntx; sty = (tt / d.ntx) % d.nty; stz = tt / (d.ntx * d.nty);
       const int sx0 = stx * G::TSX, sy0 = sty * G::TSY, sz0 = stz * G::TSZ;
-      // slot window of this (observation tile, source tile) pair from the extreme offsets
       int mnx, mxx, mny, mxy, mnz, mxz;
       abs_range(ox0 - (sx0 + G::TSX - 1), ox0 + G::OBX - 1 - sx0, mnx, mxx);
       abs_range(oy0 - (sy0 + G::TSY - 1), oy0 + G::OBY - 1 - sy0, mny, mxy);
       abs_range(oz0 - (sz0 + G::TSZ - 1), oz0 + G::OBZ - 1 - sz0, mnz, mxz);
-      const bool self = (mnx == 0 && mny == 0 && mnz == 0);
-      const int m_lo = self ? 0 : jefi_delay_fp32(jefi_q_fp32(P.g.kx, P.g.ky, P.g.kz, (float)mnx, (float)mny, (float)mnz));
-      const int m_hi = jefi_delay_fp32(jefi_q_fp32(P.g.kx, P.g.ky, P.g.kz, (float)mxx, (float)mxy, (float)mxz));
+      self = (mnx == 0 && mny == 0 && mnz == 0);
+      m_lo = self ? 0 : jefi_delay_fp32(jefi_q_fp32(P.g.kx, P.g.ky, P.g.kz, (float)mnx, (float)mny, (float)mnz));
+      m_hi = jefi_delay_fp32(jefi_q_fp32(P.g.kx, P.g.ky, P.g.kz, (float)mxx, (float)mxy, (float)mxz));
+    };
+    int item = 0;
+    for (int base = 0; base < nt; base += 32) {
+      // 32 source tiles at a time, one per lane: which of them has anything to contribute at this step?  Its window must reach a
+      // stored step >= 0 (light cone of t0; depth, reading A15) and overlap the span of steps in which the tile's ring
+      // row was not all zero (k_push_sources).  In the first steps of a run and on mostly empty grids nearly every tile drops out
+      // here, 32 per round trip.
+      int occ_first = 0x7f7f7f7f, occ_last = -1;
+      int l_stx = 0, l_sty = 0, l_stz = 0, l_mlo = 0, l_mhi = 0;
+      bool l_self = false, keep = false;
+      if (base + lane < nt) {
+        tile_window(t0 + base + lane, l_stx, l_sty, l_stz, l_mlo, l_mhi, l_self);
+        occ_first = P.tile_first[t0 + base + lane];
+        occ_last = P.tile_last[t0 + base + lane];
+        const int mcap = min(n_now, d.H - 2);                        // largest delay with a stored, emitted step
+        keep = l_mlo <= mcap && n_now - l_mlo >= occ_first && n_now - min(l_mhi, mcap) <= occ_last;
+      }
+      unsigned todo = __ballot_sync(0xffffffffu, keep);
+      while (todo) {
+      const int lsel = __ffs(todo) - 1;
+      todo &= todo - 1;
+      const int it = base + lsel;
+      const unsigned FULLW = 0xffffffffu;
+      const int t_first = __shfl_sync(FULLW, occ_first, lsel), t_last = __shfl_sync(FULLW, occ_last, lsel);
+      const int stx = __shfl_sync(FULLW, l_stx, lsel), sty = __shfl_sync(FULLW, l_sty, lsel), stz = __shfl_sync(FULLW, l_stz, lsel);
+      const int m_lo = __shfl_sync(FULLW, l_mlo, lsel), m_hi = __shfl_sync(FULLW, l_mhi, lsel);
+      const bool self = __shfl_sync(FULLW, (int)l_self, lsel) != 0;
+      const int sx0 = stx * G::TSX, sy0 = sty * G::TSY, sz0 = stz * G::TSZ;
       const int W = m_hi - m_lo + 1;
       const int npass = MULTI ? (W + WP - 1) / WP : 1;  // 1 unless the window exceeds the compiled pitch
       const size_t tile = (size_t)(t0 + it);
@@ -500,6 +528,9 @@ __global__ void __launch_bounds__(TILED_THREADS, 1) k_field_tiled(tiled_params P
         // its sources are exactly zero, so the pairs add exactly nothing and the item is not staged at all.  In the first
         // n steps of a run only sources within n c dt of an observation tile are evaluated (the light cone of t0).
         if (nvalid == 0) continue;
+        // the same for a source tile that held nothing but zeros during the steps this window reads, n - m_top + jv .. n - m_top +
+        // R - 1 (an empty region of the grid, or one the charge has not reached or has left): skipped exactly as well
+        if (n_now - m_top + R - 1 < t_first || n_now - m_top + jv > t_last) continue;
         const int s = item & 1;
         if (item >= 2) mbar_wait(barDone + 8 * s, ((item - 2) >> 1) & 1);  // consumers are done with item-2 (same stage)
         int s0 = nslot_now - (m_top - jv);  // ring slot of row jv; m_top - jv <= H - 2
@@ -539,7 +570,7 @@ __global__ void __launch_bounds__(TILED_THREADS, 1) k_field_tiled(tiled_params P
         }
         item++;
       }
-      if (++stx == d.ntx) { stx = 0; if (++sty == d.nty) { sty = 0; ++stz; } }
+      }  // tiles of this round with something to contribute
     }
     {  // terminal item: tells the consumers that nothing follows (how many items were staged depends on the light cone)
       const int s = item & 1;
@@ -978,6 +1009,7 @@ int jefi_launch_field_tiled(jefi_ctx* c, int k0, int k1, float* ex, float* ey, f
   P.to_partial = c->nsplit > 1 ? 1 : 0;
   P.step_dev = c->capturing ? c->step_dev : nullptr;
   P.ring = c->ring; P.perm = c->perm;
+  P.tile_first = c->tile_first; P.tile_last = c->tile_last;
   P.ex = ex; P.ey = ey; P.ez = ez; P.bx = bx; P.by = by; P.bz = bz;
   P.pack = reinterpret_cast<float4*>(eb_packed);
   P.partial = c->partial;

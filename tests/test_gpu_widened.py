@@ -457,3 +457,55 @@ def test_pic_step_graph_closed_loop(J, config, steps):
         assert np.linalg.norm(S[a] - So[a]) <= 1e-5 * max(np.linalg.norm(So[a]), 1e-300)
     assert min(per_step) >= 4  # every step, replayed or direct, accounts for its kernels in jefi_launch_count
     ctx.close()
+
+
+# ------------------------------------------------------------------------------------ empty source tiles / light cone of t0
+@pytest.mark.parametrize("tile", ["CELL", "DYAD"])
+@pytest.mark.parametrize("rule", ["NEAREST", "LINEAR"])
+def test_empty_source_tiles_and_unreached_windows_are_skipped_exactly(J, rule, tile):
+    """The tiled kernel does not stage (tile, pass) items whose rows are all zero: windows before t0 and source tiles that held
+    nothing during the steps the window reads (k_push_sources keeps the span of non-zero steps per tile).  Sources that live in a
+    small block which moves, vanishes for a while and comes back somewhere else; fields against the oracle at several steps, also
+    with the ring wrapped, and against the GPU's own reference kernel, which skips nothing."""
+    import torch
+
+    shape, dx = (32, 16, 24), 1e-4
+    dt = dx / (2 * C)
+    cfg = OracleConfig(*shape, dx, dx, dx, dt, delay_rule=getattr(oracle, "RULE_" + rule))
+    N = cfg.N
+    rng = np.random.default_rng(77)
+    nsteps = cfg.H + 25
+    idx = np.arange(N)
+    ii, jj, kk = idx % shape[0], (idx // shape[0]) % shape[1], idx // (shape[0] * shape[1])
+    slices = []
+    for t in range(nsteps):
+        s = np.zeros((4, N), dtype=np.float32)
+        if t < 30 or t >= cfg.H - 10:  # silent in between: tiles go empty and come back
+            x0 = (3 + t // 4) % (shape[0] - 5) if t < 30 else 20  # the block moves along x, later sits elsewhere
+            blk = (ii >= x0) & (ii < x0 + 5) & (jj >= 6) & (jj < 10) & (kk >= 9 + (0 if t < 30 else 8)) & (kk < 12 + (0 if t < 30 else 8))
+            s[:, blk] = rng.uniform(-1, 1, size=(4, int(blk.sum()))).astype(np.float32)
+            s[1:, blk] *= np.float32(C)
+        slices.append(s)
+    kw = dict(field_impl=J.JEFI_FIELD_TILED, delay_rule=getattr(J, "JEFI_DELAY_" + rule), field_tile=getattr(J, "JEFI_TILE_" + tile))
+    ctx = J.JefiContext(J.GridSpec(*shape, dx, dx, dx, dt), **kw)
+    ref = J.JefiContext(J.GridSpec(*shape, dx, dx, dx, dt), field_impl=J.JEFI_FIELD_REFERENCE, delay_rule=kw["delay_rule"])
+    orc = oracle.OracleJefi(cfg)
+    checked = 0
+    for t, s in enumerate(slices):
+        d = torch.from_numpy(s).to(ctx.device)
+        ctx.push_sources(d)
+        ref.push_sources(d)
+        orc.push_sources(*s.astype(np.float64))
+        if t in (0, 1, 2, 5, 17, 29, 31, 45, cfg.H - 11, cfg.H - 9, cfg.H + 3, nsteps - 1):
+            eb = ctx.field_step().cpu().numpy()
+            er = ref.field_step().cpu().numpy()
+            Eo, Bo = orc.field_step()
+            assert_field_parity(eb[:3], eb[3:], Eo, Bo, f"step {t} {rule} {tile}: ")
+            assert_field_parity(er[:3], er[3:], Eo, Bo, f"step {t} {rule} reference: ")
+            # cells nothing has reached are exactly zero in all three
+            Fo = np.concatenate([Eo, Bo])
+            assert np.all(eb[Fo == 0.0] == 0.0) and np.all(er[Fo == 0.0] == 0.0)
+            checked += 1
+    assert checked == 12
+    ctx.close()
+    ref.close()
