@@ -45,8 +45,8 @@ FLOP_PER_PAIR = 48.0  # 24 FMA per source-observation pair
 # `traffic` is null and `traffic_source` says the capture is stale.
 FIELD_DRAM_BYTES = {
     # (workload name, rule): (bytes, profile, kernel source sha)
-    ("cfg4_96c_field_only", "nearest"): (68.457673e9 + 707.518464e6, "profiles/r2m_field_tiled_ncu_full.md", "99ae3b3a6d6d"),
-    ("cfg4_96c_field_only", "linear"): (37.006372e9 + 705.908992e6, "profiles/r2m_field_tiled_ncu_full.md", "99ae3b3a6d6d"),
+    ("cfg4_96c_field_only", "nearest"): (93.108966e9 + 783.064576e6, "profiles/r2o_field_tiled_ncu_full.md", "a97fcdd1e225"),
+    ("cfg4_96c_field_only", "linear"): (52.037499e9 + 704.273408e6, "profiles/r2o_field_tiled_ncu_full.md", "a97fcdd1e225"),
 }
 
 
