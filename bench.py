@@ -10,7 +10,8 @@ L2 flush is needed between iterations (workloads whose ring would fit in L2 are 
 in between).  `e2e` repeats it through jefi_field_step_host with pinned HOST buffers.
 `pic` adds PIC steps/s (deposit -> push_sources -> field_step -> push_particles) over BASELINE.json's whole runs of configs
 1, 2, 3, 5 from t0, and the field-kernel time with the history at full depth;
-`paper_workloads` the pairs/s of the paper's own shapes (20^3 at kappa = 6, the 1x251x111 slab).
+`paper_workloads` the pairs/s of the paper's own shapes (20^3 at kappa = 6, the 1x251x111 slab); `paper_run` the paper's one
+printed whole-run set-up (1x251x111, 1e7 macro-particles, 1e4 steps) as a whole.
 Reference arm (--impl reference): the fp64 CPU oracle, as it stands, on a bounded sample of the same workload.
 N > 1: one process per GPU.  Under torchrun (WORLD_SIZE set) this process is one rank; without it `--gpus N` re-executes
 itself under `python -m torch.distributed.run --nproc-per-node N` so that N ranks really run.  Default: replicas
@@ -264,6 +265,33 @@ def time_pic(J, torch, device, config: int, steps: int, warmup: int) -> dict:
            "particles": int(part["x"].numel()), "alive_at_end": alive, "H": ctx.H,
            "field_kernel_ms_full_history": full_ms,
            "launches": launches, "graph": "one CUDA-graph launch per step (jefi_pic_step)", "field_impl": ctx.info["field_impl"], "tiles": ctx.tile_info}
+    ctx.close()
+    return out
+
+
+def time_paper_run(J, torch, device, count: int = 10_000_000, steps: int = 10_000) -> dict:
+    """The one whole-run time the paper prints for the method (section 3.3.2): the planar
+    emission in a 10 T B_y on 1 x 251 x 111 cells, dx = 1e-5 m, dt = 1e-13 s, 1 ns = 1e4 steps, 1e7 macro-particles, "within only
+    half an hour" on one A100 in fp64.  The same set-up (seeded stand-in for the unknown initial placement, reading A23) through
+    jefi_pic_step, timed as a whole with CUDA events: context only, another machine and precision."""
+    w = wl.SLABS["planar_emission"]
+    nx, ny, nz = w.shape
+    side = torch.cuda.Stream(device)
+    with torch.cuda.stream(side):
+        ctx = J.JefiContext(J.GridSpec(nx, ny, nz, w.dx, w.dx, w.dx, w.dt, Bext=w.Bext), device=device)
+        part = {k: torch.from_numpy(v).to(device) for k, v in wl.slab_particles("planar_emission", count).items()}
+        side.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(side)
+        for _ in range(steps):
+            ctx.pic_step(part)
+        e1.record(side)
+        side.synchronize()
+        ms = e0.elapsed_time(e1)
+        alive = int(part["alive"].sum().item())
+    out = {"workload": w.name, "grid": [nx, ny, nz], "particles": count, "steps": steps, "simulated_ns": steps * w.dt * 1e9,
+           "total_s": ms * 1e-3, "steps_per_s": 1e3 * steps / ms, "alive_at_end": alive, "field_impl": ctx.info["field_impl"], "tiles": ctx.tile_info,
+           "paper": "JefiPIC: 'within only half an hour' on one A100, fp64 (PAPER.md:372); UNIPIC: 'over 6 hours' on a Xeon workstation"}
     ctx.close()
     return out
 
@@ -565,6 +593,10 @@ def run_product(args, w: wl.FieldWorkload) -> dict:
                     out["paper_workloads"].append(time_field_workload(J, torch, device, wl.field_workload(key), "nearest", 20, 3, sm_max))
                 except Exception as e:  # noqa: BLE001
                     out["paper_workloads"].append({"config": {"workload": key}, "error": str(e)})
+            try:
+                out["paper_run"] = time_paper_run(J, torch, device)
+            except Exception as e:  # noqa: BLE001
+                out["paper_run"] = {"error": str(e)}
             try:
                 out["particle_kernels"] = time_particle_kernels(J, torch, device)
             except Exception as e:  # noqa: BLE001
