@@ -55,3 +55,19 @@ def test_product_does_not_import_the_oracle():
             if f.endswith((".py", ".c", ".h")):
                 src = open(os.path.join(dirpath, f)).read()
                 assert not re.search(r"^\s*(from|import)\s+paper_2209_07944_b200", src, flags=re.M), f
+
+
+def test_bench_traffic_table_belongs_to_this_kernel_source():
+    """bench.py's roofline.traffic comes from a committed ncu capture and is valid only for the kernel source it was taken from
+    (sha1 of csrc/jefi_field.cu + csrc/jefi_ctx.h): the table must name the current source and an existing profiles/ file."""
+    import os
+    import sys
+
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    sys.path.insert(0, root)
+    import bench
+
+    nbytes, prof = bench.field_traffic("cfg4_96c_field_only", "nearest")
+    assert nbytes is not None and nbytes > 4.74e9, prof  # at least one pass over the ring's S half (SURVEY.md 8(d))
+    assert os.path.exists(os.path.join(root, prof)), prof
+    assert bench.kernel_source_sha() in open(os.path.join(root, prof)).read()
