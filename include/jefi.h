@@ -137,6 +137,41 @@ int jefi_deposit(jefi_ctx* ctx, long np, const float* x, const float* y, const f
                  const float* uy, const float* uz, const float* qw, const unsigned char* alive, float* rho,
                  float* jx, float* jy, float* jz);
 
+/* The cell-sorted deposit for callers that cannot allocate device memory.
+ *
+ * jefi_deposit in JEFI_DEPOSIT_SORTED mode keeps its sort scratch in the context and (re)allocates it with cudaMalloc on
+ * first use and whenever np grows; creating the context allocates too.  That rules it out for a program whose device memory
+ * is all owned by its own pool after start-up (no driver allocation may happen later, or would fail against its budget) and
+ * for a step loop with a latency bound (cudaMalloc / cudaFree may synchronise the whole device).  This call needs no context
+ * and calls no cudaMalloc, cudaFree or other allocating routine, on the first call or any later one: its scratch (sort key,
+ * rank and order per particle, count and offset per sort bin, scan sums) is a fixed array of JEFI_STATIC_SCRATCH_BYTES
+ * (16 MiB) inside the library's CUDA module, held by every GPU the library is loaded on until the process exits.
+ *
+ * Computes exactly what jefi_deposit computes with shape_order 1 (Eqs. 2.15-2.19; virtual nodes dropped,
+ * PAPER.md:191; dead particles skipped), with the same kernels: same sums up to the order of the fp32 additions.
+ *   device, stream   CUDA device ordinal (made current for the call, then restored) and the cudaStream_t (NULL = legacy default
+ *                    stream) the work is enqueued on; the call does not synchronise
+ *   nx,ny,nz,dx..dz  grid, as in jefi_config;  c: speed of light, 0 -> 299792458
+ *   np, x..alive     as in jefi_deposit (DEVICE pointers, caller-owned, never modified; alive may be NULL)
+ *   rho,jx,jy,jz     OUT, DEVICE, nx*ny*nz floats each, overwritten
+ *   errbuf           HOST char[errbuf_len] that receives the text of an error (NULL / 0: no text)
+ * Limits (the scratch cannot grow): np <= JEFI_STATIC_MAX_PARTICLES and (nx+1)(ny+1)(nz+1)+1 <= JEFI_STATIC_MAX_BINS, e.g. up
+ * to a 79^3 grid.  Beyond either the call does nothing and returns JEFI_EINVAL with the limit named in errbuf; use jefi_deposit.
+ * Set-up: the first call on each device looks up the device address of the scratch (cudaGetSymbolAddress; no allocation) and
+ * caches it.  Make that first call per device before any stream capture begins.
+ * Sharing: all calls on a device use the same array, and it keeps what the last call left.  The call itself clears the part
+ * that must start at zero (the bin counters) on `stream` and overwrites the rest before reading it, so back-to-back calls on
+ * ONE stream, with any mix of grids and list lengths, are independent.  Calls whose GPU work can overlap - different streams,
+ * or different host threads - race on the array and give wrong sums: serialise them (one stream, or an event between them).
+ * Returns JEFI_OK, JEFI_EINVAL (bad argument or over a limit) or JEFI_ECUDA. */
+#define JEFI_STATIC_MAX_PARTICLES 1048576L
+#define JEFI_STATIC_MAX_BINS 524288L
+#define JEFI_STATIC_SCRATCH_BYTES 16781312L /* 3 x 4 MiB per-particle + 2 x 2 MiB per-bin + 4 KiB scan sums */
+int jefi_deposit_static(int device, void* stream, int nx, int ny, int nz, double dx, double dy, double dz, double c, long np,
+                        const float* x, const float* y, const float* z, const float* ux, const float* uy, const float* uz,
+                        const float* qw, const unsigned char* alive, float* rho, float* jx, float* jy, float* jz, char* errbuf,
+                        int errbuf_len);
+
 /* Put the caller's particle arrays in cell order, in place: first the depositing particles (alive, at least one node
  * inside the grid) grouped by base node (i,j,k) = floor(xi-.5).. with i fastest, then all others.  The order inside a
  * group is not defined.  Optional for correctness (no call depends on the order), it is what makes the warp-level

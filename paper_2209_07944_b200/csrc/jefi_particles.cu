@@ -1,5 +1,10 @@
 // libjefi: CIC deposit (Eqs. 2.15-2.19) and field interpolation +
 // relativistic Boris push + kill (row a5; PAPER.md:117-127 Eqs. 2.7-2.11, :193-205 Eq. 2.20).
+#include <string.h>
+
+#include <mutex>
+#include <string>
+
 #include "jefi_ctx.h"
 
 // Eq. (2.15)/(2.17) in grid units: node index i = floor(xi - 1/2), fraction alpha = xi - 1/2 - i.  xi - 0.5 is exact
@@ -742,5 +747,139 @@ extern "C" int jefi_debug_cell_index(jefi_ctx* c, long np, const float* x, const
   else k_cell_index<1><<<(unsigned)((np + 255) / 256), 256, 0, c->stream>>>(np, x, y, z, ijk_out);
   JEFI_CUDA_TRY(c, cudaGetLastError());
   JEFI_CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  return JEFI_OK;
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// jefi_deposit_static: the cell-sorted CIC deposit for callers that must not allocate (include/jefi.h has the contract).
+//
+// Who needs this.  Some programs that link libjefi are not free to call cudaMalloc at the moment they want a deposit: a host
+// application that gave the whole device to its own memory pool at start-up and allows no driver allocation afterwards (a
+// second allocator would overrun or fragment its budget, and a late cudaMalloc may simply fail there), or a step loop with a
+// latency bound (cudaMalloc and cudaFree can synchronise the whole device and take an unbounded time).
+// jefi_deposit with JEFI_DEPOSIT_SORTED grows context scratch with cudaMalloc on first use and whenever np grows; this entry
+// point does the same arithmetic with the same kernels, but every byte of its scratch (sort keys, ranks, the cell order, bin
+// counts, bin offsets, scan sums) lives in the fixed array below, which the library's CUDA module carries: each GPU the
+// library is loaded on reserves it when that module is loaded there, and holds it until the process exits.  No context is needed either.
+//
+// The array is shared by all calls on a device and is NOT cleared between them.  Only the bin counters have to start at zero
+// (one cudaMemsetAsync on the caller's stream per call); keys, ranks, order, offsets and scan sums are fully rewritten for
+// the first np particles / the bins of this grid before any kernel of the same call reads them, so whatever an earlier call
+// on another grid or a longer list left behind is never looked at.  Two calls that run on the GPU at the same time (different
+// streams, or two host threads) would sort into the same memory and corrupt each other: callers serialise them.
+// ------------------------------------------------------------------------------------------------------------
+namespace {
+constexpr long ST_MAX_NP = JEFI_STATIC_MAX_PARTICLES;
+constexpr long ST_MAX_BINS = JEFI_STATIC_MAX_BINS;                                  // (nx+1)(ny+1)(nz+1) + 1 must fit
+constexpr long ST_MAX_SCAN_TILES = (ST_MAX_BINS + SCAN_TILE - 1) / SCAN_TILE;
+constexpr size_t st_round(size_t b) { return (b + 255) & ~(size_t)255; }
+constexpr size_t ST_OFF_KEY = 0;
+constexpr size_t ST_OFF_RANK = ST_OFF_KEY + st_round(ST_MAX_NP * sizeof(int));
+constexpr size_t ST_OFF_ORDER = ST_OFF_RANK + st_round(ST_MAX_NP * sizeof(int));
+constexpr size_t ST_OFF_COUNT = ST_OFF_ORDER + st_round(ST_MAX_NP * sizeof(int));
+constexpr size_t ST_OFF_OFFSET = ST_OFF_COUNT + st_round(ST_MAX_BINS * sizeof(unsigned));
+constexpr size_t ST_OFF_SUMS = ST_OFF_OFFSET + st_round(ST_MAX_BINS * sizeof(unsigned));
+constexpr size_t ST_BYTES = ST_OFF_SUMS + st_round((ST_MAX_SCAN_TILES + 1) * sizeof(unsigned));
+static_assert(ST_BYTES <= JEFI_STATIC_SCRATCH_BYTES, "include/jefi.h states the size of the static scratch");
+constexpr int ST_MAX_DEVICES = 64;
+}  // namespace
+
+// The scratch itself.  In host code this name is only a handle for the runtime (a host-side shadow symbol), not a device
+// address: kernels get the address cudaGetSymbolAddress returns for the device that is current (static_scratch_base).
+static __device__ __align__(256) unsigned char g_jefi_static_scratch[JEFI_STATIC_SCRATCH_BYTES];
+
+static std::mutex g_static_mu;
+static unsigned char* g_static_base[ST_MAX_DEVICES];  // per device ordinal; NULL until the first call on that device
+
+// Device address of the scratch on `device`, which must be the current device.  Looked up once per device.
+static cudaError_t static_scratch_base(int device, unsigned char** base) {
+  std::lock_guard<std::mutex> lock(g_static_mu);
+  if (!g_static_base[device]) {
+    void* p = nullptr;
+    cudaError_t e = cudaGetSymbolAddress(&p, g_jefi_static_scratch);
+    if (e != cudaSuccess) return e;
+    g_static_base[device] = static_cast<unsigned char*>(p);
+  }
+  *base = g_static_base[device];
+  return cudaSuccess;
+}
+
+static int static_fail(char* errbuf, int errbuf_len, int code, const std::string& msg) {
+  if (errbuf && errbuf_len > 0) {
+    const size_t n = msg.size() < (size_t)errbuf_len - 1 ? msg.size() : (size_t)errbuf_len - 1;
+    memcpy(errbuf, msg.data(), n);
+    errbuf[n] = 0;
+  }
+  return code;
+}
+
+extern "C" int jefi_deposit_static(int device, void* stream, int nx, int ny, int nz, double dx, double dy, double dz, double c,
+                                   long np, const float* x, const float* y, const float* z, const float* ux, const float* uy,
+                                   const float* uz, const float* qw, const unsigned char* alive, float* rho, float* jx,
+                                   float* jy, float* jz, char* errbuf, int errbuf_len) {
+  if (errbuf && errbuf_len > 0) errbuf[0] = 0;
+  // ---- argument checks: before any CUDA call ----
+  if (nx < 1 || ny < 1 || nz < 1 || !(dx > 0) || !(dy > 0) || !(dz > 0) || c < 0)
+    return static_fail(errbuf, errbuf_len, JEFI_EINVAL, "jefi_deposit_static: nx, ny, nz >= 1 and dx, dy, dz > 0 are required");
+  if (np < 0 || !rho || !jx || !jy || !jz || (np > 0 && (!x || !y || !z || !ux || !uy || !uz || !qw)))
+    return static_fail(errbuf, errbuf_len, JEFI_EINVAL, "jefi_deposit_static: NULL array or negative np");
+  if (np > ST_MAX_NP)
+    return static_fail(errbuf, errbuf_len, JEFI_EINVAL,
+                       "jefi_deposit_static: np = " + std::to_string(np) + " exceeds JEFI_STATIC_MAX_PARTICLES = " +
+                           std::to_string(ST_MAX_NP) + " (the static scratch is fixed; use jefi_deposit for longer lists)");
+  const long nbins = (long)(nx + 1) * (ny + 1) * (nz + 1), nb = nbins + 1;
+  if (nb > ST_MAX_BINS)
+    return static_fail(errbuf, errbuf_len, JEFI_EINVAL,
+                       "jefi_deposit_static: (nx+1)(ny+1)(nz+1)+1 = " + std::to_string(nb) + " sort bins exceed JEFI_STATIC_MAX_BINS = " +
+                           std::to_string(ST_MAX_BINS) + " (the static scratch is fixed; use jefi_deposit for larger grids)");
+  if (device < 0 || device >= ST_MAX_DEVICES)
+    return static_fail(errbuf, errbuf_len, JEFI_EINVAL, "jefi_deposit_static: device ordinal out of range");
+  // ---- make `device` current for the rest of the call ----
+  struct guard_t {
+    int prev = -1;
+    bool switched = false;
+    ~guard_t() { if (switched) cudaSetDevice(prev); }
+  } guard;
+  cudaError_t e = cudaGetDevice(&guard.prev);
+  if (e == cudaSuccess && guard.prev != device) {
+    e = cudaSetDevice(device);
+    guard.switched = e == cudaSuccess;
+  }
+  unsigned char* base = nullptr;
+  if (e == cudaSuccess) e = static_scratch_base(device, &base);
+  if (e != cudaSuccess) return static_fail(errbuf, errbuf_len, JEFI_ECUDA, std::string("jefi_deposit_static: set-up: ") + cudaGetErrorString(e));
+  int* key = reinterpret_cast<int*>(base + ST_OFF_KEY);
+  int* rank = reinterpret_cast<int*>(base + ST_OFF_RANK);
+  int* order = reinterpret_cast<int*>(base + ST_OFF_ORDER);
+  unsigned* count = reinterpret_cast<unsigned*>(base + ST_OFF_COUNT);
+  unsigned* offset = reinterpret_cast<unsigned*>(base + ST_OFF_OFFSET);
+  unsigned* sums = reinterpret_cast<unsigned*>(base + ST_OFF_SUMS);
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const size_t N = (size_t)nx * ny * nz;
+#define ST_TRY(call)                                                                                                       \
+  do {                                                                                                                     \
+    cudaError_t e__ = (call);                                                                                              \
+    if (e__ != cudaSuccess) return static_fail(errbuf, errbuf_len, JEFI_ECUDA, std::string("jefi_deposit_static: " #call ": ") + cudaGetErrorString(e__)); \
+  } while (0)
+  // outputs are overwritten, as in jefi_deposit
+  ST_TRY(cudaMemsetAsync(rho, 0, N * sizeof(float), st));
+  ST_TRY(cudaMemsetAsync(jx, 0, N * sizeof(float), st));
+  ST_TRY(cudaMemsetAsync(jy, 0, N * sizeof(float), st));
+  ST_TRY(cudaMemsetAsync(jz, 0, N * sizeof(float), st));
+  if (np == 0) return JEFI_OK;
+  // the one part of the shared scratch that must start at zero: this grid's bin counters (the previous call's are stale)
+  ST_TRY(cudaMemsetAsync(count, 0, (size_t)nb * sizeof(unsigned), st));
+  const int ntiles = (int)((nb + SCAN_TILE - 1) / SCAN_TILE);
+  const unsigned pb = (unsigned)((np + 255) / 256);
+  k_sort_keys<1><<<pb, 256, 0, st>>>(nx, ny, nz, (int)nbins, np, x, y, z, alive, key, rank, count);
+  k_scan_tiles<<<ntiles, SCAN_THREADS, 0, st>>>(count, offset, nb, sums);
+  k_scan_sums<<<1, 1024, 0, st>>>(sums, ntiles);
+  k_scan_add<<<(unsigned)((nb + 255) / 256), 256, 0, st>>>(offset, nb, sums);
+  k_sort_scatter<<<pb, 256, 0, st>>>(np, key, rank, offset, order);
+  const float inv_dV = (float)(1.0 / (dx * dy * dz));
+  const float cc = (float)(c > 0 ? c : 299792458.0);
+  k_deposit_sorted<1><<<pb, 256, 0, st>>>(nx, ny, nz, inv_dV, cc, np, offset + nbins, order, alive, x, y, z, ux, uy, uz, qw, rho, jx, jy, jz);
+  ST_TRY(cudaGetLastError());
+#undef ST_TRY
   return JEFI_OK;
 }

@@ -21,6 +21,7 @@ JEFI_FIELD_AUTO, JEFI_FIELD_REFERENCE, JEFI_FIELD_TILED = 0, 1, 2
 JEFI_DEPOSIT_AUTO, JEFI_DEPOSIT_DIRECT, JEFI_DEPOSIT_SORTED, JEFI_DEPOSIT_RUNS = 0, 1, 2, 3
 JEFI_DELAY_NEAREST, JEFI_DELAY_LINEAR = 0, 1
 JEFI_TILE_AUTO, JEFI_TILE_CELL, JEFI_TILE_DYAD = 0, 1, 2
+JEFI_STATIC_MAX_PARTICLES, JEFI_STATIC_MAX_BINS = 1048576, 524288  # limits of jefi_deposit_static (include/jefi.h)
 
 EXPORTS = [
     "jefi_create", "jefi_destroy", "jefi_last_error", "jefi_get_info", "jefi_deposit", "jefi_push_sources",
@@ -28,7 +29,7 @@ EXPORTS = [
     "jefi_last_field_kernel_ms", "jefi_debug_delay_table", "jefi_debug_cell_index", "jefi_debug_history_slot",
     "jefi_debug_cell_order", "jefi_sort_particles", "jefi_field_impl_reason", "jefi_get_tile_info", "jefi_field_step_packed",
     "jefi_push_particles_packed", "jefi_field_kernel_ms", "jefi_debug_fp32_peak", "jefi_debug_check_errors", "jefi_pic_step",
-    "jefi_debug_lds128_cycles",
+    "jefi_debug_lds128_cycles", "jefi_deposit_static",
 ]
 
 
@@ -115,6 +116,9 @@ def load_library() -> C.CDLL:
     lib.jefi_field_step_packed.restype = C.c_int
     lib.jefi_push_particles_packed.argtypes = [vp, C.c_long] + [f32p] * 7 + [u8p, f32p]
     lib.jefi_push_particles_packed.restype = C.c_int
+    lib.jefi_deposit_static.argtypes = ([C.c_int, vp, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, C.c_double,
+                                         C.c_long] + [f32p] * 7 + [u8p] + [f32p] * 4 + [C.c_char_p, C.c_int])
+    lib.jefi_deposit_static.restype = C.c_int
     _lib = lib
     return lib
 
@@ -236,6 +240,35 @@ def jefi_deposit(handle: int, N: int, x, y, z, ux, uy, uz, qw, alive, rho, jx, j
     pal = _dev(alive, torch.uint8, np_, "alive") if alive is not None else 0
     pout = [_dev(t, f, N, n) for t, n in zip((rho, jx, jy, jz), ("rho", "jx", "jy", "jz"))]
     _check(handle, load_library().jefi_deposit(handle, np_, *pin, pal, *pout), "jefi_deposit")
+
+
+def jefi_deposit_static(nx: int, ny: int, nz: int, dx: float, dy: float, dz: float, x, y, z, ux, uy, uz, qw, alive, rho, jx, jy,
+                        jz, c: float = 0.0, stream: Optional[int] = None) -> None:
+    """Cell-sorted CIC deposit that allocates no device memory and needs no context (include/jefi.h, jefi_deposit_static).
+
+    For programs that may not call cudaMalloc when they deposit: all device memory belongs to their own pool after start-up, or
+    the step loop cannot afford the device-wide synchronisation an allocation can cause.  The sort scratch is a fixed 16 MiB
+    array inside libjefi's CUDA module, so the list is limited to JEFI_STATIC_MAX_PARTICLES particles and the grid to
+    (nx+1)(ny+1)(nz+1)+1 <= JEFI_STATIC_MAX_BINS; larger inputs raise JefiError (nothing is computed).  The output tensors
+    are the caller's (this binding allocates nothing either).  Every call on a device shares that one array: keep calls on one
+    stream, or order them with events; calls that overlap on the GPU corrupt each other.  Enqueues on `stream` (a
+    cudaStream_t handle; default: torch's current stream of the tensors' device) and does not synchronise.  The first call on a
+    device also looks up the array's device address; make it before starting any stream capture."""
+    import torch
+
+    f = torch.float32
+    np_ = x.numel()
+    N = nx * ny * nz
+    pin = [_dev(t, f, np_, n) for t, n in zip((x, y, z, ux, uy, uz, qw), ("x", "y", "z", "ux", "uy", "uz", "qw"))]
+    pal = _dev(alive, torch.uint8, np_, "alive") if alive is not None else 0
+    pout = [_dev(t, f, N, n) for t, n in zip((rho, jx, jy, jz), ("rho", "jx", "jy", "jz"))]
+    dev = rho.device.index or 0
+    if stream is None:
+        stream = torch.cuda.current_stream(rho.device).cuda_stream
+    err = C.create_string_buffer(512)
+    rc = load_library().jefi_deposit_static(dev, C.c_void_p(stream), nx, ny, nz, dx, dy, dz, c, np_, *pin, pal, *pout, err, len(err))
+    if rc != JEFI_OK:
+        raise JefiError(f"jefi_deposit_static failed with code {rc}: {err.value.decode()}")
 
 
 def jefi_push_particles(handle: int, N: int, x, y, z, ux, uy, uz, q_over_m, alive, ex, ey, ez, bx, by, bz) -> None:
