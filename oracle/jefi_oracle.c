@@ -20,7 +20,9 @@
  *
  * Parity pins: tests/test_oracle_*.py (P1-P15 of SURVEY.md §8(c); P16 = the gamma of the Boris rotation when E and B are
  * both non-zero, hand-computed 90-degree rotations; L1-L6 for the linear retarded-time rule; Q1-Q7 in
- * tests/test_oracle_shape2.py for the S^(2) deposit / interpolation); nothing here is "parity unpinned".
+ * tests/test_oracle_shape2.py for the S^(2) deposit / interpolation; F32 = orc_field_f32, the float-history instantiation of the
+ * field body, bitwise against orc_field_f64 on the same values and against the dense enumeration,
+ * tests/test_oracle_field.py::test_f32_history_entry_is_the_f64_entry_on_the_same_values); nothing here is "parity unpinned".
  */
 #include <math.h>
 #include <stddef.h>

@@ -410,3 +410,40 @@ def test_delay_table_nearest_step_and_no_ties_at_kappa_2():
     assert not np.any((2 * m + 1) ** 2 == 16 * q) and not np.any((2 * m - 1) ** 2 == 16 * q)  # no ties
     assert tab[0, 0, 1] == 2 and tab[0, 1, 1] == 3 and tab[1, 1, 1] == 3 and tab[0, 0, 2] == 4
     assert tab.max() <= oracle.num_dt(cfg)
+
+
+# ---------------------------------------------------------------- the float32-history entry (orc_field_f32)
+@pytest.mark.parametrize("rule", [oracle.RULE_NEAREST, oracle.RULE_LINEAR])
+def test_f32_history_entry_is_the_f64_entry_on_the_same_values(rule):
+    """oracle.field dispatches on the ring's dtype: float32 rings (what the full-size GPU parity tests and bench.py's
+    cpu_baseline pass, to keep a 335-446-slot history in host memory) go to orc_field_f32, the same Eqs. 2.4-2.6 body on a
+    `const float*` history.  Every sample is promoted to double before any arithmetic, so on float32-representable values the
+    two entries must agree BIT FOR BIT: for all cells and for a list of observation cells, on a ring that has wrapped and on
+    one still filling (zero before t0), and against the separately written dense enumeration, which never sees a float."""
+    shape, h, kappa = (5, 4, 3), (1.0, 0.8, 1.25), 1.7
+    c, eps0 = 1.0, 1.0
+    dt = h[0] / (kappa * c)
+    cfg = OracleConfig(*shape, *h, dt, c=c, eps0=eps0, delay_rule=rule)
+    rng = np.random.default_rng(32)
+    nsteps = 2 * cfg.H + 3
+    hist32 = rng.uniform(-1, 1, (nsteps, 4, cfg.N)).astype(np.float32)
+    obs = np.array([0, 7, cfg.N - 1, 13, 13], dtype=np.int64)
+    for n in (0, 2, cfg.H - 1, nsteps - 1):
+        ring32 = np.zeros((cfg.H, 4, cfg.N), dtype=np.float32)
+        for t in range(max(0, n - cfg.H + 1), n + 1):
+            ring32[t % cfg.H] = hist32[t]
+        ring64 = ring32.astype(np.float64)
+        E32, B32 = oracle.field(cfg, n, ring32)
+        E64, B64 = oracle.field(cfg, n, ring64)
+        assert E32.dtype == np.float64 and np.array_equal(E32, E64) and np.array_equal(B32, B64)
+        Eo32, Bo32 = oracle.field(cfg, n, ring32, obs)
+        assert np.array_equal(Eo32, E64[:, obs]) and np.array_equal(Bo32, B64[:, obs])
+        if rule == oracle.RULE_NEAREST:
+            Ed, Bd = dense_jefimenko(shape, h, dt, c, eps0, n, hist32.astype(np.float64))
+            assert np.allclose(E32, Ed, rtol=1e-11, atol=1e-12 * max(1e-300, np.abs(Ed).max()))
+            assert np.allclose(B32, Bd, rtol=1e-11, atol=1e-12 * max(1e-300, np.abs(Bd).max()))
+    # the two entries are told apart by dtype alone: a float32 ring whose values are NOT what the float64 ring holds must differ
+    ring64 = rng.uniform(-1, 1, (cfg.H, 4, cfg.N))
+    Ea, _ = oracle.field(cfg, 3 * cfg.H, ring64)
+    Eb, _ = oracle.field(cfg, 3 * cfg.H, ring64.astype(np.float32))
+    assert not np.array_equal(Ea, Eb) and np.allclose(Ea, Eb, rtol=0, atol=1e-6 * np.abs(Ea).max())
