@@ -95,6 +95,13 @@ typedef struct {
                            choice forms the sums of Eqs. 2.4-2.5 over the same pairs; only the order of the additions differs. */
 } jefi_config;
 
+/* Fill *cfg with the defaults (every member zero, which each member documents as "automatic" / SI value / device 0 / legacy
+ * stream) after checking that the caller's jefi_config has the size this library was built with: pass sizeof(jefi_config).
+ * The struct carries no size or version member, so a program compiled against an older header (the struct has grown over
+ * time, always at the end) would otherwise hand jefi_create uninitialised tail members.  Returns JEFI_OK, or JEFI_EINVAL if
+ * cfg is NULL or sizeof_cfg differs (text through jefi_last_error(NULL)); *cfg is not touched in that case.  Never needs a GPU. */
+int jefi_config_init(jefi_config* cfg, unsigned long sizeof_cfg);
+
 /* Create a context: allocates the ring (32*H*N_padded bytes, zeroed = "zero before t0"), builds the
  * delay table m(|di|,|dj|,|dk|) = floor(R/(c dt) + 1/2) in fp64 on the host (Eq. 2.6; nearest-step reading,
  * DESIGN.md §3 A1) and verifies on the device that the tiled kernel's fp32 delay arithmetic reproduces it for
@@ -231,7 +238,9 @@ int jefi_push_particles_packed(jefi_ctx* ctx, long np, float* x, float* y, float
  * not the legacy default stream, the sequence is captured into a CUDA graph on the first call (again whenever an argument
  * changes) and replayed as ONE launch afterwards: on small grids, where the kernels of a step take tens of microseconds, the
  * per-launch overhead is as large as the work.  The step counter lives on the device for the graph; it may be mixed freely with
- * the individual calls.  On the legacy default stream (not capturable) the four calls are simply issued in turn. */
+ * the individual calls.  The graph is also captured afresh when context state it depends on changes: the sort scratch (grown by
+ * another call with a longer list) or the run-deposit kernel JEFI_DEPOSIT_RUNS picks (it changes 64 deposits after the last
+ * jefi_sort_particles; replays count as deposits).  On the legacy default stream (not capturable) the four calls are simply issued in turn. */
 int jefi_pic_step(jefi_ctx* ctx, long np, float* x, float* y, float* z, float* ux, float* uy, float* uz, const float* qw,
                   const float* q_over_m, unsigned char* alive, float* rho, float* jx, float* jy, float* jz, float* ex, float* ey,
                   float* ez, float* bx, float* by, float* bz, float* eb_packed);
@@ -246,7 +255,9 @@ int jefi_field_step_host(jefi_ctx* ctx, const float* src_host, float* eb_host);
 long jefi_launch_count(const jefi_ctx* ctx);
 
 /* Duration in milliseconds of the most recent jefi_field_step's main kernel, measured with CUDA events on the
- * context's stream.  Synchronises on the end event.  < 0 if no field step ran. */
+ * context's stream.  Synchronises on the end event.  < 0 if no field step ran.  Steps that jefi_pic_step replays from its
+ * CUDA graph record no events (a graph holds none): after such steps this still reports the last field step that was issued
+ * directly (jefi_field_step*, or jefi_pic_step on the legacy default stream). */
 float jefi_last_field_kernel_ms(jefi_ctx* ctx);
 
 /* The same for the field step `calls_back` calls ago (0 = the most recent; the context keeps the events of its last 64

@@ -19,6 +19,17 @@ static int fail_create(jefi_ctx* c, int code, const std::string& msg) {
   return code;
 }
 
+extern "C" int jefi_config_init(jefi_config* cfg, unsigned long sizeof_cfg) {
+  if (!cfg || sizeof_cfg != sizeof(jefi_config)) {
+    g_create_err = !cfg ? "jefi_config_init: cfg is NULL"
+                        : "jefi_config_init: the caller's jefi_config has " + std::to_string(sizeof_cfg) + " bytes, this library's has " +
+                              std::to_string(sizeof(jefi_config)) + ": rebuild against this library's include/jefi.h";
+    return JEFI_EINVAL;
+  }
+  memset(cfg, 0, sizeof *cfg);
+  return JEFI_OK;
+}
+
 extern "C" const char* jefi_last_error(const jefi_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_err.c_str(); }
 
 extern "C" long jefi_launch_count(const jefi_ctx* ctx) { return ctx ? ctx->launches : 0; }
@@ -70,6 +81,7 @@ extern "C" int jefi_create(const jefi_config* cfg, jefi_ctx** out) {
   c->step_dev_value = -2;
   c->capturing = false;
   c->pic_exec = nullptr;
+  c->sort_gen = 0;
   c->pic_launches = 0;
   c->wmax = c->wpitch = 0;
   c->chunk = 0;
@@ -410,10 +422,19 @@ extern "C" int jefi_pic_step(jefi_ctx* c, long np, float* x, float* y, float* z,
   unsigned long long key[24] = {0};
   key[0] = (unsigned long long)np;
   for (int i = 0; i < 20; i++) key[1 + i] = (unsigned long long)(uintptr_t)ptrs[i];
+  // Context state the captured graph bakes in besides the caller's pointers: the sort scratch it scatters into (reallocated by
+  // any call that arrives with a longer list) and the run-deposit kernel, which jefi_deposit_impl picks from how long ago the
+  // caller's list was cell-sorted.  Either changing makes the key differ, so the step is captured afresh instead of replaying
+  // a graph that writes freed memory or keeps the kernel of the first step for ever.
+  key[21] = (unsigned long long)c->sort_gen;
+  key[22] = (c->sorted_np == np && c->deposits_since_sort < 64) ? 1ull : 0ull;
+  const bool replay = c->pic_exec && memcmp(key, c->pic_key, sizeof key) == 0;
+  if (replay && c->deposits_since_sort < (1 << 30)) c->deposits_since_sort++;  // a replay is a deposit too (capturing counts its own)
   if (!c->pic_exec || memcmp(key, c->pic_key, sizeof key) != 0) {
     if (c->pic_exec) { cudaGraphExecDestroy(c->pic_exec); c->pic_exec = nullptr; }
     int rc = jefi_prepare_deposit_scratch(c, np);
     if (rc != JEFI_OK) return rc;
+    key[21] = (unsigned long long)c->sort_gen;  // the scratch as it is now
     JEFI_CUDA_TRY(c, cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
     const long l0 = c->launches;
     c->capturing = true;

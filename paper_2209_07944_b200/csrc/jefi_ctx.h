@@ -117,6 +117,7 @@ struct jefi_ctx {
   unsigned *sort_count, *sort_offset, *sort_sums;  // per-bin counts, exclusive offsets, scan tile sums (+ grand total)
   int *sort_key, *sort_rank, *sort_order;          // per particle
   long sort_cap;
+  long sort_gen;                                   // bumped whenever the per-particle scratch is reallocated (part of jefi_pic_step's graph key)
   long sorted_np;                                  // np of the last jefi_sort_particles call (-1: none): the caller's list is
   int deposits_since_sort;                         // (nearly) cell-sorted for the next few steps, which decides the run-deposit kernel
   float4* eb_pack;                                 // jefi_push_particles: E, B packed two float4 per node

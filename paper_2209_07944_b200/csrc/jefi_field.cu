@@ -8,11 +8,13 @@
 // Kernels:
 //   k_field_reference  one thread per observation cell, all sources, delays from the fp64-built table (the paper's K1 in
 //                      fp32; used on request or when the fp32 delay arithmetic cannot be proven for a grid).
-//   k_field_tiled      warp-specialised CTA: 16 consumer warps own one 512-cell observation tile (one cell per thread) and
-//                      walk the 64-cell source tiles; a producer warp stages each tile's slot window [m_lo, m_hi] in a
-//                      two-stage shared-memory ring with TMA bulk copies (mbarrier full/done pipeline).  Compiled for two
-//                      tile geometries (8x8x8 / 4x4x4 cubes; 1x16x32 / 1x8x8 for nx <= 3 slabs), two window pitches and
-//                      the two retarded-time rules.  A window wider than the pitch is served in several passes.
+//   k_field_tiled      warp-specialised CTA: 16 consumer warps own one observation tile of 512 units (a unit = one cell, or a
+//                      dyad of two x-neighbour cells that share distance, delay and geometric factors) and walk the 64-cell
+//                      source tiles; a producer warp stages each tile's slot window [m_lo, m_hi] in a two-stage
+//                      shared-memory ring with TMA bulk copies (mbarrier full/done pipeline).  Compiled for three tile
+//                      geometries (8x8x8 / 4x4x4 cubes, one cell per thread; 16x8x8 / 4x4x4 dyads, two cells per thread:
+//                      the benchmark's; 1x16x32 / 1x8x8 for nx <= 3 slabs), two window pitches and the two retarded-time
+//                      rules.  A window wider than the pitch is served in several passes.
 //   k_reduce_partials  adds, in a fixed order, the partial sums of a launch that split the source range over CTAs.
 //   k_build_perm       once per context: the evaluation order of the 512 cells per relative tile offset.
 #include <stdio.h>
@@ -92,7 +94,7 @@ int jefi_launch_field_reference(jefi_ctx* c, int k0, int k1, float* ex, float* e
 // tiled kernel
 //
 // CTA = 16 consumer warps + 1 producer warp (544 threads), one CTA per SM.  The consumers own one observation tile
-// (G::OBX x G::OBY x G::OBZ = 512 cells, one per thread) against the source tiles [t0, t1) of the linear tile order (the
+// (G::OBX x G::OBY x G::OBZ cells = 512 units of G::CX cells, one unit per thread) against the source tiles [t0, t1) of the linear tile order (the
 // whole grid, or one chunk of it when the launch splits the source range over blockIdx.y; the pieces' partial sums are
 // then written to a [piece][6][N] buffer and added in a fixed order by k_reduce_partials).
 //
@@ -968,13 +970,17 @@ int jefi_tiled_prepare(jefi_ctx* c) {
   cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
   const int nobs = nobx * noby * nobz, ntiles = d.ntx * d.nty * d.ntz;
   choose_split(nobs, ntiles, nsm, c->cfg.field_chunk, c->chunk, c->nsplit);
-  if (c->nsplit > 1) {
+  // Partial sums of a split launch: 24 N bytes per piece (680 MB for 32 pieces at 96^3, 1.6 GB at 128^3).  When the ring already
+  // fills most of the device that allocation can fail; the split only buys L2 locality (0.5-2.6 % at 96^3, choose_split) or whole
+  // waves on small grids, so fall back to a quarter of the pieces each time and finally to one piece, which needs no buffer,
+  // rather than give up the tiled kernel.  jefi_get_tile_info reports the split that is in use.
+  while (c->nsplit > 1) {
     const size_t bytes = (size_t)c->nsplit * 6 * (size_t)d.N * sizeof(float);
-    if ((e = cudaMalloc(&c->partial, bytes)) != cudaSuccess) {
-      c->partial = nullptr;
-      c->err = std::string("partial-sum buffer (") + std::to_string(bytes) + " B): " + cudaGetErrorString(e);
-      return JEFI_ENOMEM;
-    }
+    if ((e = cudaMalloc(&c->partial, bytes)) == cudaSuccess) break;
+    c->partial = nullptr;
+    (void)cudaGetLastError();  // the failed allocation must not surface as the next launch's error
+    const int fewer = c->nsplit / 4;
+    choose_split(nobs, ntiles, nsm, fewer > 1 ? (ntiles + fewer - 1) / fewer : -1, c->chunk, c->nsplit);
   }
   // evaluation-order table over all relative tile offsets
   c->ndx = d.ntx + (d.obx / d.tsx) * (nobx - 1); c->ndy = d.nty + (d.oby / d.tsy) * (noby - 1); c->ndz = d.ntz + (d.obz / d.tsz) * (nobz - 1);

@@ -409,6 +409,7 @@ static int ensure_sort_scratch(jefi_ctx* c, long np) {
     JEFI_CUDA_TRY(c, cudaMalloc(&c->sort_rank, (size_t)np * sizeof(int)));
     JEFI_CUDA_TRY(c, cudaMalloc(&c->sort_order, (size_t)np * sizeof(int)));
     c->sort_cap = np;
+    c->sort_gen++;  // a captured PIC-step graph that scatters into the old buffers must not be replayed (jefi_pic_step compares this)
   }
   return JEFI_OK;
 }

@@ -29,7 +29,7 @@ EXPORTS = [
     "jefi_last_field_kernel_ms", "jefi_debug_delay_table", "jefi_debug_cell_index", "jefi_debug_history_slot",
     "jefi_debug_cell_order", "jefi_sort_particles", "jefi_field_impl_reason", "jefi_get_tile_info", "jefi_field_step_packed",
     "jefi_push_particles_packed", "jefi_field_kernel_ms", "jefi_debug_fp32_peak", "jefi_debug_check_errors", "jefi_pic_step",
-    "jefi_debug_lds128_cycles", "jefi_deposit_static",
+    "jefi_debug_lds128_cycles", "jefi_deposit_static", "jefi_config_init",
 ]
 
 
@@ -64,6 +64,8 @@ def load_library() -> C.CDLL:
     vp, f32p, u8p = C.c_void_p, C.c_void_p, C.c_void_p
     lib.jefi_create.argtypes = [C.POINTER(jefi_config), C.POINTER(vp)]
     lib.jefi_create.restype = C.c_int
+    lib.jefi_config_init.argtypes = [C.POINTER(jefi_config), C.c_ulong]
+    lib.jefi_config_init.restype = C.c_int
     lib.jefi_destroy.argtypes = [vp]
     lib.jefi_destroy.restype = None
     lib.jefi_last_error.argtypes = [vp]
@@ -152,9 +154,15 @@ def jefi_create(nx: int, ny: int, nz: int, dx: float, dy: float, dz: float, dt: 
                 delay_rule: int = JEFI_DELAY_NEAREST, shape_order: int = 1, field_chunk: int = 0,
                 field_tile: int = 0) -> int:
     lib = load_library()
-    cfg = jefi_config(nx, ny, nz, dx, dy, dz, dt, c, eps0, H, hist_cap, (C.c_double * 3)(*Eext),
-                      (C.c_double * 3)(*Bext), device, C.c_void_p(stream), field_impl, deposit_mode, delay_rule,
-                      shape_order, field_chunk, field_tile)
+    cfg = jefi_config()
+    if lib.jefi_config_init(C.byref(cfg), C.sizeof(jefi_config)) != JEFI_OK:  # this binding's struct is not the library's
+        msg = lib.jefi_last_error(None)
+        raise JefiError(f"jefi_config_init: {msg.decode() if msg else ''}")
+    (cfg.nx, cfg.ny, cfg.nz, cfg.dx, cfg.dy, cfg.dz, cfg.dt, cfg.c, cfg.eps0, cfg.H, cfg.hist_cap) = (nx, ny, nz, dx, dy, dz, dt, c, eps0, H, hist_cap)
+    cfg.Eext, cfg.Bext = (C.c_double * 3)(*Eext), (C.c_double * 3)(*Bext)
+    cfg.device, cfg.stream = device, C.c_void_p(stream)
+    (cfg.field_impl, cfg.deposit_mode, cfg.delay_rule, cfg.shape_order, cfg.field_chunk, cfg.field_tile) = (
+        field_impl, deposit_mode, delay_rule, shape_order, field_chunk, field_tile)
     h = C.c_void_p()
     rc = lib.jefi_create(C.byref(cfg), C.byref(h))
     if rc != JEFI_OK:
@@ -434,7 +442,7 @@ class JefiContext:
     launch per step (jefi_pic_step); the caller then keeps its own tensor work on that stream too."""
 
     def __init__(self, grid: GridSpec, device=None, field_impl: int = JEFI_FIELD_AUTO,
-                 deposit_mode: int = JEFI_DEPOSIT_AUTO, sort_every: int = 8, delay_rule: int = JEFI_DELAY_NEAREST,
+                 deposit_mode: int = JEFI_DEPOSIT_AUTO, sort_every: int = 0, delay_rule: int = JEFI_DELAY_NEAREST,
                  shape_order: int = 1, field_chunk: int = 0, packed_fields: bool = True, field_tile: int = 0):
         import torch
 
@@ -453,9 +461,11 @@ class JefiContext:
         self.info["field_impl_reason"] = jefi_field_impl_reason(self.handle)
         self.tile_info = jefi_get_tile_info(self.handle)
         self.H = self.info["H"]
-        # pic_step calls jefi_sort_particles every sort_every steps (0 = never).  Default 8: particles move at most c dt =
-        # dx/2 per step, and the deposit / push run 4-6x faster on a cell-sorted list.  A caller that
-        # matches particles by position in the arrays passes a "tag" array (permuted along) or sort_every=0.
+        # pic_step calls jefi_sort_particles every sort_every steps.  Default 0 = never: sorting permutes the caller's particle
+        # arrays in place, so it is something a caller asks for, not something that happens to it.  PIC loops that want the
+        # speed pass sort_every=8 (particles move at most c dt = dx/2 per step, and the deposit / push run 4-6x faster on a
+        # cell-sorted list) and, if they identify particles by array position, a "tag" array in the
+        # particle dict, which is permuted along.
         self.sort_every = int(sort_every)
         self._pic_steps = 0
         z = lambda k: torch.zeros((k, self.N), dtype=torch.float32, device=self.device)

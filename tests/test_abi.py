@@ -41,6 +41,30 @@ def test_create_rejects_bad_arguments_without_a_gpu():
     lib.jefi_destroy(None)
 
 
+def test_config_init_checks_the_struct_size_and_zeroes_it():
+    """jefi_config has no version member: jefi_config_init(cfg, sizeof) refuses a struct of another size (a caller built against an
+    older header) and otherwise fills in the all-zero defaults.  No GPU needed."""
+    from paper_2209_07944_b200 import jefi
+
+    lib = jefi.load_library()
+    cfg = jefi.jefi_config(5, 6, 7, 1.0, 2.0, 3.0, 4.0)
+    cfg.field_tile = 99
+    assert lib.jefi_config_init(ctypes.byref(cfg), ctypes.sizeof(jefi.jefi_config) - 12) == jefi.JEFI_EINVAL
+    assert b"rebuild" in lib.jefi_last_error(None) and cfg.nx == 5 and cfg.field_tile == 99  # untouched
+    assert lib.jefi_config_init(None, ctypes.sizeof(jefi.jefi_config)) == jefi.JEFI_EINVAL
+    assert lib.jefi_config_init(ctypes.byref(cfg), ctypes.sizeof(jefi.jefi_config)) == jefi.JEFI_OK
+    assert bytes(cfg) == bytes(ctypes.sizeof(jefi.jefi_config))
+    # the binding's mirror of the struct matches the header member for member (same count, same order)
+    text = open(os.path.join(ROOT, "include", "jefi.h")).read()
+    body = re.sub(r"/\*.*?\*/", "", text[text.index("typedef struct {"):text.index("} jefi_config;")], flags=re.S)
+    names = []
+    for decl in body.split(";"):
+        decl = decl.replace("typedef struct {", "").strip()
+        if decl:
+            names += [re.sub(r"\[.*\]", "", n).strip(" *") for n in decl.split(None, 1)[1].split(",")]
+    assert names == [f[0] for f in jefi.jefi_config._fields_], names
+
+
 def test_product_does_not_import_the_oracle():
     """The oracle is test infrastructure: nothing under the package, bench's product arm or include/ may name it."""
     pkg = os.path.join(ROOT, "paper_2209_07944_b200")

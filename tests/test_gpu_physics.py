@@ -33,7 +33,7 @@ def to_dev(part, device):
 def run_planar_emission(J, count, variant):
     w = wl.SLABS["planar_emission"]
     nx, ny, nz = w.shape
-    ctx = J.JefiContext(J.GridSpec(nx, ny, nz, w.dx, w.dx, w.dx, w.dt, Bext=w.Bext))
+    ctx = J.JefiContext(J.GridSpec(nx, ny, nz, w.dx, w.dx, w.dx, w.dt, Bext=w.Bext), sort_every=8)
     assert ctx.info["field_impl"] == J.JEFI_FIELD_TILED, ctx.info["field_impl_reason"]
     dp = to_dev(wl.slab_particles("planar_emission", count, variant), ctx.device)
     y0 = dp["y"].clone().double()
@@ -91,7 +91,7 @@ def test_time_step_insensitivity_of_the_point_emission_field(J):
     t_end = 0.6e-9
     series = {}
     for dt in (2e-14, 1e-13, 5e-12):
-        ctx = J.JefiContext(J.GridSpec(nx, ny, nz, w.dx, w.dx, w.dx, dt))
+        ctx = J.JefiContext(J.GridSpec(nx, ny, nz, w.dx, w.dx, w.dx, dt), sort_every=8)
         assert ctx.info["field_impl"] == J.JEFI_FIELD_TILED, (dt, ctx.info["field_impl_reason"])
         dp = to_dev(part, ctx.device)
         nsteps = int(round(t_end / dt))

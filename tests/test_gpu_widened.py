@@ -459,6 +459,107 @@ def test_pic_step_graph_closed_loop(J, config, steps):
     ctx.close()
 
 
+def test_pic_step_graph_past_the_ring_wrap_with_tiles_that_empty_and_refill(J):
+    """The captured graph takes n, the ring slot and the previous slot from device memory (k_advance_step), and k_push_sources
+    writes the per-tile span of non-zero steps with that device-side n.  Config 1 (16^3, H = 58) for 72 steps, EVERY step a
+    graph replay on a side stream, so the ring wraps under the graph; during steps 20-27 all particles are
+    marked dead, so every source tile empties and refills under the graph and the field kernel's tile skipping works from
+    spans the graph wrote.  Closed loop against the full fp64 oracle: fields at steps 19, 27 (silent
+    sources, earlier ones still in flight), 57, 58 (first wrapped step) and 71, trajectories at the end."""
+    import torch
+
+    w = wl.WORKLOADS[1]
+    part = wl.particles(1)
+    cfg = OracleConfig(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt)
+    assert cfg.H == 58
+    orc = oracle.OracleJefi(cfg)
+    po = {k: v.astype(np.float64) for k, v in part.items() if k != "alive"}
+    po["alive"] = part["alive"].copy()
+    steps, silent, look = 72, range(20, 28), (19, 27, 57, 58, 71)
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        ctx = J.JefiContext(J.GridSpec(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt), sort_every=0)
+        assert ctx.stream_handle != 0 and ctx.H == 58 and ctx.info["field_impl"] == J.JEFI_FIELD_TILED
+        dp = to_dev(part, ctx.device)
+        saved_gpu = saved_orc = None
+        per_step, l_prev = [], ctx.launch_count()
+        for s in range(steps):
+            if s == silent[0]:
+                saved_gpu, saved_orc = dp["alive"].clone(), po["alive"].copy()
+                dp["alive"].zero_()  # in place: the captured pointers stay the same, the graph is not re-captured
+                po["alive"][:] = 0
+            if s == silent[-1] + 1:
+                dp["alive"].copy_(saved_gpu)
+                po["alive"][:] = saved_orc
+            ctx.pic_step(dp)
+            So, Eo, Bo = orc.pic_step(po)
+            per_step.append(ctx.launch_count() - l_prev)
+            l_prev = ctx.launch_count()
+            if s in look:
+                side.synchronize()
+                eb = ctx.EB.cpu().numpy()
+                assert_field_parity(eb[:3], eb[3:], Eo, Bo, f"cfg1 graph step {s}: ")
+                S = ctx.src.cpu().numpy()
+                if s in silent:
+                    assert not S.any() and not np.any(So)  # nothing deposited, yet the fields above are not zero
+                    assert np.linalg.norm(Eo) > 0
+                for a in range(4):
+                    assert np.linalg.norm(S[a] - So[a]) <= 1e-5 * max(np.linalg.norm(So[a]), 1e-300), (s, a)
+        side.synchronize()
+        assert J.jefi_get_info(ctx.handle)["step"] == steps - 1
+        got = {k: v.cpu().numpy() for k, v in dp.items()}
+    assert len(set(per_step[1:])) == 1, per_step  # one captured graph replayed throughout: same kernel count every step
+    both = (got["alive"] == 1) & (po["alive"] == 1)
+    assert (got["alive"] != po["alive"]).sum() <= 2 and both.sum() > 0.5 * both.size
+    for k in "xyz":
+        err = np.abs(got[k][both] - po[k][both]).max() / w.n
+        print(f"cfg1 graph, 72 steps: max |d{k}| / n = {err:.2e}")
+        assert err <= 1e-5, (k, err)
+    ctx.close()
+
+
+def test_partial_sum_buffer_falls_back_to_fewer_pieces_when_memory_is_short(J):
+    """On large grids the tiled kernel splits the source range into 32 pieces whose partial sums take 24 N bytes each (0.68 GB
+    at 96^3).  When the ring leaves too little memory for that buffer, the context must keep the tiled kernel with fewer pieces
+    (a quarter each time, finally one, which needs no buffer) instead of failing over to the reference kernel.  Here the device
+    is filled up to ring + ~0.45 GB before jefi_create; the fields (shallow history, sampled cells) still meet the oracle."""
+    import torch
+
+    n, dx = 96, 1e-4
+    dt = dx / (2 * C)
+    N = n ** 3
+    cfg = OracleConfig(n, n, n, dx, dx, dx, dt)
+    dev = torch.device("cuda:0")
+    slices = [wl.history_slice(N, t, 4242, j_scale=C) for t in range(3)]
+    dsl = [torch.from_numpy(s).to(dev) for s in slices]
+    out = torch.zeros((6, N), dtype=torch.float32, device=dev)
+    torch.cuda.synchronize()
+    torch.cuda.empty_cache()
+    ring_bytes = 32 * cfg.H * (n // 4) ** 3 * 64 + (n // 4) ** 3 * cfg.H * 16  # [tile][slot] rows of 2064 B
+    free, _ = torch.cuda.mem_get_info(dev)
+    leave = ring_bytes + 450 * 2 ** 20  # < 32 pieces x 24 N = 679 MB, > 8 pieces (170 MB) + order table (~95 MB) + this test's tensors
+    hog = torch.empty(max(free - leave, 1), dtype=torch.uint8, device=dev) if free > leave else None
+    try:
+        ctx = J.JefiContext(J.GridSpec(n, n, n, dx, dx, dx, dt), packed_fields=False)
+        assert ctx.info["field_impl"] == J.JEFI_FIELD_TILED, ctx.info["field_impl_reason"]
+        split = ctx.tile_info["source_split"]
+        print(f"free {free / 2**30:.1f} GiB, left {leave / 2**30:.2f} GiB for the context: source range in {split} piece(s)")
+        assert 1 <= split < 32, ctx.tile_info
+        for d in dsl:
+            ctx.push_sources(d)
+        eb = ctx.field_step(out).cpu().numpy()
+        ctx.close()
+    finally:
+        del hog
+        torch.cuda.empty_cache()
+    ring = np.zeros((cfg.H, 4, N), dtype=np.float32)
+    for t, s in enumerate(slices):
+        ring[t] = s
+    obs = wl.sample_obs(n, 48, 4242)
+    Eo, Bo = oracle.field(cfg, 2, ring, obs)
+    assert_field_parity(eb[:3][:, obs], eb[3:][:, obs], Eo, Bo, f"96^3 with {split} piece(s): ")
+
+
 # ------------------------------------------------------------------------------------ empty source tiles / light cone of t0
 @pytest.mark.parametrize("tile", ["CELL", "DYAD"])
 @pytest.mark.parametrize("rule", ["NEAREST", "LINEAR"])
