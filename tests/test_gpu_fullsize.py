@@ -99,7 +99,7 @@ def test_config2_closed_loop_10_steps_full_oracle(J):
     cfg = OracleConfig(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt)
     import torch
 
-    ctx = J.JefiContext(J.GridSpec(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt))  # default: cell sort every 8 steps
+    ctx = J.JefiContext(J.GridSpec(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt), sort_every=8)  # cell sort every 8 steps, matched through the tag
     assert ctx.H == w.H and ctx.info["field_impl"] == J.JEFI_FIELD_TILED
     dp = to_dev(part, ctx.device)
     dp["tag"] = torch.arange(part["x"].shape[0], dtype=torch.int32, device=ctx.device)
@@ -138,7 +138,7 @@ def test_config3_closed_loop_10_steps_golden(J):
     w = wl.WORKLOADS[3]
     part = wl.particles(3)
     P = part["x"].shape[0]
-    ctx = J.JefiContext(J.GridSpec(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt))
+    ctx = J.JefiContext(J.GridSpec(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt), sort_every=8)
     assert ctx.H == w.H and ctx.info["field_impl"] == J.JEFI_FIELD_TILED
     dp = to_dev(part, ctx.device)
     dp["tag"] = torch.arange(P, dtype=torch.int32, device=ctx.device)
@@ -179,7 +179,7 @@ def test_pic_configs_sampled_parity(J, config, steps, nsample):
     """64^3 / 128^3 PIC configs: run `steps` steps on the GPU, then per-kernel parity on its own state."""
     w = wl.WORKLOADS[config]
     part = wl.particles(config)
-    ctx = J.JefiContext(J.GridSpec(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt))
+    ctx = J.JefiContext(J.GridSpec(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt), sort_every=8)
     assert ctx.H == w.H and ctx.info["field_impl"] == J.JEFI_FIELD_TILED
     dp = to_dev(part, ctx.device)
     for s in range(steps):
@@ -219,6 +219,49 @@ def test_config4_field_only_sampled_parity(J, rule, nsample):
         assert l2 <= 1e-4, f"cfg4 {name}: rel-L2 {l2:.3e}"
         assert mx <= 1e-3, f"cfg4 {name}: max-abs/rms {mx:.3e}"
     ctx.close()
+
+
+def test_config5_grid_field_at_full_history_depth_sampled_parity(J):
+    """128^3 x 128^3 (BASELINE.json configs[4]'s grid), H = 446, EVERY slot full: the one shape whose index ranges no other
+    test reaches at depth (32 768 source tiles x 446 ring rows = 30 GB, 32 source pieces, a 1.6 GB partial-sum buffer, windows
+    that wrap).  test_pic_configs_sampled_parity[5-10-1024] runs from t0 and only ever sees delays m <= 9 of 444.  Here 446
+    random slices (the config-4 recipe on the config-5 grid, J scaled by c) are pushed, then ONE jefi_field_step in the launch
+    configuration bench.py's PIC leg times, and the fp64 oracle evaluates Eqs. 2.4-2.6 at 1024 + 15 sampled
+    cells against all 2 097 151 sources; the same ring again under the second retarded-time rule (512 + 15 cells)."""
+    import torch
+
+    w = wl.WORKLOADS[5]
+    avail_gb = 0.0
+    for line in open("/proc/meminfo"):
+        if line.startswith("MemAvailable:"):
+            avail_gb = int(line.split()[1]) / 1e6
+    ring_gb = w.H * 4 * w.N * 4 / 1e9
+    if avail_gb < ring_gb + 8:
+        pytest.skip(f"host has {avail_gb:.0f} GB available; the oracle's fp32 ring of this case needs {ring_gb:.0f} GB")
+    ring = np.empty((w.H, 4, w.N), dtype=np.float32)
+    for t in range(w.H):
+        ring[t] = wl.history_slice(w.N, t, w.seed, j_scale=wl.C_SI)
+    for rule, nsample in (("NEAREST", 1024), ("LINEAR", 512)):
+        ctx = J.JefiContext(J.GridSpec(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt), delay_rule=getattr(J, "JEFI_DELAY_" + rule))
+        assert ctx.H == w.H == 446 and ctx.info["field_impl"] == J.JEFI_FIELD_TILED, ctx.info["field_impl_reason"]
+        assert ctx.tile_info["obs_tile"] == (16, 8, 8) and ctx.tile_info["source_split"] == 32, ctx.tile_info
+        for t in range(w.H):
+            ctx.push_sources(torch.from_numpy(ring[t]).to(ctx.device))
+        ctx.field_step()
+        ms = ctx.last_field_kernel_ms()
+        cfg = OracleConfig(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt, delay_rule=getattr(oracle, "RULE_" + rule))
+        obs = wl.sample_obs(w.n, nsample, w.seed)
+        Eo, Bo = oracle.field(cfg, w.H - 1, ring, obs)
+        eb = ctx.EB.cpu().numpy()
+        for name, F, Fo in (("E", eb[:3][:, obs], Eo), ("B", eb[3:][:, obs], Bo)):
+            l2, mx = sampled_field_err(F, Fo)
+            print(f"cfg5 grid, full depth, {rule}: {name} rel-L2 {l2:.2e}, max-abs/rms {mx:.2e}, field kernel {ms:.0f} ms")
+            assert l2 <= 1e-4, f"cfg5 full depth {rule} {name}: rel-L2 {l2:.3e}"
+            assert mx <= 1e-3, f"cfg5 full depth {rule} {name}: max-abs/rms {mx:.3e}"
+        assert np.isfinite(eb).all()
+        ctx.close()
+        del ctx
+        torch.cuda.empty_cache()
 
 
 @pytest.mark.parametrize("which,count,steps", [("point_emission", 100000, 12), ("column_in_By", 100000, 8)])
@@ -279,12 +322,15 @@ def test_paper_slab_workloads_closed_loop(J, which, count, steps):
     # of cells around the charge (peak/RMS ~ 15-75), so the max-norm bound is taken against the peak (reading A20b; both forms
     # are printed).  B of the point emission is ill-conditioned in the sources: the emission is isotropic, so B is the small
     # residual of cancelling currents and its J-dot term a difference of two nearly equal deposits; sources within the
-    # deposit bound of the oracle's already move it by `sens` (~1e-4 .. 1e-3).  Bound: max(1e-4, sens).
+    # deposit bound of the oracle's already move it by `sens` (~1e-4 .. 1e-3).  Bound: 1e-4, and max(1e-4, sens) for that one case;
+    # `sens` is printed for every case.
     for name, F, Fo, FoP in (("E", eb[:3], Eo, EoP), ("B", eb[3:], Bo, BoP)):
         l2, mx_rms = sampled_field_err(F, Fo)
         mx_peak = np.abs(F - Fo).max() / np.abs(Fo).max()
         sens = np.linalg.norm(FoP - Fo) / np.linalg.norm(Fo)
-        tol = max(1e-4, sens)
+        # north_star's 1e-4 everywhere; the sensitivity bound only for the one named case measured at the bar itself (B of the
+        # point emission: 3e-5 .. 1e-4 from run to run with the order of the deposit's atomics, DESIGN.md section 3 A20b)
+        tol = max(1e-4, sens) if (which, name) == ("point_emission", "B") else 1e-4
         print(f"{which} {name} closed loop: rel-L2 {l2:.2e} (oracle fields under a 1e-5 source perturbation move by {sens:.2e}; bound {tol:.2e})  "
               f"max-abs/RMS {mx_rms:.2e}  max-abs/peak {mx_peak:.2e}  peak/RMS {np.abs(Fo).max() / (np.linalg.norm(Fo) / np.sqrt(Fo.size)):.1f}")
         assert l2 <= tol and mx_peak <= 1e-3, (which, name, l2, tol, mx_peak, ctx.info["field_impl"])
