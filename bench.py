@@ -14,9 +14,11 @@ in between).  `e2e` repeats it through jefi_field_step_host with pinned HOST buf
 printed whole-run set-up (1x251x111, 1e7 macro-particles, 1e4 steps) as a whole.
 Reference arm (--impl reference): the fp64 CPU oracle, as it stands, on a bounded sample of the same workload.
 N > 1: one process per GPU.  Under torchrun (WORLD_SIZE set) this process is one rank; without it `--gpus N` re-executes
-itself under `python -m torch.distributed.run --nproc-per-node N` so that N ranks really run.  Default: replicas
-(every rank runs the same workload on its own GPU, no data-path collective); `--shard obs` splits the
-observation planes of ONE step over the ranks and assembles E, B with an NCCL all-reduce.
+itself under `python -m torch.distributed.run --nproc-per-node N` so that N ranks really run.  Default for N > 1: `--shard obs`
+(DESIGN.md section 9): the observation planes of ONE field step are split over the ranks, E, B are
+assembled with an NCCL all-gather, `"scaling": "strong"`; the `pic_sharded` leg runs whole PIC steps that way (particles dealt
+to ranks, all-reduce of rho, J, slab solve, all-gather of E, B: paper_2209_07944_b200/sharded.py).  `--shard replicas`: every
+rank runs the same workload on its own GPU with no data-path collective (`"scaling": "weak"`).
 """
 from __future__ import annotations
 
@@ -46,8 +48,17 @@ FLOP_PER_PAIR = 48.0  # 24 FMA per source-observation pair
 # `traffic` is null and `traffic_source` says the capture is stale.
 FIELD_DRAM_BYTES = {
     # (workload name, rule): (bytes, profile, kernel source sha)
-    ("cfg4_96c_field_only", "nearest"): (93.108966e9 + 783.064576e6, "profiles/r2o_field_tiled_ncu_full.md", "a97fcdd1e225"),
-    ("cfg4_96c_field_only", "linear"): (52.037499e9 + 704.273408e6, "profiles/r2o_field_tiled_ncu_full.md", "a97fcdd1e225"),
+    ("cfg4_96c_field_only", "nearest"): (91.143151e9 + 707.036928e6, "profiles/r3b_field_tiled_ncu_full.md", "cece236078a7"),
+    ("cfg4_96c_field_only", "linear"): (53.111260e9 + 706.341376e6, "profiles/r3b_field_tiled_ncu_full.md", "cece236078a7"),
+}
+# From the same captures: how busy the FMA pipe and the shared-memory data pipe were (sm__pipe_fma_cycles_active and
+# l1tex__data_pipe_lsu_wavefronts_mem_shared, % of peak sustained elapsed) and the FP32 lane-operations the kernel EXECUTES per
+# source-observation pair ((64 FFMA2 + 32 (FFMA + FMUL + FADD)) thread-instructions / pairs).  `roofline.achieved` counts the
+# survey's 48 FLOP per pair whatever the kernel executes, so it is an ALGORITHMIC rate: the dyad geometry evaluates distance,
+# delay and geometric factors once for two pairs and executes fewer.  These figures say how full the pipes really were.
+FIELD_PIPES = {
+    ("cfg4_96c_field_only", "nearest"): {"fma_pipe_busy": 0.679, "smem_data_pipe_busy": 0.947, "fp32_lane_ops_per_pair": 20.2},
+    ("cfg4_96c_field_only", "linear"): {"fma_pipe_busy": 0.698, "smem_data_pipe_busy": 0.778, "fp32_lane_ops_per_pair": None},
 }
 
 
@@ -67,6 +78,14 @@ def field_traffic(name: str, rule: str):
     if sha != kernel_source_sha():
         return None, f"stale: {prof} was captured on kernel source {sha}, this build is {kernel_source_sha()}"
     return nbytes, prof
+
+
+def field_pipes(name: str, rule: str):
+    """Pipe utilisation of the field kernel from the sha-matched ncu capture (None when there is none for this source)."""
+    ent = FIELD_DRAM_BYTES.get((name, rule))
+    if ent is None or ent[2] != kernel_source_sha():
+        return None
+    return FIELD_PIPES.get((name, rule))
 
 
 def log(*a):
@@ -160,8 +179,16 @@ def host_ring(w: wl.FieldWorkload) -> np.ndarray:
 
 def workload_config(w: wl.FieldWorkload, rule: str) -> dict:
     """The `config` object both arms print (same keys, so that the driver can match the two lines)."""
+    ring_gb = 32.0 * w.H * w.N / 1e9  # the device ring of the product arm (32 B per cell-slot, before tile padding)
     return {"workload": w.name, "grid": list(w.shape), "H": w.H, "dx": w.h[0], "dt": w.dt, "kappa": round(w.kappa, 6),
-            "pairs_per_step": float(w.N) * float(w.N - 1), "delay_rule": rule}
+            "pairs_per_step": float(w.N) * float(w.N - 1), "delay_rule": rule,
+            "l2": (f"inputs ({ring_gb:.1f} GB ring) larger than L2, no flush" if not ring_needs_flush(32 * w.H * w.N)
+                   else "512 MB fill between timed steps")}
+
+
+def ring_needs_flush(ring_bytes: float) -> bool:
+    """Inputs larger than L2 need no flush; a ring that would (nearly) fit in the 126 MB L2 is flushed between timed steps."""
+    return ring_bytes < 512 * 1024 * 1024
 
 
 def run_reference(args, w: wl.FieldWorkload) -> dict:
@@ -201,19 +228,53 @@ def max_over_ranks(dist, ms: float, device) -> float:
     return float(t.item())
 
 
-def assemble_slabs(dist, EB, plane: int, k0: int, k1: int) -> None:
-    """--shard obs: every rank has computed the observation planes [k0, k1) of EB ([6][N], plane = nx*ny cells per
-    z-plane); zero the rest and sum over ranks, so that every rank ends up with the whole E, B (24 N bytes over NVLink,
-    the all-gather of SURVEY.md §8(e) written as an all-reduce because slabs need not be equal)."""
-    EB[:, :plane * k0] = 0
-    EB[:, plane * k1:] = 0
-    if dist is not None:
-        dist.all_reduce(EB, op=dist.ReduceOp.SUM)
+def assemble_slabs(dist, EB, plane: int, ranges, rank: int) -> None:
+    """--shard obs: rank r has computed the observation planes ranges[r] = [k0, k1) of EB ([6][N], plane = nx*ny cells per
+    z-plane); one all-gather over the slabs (24 N bytes per rank) leaves every rank with the whole E, B."""
+    from paper_2209_07944_b200.sharded import gather_slabs
+
+    gather_slabs(dist, EB, plane, ranges, rank)
 
 
 def aggregate_rate(world: int, pairs_per_rank: float, ms_max: float) -> float:
     """Whole-job Gpairs/s: every rank processed pairs_per_rank pairs (replicas) in ms_max."""
     return world * pairs_per_rank / (ms_max * 1e-3) / 1e9
+
+
+def time_pic_sharded(J, torch, device, dist, rank: int, world: int, config: int, steps: int, warmup: int) -> dict:
+    """Whole PIC steps of one config over `world` ranks (paper_2209_07944_b200/sharded.py): particles dealt
+    to the ranks, per step one all-reduce of rho, J (16 N bytes) and one all-gather of E, B (24 N bytes), each rank solving its
+    observation slab.  `steps` steps from t0 on a fresh context, CUDA events on every rank, max over ranks.  Every rank calls this."""
+    from paper_2209_07944_b200.sharded import ShardedPic, deal_particles
+
+    w = wl.WORKLOADS[config]
+    mine0 = deal_particles(wl.particles(config), rank, world)
+
+    def run(nsteps: int):
+        ctx = J.JefiContext(J.GridSpec(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt), device=device, packed_fields=False)
+        dp = {k: torch.from_numpy(np.ascontiguousarray(v)).to(device) for k, v in mine0.items()}
+        sp = ShardedPic(ctx, dist, rank, world)
+        dist.barrier()
+        torch.cuda.synchronize(device)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(nsteps):
+            sp.step(dp)
+        e1.record()
+        dist.barrier()
+        torch.cuda.synchronize(device)
+        alive = dp["alive"].sum().to(torch.float64).reshape(1)
+        dist.all_reduce(alive)
+        res = (e0.elapsed_time(e1), int(alive.item()), sp.ranges, sp.bytes_per_step, ctx.info["field_impl"])
+        ctx.close()
+        return res
+
+    run(warmup)
+    ms, alive, ranges, nbytes, impl = run(steps)
+    ms = max_over_ranks(dist, ms, device)
+    return {"workload": w.name, "ranks": world, "steps": steps, "from": "t0", "total_ms": ms, "steps_per_s": 1e3 * steps / ms,
+            "alive_at_end": alive, "slabs": ranges, "bytes_per_step_per_rank": nbytes, "field_impl": impl,
+            "how": "ShardedPic.step: deposit, all-reduce(rho, J), push_sources, field_step_slab, all-gather(E, B), push_particles"}
 
 
 def time_pic(J, torch, device, config: int, steps: int, warmup: int) -> dict:
@@ -229,14 +290,14 @@ def time_pic(J, torch, device, config: int, steps: int, warmup: int) -> dict:
     side = torch.cuda.Stream(device)
     with torch.cuda.stream(side):
         if warmup > 0:
-            wctx = J.JefiContext(J.GridSpec(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt), device=device)
+            wctx = J.JefiContext(J.GridSpec(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt), device=device, sort_every=8)
             wpart = {k: torch.from_numpy(v).to(device) for k, v in wl.particles(config).items()}
             for _ in range(warmup):
                 wctx.pic_step(wpart)
             side.synchronize()
             wctx.close()
             del wpart
-        ctx = J.JefiContext(J.GridSpec(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt), device=device)
+        ctx = J.JefiContext(J.GridSpec(w.n, w.n, w.n, w.dx, w.dx, w.dx, w.dt), device=device, sort_every=8)
         part = {k: torch.from_numpy(v).to(device) for k, v in wl.particles(config).items()}
         side.synchronize()
         evs = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
@@ -278,7 +339,7 @@ def time_paper_run(J, torch, device, count: int = 10_000_000, steps: int = 10_00
     nx, ny, nz = w.shape
     side = torch.cuda.Stream(device)
     with torch.cuda.stream(side):
-        ctx = J.JefiContext(J.GridSpec(nx, ny, nz, w.dx, w.dx, w.dx, w.dt, Bext=w.Bext), device=device)
+        ctx = J.JefiContext(J.GridSpec(nx, ny, nz, w.dx, w.dx, w.dx, w.dt, Bext=w.Bext), device=device, sort_every=8)
         part = {k: torch.from_numpy(v).to(device) for k, v in wl.slab_particles("planar_emission", count).items()}
         side.synchronize()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -289,8 +350,37 @@ def time_paper_run(J, torch, device, count: int = 10_000_000, steps: int = 10_00
         side.synchronize()
         ms = e0.elapsed_time(e1)
         alive = int(part["alive"].sum().item())
+        # what a step of this workload is made of: 200 further steps through the five individual calls
+        # (the graph's contents, issued one by one) with a CUDA event between calls; the state is the run's own at its end
+        names = ("sort_every_8", "deposit", "push_sources", "field_step_packed", "push_particles_packed")
+        tot = {k: 0.0 for k in names}
+        bsteps = 200
+        evs = []
+        for i in range(bsteps):
+            ev = [torch.cuda.Event(enable_timing=True) for _ in range(6)]
+            ev[0].record(side)
+            if i % 8 == 0:
+                ctx.sort_particles(part)
+            ev[1].record(side)
+            ctx.deposit(part)
+            ev[2].record(side)
+            ctx.push_sources()
+            ev[3].record(side)
+            ctx.field_step_packed()
+            ev[4].record(side)
+            ctx.push_particles_packed(part)
+            ev[5].record(side)
+            evs.append(ev)
+        side.synchronize()
+        for ev in evs:
+            for j, k in enumerate(names):
+                tot[k] += ev[j].elapsed_time(ev[j + 1])
+        breakdown = {k: v / bsteps for k, v in tot.items()}
+        breakdown["sum_ms_per_step"] = sum(tot.values()) / bsteps
+        breakdown["how"] = f"{bsteps} steps after the run, the five C-ABI calls issued one by one on the same stream, CUDA events between them (ms per step)"
     out = {"workload": w.name, "grid": [nx, ny, nz], "particles": count, "steps": steps, "simulated_ns": steps * w.dt * 1e9,
            "total_s": ms * 1e-3, "steps_per_s": 1e3 * steps / ms, "alive_at_end": alive, "field_impl": ctx.info["field_impl"], "tiles": ctx.tile_info,
+           "ms_per_call": breakdown,
            "paper": "JefiPIC: 'within only half an hour' on one A100, fp64 (PAPER.md:372); UNIPIC: 'over 6 hours' on a Xeon workstation"}
     ctx.close()
     return out
@@ -444,7 +534,7 @@ def run_product(args, w: wl.FieldWorkload) -> dict:
                         delay_rule=J.JEFI_DELAY_LINEAR if args.delay_rule == "linear" else J.JEFI_DELAY_NEAREST)
     N, H = w.N, ctx.H
     assert H == w.H
-    keep_host = (rank == 0 and world == 1 and not args.no_cpu_baseline)
+    keep_host = (rank == 0 and not args.no_cpu_baseline)  # rank 0 times the oracle at every N (after the timed region; the other ranks wait)
     ring_host = np.empty((H, 4, N), dtype=np.float32) if keep_host else None
     log(f"[rank {rank}/{world}] {w.name}: N={N} H={H} ring={ctx.info['ring_bytes'] / 1e9:.2f} GB; {ctx.info['field_impl_reason']}")
     t0 = time.perf_counter()
@@ -460,7 +550,7 @@ def run_product(args, w: wl.FieldWorkload) -> dict:
     fresh = [torch.from_numpy(w.slice(H + i)).to(device) for i in range(min(nfresh, 8))]
     pairs = float(N) * float(N - 1)
     # inputs larger than L2 need no flush; a ring that would (nearly) fit in the 126 MB L2 is flushed between steps
-    need_flush = ctx.info["ring_bytes"] < 512 * 1024 * 1024
+    need_flush = ring_needs_flush(32 * H * N)  # the same rule workload_config() states in `config.l2` (both arms print it)
     flush = torch.empty(128 * 1024 * 1024, dtype=torch.float32, device=device) if need_flush else None
 
     def barrier():
@@ -472,13 +562,14 @@ def run_product(args, w: wl.FieldWorkload) -> dict:
     # assembled over NVLink (strong scaling of ONE field step).  Default: replicas.
     shard = args.shard == "obs" and dist is not None
     nz = w.shape[2]
-    k0, k1 = ctx.slab_range(rank, world) if shard else (0, nz)
+    ranges = [ctx.slab_range(r, world) for r in range(world)] if shard else [(0, nz)]
+    k0, k1 = ranges[rank] if shard else (0, nz)
     plane = w.shape[0] * w.shape[1]
 
     def field_step():
         if shard:
             ctx.field_step_slab(k0, k1)
-            assemble_slabs(dist, ctx.EB, plane, k0, k1)
+            assemble_slabs(dist, ctx.EB, plane, ranges, rank)
         else:
             ctx.field_step()
 
@@ -543,10 +634,14 @@ def run_product(args, w: wl.FieldWorkload) -> dict:
               "ffma_3reg": J.jefi_debug_fp32_peak(ctx.handle, 2), "ffma2_3reg": J.jefi_debug_fp32_peak(ctx.handle, 3)} if rank == 0 else None)
     lds = ({k: J.jefi_debug_lds128_cycles(ctx.handle, i) for i, k in enumerate(("broadcast", "lane_pairs_share", "32_rows", "one_pair_differs",
                                                                                 "pairs_share_rows_8_apart"))} if rank == 0 else None)
-    impl, reason, tiles = ctx.info["field_impl"], ctx.info["field_impl_reason"], ctx.tile_info
+    impl, reason, tiles, ring_bytes = ctx.info["field_impl"], ctx.info["field_impl_reason"], ctx.tile_info, ctx.info["ring_bytes"]
     ctx.close()
     del flush
     torch.cuda.empty_cache()
+
+    pic_sharded = None
+    if dist is not None and shard and not args.no_pic:  # every rank takes part; BASELINE.json's config 3 for its 200 steps from t0
+        pic_sharded = time_pic_sharded(J, torch, device, dist, rank, world, 3, 200, 3)
 
     out = None
     if rank == 0:
@@ -554,16 +649,21 @@ def run_product(args, w: wl.FieldWorkload) -> dict:
         peak = fp32_peak_tflops(sm_max)
         achieved = FLOP_PER_PAIR * pairs_per_launch / (kernel_ms * 1e-3) / 1e12
         traffic, traffic_src = field_traffic(w.name, args.delay_rule)
-        cfg = workload_config(w, args.delay_rule)
-        cfg.update({"l2": "512 MB fill between timed steps" if need_flush else f"inputs ({ctx.info['ring_bytes'] / 1e9:.1f} GB ring) larger than L2, no flush",
-                    "parallelism": ("obs_slabs" if shard else "replicas") if dist is not None else "single", "field_impl": impl,
-                    "field_impl_reason": reason, "tiles": tiles})
+        cfg = workload_config(w, args.delay_rule)  # identical in both arms; what only this arm has goes to `launch`
+        launch = {"parallelism": ("obs_slabs" if shard else "replicas") if dist is not None else "single", "field_impl": impl,
+                  "field_impl_reason": reason, "tiles": tiles, "ring_bytes": ring_bytes}
+        pipes = field_pipes(w.name, args.delay_rule)
         out = {"metric": "jefimenko_source_obs_pairs_per_s", "value": value, "unit": "Gpairs/s", "n_gpus": world,
                "steps": args.steps, "warmup": args.warmup, "ms_per_step": step_ms_max, "higher_is_better": True,
                "scaling": "strong" if shard else "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-               "config": cfg,
+               "config": cfg, "launch": launch,
                "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
                             "traffic": traffic, "traffic_source": traffic_src,
+                            "achieved_kind": "algorithmic: 48 FLOP (24 FMA, SURVEY.md 8(d)) per source-observation pair x pairs / kernel time, "
+                                             "whatever the kernel executes; fma_pipe_busy is the pipe's own utilisation",
+                            "fma_pipe_busy": pipes["fma_pipe_busy"] if pipes else None,
+                            "smem_data_pipe_busy": pipes["smem_data_pipe_busy"] if pipes else None,
+                            "fp32_lane_ops_per_pair_executed": pipes["fp32_lane_ops_per_pair"] if pipes else None,
                             "kernel": "k_field_tiled" if impl == 2 else "k_field_reference",
                             "kernel_ms": kernel_ms, "kernel_ms_source": f"CUDA events around the field kernel of the {len(kms)} timed steps",
                             "flop_per_pair": FLOP_PER_PAIR, "peak_source": PEAK_SOURCE, "kernel_source_sha": kernel_source_sha(),
@@ -578,6 +678,8 @@ def run_product(args, w: wl.FieldWorkload) -> dict:
                "e2e": {"value": e2e_val, "unit": "Gpairs/s", "h2d_bytes_per_step": 16 * N, "d2h_bytes_per_step": 24 * N,
                        "ms_per_step": e2e_ms_max, "checksum_abs_ex": checksum},
                "gpu_launches": int(launches), "clocks": clocks}
+        if pic_sharded is not None:
+            out["pic_sharded"] = pic_sharded
         if not args.no_pic and world == 1:
             out["pic"] = []
             for cfgno, st, wu in ((1, 64, 3), (2, 100, 3), (3, 200, 3), (5, 50, 2)):  # BASELINE.json's run lengths
@@ -639,8 +741,8 @@ def main():
                     "the paper's own shapes: analytic20 (20^3, kappa = 6), slab251 (1x251x111), slab101")
     ap.add_argument("--no-pic", action="store_true", help="skip the PIC steps/s, paper-workload and particle-kernel legs")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--shard", default="replicas", choices=["replicas", "obs"],
-                    help="N > 1: replicas (default, weak scaling) or observation z-slabs of one field step (strong scaling)")
+    ap.add_argument("--shard", default="obs", choices=["replicas", "obs"],
+                    help="N > 1: observation z-slabs of one field step (default, strong scaling) or replicas (weak scaling)")
     ap.add_argument("--delay-rule", default="nearest", choices=["nearest", "linear"],
                     help="retarded-time rule: nearest = BASELINE.json's configs (reading A1); linear = second rule (A22)")
     ap.add_argument("--particles-only", action="store_true", help="only the deposit/push HBM-roofline leg (for ncu captures)")

@@ -116,10 +116,11 @@ def _slab_worker(rank: int, world: int, port: int, out):
 
     nx, ny, nz = 5, 4, 20
     full = torch.arange(6 * nx * ny * nz, dtype=torch.float32).reshape(6, -1) + 1.0  # what a 1-GPU field step would give
-    k0, k1 = slab_range(nz, rank, world)
+    ranges = [slab_range(nz, r, world) for r in range(world)]  # (0, 8) and (8, 20): unequal slabs, the gather pads the narrow one
+    k0, k1 = ranges[rank]
     mine = torch.full_like(full, 123.0)  # stale values outside the slab must not leak into the result
     mine[:, nx * ny * k0:nx * ny * k1] = full[:, nx * ny * k0:nx * ny * k1]
-    bench.assemble_slabs(dist, mine, nx * ny, k0, k1)
+    bench.assemble_slabs(dist, mine, nx * ny, ranges, rank)
     out.put((rank, bool(torch.equal(mine, full))))
     dist.barrier()
     dist.destroy_process_group()
@@ -130,6 +131,92 @@ def test_slab_assembly_gloo_world2():
     q = ctx.Queue()
     port = _free_port()
     procs = [ctx.Process(target=_slab_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = sorted(q.get(timeout=120) for _ in procs)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    assert res == [(0, True), (1, True)]
+
+
+def test_deal_range_covers_every_particle_once():
+    """Host logic of the sharded PIC step (paper_2209_07944_b200/sharded.py): particles are dealt to ranks in contiguous blocks."""
+    import numpy as np
+
+    from paper_2209_07944_b200.sharded import deal_particles, deal_range
+
+    for count in (0, 1, 7, 4096, 1000003):
+        for world in (1, 2, 3, 8):
+            r = [deal_range(count, k, world) for k in range(world)]
+            assert r[0][0] == 0 and r[-1][1] == count and all(a[1] == b[0] for a, b in zip(r, r[1:]))
+            assert max(b - a for a, b in r) - min(b - a for a, b in r) <= 1
+    part = {"x": np.arange(10.0), "alive": np.ones(10, np.uint8)}
+    a, b = deal_particles(part, 0, 2), deal_particles(part, 1, 2)
+    assert np.array_equal(np.concatenate([a["x"], b["x"]]), part["x"]) and a["alive"].size == 5
+    a["x"][0] = -1.0
+    assert part["x"][0] == 0.0  # copies, not views
+
+
+def _sharded_step_worker(rank: int, world: int, port: int, out):
+    """The six stages of ShardedPic.step with a stand-in context that records the calls and does integer-valued 'physics', so the
+    exchanges can be checked exactly on CPU tensors: what each rank deposits, that sources are summed, slabs gathered."""
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    from paper_2209_07944_b200.jefi import GridSpec, slab_range
+    from paper_2209_07944_b200.sharded import ShardedPic
+
+    class FakeCtx:
+        def __init__(self):
+            self.grid = GridSpec(3, 2, 20, 1.0, 1.0, 1.0, 1.0)
+            self.N = self.grid.N
+            self.src = torch.zeros((4, self.N))
+            self.EB = torch.full((6, self.N), -7.0)
+            self.calls = []
+
+        def slab_range(self, r, w):
+            return slab_range(self.grid.nz, r, w)
+
+        def deposit(self, part):
+            self.calls.append("deposit")
+            self.src.zero_()
+            self.src[:, part["cell"]] += part["q"]  # each rank's own particles only
+
+        def push_sources(self):
+            self.calls.append("push_sources")
+            self.pushed = self.src.clone()
+
+        def field_step_slab(self, k0, k1):
+            self.calls.append(("slab", k0, k1))
+            p = self.grid.nx * self.grid.ny
+            comp = torch.arange(6.0).reshape(6, 1)
+            self.EB[:, p * k0:p * k1] = self.pushed[0, p * k0:p * k1] * 10.0 + comp  # a function of the SUMMED sources
+
+        def push_particles(self, part):
+            self.calls.append("push_particles")
+            part["seen_E"] = self.EB[0, part["cell"]].clone()
+
+    ctx = FakeCtx()
+    sp = ShardedPic(ctx, dist, rank, world)
+    part = {"cell": torch.tensor([5 + rank, 100]), "q": torch.tensor([1.0 + rank, 2.0])}  # cell 100 gets charge from both ranks
+    sp.step(part)
+    expect_src = torch.zeros(ctx.N)
+    expect_src[5], expect_src[6], expect_src[100] = 1.0, 2.0, 4.0
+    ok = torch.equal(ctx.pushed[0], expect_src)
+    ok &= torch.equal(ctx.EB, expect_src * 10.0 + torch.arange(6.0).reshape(6, 1))  # whole grid, both slabs, on every rank
+    ok &= ctx.calls == ["deposit", "push_sources", ("slab",) + slab_range(20, rank, world), "push_particles"]
+    ok &= torch.equal(part["seen_E"], torch.tensor([10.0 * (1.0 + rank), 40.0]))  # the push sees fields of cells the OTHER rank solved
+    ok &= sp.bytes_per_step == {"all_reduce_rho_J": 16 * ctx.N, "all_gather_E_B": 24 * ctx.N}
+    out.put((rank, bool(ok)))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_sharded_pic_step_exchanges_gloo_world2():
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_sharded_step_worker, args=(r, 2, port, q)) for r in range(2)]
     for p in procs:
         p.start()
     res = sorted(q.get(timeout=120) for _ in procs)
