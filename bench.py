@@ -330,6 +330,10 @@ def time_pic(J, torch, device, config: int, steps: int, warmup: int) -> dict:
     return out
 
 
+# Table 1 of the paper, JefiPIC column: step -> (maximum displacement / m, maximum velocity / (m/s)) at 0.4 and 0.6 ns
+TABLE1 = {4000: (8.43e-4, 2.20e6), 6000: (1.29e-3, 2.25e6)}
+
+
 def time_paper_run(J, torch, device, count: int = 10_000_000, steps: int = 10_000) -> dict:
     """The one whole-run time the paper prints for the method (section 3.3.2): the planar
     emission in a 10 T B_y on 1 x 251 x 111 cells, dx = 1e-5 m, dt = 1e-13 s, 1 ns = 1e4 steps, 1e7 macro-particles, "within only
@@ -341,11 +345,20 @@ def time_paper_run(J, torch, device, count: int = 10_000_000, steps: int = 10_00
     with torch.cuda.stream(side):
         ctx = J.JefiContext(J.GridSpec(nx, ny, nz, w.dx, w.dx, w.dx, w.dt, Bext=w.Bext), device=device, sort_every=8)
         part = {k: torch.from_numpy(v).to(device) for k, v in wl.slab_particles("planar_emission", count).items()}
+        part["tag"] = torch.arange(count, dtype=torch.int32, device=device)  # permuted along by the cell sort: particle identity
+        y0 = part["y"].clone()
         side.synchronize()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        table1 = {}
         e0.record(side)
-        for _ in range(steps):
+        for i in range(steps):
             ctx.pic_step(part)
+            if i + 1 in TABLE1:  # the paper's two read-out times (Table 1), with the paper's own particle count
+                al = part["alive"].bool()
+                dy = (part["y"][al].double() - y0[part["tag"][al].long()].double()).max() * w.dx
+                u = [part[k][al].double() for k in ("ux", "uy", "uz")]
+                vy = (u[1] / (1 + u[0] ** 2 + u[1] ** 2 + u[2] ** 2).sqrt()).max() * wl.C_SI
+                table1[i + 1] = (dy, vy)  # device scalars: read back after the timed region
         e1.record(side)
         side.synchronize()
         ms = e0.elapsed_time(e1)
@@ -381,6 +394,9 @@ def time_paper_run(J, torch, device, count: int = 10_000_000, steps: int = 10_00
     out = {"workload": w.name, "grid": [nx, ny, nz], "particles": count, "steps": steps, "simulated_ns": steps * w.dt * 1e9,
            "total_s": ms * 1e-3, "steps_per_s": 1e3 * steps / ms, "alive_at_end": alive, "field_impl": ctx.info["field_impl"], "tiles": ctx.tile_info,
            "ms_per_call": breakdown,
+           "table1": {f"{k * w.dt * 1e9:.1f} ns": {"max_displacement_m": float(d), "paper_jefipic_m": TABLE1[k][0], "ratio": float(d) / TABLE1[k][0],
+                                                   "max_vy_m_per_s": float(v), "paper_jefipic_m_per_s": TABLE1[k][1], "ratio_v": float(v) / TABLE1[k][1]}
+                      for k, (d, v) in table1.items()},
            "paper": "JefiPIC: 'within only half an hour' on one A100, fp64 (PAPER.md:372); UNIPIC: 'over 6 hours' on a Xeon workstation"}
     ctx.close()
     return out
@@ -746,6 +762,7 @@ def main():
     ap.add_argument("--delay-rule", default="nearest", choices=["nearest", "linear"],
                     help="retarded-time rule: nearest = BASELINE.json's configs (reading A1); linear = second rule (A22)")
     ap.add_argument("--particles-only", action="store_true", help="only the deposit/push HBM-roofline leg (for ncu captures)")
+    ap.add_argument("--paper-run-only", action="store_true", help="only the paper_run leg (1x251x111, 1e7 macro-particles, 1e4 steps)")
     ap.add_argument("--cpu-obs", type=int, default=4096, help="observation cells of the cpu_baseline sample")
     ap.add_argument("--ref-obs", type=int, default=1024, help="observation cells per step of --impl reference")
     args = ap.parse_args()
@@ -766,6 +783,13 @@ def main():
 
         J.load_library()
         res = time_particle_kernels(J, torch, torch.device("cuda:0"), reps=max(1, args.steps))
+    elif args.paper_run_only:
+        import torch
+
+        from paper_2209_07944_b200 import jefi as J
+
+        J.load_library()
+        res = {"paper_run": time_paper_run(J, torch, torch.device("cuda:0"))}
     elif args.impl == "reference":
         if rank != 0:
             log(f"[reference] rank {rank} of {world}: idle (rank 0 alone runs the CPU oracle)")
